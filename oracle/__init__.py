@@ -1,0 +1,209 @@
+"""oracle/ -- TEST INFRASTRUCTURE, NOT THE PRODUCT.
+
+numpy/ctypes front end of `sorf_oracle.c`, the plain FP64 CPU statement of the SORF hot path
+(eq. 14-17, 20; see the C file's header for readings and pins).  Only `tests/`,
+`__graft_entry__.smoke()` and `bench.py`'s cpu_baseline / `--impl reference` legs may import
+this package; the product (`paper_2206_01580_b200/`) never does, and this package never
+imports the product.  Arguments are plain numpy arrays and scalars (the same fp32/int8/int32
+arrays the GPU library is given); results are float64.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+import subprocess
+from typing import Optional
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "sorf_oracle.c")
+_LIB = os.path.join(_HERE, "libsorf_oracle.so")
+_lib = None
+
+
+def build(force: bool = False) -> str:
+    """Compile sorf_oracle.c with gcc (-O2, no fast-math, OpenMP)."""
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+        tmp = _LIB + f".tmp{os.getpid()}"
+        subprocess.check_call(["gcc", "-O2", "-std=c99", "-fopenmp", "-fPIC", "-shared", _SRC, "-o", tmp, "-lm"])
+        os.replace(tmp, _LIB)
+    return _LIB
+
+
+def _load():
+    global _lib
+    if _lib is None:
+        _lib = ctypes.CDLL(build())
+        _lib.qo_scale.restype = ctypes.c_double
+        _lib.qo_scale.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.c_double]
+        _lib.qo_num_threads.restype = ctypes.c_int
+    return _lib
+
+
+def _p(a: Optional[np.ndarray]):
+    return None if a is None else a.ctypes.data_as(ctypes.c_void_p)
+
+
+def _f32(a):
+    return np.ascontiguousarray(a, dtype=np.float32)
+
+
+def _i32(a):
+    return np.ascontiguousarray(a, dtype=np.int32)
+
+
+def _i8(a):
+    return np.ascontiguousarray(a, dtype=np.int8)
+
+
+_I, _L, _D = ctypes.c_int, ctypes.c_int64, ctypes.c_double
+
+
+def num_threads() -> int:
+    return int(_load().qo_num_threads())
+
+
+def fwht(v: np.ndarray) -> np.ndarray:
+    """Unnormalised natural-order Walsh-Hadamard transform of a length-2^n vector (L163-167)."""
+    out = np.array(v, dtype=np.float64, copy=True)
+    _load().qo_fwht(_p(out), _I(out.shape[0]))
+    return out
+
+
+def scale(d: int, T: int, sigma: float) -> float:
+    return float(_load().qo_scale(d, T, float(sigma)))
+
+
+def sorf_u(x_I, e: int, d: int, D: int, T: int, sigma: float, signs) -> np.ndarray:
+    """u = W_e x_I (eq. 20), length D, stack-major."""
+    x_I, signs = _f32(x_I), _i8(signs)
+    u = np.empty(D, dtype=np.float64)
+    _load().qo_sorf_u(_p(x_I), _I(e), _I(d), _I(D), _I(T), _D(sigma), _p(signs), _p(u))
+    return u
+
+
+def forward(x, elem, mol_off, d, D, T, sigma, signs, bias) -> np.ndarray:
+    """Z[n_mol, D] (eq. 14 + eq. 15)."""
+    x, elem, mol_off, signs, bias = _f32(x), _i32(elem), _i32(mol_off), _i8(signs), _f32(bias)
+    n_mol = mol_off.shape[0] - 1
+    Z = np.empty((n_mol, D), dtype=np.float64)
+    _load().qo_forward(_p(x), _p(elem), _p(mol_off), _L(elem.shape[0]), _I(n_mol), _I(d), _I(D), _I(T),
+                       _D(sigma), _p(signs), _p(bias), _p(Z))
+    return Z
+
+
+def energy(Z, alpha) -> np.ndarray:
+    Z = np.ascontiguousarray(Z, dtype=np.float64)
+    alpha = _f32(alpha)
+    out = np.empty(Z.shape[0], dtype=np.float64)
+    _load().qo_energy(_p(Z), _p(alpha), _I(Z.shape[0]), _I(Z.shape[1]), _p(out))
+    return out
+
+
+def backward_g(x, elem, d, D, T, sigma, signs, bias, alpha) -> np.ndarray:
+    """g[n_atoms, d] = dE/dx (chain rule through eq. 14 and the transposed eq. 20)."""
+    x, elem, signs, bias, alpha = _f32(x), _i32(elem), _i8(signs), _f32(bias), _f32(alpha)
+    g = np.empty((elem.shape[0], d), dtype=np.float64)
+    _load().qo_backward_g(_p(x), _p(elem), _L(elem.shape[0]), _I(d), _I(D), _I(T), _D(sigma), _p(signs),
+                          _p(bias), _p(alpha), _p(g))
+    return g
+
+
+def forces_dense(g, mol_off, d, dense, dense_off) -> np.ndarray:
+    g = np.ascontiguousarray(g, dtype=np.float64)
+    mol_off, dense = _i32(mol_off), _f32(dense)
+    dense_off = np.ascontiguousarray(dense_off, dtype=np.int64)
+    F = np.zeros((g.shape[0], 3), dtype=np.float64)
+    _load().qo_forces_dense(_p(g), _p(mol_off), _I(mol_off.shape[0] - 1), _I(d), _p(dense), _p(dense_off), _p(F))
+    return F
+
+
+def forces_neighbor(g, d, nbr_idx, nbr_val) -> np.ndarray:
+    g = np.ascontiguousarray(g, dtype=np.float64)
+    nbr_idx, nbr_val = _i32(nbr_idx), _f32(nbr_val)
+    F = np.zeros((g.shape[0], 3), dtype=np.float64)
+    _load().qo_forces_neighbor(_p(g), _L(g.shape[0]), _I(d), _I(nbr_idx.shape[1]), _p(nbr_idx), _p(nbr_val), _p(F))
+    return F
+
+
+def force_rows_dense(x, elem, mol_off, d, D, T, sigma, signs, bias, dense, dense_off) -> np.ndarray:
+    """G[3 n_atoms, D] = -dZ/dr, rows (M, j, k) (L137, reading A8)."""
+    x, elem, mol_off, signs, bias, dense = _f32(x), _i32(elem), _i32(mol_off), _i8(signs), _f32(bias), _f32(dense)
+    dense_off = np.ascontiguousarray(dense_off, dtype=np.int64)
+    G = np.zeros((3 * elem.shape[0], D), dtype=np.float64)
+    _load().qo_force_rows_dense(_p(x), _p(elem), _p(mol_off), _I(mol_off.shape[0] - 1), _I(d), _I(D), _I(T),
+                                _D(sigma), _p(signs), _p(bias), _p(dense), _p(dense_off), _p(G))
+    return G
+
+
+def force_rows_neighbor(x, elem, d, D, T, sigma, signs, bias, nbr_idx, nbr_val) -> np.ndarray:
+    x, elem, signs, bias = _f32(x), _i32(elem), _i8(signs), _f32(bias)
+    nbr_idx, nbr_val = _i32(nbr_idx), _f32(nbr_val)
+    G = np.zeros((3 * elem.shape[0], D), dtype=np.float64)
+    _load().qo_force_rows_neighbor(_p(x), _p(elem), _L(elem.shape[0]), _I(d), _I(D), _I(T), _D(sigma), _p(signs),
+                                   _p(bias), _I(nbr_idx.shape[1]), _p(nbr_idx), _p(nbr_val), _p(G))
+    return G
+
+
+def normal_equations(A, y):
+    """(ZtZ, Zty) = (A^T A, A^T y) in FP64 from the fp32 rows the GPU is given (eq. 16-17)."""
+    A, y = _f32(A), _f32(y)
+    rows, D = A.shape
+    ZtZ = np.empty((D, D), dtype=np.float64)
+    Zty = np.empty(D, dtype=np.float64)
+    _load().qo_normal_equations(_p(A), _p(y), _L(rows), _I(D), _p(ZtZ), _p(Zty))
+    return ZtZ, Zty
+
+
+def gram_entries(A, ii, jj) -> np.ndarray:
+    A, ii, jj = _f32(A), _i32(ii), _i32(jj)
+    out = np.empty(ii.shape[0], dtype=np.float64)
+    _load().qo_gram_entries(_p(A), _L(A.shape[0]), _I(A.shape[1]), _p(ii), _p(jj), _L(ii.shape[0]), _p(out))
+    return out
+
+
+def gram_rows(A, y, ii):
+    A, ii = _f32(A), _i32(ii)
+    y = None if y is None else _f32(y)
+    out = np.empty((ii.shape[0], A.shape[1]), dtype=np.float64)
+    out_y = np.empty(ii.shape[0], dtype=np.float64)
+    _load().qo_gram_rows(_p(A), _p(y), _L(A.shape[0]), _I(A.shape[1]), _p(ii), _I(ii.shape[0]), _p(out), _p(out_y))
+    return out, out_y
+
+
+# ---- conveniences over a workloads.Workload-shaped object (attribute access only; no import) ----
+
+def _m(w):
+    m = w.model
+    return m.d, m.D, m.T, m.sigma, m.signs, m.bias
+
+
+def forward_w(w) -> np.ndarray:
+    return forward(w.x, w.elem, w.mol_off, *_m(w))
+
+
+def backward_g_w(w, alpha=None) -> np.ndarray:
+    return backward_g(w.x, w.elem, *_m(w), w.alpha if alpha is None else alpha)
+
+
+def forces_w(w, alpha=None) -> np.ndarray:
+    """F[n_atoms, 3] = -dE/dr through the supplied descriptor gradient (a5 + a6)."""
+    g = backward_g_w(w, alpha)
+    if w.grad.layout == "dense":
+        return forces_dense(g, w.mol_off, w.model.d, w.grad.dense, w.grad.dense_off)
+    return forces_neighbor(g, w.model.d, w.grad.nbr_idx, w.grad.nbr_val)
+
+
+def force_rows_w(w) -> np.ndarray:
+    if w.grad.layout == "dense":
+        return force_rows_dense(w.x, w.elem, w.mol_off, *_m(w), w.grad.dense, w.grad.dense_off)
+    return force_rows_neighbor(w.x, w.elem, *_m(w), w.grad.nbr_idx, w.grad.nbr_val)
+
+
+def predict_w(w, alpha=None):
+    """(energies[n_mol], forces[n_atoms, 3] or None): eq. 15 and F = -dE/dr."""
+    a = w.alpha if alpha is None else alpha
+    E = energy(forward_w(w), a)
+    F = forces_w(w, a) if w.grad is not None else None
+    return E, F
