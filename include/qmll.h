@@ -1,0 +1,137 @@
+/* qmll.h -- C-ABI of the B200 (sm_100a) SORF hot path of QML-Lightning (arXiv 2206.01580).
+ *
+ * Citations are /root/reference/PAPER.md line numbers + equation; "A<n>" are the readings of
+ * DESIGN.md (section "Readings of the paper").
+ *
+ * Conventions for every call
+ *   - ALL data pointers are DEVICE pointers (cudaMalloc'ed / torch CUDA tensors), caller-owned,
+ *     row-major, densely packed, naturally aligned to 16 bytes.  The two parameter structs
+ *     themselves (qmll_sorf_params, qmll_grad) live in HOST memory.
+ *   - The library allocates nothing persistent and keeps no state between calls; scratch comes from
+ *     `workspace` (device memory, 256-byte aligned, size from qmll_workspace_bytes()).
+ *   - Calls enqueue work on `cuda_stream` (a cudaStream_t cast to void*, NULL = default stream) and
+ *     return without synchronising; outputs are valid once the stream has been synchronised.
+ *   - Return value: QMLL_OK (0) or a negative qmll_status.  No exceptions cross the boundary.  Only
+ *     host-visible arguments are checked; device-side contents that break the documented contract
+ *     (elem[i] >= n_elem, non-monotone mol_off, signs other than +1/-1, nbr_idx >= n_atoms) are
+ *     undefined behaviour.
+ *   - There is no CPU fallback: on a machine without an sm_100 device every compute call returns
+ *     QMLL_ERR_UNSUPPORTED / QMLL_ERR_CUDA.
+ *
+ * Notation: n_atoms atoms in n_mol molecules (atoms of a molecule contiguous),
+ * descriptor length d (power of two), D = N_F features = n_s stacks of d, T = N_transform,
+ * S[e,s,t,:] the Rademacher diagonal D_{t+1} of element e and stack s, H the unnormalised
+ * Sylvester-Walsh-Hadamard matrix in natural order (L163-165), c = sqrt(d)/sigma * d^(-T/2) (A2).
+ */
+#ifndef QMLL_H_
+#define QMLL_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+  QMLL_OK = 0,
+  QMLL_ERR_INVALID_ARG = -1, /* null pointer, d not a power of two, D % d != 0, T not in 1..3, sigma <= 0,
+                                negative sizes, bad gradient layout                                         */
+  QMLL_ERR_UNSUPPORTED = -2, /* d outside 16..1024 (see qmll_sorf_params), device is not sm_100             */
+  QMLL_ERR_WORKSPACE = -3,   /* workspace NULL / too small / misaligned                                      */
+  QMLL_ERR_CUDA = -4         /* a CUDA runtime / driver call or a kernel launch failed                       */
+} qmll_status;
+
+/* The SORF "model" minus alpha (eq. 20, eq. 14; A1-A7). */
+typedef struct {
+  int32_t d;           /* descriptor length: power of two, supported 16, 32, 64, 128, 256, 512, 1024          */
+  int32_t D;           /* number of features N_F, a positive multiple of d                                    */
+  int32_t n_transform; /* T in {1, 2, 3}                                                                       */
+  int32_t n_elem;      /* number of element classes E >= 1                                                     */
+  float sigma;         /* kernel width > 0                                                                     */
+  const int8_t* signs; /* device [E, D/d, T, d], entries +1 / -1; t = 0 is D_1 and multiplies x (A4)          */
+  const float* bias;   /* device [E, D], b in [0, 2 pi] (eq. 14); per element (A6)                            */
+} qmll_sorf_params;
+
+enum { QMLL_GRAD_NONE = 0, QMLL_GRAD_DENSE = 1, QMLL_GRAD_NEIGHBOR = 2 };
+
+/* Descriptor gradient d x_I[m] / d r_{j,k} in one of two layouts (A12, A13). */
+typedef struct {
+  int32_t layout;           /* QMLL_GRAD_DENSE or QMLL_GRAD_NEIGHBOR                                          */
+  const float* dense;       /* DENSE: molecules concatenated; molecule M with n atoms holds [n, d, n, 3] =     */
+                            /*        (I, m, j, k), I and j local atom indices                                 */
+  const int64_t* dense_off; /* DENSE: device [n_mol + 1] offsets (in floats) of each molecule's block,        */
+                            /*        dense_off[M+1] - dense_off[M] = 3 d n_M^2                                */
+  const int32_t* nbr_idx;   /* NEIGHBOR: device [n_atoms, K]: global atom index j, or -1 = padding            */
+  const float* nbr_val;     /* NEIGHBOR: device [n_atoms, K, d, 3] = d x_I[m] / d r_{j,k}, j = nbr_idx[I, q];  */
+                            /*        self and duplicate j are legal and ACCUMULATE                            */
+  int32_t K;                /* NEIGHBOR: neighbours per atom                                                    */
+} qmll_grad;
+
+/* Steps a1-a3 (+a7): Z[M, l] = sum_{I in M} sqrt(2/D) cos((W_{e_I} x_I)[l] + b[e_I, l])
+ * (eq. 20, eq. 14, eq. 15), l = s*d + m (A5).
+ * If `grad` and `G` are given also the force rows (derivative features, L137; sign A8)
+ *   G[3*j + k, l] = -dZ[M(j), l] / d r_{j,k} = sum_I sqrt(2/D) sin(u_I[l] + b[e_I, l]) (W_{e_I} dx_I[:, j, k])[l]
+ * so that [Z; G] alpha = [E; F].  Rows of G are ordered by global atom index j then k = x, y, z.
+ *   x        [n_atoms, d] fp32          elem  [n_atoms] int32 in [0, n_elem)
+ *   mol_off  [n_mol + 1] int32, mol_off[0] = 0, mol_off[n_mol] = n_atoms, non-decreasing (empty molecules legal)
+ *   Z        [n_mol, D] fp32, overwritten (may be NULL if only G is wanted)
+ *   G        [3 n_atoms, D] fp32, overwritten; NULL unless grad != NULL
+ * n_atoms == 0 or n_mol == 0 is legal (Z rows of empty molecules are zero). */
+int qmll_sorf_forward(const qmll_sorf_params* p, const float* x, const int32_t* elem, const int32_t* mol_off,
+                      int64_t n_atoms, int32_t n_mol, const qmll_grad* grad, float* Z, float* G,
+                      void* workspace, size_t workspace_bytes, void* cuda_stream);
+
+/* Steps a1, a5, a6: F[j, k] = -dE/dr_{j,k} with E = sum_M Z[M, :] . alpha  (eq. 15; F = -dE/dr,
+ * eq. 5/10 L63, L90): q[l] = -sqrt(2/D) alpha[l] sin(u_I[l] + b); g_I = sum_s W_{e,s}^T q_s (transposed
+ * Hadamard / sign chain, L268 "backwards pass"); F[j,k] = -sum_I sum_m g_I[m] dx_I[m]/dr_{j,k}.
+ *   alpha [D] fp32;  grad required;  forces [n_atoms, 3] fp32, overwritten. */
+int qmll_sorf_backward_forces(const qmll_sorf_params* p, const float* x, const int32_t* elem,
+                              const int32_t* mol_off, int64_t n_atoms, int32_t n_mol, const float* alpha,
+                              const qmll_grad* grad, float* forces, void* workspace, size_t workspace_bytes,
+                              void* cuda_stream);
+
+/* Step a8: normal equations (eq. 16, eq. 17; FP32 round-off remark L351):
+ *   ZtZ (+)= A^T A,  Zty (+)= A^T y   for a block of rows A [rows, D] fp32 (rows of Z and/or G), y [rows] fp32.
+ * ZtZ [D, D] fp32 is stored full and exactly symmetric; Zty [D] fp32.  accumulate = 0 overwrites, 1 adds to the
+ * existing (symmetric) content.  The product runs on the tensor cores in 3xTF32 with the row dimension cut
+ * into chunks that are summed in fp32 round-to-nearest.  lambda*I and the solve are the caller's (A10).
+ * rows == 0 is legal (accumulate = 0 then zeroes the outputs).  y and Zty may both be NULL (ZtZ only). */
+int qmll_normal_equations(const float* A, const float* y, int64_t rows, int32_t D, int32_t accumulate,
+                          float* ZtZ, float* Zty, void* workspace, size_t workspace_bytes, void* cuda_stream);
+
+/* Steps a1-a6 composed: energies[M] = Z[M, :] . alpha (eq. 15) and, if grad != NULL, forces as in
+ * qmll_sorf_backward_forces, from one pass that shares u between cos and sin; Z is never materialised.
+ *   energies [n_mol] fp32, overwritten;  forces [n_atoms, 3] fp32 or NULL (then grad must be NULL). */
+int qmll_predict(const qmll_sorf_params* p, const float* x, const int32_t* elem, const int32_t* mol_off,
+                 int64_t n_atoms, int32_t n_mol, const float* alpha, const qmll_grad* grad, float* energies,
+                 float* forces, void* workspace, size_t workspace_bytes, void* cuda_stream);
+
+enum {
+  QMLL_CALL_FORWARD = 0,         /* qmll_sorf_forward without grad            */
+  QMLL_CALL_FORWARD_GRAD = 1,    /* qmll_sorf_forward with grad and G         */
+  QMLL_CALL_BACKWARD_FORCES = 2, /* qmll_sorf_backward_forces                 */
+  QMLL_CALL_NORMAL_EQUATIONS = 3,/* qmll_normal_equations (uses rows and p->D; p->d may be 0) */
+  QMLL_CALL_PREDICT = 4          /* qmll_predict                              */
+};
+
+/* Scratch bytes the named call needs for these sizes (host-side arithmetic only, no CUDA call).
+ * For QMLL_CALL_NORMAL_EQUATIONS this is the size that lets all `rows` be staged in one panel; the call
+ * also runs (in several panels) with any workspace of at least qmll_normal_equations_min_workspace(D). */
+size_t qmll_workspace_bytes(int which_call, const qmll_sorf_params* p, int64_t n_atoms, int32_t n_mol,
+                            int64_t rows);
+size_t qmll_normal_equations_min_workspace(int32_t D);
+
+/* Static description of a status code; for QMLL_ERR_CUDA the text of the last CUDA error seen by this
+ * thread is appended.  The returned pointer stays valid until the next call from the same thread. */
+const char* qmll_status_string(int status);
+
+/* Counters for benchmarks: number of kernel launches issued by this library since the last reset
+ * (process-wide, host-side counter). */
+int64_t qmll_launch_count(void);
+void qmll_reset_launch_count(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* QMLL_H_ */

@@ -1,0 +1,252 @@
+"""paper_2206_01580_b200 -- B200 (sm_100a) SORF hot path of QML-Lightning (arXiv 2206.01580).
+
+Thin Python binding over the C-ABI library `libqmll.so` declared in include/qmll.h: argument marshalling
+only (torch CUDA tensors -> device pointers, the current torch stream -> cudaStream_t).  Every step of the
+path runs in the library's CUDA kernels; there is no CPU or PyTorch fallback, and importing the compute
+functions fails loudly if the library is missing.  PyTorch is used for device memory and streams only.
+
+    from paper_2206_01580_b200 import SorfParams, Grad, qmll_sorf_forward, qmll_sorf_backward_forces, \
+        qmll_normal_equations, qmll_predict
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from dataclasses import dataclass
+from typing import Optional
+
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libqmll.so")
+
+QMLL_GRAD_DENSE, QMLL_GRAD_NEIGHBOR = 1, 2
+CALL_FORWARD, CALL_FORWARD_GRAD, CALL_BACKWARD_FORCES, CALL_NORMAL_EQUATIONS, CALL_PREDICT = range(5)
+
+EXPORTS = ("qmll_sorf_forward", "qmll_sorf_backward_forces", "qmll_normal_equations", "qmll_predict",
+           "qmll_workspace_bytes", "qmll_normal_equations_min_workspace", "qmll_status_string",
+           "qmll_launch_count", "qmll_reset_launch_count")
+
+
+class _CParams(ctypes.Structure):
+    _fields_ = [("d", ctypes.c_int32), ("D", ctypes.c_int32), ("n_transform", ctypes.c_int32),
+                ("n_elem", ctypes.c_int32), ("sigma", ctypes.c_float), ("signs", ctypes.c_void_p),
+                ("bias", ctypes.c_void_p)]
+
+
+class _CGrad(ctypes.Structure):
+    _fields_ = [("layout", ctypes.c_int32), ("dense", ctypes.c_void_p), ("dense_off", ctypes.c_void_p),
+                ("nbr_idx", ctypes.c_void_p), ("nbr_val", ctypes.c_void_p), ("K", ctypes.c_int32)]
+
+
+class QmllError(RuntimeError):
+    def __init__(self, status: int, text: str):
+        super().__init__(f"qmll status {status}: {text}")
+        self.status = status
+
+
+_lib = None
+
+
+def load_library() -> ctypes.CDLL:
+    """dlopen libqmll.so (built by paper_2206_01580_b200.build / __graft_entry__.build)."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise ImportError(f"{LIB_PATH} is missing: run `python -m paper_2206_01580_b200.build` "
+                          "(there is no fallback path)")
+    lib = ctypes.CDLL(LIB_PATH)
+    vp, i32, i64, sz = ctypes.c_void_p, ctypes.c_int32, ctypes.c_int64, ctypes.c_size_t
+    pp, gp = ctypes.POINTER(_CParams), ctypes.POINTER(_CGrad)
+    lib.qmll_sorf_forward.argtypes = [pp, vp, vp, vp, i64, i32, gp, vp, vp, vp, sz, vp]
+    lib.qmll_sorf_backward_forces.argtypes = [pp, vp, vp, vp, i64, i32, vp, gp, vp, vp, sz, vp]
+    lib.qmll_normal_equations.argtypes = [vp, vp, i64, i32, i32, vp, vp, vp, sz, vp]
+    lib.qmll_predict.argtypes = [pp, vp, vp, vp, i64, i32, vp, gp, vp, vp, vp, sz, vp]
+    for name in ("qmll_sorf_forward", "qmll_sorf_backward_forces", "qmll_normal_equations", "qmll_predict"):
+        getattr(lib, name).restype = ctypes.c_int
+    lib.qmll_workspace_bytes.argtypes = [ctypes.c_int, pp, i64, i32, i64]
+    lib.qmll_workspace_bytes.restype = sz
+    lib.qmll_normal_equations_min_workspace.argtypes = [i32]
+    lib.qmll_normal_equations_min_workspace.restype = sz
+    lib.qmll_status_string.argtypes = [ctypes.c_int]
+    lib.qmll_status_string.restype = ctypes.c_char_p
+    lib.qmll_launch_count.restype = i64
+    lib.qmll_reset_launch_count.restype = None
+    _lib = lib
+    return lib
+
+
+def _check(status: int) -> None:
+    if status != 0:
+        raise QmllError(status, load_library().qmll_status_string(status).decode())
+
+
+def _dev(t: Optional[torch.Tensor], dtype, name: str):
+    if t is None:
+        return None
+    if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == dtype and t.is_contiguous()):
+        raise TypeError(f"{name}: expected a contiguous CUDA tensor of dtype {dtype}")
+    return ctypes.c_void_p(t.data_ptr())
+
+
+def _stream() -> ctypes.c_void_p:
+    return ctypes.c_void_p(torch.cuda.current_stream().cuda_stream)
+
+
+@dataclass
+class SorfParams:
+    """qmll_sorf_params: signs int8 [E, D/d, T, d] and bias fp32 [E, D] are CUDA tensors."""
+    d: int
+    D: int
+    n_transform: int
+    n_elem: int
+    sigma: float
+    signs: torch.Tensor
+    bias: torch.Tensor
+
+    def c(self) -> _CParams:
+        return _CParams(self.d, self.D, self.n_transform, self.n_elem, float(self.sigma),
+                        _dev(self.signs, torch.int8, "signs"), _dev(self.bias, torch.float32, "bias"))
+
+
+@dataclass
+class Grad:
+    """qmll_grad: dense (flat fp32 + int64 offsets [n_mol+1]) or neighbour (int32 [n,K] + fp32 [n,K,d,3])."""
+    layout: int
+    dense: Optional[torch.Tensor] = None
+    dense_off: Optional[torch.Tensor] = None
+    nbr_idx: Optional[torch.Tensor] = None
+    nbr_val: Optional[torch.Tensor] = None
+    K: int = 0
+
+    @staticmethod
+    def make_dense(dense: torch.Tensor, dense_off: torch.Tensor) -> "Grad":
+        return Grad(QMLL_GRAD_DENSE, dense=dense, dense_off=dense_off)
+
+    @staticmethod
+    def make_neighbor(nbr_idx: torch.Tensor, nbr_val: torch.Tensor) -> "Grad":
+        return Grad(QMLL_GRAD_NEIGHBOR, nbr_idx=nbr_idx, nbr_val=nbr_val, K=int(nbr_idx.shape[1]))
+
+    def c(self) -> _CGrad:
+        return _CGrad(self.layout, _dev(self.dense, torch.float32, "dense"),
+                      _dev(self.dense_off, torch.int64, "dense_off"), _dev(self.nbr_idx, torch.int32, "nbr_idx"),
+                      _dev(self.nbr_val, torch.float32, "nbr_val"), int(self.K))
+
+
+_workspaces: dict = {}
+
+
+def workspace(nbytes: int, device) -> torch.Tensor:
+    """A cached, grow-only scratch tensor per device (torch allocations are 512-byte aligned)."""
+    key = torch.device(device).index or 0
+    ws = _workspaces.get(key)
+    if ws is None or ws.numel() < nbytes:
+        _workspaces.pop(key, None)
+        ws = None
+        ws = torch.empty(max(int(nbytes), 256), dtype=torch.uint8, device=device)
+        _workspaces[key] = ws
+    return ws
+
+
+def release_workspaces() -> None:
+    _workspaces.clear()
+
+
+def workspace_bytes(which: int, p: SorfParams, n_atoms: int = 0, n_mol: int = 0, rows: int = 0) -> int:
+    cp = p.c()
+    return int(load_library().qmll_workspace_bytes(which, ctypes.byref(cp), n_atoms, n_mol, rows))
+
+
+def _problem(x, elem, mol_off):
+    n_atoms, n_mol = int(elem.shape[0]), int(mol_off.shape[0]) - 1
+    return (_dev(x, torch.float32, "x"), _dev(elem, torch.int32, "elem"), _dev(mol_off, torch.int32, "mol_off"),
+            n_atoms, n_mol)
+
+
+def qmll_sorf_forward(p: SorfParams, x, elem, mol_off, grad: Optional[Grad] = None, Z=None, G=None,
+                      want_Z: bool = True):
+    """Z [n_mol, D] (and G [3 n_atoms, D] when `grad` is given): include/qmll.h qmll_sorf_forward."""
+    lib = load_library()
+    xp, ep, mp, n_atoms, n_mol = _problem(x, elem, mol_off)
+    if Z is None and want_Z:
+        Z = torch.empty((n_mol, p.D), dtype=torch.float32, device=x.device)
+    if grad is not None and G is None:
+        G = torch.empty((3 * n_atoms, p.D), dtype=torch.float32, device=x.device)
+    cp = p.c()
+    cg = grad.c() if grad is not None else None
+    nb = lib.qmll_workspace_bytes(CALL_FORWARD_GRAD if grad is not None else CALL_FORWARD, ctypes.byref(cp),
+                                  n_atoms, n_mol, 0)
+    ws = workspace(nb, x.device)
+    _check(lib.qmll_sorf_forward(ctypes.byref(cp), xp, ep, mp, n_atoms, n_mol,
+                                 ctypes.byref(cg) if cg is not None else None, _dev(Z, torch.float32, "Z"),
+                                 _dev(G, torch.float32, "G"), ctypes.c_void_p(ws.data_ptr()), ws.numel(), _stream()))
+    return (Z, G) if grad is not None else Z
+
+
+def qmll_sorf_backward_forces(p: SorfParams, x, elem, mol_off, alpha, grad: Grad, forces=None):
+    """forces [n_atoms, 3] = -dE/dr: include/qmll.h qmll_sorf_backward_forces."""
+    lib = load_library()
+    xp, ep, mp, n_atoms, n_mol = _problem(x, elem, mol_off)
+    if forces is None:
+        forces = torch.empty((n_atoms, 3), dtype=torch.float32, device=x.device)
+    cp, cg = p.c(), grad.c()
+    nb = lib.qmll_workspace_bytes(CALL_BACKWARD_FORCES, ctypes.byref(cp), n_atoms, n_mol, 0)
+    ws = workspace(nb, x.device)
+    _check(lib.qmll_sorf_backward_forces(ctypes.byref(cp), xp, ep, mp, n_atoms, n_mol,
+                                         _dev(alpha, torch.float32, "alpha"), ctypes.byref(cg),
+                                         _dev(forces, torch.float32, "forces"), ctypes.c_void_p(ws.data_ptr()),
+                                         ws.numel(), _stream()))
+    return forces
+
+
+def qmll_predict(p: SorfParams, x, elem, mol_off, alpha, grad: Optional[Grad] = None, energies=None, forces=None):
+    """(energies [n_mol], forces [n_atoms, 3] or None): include/qmll.h qmll_predict."""
+    lib = load_library()
+    xp, ep, mp, n_atoms, n_mol = _problem(x, elem, mol_off)
+    if energies is None:
+        energies = torch.empty((n_mol,), dtype=torch.float32, device=x.device)
+    if grad is not None and forces is None:
+        forces = torch.empty((n_atoms, 3), dtype=torch.float32, device=x.device)
+    cp = p.c()
+    cg = grad.c() if grad is not None else None
+    nb = lib.qmll_workspace_bytes(CALL_PREDICT, ctypes.byref(cp), n_atoms, n_mol, 0)
+    ws = workspace(nb, x.device)
+    _check(lib.qmll_predict(ctypes.byref(cp), xp, ep, mp, n_atoms, n_mol, _dev(alpha, torch.float32, "alpha"),
+                            ctypes.byref(cg) if cg is not None else None, _dev(energies, torch.float32, "energies"),
+                            _dev(forces, torch.float32, "forces"), ctypes.c_void_p(ws.data_ptr()), ws.numel(),
+                            _stream()))
+    return energies, forces
+
+
+def qmll_normal_equations(A, y=None, ZtZ=None, Zty=None, accumulate: bool = False,
+                          workspace_limit: Optional[int] = None):
+    """(ZtZ [D, D], Zty [D] or None) (+)= (A^T A, A^T y): include/qmll.h qmll_normal_equations."""
+    lib = load_library()
+    rows, D = int(A.shape[0]), int(A.shape[1])
+    if ZtZ is None:
+        if accumulate:
+            raise ValueError("accumulate=True needs ZtZ")
+        ZtZ = torch.empty((D, D), dtype=torch.float32, device=A.device)
+    if y is not None and Zty is None:
+        if accumulate:
+            raise ValueError("accumulate=True needs Zty")
+        Zty = torch.empty((D,), dtype=torch.float32, device=A.device)
+    cp = _CParams(0, D, 0, 0, 0.0, None, None)
+    nb = int(lib.qmll_workspace_bytes(CALL_NORMAL_EQUATIONS, ctypes.byref(cp), 0, 0, rows))
+    if workspace_limit is not None:
+        nb = max(min(nb, int(workspace_limit)), int(lib.qmll_normal_equations_min_workspace(D)))
+    ws = workspace(nb, A.device)
+    _check(lib.qmll_normal_equations(_dev(A, torch.float32, "A") if rows > 0 else None, _dev(y, torch.float32, "y"),
+                                     rows, D, 1 if accumulate else 0, _dev(ZtZ, torch.float32, "ZtZ"),
+                                     _dev(Zty, torch.float32, "Zty"), ctypes.c_void_p(ws.data_ptr()),
+                                     min(ws.numel(), nb), _stream()))
+    return ZtZ, Zty
+
+
+def launch_count() -> int:
+    return int(load_library().qmll_launch_count())
+
+
+def reset_launch_count() -> None:
+    load_library().qmll_reset_launch_count()

@@ -1,0 +1,214 @@
+// qmll_api.cu -- the C-ABI of include/qmll.h: host-side argument checks, workspace carving and the
+// sequencing of the kernels.  Every step of the path runs in the kernels; nothing is computed on the host.
+#include <atomic>
+#include <stdio.h>
+#include <string.h>
+
+#include "qmll_common.cuh"
+
+namespace qmll {
+
+static thread_local char g_err_text[512] = "";
+static std::atomic<long long> g_launches{0};
+
+void note_cuda_error(cudaError_t err, const char* where) {
+  snprintf(g_err_text, sizeof(g_err_text), "%s: %s", where, cudaGetErrorString(err));
+  cudaGetLastError();  // clear the sticky-less error state
+}
+void count_launch(int n) { g_launches.fetch_add(n, std::memory_order_relaxed); }
+
+static int check_params(const qmll_sorf_params* p) {
+  if (!p || !p->signs || !p->bias) return QMLL_ERR_INVALID_ARG;
+  if (p->d <= 0 || (p->d & (p->d - 1)) != 0) return QMLL_ERR_INVALID_ARG;
+  if (p->D <= 0 || p->D % p->d != 0) return QMLL_ERR_INVALID_ARG;
+  if (p->n_transform < 1 || p->n_transform > 3) return QMLL_ERR_INVALID_ARG;
+  if (p->n_elem < 1 || !(p->sigma > 0.f)) return QMLL_ERR_INVALID_ARG;
+  if (!sorf_supported_d(p->d)) return QMLL_ERR_UNSUPPORTED;
+  return QMLL_OK;
+}
+
+static int check_problem(const float* x, const int32_t* elem, const int32_t* mol_off, int64_t n_atoms,
+                         int32_t n_mol) {
+  if (n_atoms < 0 || n_mol < 0 || n_atoms > 0x7fffff00LL) return QMLL_ERR_INVALID_ARG;
+  if (!mol_off) return QMLL_ERR_INVALID_ARG;
+  if (n_atoms > 0 && (!x || !elem || n_mol == 0)) return QMLL_ERR_INVALID_ARG;
+  return QMLL_OK;
+}
+
+static int check_grad(const qmll_grad* g) {
+  if (!g) return QMLL_ERR_INVALID_ARG;
+  if (g->layout == QMLL_GRAD_DENSE) return (g->dense && g->dense_off) ? QMLL_OK : QMLL_ERR_INVALID_ARG;
+  if (g->layout == QMLL_GRAD_NEIGHBOR) {
+    if (g->K < 0) return QMLL_ERR_INVALID_ARG;
+    return (g->K == 0 || (g->nbr_idx && g->nbr_val)) ? QMLL_OK : QMLL_ERR_INVALID_ARG;
+  }
+  return QMLL_ERR_INVALID_ARG;
+}
+
+static int check_device() {
+  int dev = 0, major = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e == cudaSuccess) e = cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev);
+  if (e != cudaSuccess) { note_cuda_error(e, "cudaGetDevice"); return QMLL_ERR_CUDA; }
+  return major == 10 ? QMLL_OK : QMLL_ERR_UNSUPPORTED;
+}
+
+static int check_ws(void* ws, size_t have, size_t need) {
+  if (need == 0) return QMLL_OK;
+  if (!ws || ((uintptr_t)ws & 255) != 0 || have < need) return QMLL_ERR_WORKSPACE;
+  return QMLL_OK;
+}
+
+static size_t zs_bytes(const qmll_sorf_params* p, int64_t n_atoms) {
+  return align_up((size_t)n_atoms * p->D * sizeof(float), 256) + 256;
+}
+static size_t g_bytes(const qmll_sorf_params* p, int64_t n_atoms) {
+  return align_up((size_t)n_atoms * p->d * sizeof(float), 256) + 256;
+}
+static size_t e_bytes(int32_t n_mol) { return align_up((size_t)n_mol * sizeof(double), 256) + 256; }
+
+static int contract(const qmll_grad* grad, const float* g, const SorfProblem& pr, float* forces, cudaStream_t st) {
+  if (grad->layout == QMLL_GRAD_DENSE)
+    return contract_dense(g, pr.mol_off, pr.n_mol, pr.n_atoms, pr.p->d, grad->dense, grad->dense_off, forces, st);
+  return contract_neighbor(g, pr.n_atoms, pr.p->d, grad->K, grad->nbr_idx, grad->nbr_val, forces, st);
+}
+
+// shared body of qmll_sorf_backward_forces and qmll_predict
+static int backward_impl(const qmll_sorf_params* p, const float* x, const int32_t* elem, const int32_t* mol_off,
+                         int64_t n_atoms, int32_t n_mol, const float* alpha, const qmll_grad* grad, float* energies,
+                         float* forces, void* workspace, size_t workspace_bytes, cudaStream_t st, int which) {
+  int rc = check_params(p);
+  if (rc) return rc;
+  rc = check_problem(x, elem, mol_off, n_atoms, n_mol);
+  if (rc) return rc;
+  if (!alpha) return QMLL_ERR_INVALID_ARG;
+  if (forces) { rc = check_grad(grad); if (rc) return rc; }
+  else if (grad) return QMLL_ERR_INVALID_ARG;
+  if (!forces && !energies) return QMLL_ERR_INVALID_ARG;
+  rc = check_device();
+  if (rc) return rc;
+  rc = check_ws(workspace, workspace_bytes, qmll_workspace_bytes(which, p, n_atoms, n_mol, 0));
+  if (rc) return rc;
+
+  Carver ws(workspace, workspace_bytes);
+  SorfTables t;
+  rc = sorf_prepare_tables(p, alpha, ws, &t, st);
+  if (rc) return rc;
+  float* g = forces ? ws.take<float>((size_t)n_atoms * p->d) : nullptr;
+  double* eacc = energies ? ws.take<double>((size_t)n_mol) : nullptr;
+  if (!ws.fits()) return QMLL_ERR_WORKSPACE;
+  if (eacc && n_mol > 0) QMLL_CUDA_TRY(cudaMemsetAsync(eacc, 0, (size_t)n_mol * sizeof(double), st));
+  SorfProblem pr{p, x, elem, mol_off, n_atoms, n_mol};
+  rc = sorf_launch_backward(pr, t, g, eacc, st);
+  if (rc) return rc;
+  if (energies) { rc = sorf_finish_energies(eacc, energies, n_mol, st); if (rc) return rc; }
+  if (forces) { rc = contract(grad, g, pr, forces, st); if (rc) return rc; }
+  return QMLL_OK;
+}
+
+}  // namespace qmll
+
+using namespace qmll;
+
+extern "C" {
+
+size_t qmll_normal_equations_min_workspace(int32_t D) { return D > 0 ? syrk_min_workspace(D) : 0; }
+
+size_t qmll_workspace_bytes(int which_call, const qmll_sorf_params* p, int64_t n_atoms, int32_t n_mol,
+                            int64_t rows) {
+  if (!p) return 0;
+  if (which_call == QMLL_CALL_NORMAL_EQUATIONS) return p->D > 0 ? syrk_full_workspace(rows, p->D) : 0;
+  if (p->d <= 0 || p->D <= 0 || p->D % p->d != 0 || p->n_elem < 1 || p->n_transform < 1 || !sorf_supported_d(p->d))
+    return 0;
+  if (n_atoms < 0) n_atoms = 0;
+  if (n_mol < 0) n_mol = 0;
+  switch (which_call) {
+    case QMLL_CALL_FORWARD: return sorf_tables_bytes(p, false);
+    case QMLL_CALL_FORWARD_GRAD: return sorf_tables_bytes(p, false) + zs_bytes(p, n_atoms);
+    case QMLL_CALL_BACKWARD_FORCES: return sorf_tables_bytes(p, true) + g_bytes(p, n_atoms);
+    case QMLL_CALL_PREDICT: return sorf_tables_bytes(p, true) + g_bytes(p, n_atoms) + e_bytes(n_mol);
+    default: return 0;
+  }
+}
+
+int qmll_sorf_forward(const qmll_sorf_params* p, const float* x, const int32_t* elem, const int32_t* mol_off,
+                      int64_t n_atoms, int32_t n_mol, const qmll_grad* grad, float* Z, float* G, void* workspace,
+                      size_t workspace_bytes, void* cuda_stream) {
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  int rc = check_params(p);
+  if (rc) return rc;
+  rc = check_problem(x, elem, mol_off, n_atoms, n_mol);
+  if (rc) return rc;
+  if ((G != nullptr) != (grad != nullptr)) return QMLL_ERR_INVALID_ARG;
+  if (!Z && !G) return QMLL_ERR_INVALID_ARG;
+  if (grad) { rc = check_grad(grad); if (rc) return rc; }
+  rc = check_device();
+  if (rc) return rc;
+  rc = check_ws(workspace, workspace_bytes,
+                qmll_workspace_bytes(grad ? QMLL_CALL_FORWARD_GRAD : QMLL_CALL_FORWARD, p, n_atoms, n_mol, 0));
+  if (rc) return rc;
+  Carver ws(workspace, workspace_bytes);
+  SorfTables t;
+  rc = sorf_prepare_tables(p, nullptr, ws, &t, st);
+  if (rc) return rc;
+  float* zs = grad ? ws.take<float>((size_t)n_atoms * p->D) : nullptr;
+  if (!ws.fits()) return QMLL_ERR_WORKSPACE;
+  SorfProblem pr{p, x, elem, mol_off, n_atoms, n_mol};
+  rc = sorf_launch_forward(pr, t, Z, zs, st);
+  if (rc) return rc;
+  if (grad) {
+    if (grad->layout == QMLL_GRAD_DENSE)
+      rc = sorf_launch_force_rows_dense(pr, t, zs, grad->dense, grad->dense_off, G, st);
+    else
+      rc = sorf_launch_force_rows_neighbor(pr, t, zs, grad->nbr_idx, grad->nbr_val, grad->K, G, st);
+  }
+  return rc;
+}
+
+int qmll_sorf_backward_forces(const qmll_sorf_params* p, const float* x, const int32_t* elem,
+                              const int32_t* mol_off, int64_t n_atoms, int32_t n_mol, const float* alpha,
+                              const qmll_grad* grad, float* forces, void* workspace, size_t workspace_bytes,
+                              void* cuda_stream) {
+  if (!forces || !grad) return QMLL_ERR_INVALID_ARG;
+  return backward_impl(p, x, elem, mol_off, n_atoms, n_mol, alpha, grad, nullptr, forces, workspace,
+                       workspace_bytes, static_cast<cudaStream_t>(cuda_stream), QMLL_CALL_BACKWARD_FORCES);
+}
+
+int qmll_predict(const qmll_sorf_params* p, const float* x, const int32_t* elem, const int32_t* mol_off,
+                 int64_t n_atoms, int32_t n_mol, const float* alpha, const qmll_grad* grad, float* energies,
+                 float* forces, void* workspace, size_t workspace_bytes, void* cuda_stream) {
+  if (!energies) return QMLL_ERR_INVALID_ARG;
+  return backward_impl(p, x, elem, mol_off, n_atoms, n_mol, alpha, grad, energies, forces, workspace,
+                       workspace_bytes, static_cast<cudaStream_t>(cuda_stream), QMLL_CALL_PREDICT);
+}
+
+int qmll_normal_equations(const float* A, const float* y, int64_t rows, int32_t D, int32_t accumulate, float* ZtZ,
+                          float* Zty, void* workspace, size_t workspace_bytes, void* cuda_stream) {
+  if (rows < 0 || D <= 0 || !ZtZ) return QMLL_ERR_INVALID_ARG;
+  if (rows > 0 && !A) return QMLL_ERR_INVALID_ARG;
+  if ((y != nullptr) != (Zty != nullptr)) return QMLL_ERR_INVALID_ARG;
+  if (D % 4 != 0) return QMLL_ERR_UNSUPPORTED;  // TMA row pitch / 16-byte alignment of A rows
+  int rc = check_device();
+  if (rc) return rc;
+  return syrk_normal_equations(A, y, rows, D, accumulate, ZtZ, Zty, workspace, workspace_bytes,
+                               static_cast<cudaStream_t>(cuda_stream));
+}
+
+const char* qmll_status_string(int status) {
+  static thread_local char buf[640];
+  switch (status) {
+    case QMLL_OK: return "QMLL_OK";
+    case QMLL_ERR_INVALID_ARG: return "QMLL_ERR_INVALID_ARG: invalid argument";
+    case QMLL_ERR_UNSUPPORTED: return "QMLL_ERR_UNSUPPORTED: unsupported size or device (needs sm_100, d in 16..1024)";
+    case QMLL_ERR_WORKSPACE: return "QMLL_ERR_WORKSPACE: workspace missing, misaligned or too small";
+    case QMLL_ERR_CUDA:
+      snprintf(buf, sizeof(buf), "QMLL_ERR_CUDA: %s", g_err_text);
+      return buf;
+    default: return "unknown qmll status";
+  }
+}
+
+int64_t qmll_launch_count(void) { return g_launches.load(); }
+void qmll_reset_launch_count(void) { g_launches.store(0); }
+
+}  // extern "C"

@@ -1,0 +1,97 @@
+// qmll_common.cuh -- shared host-side plumbing of the CUDA library (error handling, launch counter,
+// workspace carving).  Internal to paper_2206_01580_b200/csrc; never included by oracle/.
+#pragma once
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <stddef.h>
+
+#include "../../include/qmll.h"
+
+namespace qmll {
+
+// Records the last CUDA error text for qmll_status_string (thread-local).
+void note_cuda_error(cudaError_t err, const char* where);
+void count_launch(int n = 1);
+
+#define QMLL_CUDA_TRY(expr)                                  \
+  do {                                                       \
+    cudaError_t _e = (expr);                                 \
+    if (_e != cudaSuccess) {                                 \
+      ::qmll::note_cuda_error(_e, #expr);                    \
+      return QMLL_ERR_CUDA;                                  \
+    }                                                        \
+  } while (0)
+
+// After a kernel launch: counts it and turns a launch error into QMLL_ERR_CUDA.
+#define QMLL_LAUNCH_CHECK(name)                              \
+  do {                                                       \
+    ::qmll::count_launch();                                  \
+    cudaError_t _e = cudaGetLastError();                     \
+    if (_e != cudaSuccess) {                                 \
+      ::qmll::note_cuda_error(_e, name);                     \
+      return QMLL_ERR_CUDA;                                  \
+    }                                                        \
+  } while (0)
+
+static inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+
+// Bump allocator over the caller's workspace; `fits()` tells whether everything carved so far fits.
+struct Carver {
+  char* base;
+  size_t size;
+  size_t used = 0;
+  Carver(void* b, size_t s) : base(static_cast<char*>(b)), size(s) {}
+  template <typename T>
+  T* take(size_t count) {
+    size_t off = align_up(used, 256);
+    used = off + count * sizeof(T);
+    return reinterpret_cast<T*>(base ? base + off : nullptr);
+  }
+  bool fits() const { return used <= size; }
+};
+
+// ---- SORF (sorf_kernels.cu) ----------------------------------------------------------------------
+struct SorfProblem {
+  const qmll_sorf_params* p;
+  const float* x;
+  const int32_t* elem;
+  const int32_t* mol_off;
+  int64_t n_atoms;
+  int32_t n_mol;
+};
+
+// Permuted / packed copies of the model tables living in the workspace (layouts in sorf_kernels.cu).
+struct SorfTables {
+  uint32_t* sign_bits;  // [E][T][EW][n_s*P]
+  float* bias_rev;      // [E][Ereg/4][n_s*P][4]   bias / (2 pi)
+  float* alpha_s;       // [Ereg/4][n_s*P][4]      alpha * sqrt(2/D)   (may be unused)
+};
+
+size_t sorf_tables_bytes(const qmll_sorf_params* p, bool with_alpha);
+int sorf_prepare_tables(const qmll_sorf_params* p, const float* alpha, Carver& ws, SorfTables* t,
+                        cudaStream_t st);
+int sorf_launch_forward(const SorfProblem& pr, const SorfTables& t, float* Z, float* zs_out, cudaStream_t st);
+int sorf_launch_backward(const SorfProblem& pr, const SorfTables& t, float* g_out, double* energy_acc,
+                         cudaStream_t st);
+int sorf_launch_force_rows_dense(const SorfProblem& pr, const SorfTables& t, const float* zs,
+                                 const float* dense, const int64_t* dense_off, float* G, cudaStream_t st);
+int sorf_launch_force_rows_neighbor(const SorfProblem& pr, const SorfTables& t, const float* zs,
+                                    const int32_t* nbr_idx, const float* nbr_val, int K, float* G,
+                                    cudaStream_t st);
+int sorf_finish_energies(const double* energy_acc, float* energies, int32_t n_mol, cudaStream_t st);
+bool sorf_supported_d(int d);
+
+// ---- gradient contraction (contract_kernels.cu) ------------------------------------------------------
+int contract_dense(const float* g, const int32_t* mol_off, int32_t n_mol, int64_t n_atoms, int d,
+                   const float* dense, const int64_t* dense_off, float* forces, cudaStream_t st);
+int contract_neighbor(const float* g, int64_t n_atoms, int d, int K, const int32_t* nbr_idx,
+                      const float* nbr_val, float* forces, cudaStream_t st);
+
+// ---- normal equations (syrk_tcgen05.cu) ----------------------------------------------------------------
+size_t syrk_min_workspace(int32_t D);
+size_t syrk_full_workspace(int64_t rows, int32_t D);
+int syrk_normal_equations(const float* A, const float* y, int64_t rows, int32_t D, int accumulate, float* ZtZ,
+                          float* Zty, void* ws, size_t ws_bytes, cudaStream_t st);
+
+}  // namespace qmll

@@ -1,0 +1,157 @@
+// sorf_dispatch.cu -- table packing kernels, workspace layout of the packed tables and the switch over the
+// supported descriptor lengths (the kernels themselves are instantiated in sorf_d*.cu).
+#include "sorf_kernels.cuh"
+
+namespace qmll {
+
+// ------------------------------------------------------------------------------------------------
+// Table packing.  gl = s*P + p is the "global lane" of stack s, sub-lane p; n_gl = n_s*P.
+//   sign_bits[((e*T + t)*EW + k)*n_gl + gl]  bit i  <->  S[e, s, t, p*E + 32k + i] == -1
+//   bias_rev [((e*E4 + j4)*n_gl + gl)*4 + i]        =   b[e, s*d + p*E + 4 j4 + i] / (2 pi)
+//   alpha_s  [(j4*n_gl + gl)*4 + i]                 =   alpha[s*d + p*E + 4 j4 + i] * sqrt(2/D)
+// so that a warp's loads of any of them are contiguous.
+// ------------------------------------------------------------------------------------------------
+__global__ void pack_signs_kernel(const int8_t* __restrict__ signs, uint32_t* __restrict__ out, int n_elem,
+                                  int n_s, int T, int d, int E, int P, int EW) {
+  const int n_gl = n_s * P;
+  const long long total = (long long)n_elem * T * EW * n_gl;
+  for (long long idx = blockIdx.x * (long long)blockDim.x + threadIdx.x; idx < total;
+       idx += (long long)gridDim.x * blockDim.x) {
+    int gl = (int)(idx % n_gl);
+    long long r = idx / n_gl;
+    int k = (int)(r % EW); r /= EW;
+    int t = (int)(r % T);
+    int e = (int)(r / T);
+    int s = gl / P, p = gl % P;
+    const int8_t* src = signs + (((size_t)e * n_s + s) * T + t) * d + p * E + 32 * k;
+    int nb = E - 32 * k < 32 ? E - 32 * k : 32;
+    uint32_t w = 0;
+    for (int i = 0; i < nb; ++i) w |= (src[i] < 0 ? 1u : 0u) << i;
+    out[idx] = w;
+  }
+}
+
+__global__ void permute_table_kernel(const float* __restrict__ in /* [rows, D] */, float* __restrict__ out,
+                                     int rows, int n_s, int d, int E, int P, float scale) {
+  const int n_gl = n_s * P, E4 = E / 4;
+  const long long D = (long long)n_s * d;
+  const long long total = (long long)rows * E4 * n_gl * 4;
+  for (long long idx = blockIdx.x * (long long)blockDim.x + threadIdx.x; idx < total;
+       idx += (long long)gridDim.x * blockDim.x) {
+    int i = (int)(idx & 3);
+    long long r = idx >> 2;
+    int gl = (int)(r % n_gl); r /= n_gl;
+    int j4 = (int)(r % E4);
+    int e = (int)(r / E4);
+    int s = gl / P, p = gl % P;
+    out[idx] = in[e * D + (long long)s * d + p * E + 4 * j4 + i] * scale;
+  }
+}
+
+
+__global__ void finish_energies_kernel(const double* __restrict__ acc, float* __restrict__ out, int n) {
+  int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < n) out[i] = (float)acc[i];
+}
+
+int device_sm_count() {
+  static int cached = 0;
+  if (cached == 0) {
+    int dev = 0, n = 0;
+    if (cudaGetDevice(&dev) == cudaSuccess &&
+        cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && n > 0)
+      cached = n;
+    else
+      return 148;
+  }
+  return cached;
+}
+
+bool sorf_supported_d(int d) { return d >= 16 && d <= 1024 && (d & (d - 1)) == 0; }
+
+static void shape_of(int d, int* E, int* P) {
+  *E = d < 128 ? d : 128;
+  *P = d / *E;
+}
+
+size_t sorf_tables_bytes(const qmll_sorf_params* p, bool with_alpha) {
+  int E, P;
+  shape_of(p->d, &E, &P);
+  const size_t n_gl = (size_t)(p->D / p->d) * P, EW = (E + 31) / 32;
+  size_t b = align_up((size_t)p->n_elem * p->n_transform * EW * n_gl * 4, 256);
+  b += align_up((size_t)p->n_elem * p->D * 4, 256);
+  if (with_alpha) b += align_up((size_t)p->D * 4, 256);
+  return b + 256;
+}
+
+int sorf_prepare_tables(const qmll_sorf_params* p, const float* alpha, Carver& ws, SorfTables* t,
+                        cudaStream_t st) {
+  int E, P;
+  shape_of(p->d, &E, &P);
+  const int n_s = p->D / p->d, EW = (E + 31) / 32;
+  const size_t n_gl = (size_t)n_s * P;
+  t->sign_bits = ws.take<uint32_t>((size_t)p->n_elem * p->n_transform * EW * n_gl);
+  t->bias_rev = ws.take<float>((size_t)p->n_elem * p->D);
+  t->alpha_s = alpha ? ws.take<float>((size_t)p->D) : nullptr;
+  if (!ws.fits()) return QMLL_ERR_WORKSPACE;
+  const int threads = 256;
+  auto blocks = [&](size_t n) { size_t b = (n + threads - 1) / threads; return (unsigned)(b > 65535 ? 65535 : (b ? b : 1)); };
+  pack_signs_kernel<<<blocks((size_t)p->n_elem * p->n_transform * EW * n_gl), threads, 0, st>>>(
+      p->signs, t->sign_bits, p->n_elem, n_s, p->n_transform, p->d, E, P, EW);
+  QMLL_LAUNCH_CHECK("pack_signs_kernel");
+  permute_table_kernel<<<blocks((size_t)p->n_elem * p->D), threads, 0, st>>>(
+      p->bias, t->bias_rev, p->n_elem, n_s, p->d, E, P, (float)(1.0 / (2.0 * M_PI)));
+  QMLL_LAUNCH_CHECK("permute_table_kernel(bias)");
+  if (alpha) {
+    permute_table_kernel<<<blocks((size_t)p->D), threads, 0, st>>>(alpha, t->alpha_s, 1, n_s, p->d, E, P,
+                                                                   (float)sqrt(2.0 / (double)p->D));
+    QMLL_LAUNCH_CHECK("permute_table_kernel(alpha)");
+  }
+  return QMLL_OK;
+}
+
+#define QMLL_SWITCH_D(d, CALL)                    \
+  switch (d) {                                    \
+    case 16: return CALL(d16);                    \
+    case 32: return CALL(d32);                    \
+    case 64: return CALL(d64);                    \
+    case 128: return CALL(d128);                  \
+    case 256: return CALL(d256);                  \
+    case 512: return CALL(d512);                  \
+    case 1024: return CALL(d1024);                \
+    default: return QMLL_ERR_UNSUPPORTED;         \
+  }
+
+int sorf_launch_forward(const SorfProblem& pr, const SorfTables& t, float* Z, float* zs_out, cudaStream_t st) {
+#define CALL(TAG) sorf_forward_##TAG(pr, t, Z, zs_out, st)
+  QMLL_SWITCH_D(pr.p->d, CALL)
+#undef CALL
+}
+int sorf_launch_backward(const SorfProblem& pr, const SorfTables& t, float* g_out, double* energy_acc,
+                         cudaStream_t st) {
+#define CALL(TAG) sorf_backward_##TAG(pr, t, g_out, energy_acc, st)
+  QMLL_SWITCH_D(pr.p->d, CALL)
+#undef CALL
+}
+int sorf_launch_force_rows_dense(const SorfProblem& pr, const SorfTables& t, const float* zs,
+                                 const float* dense, const int64_t* dense_off, float* G, cudaStream_t st) {
+#define CALL(TAG) sorf_force_rows_dense_##TAG(pr, t, zs, dense, dense_off, G, st)
+  QMLL_SWITCH_D(pr.p->d, CALL)
+#undef CALL
+}
+int sorf_launch_force_rows_neighbor(const SorfProblem& pr, const SorfTables& t, const float* zs,
+                                    const int32_t* nbr_idx, const float* nbr_val, int K, float* G,
+                                    cudaStream_t st) {
+#define CALL(TAG) sorf_force_rows_neighbor_##TAG(pr, t, zs, nbr_idx, nbr_val, K, G, st)
+  QMLL_SWITCH_D(pr.p->d, CALL)
+#undef CALL
+}
+
+int sorf_finish_energies(const double* energy_acc, float* energies, int32_t n_mol, cudaStream_t st) {
+  if (n_mol == 0) return QMLL_OK;
+  finish_energies_kernel<<<(n_mol + 255) / 256, 256, 0, st>>>(energy_acc, energies, n_mol);
+  QMLL_LAUNCH_CHECK("finish_energies_kernel");
+  return QMLL_OK;
+}
+
+}  // namespace qmll

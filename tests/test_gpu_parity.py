@@ -1,0 +1,168 @@
+"""GPU parity: the CUDA path (through the C-ABI library, via the thin binding) against the FP64 oracle on the
+same seeded inputs.  Tolerances are BASELINE.json:north_star's: relative Frobenius error <= 1e-5 for Z,
+energies and ZtZ (also used for G and Zty), <= 1e-4 for forces.
+"""
+import numpy as np
+import pytest
+
+import oracle
+from workloads import make_workload, tiny_workload
+
+pytestmark = pytest.mark.gpu
+
+TOL, TOL_F = 1e-5, 1e-4
+
+
+def rel(a, b):
+    a = np.asarray(a, dtype=np.float64)
+    b = np.asarray(b, dtype=np.float64)
+    den = np.linalg.norm(b)
+    return float(np.linalg.norm(a - b) / den) if den > 0 else float(np.linalg.norm(a))
+
+
+@pytest.fixture(scope="module")
+def q():
+    import torch
+    import paper_2206_01580_b200 as pkg
+    from paper_2206_01580_b200 import workload_io
+    pkg.load_library()
+    assert torch.cuda.is_available()
+    return pkg, workload_io, torch
+
+
+def run_all(q, w, check_ne=True):
+    """Runs every export on workload w and compares with the oracle."""
+    pkg, wio, torch = q
+    dp = wio.device_problem(w)
+    Zo = oracle.forward_w(w)
+    # forward
+    Z = pkg.qmll_sorf_forward(dp.params, dp.x, dp.elem, dp.mol_off)
+    torch.cuda.synchronize()
+    assert rel(Z.cpu().numpy(), Zo) <= TOL
+    Eo = oracle.energy(Zo, w.alpha)
+    if w.grad is None:
+        E, F = pkg.qmll_predict(dp.params, dp.x, dp.elem, dp.mol_off, dp.alpha)
+        assert F is None
+        assert rel(E.cpu().numpy(), Eo) <= TOL
+        return
+    # forward + force rows
+    Z2, G = pkg.qmll_sorf_forward(dp.params, dp.x, dp.elem, dp.mol_off, dp.grad)
+    Go = oracle.force_rows_w(w)
+    assert rel(Z2.cpu().numpy(), Zo) <= TOL
+    assert rel(G.cpu().numpy(), Go) <= TOL
+    # predict and backward
+    Fo = oracle.forces_w(w)
+    E, F = pkg.qmll_predict(dp.params, dp.x, dp.elem, dp.mol_off, dp.alpha, dp.grad)
+    assert rel(E.cpu().numpy(), Eo) <= TOL
+    assert rel(F.cpu().numpy(), Fo) <= TOL_F
+    F2 = pkg.qmll_sorf_backward_forces(dp.params, dp.x, dp.elem, dp.mol_off, dp.alpha, dp.grad)
+    assert rel(F2.cpu().numpy(), Fo) <= TOL_F
+    # G alpha = F (JVP/VJP consistency on the GPU results themselves, in fp64 on the host)
+    if F.numel() > 0:
+        Ga = G.cpu().numpy().astype(np.float64) @ w.alpha.astype(np.float64)
+        assert rel(Ga.reshape(-1, 3), Fo) <= TOL_F
+    if check_ne:
+        A = torch.cat([Z2, G]).contiguous()
+        y = dp.y
+        ZtZ, Zty = pkg.qmll_normal_equations(A, y)
+        An = A.cpu().numpy()
+        ZtZo, Ztyo = oracle.normal_equations(An, w.y)
+        ZtZn = ZtZ.cpu().numpy()
+        assert rel(ZtZn, ZtZo) <= TOL
+        assert rel(Zty.cpu().numpy(), Ztyo) <= TOL
+        assert np.array_equal(ZtZn, ZtZn.T)
+
+
+def test_c1_full(q):
+    run_all(q, make_workload("c1"))
+
+
+@pytest.mark.parametrize("T", [1, 2, 3])
+@pytest.mark.parametrize("d,D", [(16, 64), (32, 96), (64, 448), (128, 4224), (256, 1024), (512, 1024), (1024, 2048)])
+def test_tiny_ragged_dense(q, d, D, T):
+    # ragged molecules incl. empty ones and one longer than a chunk; D/d not a multiple of the warp's stack count
+    counts = [3, 0, 1, 7, 0, 40, 2, 5]
+    if d >= 512:
+        counts = [3, 0, 5, 2]
+    w = tiny_workload(seed=1000 + d + T, d=d, D=D, T=T, sigma=1.5 * np.sqrt(d) / 4, counts=counts, n_elem=3,
+                      grad="dense", x_std=1.0)
+    run_all(q, w, check_ne=(d == 64))
+
+
+@pytest.mark.parametrize("d,D", [(64, 256), (128, 1024), (256, 2048)])
+def test_tiny_neighbor(q, d, D):
+    w = tiny_workload(seed=77 + d, d=d, D=D, T=3, sigma=np.sqrt(d) / 2, counts=[50, 0, 13], n_elem=2,
+                      grad="neighbor", K=6)
+    run_all(q, w, check_ne=False)
+
+
+def test_c2_reduced(q):
+    run_all(q, make_workload("c2", n_mol=12, D=2048))
+
+
+def test_c3_reduced(q):
+    run_all(q, make_workload("c3", n_mol=700, D=4096))
+
+
+def test_c4_reduced(q):
+    run_all(q, make_workload("c4", n_mol=6, D=2048), check_ne=False)
+    run_all(q, make_workload("c4", n_mol=4, D=1024, part="infer"), check_ne=False)
+
+
+def test_c5_reduced(q):
+    run_all(q, make_workload("c5", n_atoms=1500, D=4096, K=8))
+
+
+def test_empty_inputs(q):
+    pkg, wio, torch = q
+    w = tiny_workload(seed=5, d=64, D=128, T=3, sigma=2.0, counts=[0, 0], grad=None)
+    dp = wio.device_problem(w)
+    Z = pkg.qmll_sorf_forward(dp.params, dp.x, dp.elem, dp.mol_off)
+    assert Z.shape == (2, 128) and float(Z.abs().max()) == 0.0
+    E, _ = pkg.qmll_predict(dp.params, dp.x, dp.elem, dp.mol_off, dp.alpha)
+    assert float(E.abs().max()) == 0.0
+
+
+@pytest.mark.parametrize("rows,D", [(1, 256), (777, 384), (1500, 128), (2500, 520), (4096, 1024)])
+def test_normal_equations_shapes(q, rows, D):
+    pkg, wio, torch = q
+    rng = np.random.default_rng(rows + D)
+    # correlated, non-zero-mean rows (like Z of near-identical molecules): the hard case for fp32 accumulation
+    A = (0.7 + 0.3 * rng.standard_normal((rows, D))).astype(np.float32)
+    y = rng.standard_normal(rows).astype(np.float32)
+    Ad, yd = torch.from_numpy(A).cuda(), torch.from_numpy(y).cuda()
+    ZtZ, Zty = pkg.qmll_normal_equations(Ad, yd)
+    ZtZo, Ztyo = oracle.normal_equations(A, y)
+    assert rel(ZtZ.cpu().numpy(), ZtZo) <= TOL
+    assert rel(Zty.cpu().numpy(), Ztyo) <= TOL
+    # accumulate a second block, with a workspace that forces several panels
+    B = rng.standard_normal((rows, D)).astype(np.float32)
+    yb = rng.standard_normal(rows).astype(np.float32)
+    pkg.qmll_normal_equations(torch.from_numpy(B).cuda(), torch.from_numpy(yb).cuda(), ZtZ=ZtZ, Zty=Zty,
+                              accumulate=True, workspace_limit=0)
+    ZtZo2, Ztyo2 = oracle.normal_equations(B, yb)
+    Zn = ZtZ.cpu().numpy()
+    assert rel(Zn, ZtZo + ZtZo2) <= TOL
+    assert rel(Zty.cpu().numpy(), Ztyo + Ztyo2) <= TOL
+    assert np.array_equal(Zn, Zn.T)
+
+
+def test_normal_equations_zero_rows(q):
+    pkg, wio, torch = q
+    A = torch.empty((0, 256), dtype=torch.float32, device="cuda")
+    y = torch.empty((0,), dtype=torch.float32, device="cuda")
+    ZtZ, Zty = pkg.qmll_normal_equations(A, y)
+    assert float(ZtZ.abs().max()) == 0.0 and float(Zty.abs().max()) == 0.0
+
+
+def test_error_codes(q):
+    pkg, wio, torch = q
+    w = tiny_workload(seed=9, d=64, D=128, T=3, sigma=2.0, counts=[2], grad="dense")
+    dp = wio.device_problem(w)
+    bad = pkg.SorfParams(d=48, D=96, n_transform=3, n_elem=3, sigma=1.0, signs=dp.params.signs, bias=dp.params.bias)
+    with pytest.raises(pkg.QmllError) as ei:
+        pkg.qmll_sorf_forward(bad, dp.x, dp.elem, dp.mol_off)
+    assert ei.value.status == -1
+    bad2 = pkg.SorfParams(d=64, D=128, n_transform=4, n_elem=3, sigma=1.0, signs=dp.params.signs, bias=dp.params.bias)
+    with pytest.raises(pkg.QmllError):
+        pkg.qmll_sorf_forward(bad2, dp.x, dp.elem, dp.mol_off)
