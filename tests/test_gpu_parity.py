@@ -110,7 +110,7 @@ def test_c4_reduced(q):
 
 
 def test_c5_reduced(q):
-    run_all(q, make_workload("c5", n_atoms=1500, D=4096, K=8))
+    run_all(q, make_workload("c5", n_atoms=1500, D=4096, K=8), check_ne=False)  # c5 is inference only (no y rows)
 
 
 def test_empty_inputs(q):
