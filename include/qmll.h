@@ -131,6 +131,13 @@ const char* qmll_status_string(int status);
 int64_t qmll_launch_count(void);
 void qmll_reset_launch_count(void);
 
+/* Measurement aid (bench.py roofline): when enabled, every launch of the tensor-core kernel inside
+ * qmll_normal_equations is bracketed by CUDA events on the caller's stream.  The collect call waits for them,
+ * returns the summed kernel time in ms and the number of launches since the last collect, and frees them
+ * (at most 4096 launches are recorded between collects).  Not thread-safe. */
+void qmll_time_normal_equations_kernel(int enable);
+int qmll_collect_normal_equations_kernel_ms(double* total_ms, int* launches);
+
 #ifdef __cplusplus
 }
 #endif

@@ -25,7 +25,8 @@ CALL_FORWARD, CALL_FORWARD_GRAD, CALL_BACKWARD_FORCES, CALL_NORMAL_EQUATIONS, CA
 
 EXPORTS = ("qmll_sorf_forward", "qmll_sorf_backward_forces", "qmll_normal_equations", "qmll_predict",
            "qmll_workspace_bytes", "qmll_normal_equations_min_workspace", "qmll_status_string",
-           "qmll_launch_count", "qmll_reset_launch_count")
+           "qmll_launch_count", "qmll_reset_launch_count", "qmll_time_normal_equations_kernel",
+           "qmll_collect_normal_equations_kernel_ms")
 
 
 class _CParams(ctypes.Structure):
@@ -73,6 +74,11 @@ def load_library() -> ctypes.CDLL:
     lib.qmll_status_string.restype = ctypes.c_char_p
     lib.qmll_launch_count.restype = i64
     lib.qmll_reset_launch_count.restype = None
+    lib.qmll_time_normal_equations_kernel.argtypes = [ctypes.c_int]
+    lib.qmll_time_normal_equations_kernel.restype = None
+    lib.qmll_collect_normal_equations_kernel_ms.argtypes = [ctypes.POINTER(ctypes.c_double),
+                                                            ctypes.POINTER(ctypes.c_int)]
+    lib.qmll_collect_normal_equations_kernel_ms.restype = ctypes.c_int
     _lib = lib
     return lib
 
@@ -250,3 +256,14 @@ def launch_count() -> int:
 
 def reset_launch_count() -> None:
     load_library().qmll_reset_launch_count()
+
+
+def time_normal_equations_kernel(enable: bool) -> None:
+    load_library().qmll_time_normal_equations_kernel(1 if enable else 0)
+
+
+def collect_normal_equations_kernel_ms():
+    """(summed ms, launches) of the tcgen05 kernel since the last collect (waits for the events)."""
+    ms, n = ctypes.c_double(0.0), ctypes.c_int(0)
+    _check(load_library().qmll_collect_normal_equations_kernel_ms(ctypes.byref(ms), ctypes.byref(n)))
+    return float(ms.value), int(n.value)

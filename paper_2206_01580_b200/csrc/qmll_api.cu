@@ -208,6 +208,12 @@ const char* qmll_status_string(int status) {
   }
 }
 
+void qmll_time_normal_equations_kernel(int enable) { syrk_set_timing(enable != 0); }
+int qmll_collect_normal_equations_kernel_ms(double* total_ms, int* launches) {
+  if (!total_ms || !launches) return QMLL_ERR_INVALID_ARG;
+  return syrk_collect_timing(total_ms, launches);
+}
+
 int64_t qmll_launch_count(void) { return g_launches.load(); }
 void qmll_reset_launch_count(void) { g_launches.store(0); }
 

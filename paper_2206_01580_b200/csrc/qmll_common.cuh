@@ -94,4 +94,7 @@ size_t syrk_full_workspace(int64_t rows, int32_t D);
 int syrk_normal_equations(const float* A, const float* y, int64_t rows, int32_t D, int accumulate, float* ZtZ,
                           float* Zty, void* ws, size_t ws_bytes, cudaStream_t st);
 
+void syrk_set_timing(bool on);
+int syrk_collect_timing(double* total_ms, int* launches);
+
 }  // namespace qmll

@@ -377,6 +377,28 @@ static int make_map(CUtensorMap* map, float* base, int D, long long R_pad) {
   return QMLL_OK;
 }
 
+// Optional per-launch timing of the tcgen05 kernel (bench.py's roofline): events on the caller's stream.
+static bool g_timing = false;
+struct TimedLaunch { cudaEvent_t a, b; };
+static TimedLaunch g_timed[4096];
+static int g_n_timed = 0;
+void syrk_set_timing(bool on) { g_timing = on; }
+int syrk_collect_timing(double* total_ms, int* launches) {
+  double tot = 0.0;
+  for (int i = 0; i < g_n_timed; ++i) {
+    float ms = 0.f;
+    QMLL_CUDA_TRY(cudaEventSynchronize(g_timed[i].b));
+    QMLL_CUDA_TRY(cudaEventElapsedTime(&ms, g_timed[i].a, g_timed[i].b));
+    tot += ms;
+    cudaEventDestroy(g_timed[i].a);
+    cudaEventDestroy(g_timed[i].b);
+  }
+  *total_ms = tot;
+  *launches = g_n_timed;
+  g_n_timed = 0;
+  return QMLL_OK;
+}
+
 static long long pad_rows(long long r) { return (r + kRowPad - 1) / kRowPad * kRowPad; }
 
 size_t syrk_min_workspace(int32_t D) { return (size_t)2 * D * kChunkRows * sizeof(float) + 1024; }
@@ -423,9 +445,19 @@ int syrk_normal_equations(const float* A, const float* y, int64_t rows, int32_t 
     if (rc != QMLL_OK) return rc;
     rc = make_map(&map_lo, At_lo, D, rp);
     if (rc != QMLL_OK) return rc;
+    const bool timed = g_timing && g_n_timed < 4096;
+    if (timed) {
+      QMLL_CUDA_TRY(cudaEventCreate(&g_timed[g_n_timed].a));
+      QMLL_CUDA_TRY(cudaEventCreate(&g_timed[g_n_timed].b));
+      QMLL_CUDA_TRY(cudaEventRecord(g_timed[g_n_timed].a, st));
+    }
     syrk_tcgen05_kernel<<<grid, kSyrkThreads, kSmemBytes, st>>>(map_hi, map_lo, ZtZ, D, (int)(rp / kBK), n_tiles,
                                                               first_store);
     QMLL_LAUNCH_CHECK("syrk_tcgen05_kernel");
+    if (timed) {
+      QMLL_CUDA_TRY(cudaEventRecord(g_timed[g_n_timed].b, st));
+      ++g_n_timed;
+    }
     first_store = 0;
   }
   dim3 g3((unsigned)((D + 31) / 32), (unsigned)((D + 31) / 32));
