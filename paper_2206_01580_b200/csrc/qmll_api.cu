@@ -186,7 +186,7 @@ int qmll_normal_equations(const float* A, const float* y, int64_t rows, int32_t 
                           float* Zty, void* workspace, size_t workspace_bytes, void* cuda_stream) {
   if (rows < 0 || D <= 0 || !ZtZ) return QMLL_ERR_INVALID_ARG;
   if (rows > 0 && !A) return QMLL_ERR_INVALID_ARG;
-  if ((y != nullptr) != (Zty != nullptr)) return QMLL_ERR_INVALID_ARG;
+  if (rows > 0 && (y != nullptr) != (Zty != nullptr)) return QMLL_ERR_INVALID_ARG;
   if (D % 4 != 0) return QMLL_ERR_UNSUPPORTED;  // TMA row pitch / 16-byte alignment of A rows
   int rc = check_device();
   if (rc) return rc;

@@ -14,6 +14,7 @@
 //      triangle are computed.
 //   3. mirror_lower_kernel: C[i, j] = C[j, i] for i < j  -> full, exactly symmetric matrix.
 #include <cuda.h>
+#include <stdlib.h>
 
 #include "qmll_common.cuh"
 
@@ -24,9 +25,21 @@ constexpr int kBN = 256;          // tile extent along J (MMA N, TMEM columns)
 constexpr int kBK = 32;           // rows per pipeline stage = one 128-byte swizzle span of fp32
 constexpr int kUmmaK = 8;         // rows per tcgen05.mma kind::tf32 (32 bytes)
 constexpr int kStages = 2;
-constexpr int kChunkRows = 1024;  // rows accumulated in TMEM before a drain (fp32 RN sum across chunks)
+constexpr int kChunkRows = 1024;  // panel granularity (rows); the TMEM drain interval is chunk_rows() <= this
+// Rows accumulated in TMEM before a drain.  The tensor core truncates (rounds toward zero) every accumulate, a
+// bias of ~2e-8 per MMA relative to the running sum, so long same-sign sums (Gram diagonals, coherent Z columns)
+// need short chunks; chunk partials are summed in fp32 round-to-nearest.  QMLL_CHUNK_ROWS overrides (tuning).
+static int chunk_rows() {
+  static int v = 0;
+  if (v == 0) {
+    v = 128;
+    const char* e = getenv("QMLL_CHUNK_ROWS");
+    if (e) { int t = atoi(e); if (t >= 32 && t <= 1024 && t % 32 == 0) v = t; }
+  }
+  return v;
+}
 constexpr int kRowPad = 64;       // panels are padded with zero rows to a multiple of this
-constexpr int kSyrkThreads = 192; // warp 0 TMA producer, warp 1 MMA issuer, warps 2..5 epilogue
+constexpr int kSyrkThreads = 320; // warp 0 TMA producer, warp 1 MMA issuer, warps 2..9 epilogue
 constexpr uint32_t kTileABytes = kBM * kBK * 4;             // 16 KB
 constexpr uint32_t kTileBBytes = kBN * kBK * 4;             // 32 KB
 constexpr uint32_t kStageBytes = 2 * kTileABytes + 2 * kTileBBytes;  // hi + lo of both operands: 96 KB
@@ -174,7 +187,7 @@ __host__ __device__ inline int tiles_in_row(int tj, int n_ti) { return (2 * tj +
 __global__ void __launch_bounds__(kSyrkThreads, 1)
 syrk_tcgen05_kernel(const __grid_constant__ CUtensorMap map_hi, const __grid_constant__ CUtensorMap map_lo,
                     float* __restrict__ C, int D, int n_kb /* 32-row blocks in the panel */, int n_tiles,
-                    int first_store) {
+                    int first_store, int kb_per_chunk) {
   extern __shared__ uint8_t smem_raw[];
   uint8_t* smem = reinterpret_cast<uint8_t*>(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
   uint64_t* bars = reinterpret_cast<uint64_t*>(smem + kStages * kStageBytes);
@@ -186,12 +199,11 @@ syrk_tcgen05_kernel(const __grid_constant__ CUtensorMap map_hi, const __grid_con
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int n_ti = (D + kBM - 1) / kBM;
-  const int kb_per_chunk = kChunkRows / kBK;
   const int n_chunks = (n_kb + kb_per_chunk - 1) / kb_per_chunk;
 
   if (threadIdx.x == 0) {
     for (int s = 0; s < kStages; ++s) { mbar_init(&full_bar[s], 1); mbar_init(&empty_bar[s], 1); }
-    for (int b = 0; b < 2; ++b) { mbar_init(&tfull_bar[b], 1); mbar_init(&tempty_bar[b], 4); }
+    for (int b = 0; b < 2; ++b) { mbar_init(&tfull_bar[b], 1); mbar_init(&tempty_bar[b], 8); }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
   }
@@ -265,45 +277,49 @@ syrk_tcgen05_kernel(const __grid_constant__ CUtensorMap map_hi, const __grid_con
       }
     }
   } else {
-    // ===================== epilogue warps 2..5 =====================
+    // ===================== epilogue warps 2..9 =====================
+    // Two warps per TMEM lane quarter; each owns half of the 256 accumulator columns.  Chunk partials are summed
+    // in REGISTERS (128 fp32 per thread, round-to-nearest) so that draining TMEM every few hundred rows costs only
+    // tcgen05.ld + FADD; C is touched once per tile.
     const int quarter = warp & 3;  // TMEM lanes [32 q, 32 q + 32) are the ones this warp may read
+    const int chalf = (warp - 2) >> 2;  // 0: columns [0,128), 1: columns [128,256)
     const int i_loc = quarter * 32 + lane;
     uint32_t item = 0;
     for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
       int tj = 0, rem = tile;
       while (rem >= tiles_in_row(tj, n_ti)) { rem -= tiles_in_row(tj, n_ti); ++tj; }
-      const int I0 = rem * kBM, J0 = tj * kBN;
+      const int I0 = rem * kBM, J0 = tj * kBN + chalf * 128;
       const int col = I0 + i_loc;  // column of C this thread writes (transposed store)
+      float acc[128];
+#pragma unroll
+      for (int j = 0; j < 128; ++j) acc[j] = 0.f;
       for (int ch = 0; ch < n_chunks; ++ch, ++item) {
         const uint32_t buf = item & 1, tph = (item >> 1) & 1;
         mbar_wait(&tfull_bar[buf], tph);
         tcgen05_fence_after();
-        const bool store_only = first_store && ch == 0;
-#pragma unroll 1
-        for (int c0 = 0; c0 < kBN; c0 += 32) {
+        const uint32_t taddr = tmem_base + ((uint32_t)(quarter * 32) << 16) + buf * kBN + chalf * 128;
+#pragma unroll
+        for (int c0 = 0; c0 < 128; c0 += 32) {
           uint32_t r[32];
-          tmem_ld_32x32b_x32(tmem_base + ((uint32_t)(quarter * 32) << 16) + buf * kBN + c0, r);
+          tmem_ld_32x32b_x32(taddr + c0, r);
           tmem_ld_wait();
-          if (c0 + 32 == kBN) {  // all TMEM reads of this accumulator are done: hand it back to the MMA warp
-            tcgen05_fence_before();
-            __syncwarp();
-            if (lane == 0) mbar_arrive(&tempty_bar[buf]);
-          }
-          if (col < D) {
-            float* dst = C + (size_t)(J0 + c0) * D + col;
-            float old[32];
-            if (!store_only) {
 #pragma unroll
-              for (int jj = 0; jj < 32; ++jj) old[jj] = (J0 + c0 + jj < D) ? dst[(size_t)jj * D] : 0.f;
-            } else {
-#pragma unroll
-              for (int jj = 0; jj < 32; ++jj) old[jj] = 0.f;
-            }
-#pragma unroll
-            for (int jj = 0; jj < 32; ++jj)
-              if (J0 + c0 + jj < D) dst[(size_t)jj * D] = old[jj] + __uint_as_float(r[jj]);
-          }
+          for (int jj = 0; jj < 32; ++jj) acc[c0 + jj] += __uint_as_float(r[jj]);
         }
+        tcgen05_fence_before();  // all TMEM reads of this warp are done: hand the accumulator back
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&tempty_bar[buf]);
+      }
+      if (col < D) {
+        float* dst = C + (size_t)J0 * D + col;
+        if (!first_store) {
+#pragma unroll
+          for (int j = 0; j < 128; ++j)
+            if (J0 + j < D) acc[j] += __ldcg(dst + (size_t)j * D);
+        }
+#pragma unroll
+        for (int j = 0; j < 128; ++j)
+          if (J0 + j < D) __stcg(dst + (size_t)j * D, acc[j]);
       }
     }
   }
@@ -452,7 +468,7 @@ int syrk_normal_equations(const float* A, const float* y, int64_t rows, int32_t 
       QMLL_CUDA_TRY(cudaEventRecord(g_timed[g_n_timed].a, st));
     }
     syrk_tcgen05_kernel<<<grid, kSyrkThreads, kSmemBytes, st>>>(map_hi, map_lo, ZtZ, D, (int)(rp / kBK), n_tiles,
-                                                              first_store);
+                                                              first_store, chunk_rows() / kBK);
     QMLL_LAUNCH_CHECK("syrk_tcgen05_kernel");
     if (timed) {
       QMLL_CUDA_TRY(cudaEventRecord(g_timed[g_n_timed].b, st));
