@@ -122,27 +122,41 @@ sorf_forward_kernel(const float* __restrict__ x, const int32_t* __restrict__ ele
 //   transposed chain;  reduce-scatter over the SPW stack lanes (shuffles), accumulate over stack groups.
 // energy_acc[mol] (double, pre-zeroed) receives one atomicAdd per (task, molecule).
 // ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ float select_f32(bool c, float a, float b) {
+  float r;
+  asm("{\n.reg .pred p;\nsetp.ne.u32 p, %3, 0;\nselp.f32 %0, %1, %2, p;\n}" : "=f"(r) : "f"(a), "f"(b), "r"((unsigned)c));
+  return r;
+}
+
 template <typename S>
 struct StackReduce {
   static constexpr bool kScatter = (S::E >= S::SPW);
   static constexpr int R = kScatter ? S::E / S::SPW : S::E;  // values a lane ends up owning
+  static constexpr int kLogSPW = S::SPW == 32 ? 5 : S::SPW == 16 ? 4 : S::SPW == 8 ? 3 : 2;
+  // One halving step: lanes whose bit `mask` is clear keep the lower half of the live elements and receive the
+  // partner's lower half; the others keep / receive the upper half.  K is a template parameter so that every
+  // register index is a compile-time constant (a runtime `half` sends v[] to local memory).
+  template <int K>
+  __device__ static __forceinline__ void step(float (&v)[S::E], int lane, int& jbase) {
+    if constexpr (K < kLogSPW) {
+      constexpr int mask = S::P << K;
+      constexpr int half = S::E >> (K + 1);
+      const bool up = (lane & mask) != 0;
+#pragma unroll
+      for (int i = 0; i < half; ++i) {
+        const float send = select_f32(up, v[i], v[i + half]);
+        const float keep = select_f32(up, v[i + half], v[i]);
+        v[i] = keep + __shfl_xor_sync(0xffffffffu, send, mask);
+      }
+      if (up) jbase += half;
+      step<K + 1>(v, lane, jbase);
+    }
+  }
   // Sums v over the SPW stack lanes that share p.  Scatter form: lane keeps elements [jbase, jbase + R).
   __device__ static __forceinline__ void run(float (&v)[S::E], int lane, int& jbase) {
     jbase = 0;
     if constexpr (kScatter) {
-#pragma unroll
-      for (int k = 0; (1 << k) < S::SPW; ++k) {
-        const int mask = S::P << k;
-        const int half = S::E >> (k + 1);
-        const bool up = (lane & mask) != 0;
-#pragma unroll
-        for (int i = 0; i < half; ++i) {
-          const float send = up ? v[i] : v[i + half];
-          const float keep = up ? v[i + half] : v[i];
-          v[i] = keep + __shfl_xor_sync(0xffffffffu, send, mask);
-        }
-        if (up) jbase += half;
-      }
+      step<0>(v, lane, jbase);
     } else {
 #pragma unroll
       for (int mask = S::P; mask < kWarp; mask <<= 1) {
