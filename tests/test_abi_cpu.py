@@ -1,0 +1,81 @@
+"""CPU-only checks of the boundary: the C-ABI library builds for sm_100a, loads, and exports every symbol that
+include/qmll.h declares; host-side argument checks and workspace arithmetic work without a GPU (no compute)."""
+import ctypes
+import os
+import re
+
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def lib():
+    from paper_2206_01580_b200 import build as qbuild
+    qbuild.build()
+    import paper_2206_01580_b200 as pkg
+    return pkg, pkg.load_library()
+
+
+def declared_symbols():
+    text = open(os.path.join(ROOT, "include", "qmll.h")).read()
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    return sorted(set(re.findall(r"\b(qmll_[a-z_0-9]+)\s*\(", text)))
+
+
+def test_header_symbols_are_exported(lib):
+    pkg, l = lib
+    names = declared_symbols()
+    assert {"qmll_sorf_forward", "qmll_sorf_backward_forces", "qmll_normal_equations", "qmll_predict"} <= set(names)
+    for n in names:
+        assert hasattr(l, n), n
+    assert set(pkg.EXPORTS) <= set(names)
+
+
+def test_status_strings(lib):
+    pkg, l = lib
+    assert l.qmll_status_string(0) == b"QMLL_OK"
+    for code in (-1, -2, -3, -4):
+        assert l.qmll_status_string(code).startswith(b"QMLL_ERR")
+
+
+def test_workspace_arithmetic(lib):
+    pkg, l = lib
+    p = pkg._CParams(128, 8192, 3, 5, 8.0, None, None)
+    fwd = l.qmll_workspace_bytes(pkg.CALL_FORWARD, ctypes.byref(p), 21000, 1000, 0)
+    fwdg = l.qmll_workspace_bytes(pkg.CALL_FORWARD_GRAD, ctypes.byref(p), 21000, 1000, 0)
+    pred = l.qmll_workspace_bytes(pkg.CALL_PREDICT, ctypes.byref(p), 21000, 1000, 0)
+    assert fwd >= 5 * 8192 * 4 + 5 * 64 * 3 * 128 // 8          # permuted bias + packed sign bits
+    assert fwdg - fwd >= 21000 * 8192 * 4                        # per-atom sin table for the force rows
+    assert pred >= fwd + 21000 * 128 * 4 + 1000 * 8
+    ne = l.qmll_workspace_bytes(pkg.CALL_NORMAL_EQUATIONS, ctypes.byref(p), 0, 0, 64000)
+    assert ne >= 2 * 8192 * 64000 * 4
+    assert 0 < l.qmll_normal_equations_min_workspace(8192) <= ne
+    bad = pkg._CParams(100, 8192, 3, 5, 8.0, None, None)          # d not a power of two
+    assert l.qmll_workspace_bytes(pkg.CALL_FORWARD, ctypes.byref(bad), 10, 1, 0) == 0
+
+
+def test_host_side_argument_checks_need_no_gpu(lib):
+    pkg, l = lib
+    # null parameter struct / invalid sizes are rejected before any CUDA call
+    assert l.qmll_sorf_forward(None, None, None, None, 0, 0, None, None, None, None, 0, None) == -1
+    assert l.qmll_normal_equations(None, None, -1, 256, 0, None, None, None, 0, None) == -1
+    assert l.qmll_predict(None, None, None, None, 0, 0, None, None, None, None, None, 0, None) == -1
+    assert l.qmll_sorf_backward_forces(None, None, None, None, 0, 0, None, None, None, None, 0, None) == -1
+
+
+def test_launch_counter(lib):
+    pkg, l = lib
+    pkg.reset_launch_count()
+    assert pkg.launch_count() == 0
+
+
+def test_product_never_imports_oracle():
+    pkgdir = os.path.join(ROOT, "paper_2206_01580_b200")
+    for dirpath, _, files in os.walk(pkgdir):
+        for f in files:
+            if f.endswith((".py", ".cu", ".cuh", ".h")):
+                text = open(os.path.join(dirpath, f)).read()
+                assert "import oracle" not in text and "from oracle" not in text and "sorf_oracle" not in text, f
+    otext = open(os.path.join(ROOT, "oracle", "__init__.py")).read() + open(os.path.join(ROOT, "oracle", "sorf_oracle.c")).read()
+    assert "import paper_2206_01580_b200" not in otext and "qmll.h" not in otext
