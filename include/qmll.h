@@ -66,6 +66,8 @@ typedef struct {
   const float* nbr_val;     /* NEIGHBOR: device [n_atoms, K, d, 3] = d x_I[m] / d r_{j,k}, j = nbr_idx[I, q];  */
                             /*        self and duplicate j are legal and ACCUMULATE                            */
   int32_t K;                /* NEIGHBOR: neighbours per atom                                                    */
+  int64_t dense_floats;     /* DENSE: total number of floats in `dense` (= dense_off[n_mol]); the host needs it to */
+                            /*        size the workspace copy made by qmll_sorf_forward (columns made contiguous)  */
 } qmll_grad;
 
 /* Steps a1-a3 (+a7): Z[M, l] = sum_{I in M} sqrt(2/D) cos((W_{e_I} x_I)[l] + b[e_I, l])
@@ -116,6 +118,7 @@ enum {
 };
 
 /* Scratch bytes the named call needs for these sizes (host-side arithmetic only, no CUDA call).
+ * For QMLL_CALL_FORWARD_GRAD with a dense gradient pass rows = grad->dense_floats (0 for a neighbour gradient).
  * For QMLL_CALL_NORMAL_EQUATIONS this is the size that lets all `rows` be staged in one panel; the call
  * also runs (in several panels) with any workspace of at least qmll_normal_equations_min_workspace(D). */
 size_t qmll_workspace_bytes(int which_call, const qmll_sorf_params* p, int64_t n_atoms, int32_t n_mol,

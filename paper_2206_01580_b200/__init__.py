@@ -37,7 +37,8 @@ class _CParams(ctypes.Structure):
 
 class _CGrad(ctypes.Structure):
     _fields_ = [("layout", ctypes.c_int32), ("dense", ctypes.c_void_p), ("dense_off", ctypes.c_void_p),
-                ("nbr_idx", ctypes.c_void_p), ("nbr_val", ctypes.c_void_p), ("K", ctypes.c_int32)]
+                ("nbr_idx", ctypes.c_void_p), ("nbr_val", ctypes.c_void_p), ("K", ctypes.c_int32),
+                ("dense_floats", ctypes.c_int64)]
 
 
 class QmllError(RuntimeError):
@@ -137,7 +138,8 @@ class Grad:
     def c(self) -> _CGrad:
         return _CGrad(self.layout, _dev(self.dense, torch.float32, "dense"),
                       _dev(self.dense_off, torch.int64, "dense_off"), _dev(self.nbr_idx, torch.int32, "nbr_idx"),
-                      _dev(self.nbr_val, torch.float32, "nbr_val"), int(self.K))
+                      _dev(self.nbr_val, torch.float32, "nbr_val"), int(self.K),
+                      int(self.dense.numel()) if self.dense is not None else 0)
 
 
 _workspaces: dict = {}
@@ -181,8 +183,9 @@ def qmll_sorf_forward(p: SorfParams, x, elem, mol_off, grad: Optional[Grad] = No
         G = torch.empty((3 * n_atoms, p.D), dtype=torch.float32, device=x.device)
     cp = p.c()
     cg = grad.c() if grad is not None else None
+    dense_floats = int(grad.dense.numel()) if (grad is not None and grad.dense is not None) else 0
     nb = lib.qmll_workspace_bytes(CALL_FORWARD_GRAD if grad is not None else CALL_FORWARD, ctypes.byref(cp),
-                                  n_atoms, n_mol, 0)
+                                  n_atoms, n_mol, dense_floats)
     ws = workspace(nb, x.device)
     _check(lib.qmll_sorf_forward(ctypes.byref(cp), xp, ep, mp, n_atoms, n_mol,
                                  ctypes.byref(cg) if cg is not None else None, _dev(Z, torch.float32, "Z"),

@@ -37,7 +37,8 @@ static int check_problem(const float* x, const int32_t* elem, const int32_t* mol
 
 static int check_grad(const qmll_grad* g) {
   if (!g) return QMLL_ERR_INVALID_ARG;
-  if (g->layout == QMLL_GRAD_DENSE) return (g->dense && g->dense_off) ? QMLL_OK : QMLL_ERR_INVALID_ARG;
+  if (g->layout == QMLL_GRAD_DENSE)
+    return (g->dense && g->dense_off && g->dense_floats >= 0) ? QMLL_OK : QMLL_ERR_INVALID_ARG;
   if (g->layout == QMLL_GRAD_NEIGHBOR) {
     if (g->K < 0) return QMLL_ERR_INVALID_ARG;
     return (g->K == 0 || (g->nbr_idx && g->nbr_val)) ? QMLL_OK : QMLL_ERR_INVALID_ARG;
@@ -124,7 +125,8 @@ size_t qmll_workspace_bytes(int which_call, const qmll_sorf_params* p, int64_t n
   if (n_mol < 0) n_mol = 0;
   switch (which_call) {
     case QMLL_CALL_FORWARD: return sorf_tables_bytes(p, false);
-    case QMLL_CALL_FORWARD_GRAD: return sorf_tables_bytes(p, false) + zs_bytes(p, n_atoms);
+    case QMLL_CALL_FORWARD_GRAD:
+      return sorf_tables_bytes(p, false) + zs_bytes(p, n_atoms) + align_up((size_t)(rows > 0 ? rows : 0) * 4, 256) + 256;
     case QMLL_CALL_BACKWARD_FORCES: return sorf_tables_bytes(p, true) + g_bytes(p, n_atoms);
     case QMLL_CALL_PREDICT: return sorf_tables_bytes(p, true) + g_bytes(p, n_atoms) + e_bytes(n_mol);
     default: return 0;
@@ -145,7 +147,8 @@ int qmll_sorf_forward(const qmll_sorf_params* p, const float* x, const int32_t* 
   rc = check_device();
   if (rc) return rc;
   rc = check_ws(workspace, workspace_bytes,
-                qmll_workspace_bytes(grad ? QMLL_CALL_FORWARD_GRAD : QMLL_CALL_FORWARD, p, n_atoms, n_mol, 0));
+                qmll_workspace_bytes(grad ? QMLL_CALL_FORWARD_GRAD : QMLL_CALL_FORWARD, p, n_atoms, n_mol,
+                                     (grad && grad->layout == QMLL_GRAD_DENSE) ? grad->dense_floats : 0));
   if (rc) return rc;
   Carver ws(workspace, workspace_bytes);
   SorfTables t;
@@ -157,8 +160,13 @@ int qmll_sorf_forward(const qmll_sorf_params* p, const float* x, const int32_t* 
   rc = sorf_launch_forward(pr, t, Z, zs, st);
   if (rc) return rc;
   if (grad) {
-    if (grad->layout == QMLL_GRAD_DENSE)
-      rc = sorf_launch_force_rows_dense(pr, t, zs, grad->dense, grad->dense_off, G, st);
+    if (grad->layout == QMLL_GRAD_DENSE) {
+      float* gt = ws.take<float>((size_t)grad->dense_floats);
+      if (!ws.fits()) return QMLL_ERR_WORKSPACE;
+      rc = sorf_transpose_dense(pr, grad->dense, grad->dense_off, gt, st);
+      if (rc) return rc;
+      rc = sorf_launch_force_rows_dense(pr, t, zs, gt, grad->dense_off, G, st);
+    }
     else
       rc = sorf_launch_force_rows_neighbor(pr, t, zs, grad->nbr_idx, grad->nbr_val, grad->K, G, st);
   }

@@ -79,6 +79,8 @@ int sorf_launch_force_rows_dense(const SorfProblem& pr, const SorfTables& t, con
 int sorf_launch_force_rows_neighbor(const SorfProblem& pr, const SorfTables& t, const float* zs,
                                     const int32_t* nbr_idx, const float* nbr_val, int K, float* G,
                                     cudaStream_t st);
+int sorf_transpose_dense(const SorfProblem& pr, const float* dense, const int64_t* dense_off, float* gt,
+                         cudaStream_t st);
 int sorf_finish_energies(const double* energy_acc, float* energies, int32_t n_mol, cudaStream_t st);
 bool sorf_supported_d(int d);
 

@@ -54,6 +54,43 @@ __global__ void finish_energies_kernel(const double* __restrict__ acc, float* __
   if (i < n) out[i] = (float)acc[i];
 }
 
+// Dense gradient [n, d, n, 3] = (I, m, j, k)  ->  [n, n, 3, d] = (I, j, k, m) per molecule: every gradient column
+// becomes d contiguous floats (what the force-row kernel stages with one bulk copy).  Block = one atom I: a
+// [d, 3n] -> [3n, d] transposition through 32 x 96 shared-memory tiles, coalesced on both sides.
+__global__ void __launch_bounds__(256)
+transpose_dense_kernel(const float* __restrict__ dense, const int64_t* __restrict__ dense_off,
+                       const int32_t* __restrict__ mol_off, int n_mol, int d, float* __restrict__ gt) {
+  __shared__ float tile[32][97];
+  const int Ig = blockIdx.x;
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const int M = owner_molecule(mol_off, n_mol, Ig);
+  const int a0 = __ldg(mol_off + M), n = __ldg(mol_off + M + 1) - a0;
+  const int ncol = 3 * n;
+  const size_t base = (size_t)__ldg(dense_off + M) + (size_t)(Ig - a0) * d * ncol;
+  const float* src = dense + base;  // [d][ncol]
+  float* dst = gt + base;           // [ncol][d]
+  for (int c0 = 0; c0 < ncol; c0 += 96) {
+    const int nc = ncol - c0 < 96 ? ncol - c0 : 96;
+    for (int m0 = 0; m0 < d; m0 += 32) {
+      const int nm = d - m0 < 32 ? d - m0 : 32;
+      __syncthreads();
+      for (int rr = warp; rr < nm; rr += 8)
+        for (int cc = lane; cc < nc; cc += 32) tile[rr][cc] = __ldcs(src + (size_t)(m0 + rr) * ncol + c0 + cc);
+      __syncthreads();
+      for (int cc = warp; cc < nc; cc += 8)
+        if (lane < nm) dst[(size_t)(c0 + cc) * d + m0 + lane] = tile[lane][cc];
+    }
+  }
+}
+
+int sorf_transpose_dense(const SorfProblem& pr, const float* dense, const int64_t* dense_off, float* gt,
+                         cudaStream_t st) {
+  if (pr.n_atoms == 0) return QMLL_OK;
+  transpose_dense_kernel<<<(unsigned)pr.n_atoms, 256, 0, st>>>(dense, dense_off, pr.mol_off, pr.n_mol, pr.p->d, gt);
+  QMLL_LAUNCH_CHECK("transpose_dense_kernel");
+  return QMLL_OK;
+}
+
 int device_sm_count() {
   static int cached = 0;
   if (cached == 0) {

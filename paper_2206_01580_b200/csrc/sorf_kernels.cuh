@@ -9,6 +9,7 @@
 
 #include "qmll_common.cuh"
 #include "sorf_device.cuh"
+#include "ptx_utils.cuh"
 
 namespace qmll {
 
@@ -259,15 +260,30 @@ sorf_backward_kernel(const float* __restrict__ x, const int32_t* __restrict__ el
 // I in the shared-memory accumulators; the finished [SPW, d] slab of G row r is then written once.
 //   G[r, l] = c * sum_I zs_I[l] * (H S_T ... H S_1 dx_I[:, j, k])[l]
 // ------------------------------------------------------------------------------------------------
+// `gt` is the gradient with each column made contiguous ([n, n, 3, d] = (I, j, k, m) per molecule, written by
+// transpose_dense_kernel); the column of the next atom is staged in shared memory by a 1-D TMA bulk copy while
+// the current one runs through the chain (2-deep ring per warp, one mbarrier per slot).
+template <typename S>
+struct ColStage {
+  static constexpr int kSlice = S::E + 4;                 // floats per lane slice (+16 B: no bank conflicts for P > 1)
+  static constexpr int kBufFloats = S::P * kSlice;        // one staged column
+  static constexpr size_t kBytes = (size_t)(kFwdThreads / kWarp) * 2 * (kBufFloats * sizeof(float) + sizeof(uint64_t));
+};
+
 template <typename S>
 __global__ void __launch_bounds__(kFwdThreads, (S::E >= 128 ? 3 : 4))
 sorf_force_rows_dense_kernel(const int32_t* __restrict__ elem, const int32_t* __restrict__ mol_off, int n_atoms,
                              int n_mol, int n_s, int T, float c, const uint32_t* __restrict__ sign_bits,
-                             const float* __restrict__ zs, const float* __restrict__ dense,
+                             const float* __restrict__ zs, const float* __restrict__ gt,
                              const int64_t* __restrict__ dense_off, float* __restrict__ G, int n_sg) {
   extern __shared__ float4 acc[];
+  using CS = ColStage<S>;
+  constexpr int kWarps = kFwdThreads / kWarp;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  const long long task = (long long)blockIdx.x * (kFwdThreads / kWarp) + warp;
+  float* colbuf = reinterpret_cast<float*>(acc + S::E4 * kFwdThreads) + warp * 2 * CS::kBufFloats;
+  uint64_t* bars = reinterpret_cast<uint64_t*>(reinterpret_cast<float*>(acc + S::E4 * kFwdThreads) +
+                                               kWarps * 2 * CS::kBufFloats) + warp * 2;
+  const long long task = (long long)blockIdx.x * kWarps + warp;
   if (task >= 3LL * n_atoms * n_sg) return;
   const int sg = (int)(task % n_sg);
   const long long r = task / n_sg;
@@ -280,18 +296,43 @@ sorf_force_rows_dense_kernel(const int32_t* __restrict__ elem, const int32_t* __
   const int M = owner_molecule(mol_off, n_mol, jg);
   const int a0 = __ldg(mol_off + M), n = __ldg(mol_off + M + 1) - a0;
   const int jl = jg - a0;
-  const float* dxM = dense + __ldg(dense_off + M);
-  const size_t cstride = (size_t)3 * n;  // floats between consecutive m of one column
+  // column (I, jl, k) of molecule M: d contiguous floats; consecutive I are 3*n*d floats apart
+  const float* col0 = gt + __ldg(dense_off + M) + ((size_t)jl * 3 + k) * S::d;
+  const size_t istride = (size_t)3 * n * S::d;
+
+  if (lane == 0) {
+    mbar_init(&bars[0], 1);
+    mbar_init(&bars[1], 1);
+    fence_mbarrier_init();
+  }
+  __syncwarp();
+  auto stage = [&](int I) {  // lane 0 only
+    uint64_t* bar = &bars[I & 1];
+    float* dst = colbuf + (I & 1) * CS::kBufFloats;
+    mbar_expect_tx(bar, S::d * sizeof(float));
+#pragma unroll
+    for (int pp = 0; pp < S::P; ++pp)
+      bulk_copy_g2s(dst + pp * CS::kSlice, col0 + (size_t)I * istride + pp * S::E, S::E * sizeof(float), bar);
+  };
+  if (lane == 0) stage(0);
 
   zero_acc<S>(acc, tid);
   const float4* zs4 = reinterpret_cast<const float4*>(zs);
 #pragma unroll 1
   for (int I = 0; I < n; ++I) {
+    if (lane == 0 && I + 1 < n) stage(I + 1);  // slot (I+1)&1 was last read in iteration I-1 (warp-synced below)
     const int e = __ldg(elem + a0 + I);
-    const float* col = dxM + ((size_t)I * S::d + p * S::E) * cstride + (size_t)jl * 3 + k;
+    mbar_wait(&bars[I & 1], (uint32_t)((I >> 1) & 1));
     float v[S::E];
+    {
+      const float4* src = reinterpret_cast<const float4*>(colbuf + (I & 1) * CS::kBufFloats + p * CS::kSlice);
 #pragma unroll
-    for (int j = 0; j < S::E; ++j) v[j] = __ldg(col + (size_t)j * cstride);
+      for (int q = 0; q < S::E4; ++q) {
+        const float4 t = src[q];
+        v[4 * q + 0] = t.x; v[4 * q + 1] = t.y; v[4 * q + 2] = t.z; v[4 * q + 3] = t.w;
+      }
+    }
+    __syncwarp();
     chain_forward<S>(v, sign_bits, e, T, n_gl, gl, p);
     const float4* z4 = zs4 + (size_t)(a0 + I) * S::E4 * n_gl + gl;
 #pragma unroll
@@ -414,8 +455,9 @@ struct SorfLaunch {
     const long long grid = (tasks + kWarpsPerBlock - 1) / kWarpsPerBlock;
     if (grid > 0x7fffffffLL) return QMLL_ERR_UNSUPPORTED;
     auto kern = sorf_force_rows_dense_kernel<S>;
-    QMLL_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kAccBytes));
-    kern<<<(unsigned)grid, kFwdThreads, kAccBytes, st>>>(pr.elem, pr.mol_off, n_atoms, pr.n_mol, n_s,
+    const size_t smem = kAccBytes + ColStage<S>::kBytes;
+    QMLL_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    kern<<<(unsigned)grid, kFwdThreads, smem, st>>>(pr.elem, pr.mol_off, n_atoms, pr.n_mol, n_s,
                                                          p->n_transform, c_of(p), t.sign_bits, zs, dense,
                                                          dense_off, G, n_sg);
     QMLL_LAUNCH_CHECK("sorf_force_rows_dense_kernel");
