@@ -1,6 +1,5 @@
-// sorf_d128.cu -- instantiates the fused SORF kernels for descriptor length 128 (E = 128 elements per lane,
-// P = 1 lanes per vector); see sorf_kernels.cuh.
+// sorf_d128.cu -- instantiates the fused SORF kernels for descriptor length 128; see sorf_kernels.cuh.
 #include "sorf_kernels.cuh"
 namespace qmll {
-QMLL_DEFINE_SORF_SHAPE(d128, 128, 1)
+QMLL_DEFINE_SORF_SHAPE_D(d128, 128)
 }

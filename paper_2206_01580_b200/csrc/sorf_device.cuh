@@ -16,6 +16,14 @@ namespace qmll {
 
 constexpr int kWarp = 32;
 
+// Elements per lane: the whole vector for d <= QMLL_MAX_E, else QMLL_MAX_E with P = d / QMLL_MAX_E lanes per vector.
+#ifndef QMLL_MAX_E
+#define QMLL_MAX_E 128
+#endif
+constexpr int shape_E(int d) { return d < QMLL_MAX_E ? d : QMLL_MAX_E; }
+constexpr int shape_P(int d) { return d / shape_E(d); }
+constexpr int ilog2(int v) { return v <= 1 ? 0 : 1 + ilog2(v >> 1); }
+
 template <int E_, int P_>
 struct Shape {
   static constexpr int E = E_;             // elements per lane
@@ -25,7 +33,7 @@ struct Shape {
   static constexpr int EW = (E_ + 31) / 32;  // 32-bit sign words per lane and transform
   static constexpr int E4 = E_ / 4;        // float4 groups per lane
   static_assert(E_ >= 16 && E_ <= 128 && (E_ & (E_ - 1)) == 0, "E");
-  static_assert(P_ >= 1 && P_ <= 8 && (P_ & (P_ - 1)) == 0, "P");
+  static_assert(P_ >= 1 && P_ <= 16 && (P_ & (P_ - 1)) == 0, "P");
 };
 
 // v <- H_d v (unnormalised, natural order): any order of the butterfly stages gives the same matrix.

@@ -107,8 +107,8 @@ int device_sm_count() {
 bool sorf_supported_d(int d) { return d >= 16 && d <= 1024 && (d & (d - 1)) == 0; }
 
 static void shape_of(int d, int* E, int* P) {
-  *E = d < 128 ? d : 128;
-  *P = d / *E;
+  *E = shape_E(d);
+  *P = shape_P(d);
 }
 
 size_t sorf_tables_bytes(const qmll_sorf_params* p, bool with_alpha) {

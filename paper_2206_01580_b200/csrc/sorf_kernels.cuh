@@ -133,7 +133,7 @@ template <typename S>
 struct StackReduce {
   static constexpr bool kScatter = (S::E >= S::SPW);
   static constexpr int R = kScatter ? S::E / S::SPW : S::E;  // values a lane ends up owning
-  static constexpr int kLogSPW = S::SPW == 32 ? 5 : S::SPW == 16 ? 4 : S::SPW == 8 ? 3 : 2;
+  static constexpr int kLogSPW = ilog2(S::SPW);
   // One halving step: lanes whose bit `mask` is clear keep the lower half of the live elements and receive the
   // partner's lower half; the others keep / receive the upper half.  K is a template parameter so that every
   // register index is a compile-time constant (a runtime `half` sends v[] to local memory).
@@ -491,6 +491,7 @@ struct SorfLaunch {
   int sorf_force_rows_neighbor_##TAG(const SorfProblem&, const SorfTables&, const float*, const int32_t*,      \
                                      const float*, int, float*, cudaStream_t);
 
+#define QMLL_DEFINE_SORF_SHAPE_D(TAG, D_) QMLL_DEFINE_SORF_SHAPE(TAG, shape_E(D_), shape_P(D_))
 #define QMLL_DEFINE_SORF_SHAPE(TAG, E_, P_)                                                                   \
   int sorf_forward_##TAG(const SorfProblem& pr, const SorfTables& t, float* Z, float* zs, cudaStream_t st) {   \
     return SorfLaunch<Shape<E_, P_>>::forward(pr, t, Z, zs, st);                                               \
