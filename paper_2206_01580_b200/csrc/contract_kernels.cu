@@ -34,9 +34,23 @@ contract_dense_kernel(const float* __restrict__ g, const int32_t* __restrict__ m
     float acc = 0.f;
     if (rl < RL) {
       const float* ptr = dx + (size_t)col;
-#pragma unroll 8
-      for (long long r = r0 + rl; r < r1; r += RL) acc = fmaf(__ldg(gM + r), __ldg(ptr + (size_t)r * ncol), acc);
-      atomicAdd(&sacc[col], acc);
+      long long r = r0 + rl;
+      float acc2 = 0.f;
+      // 8 independent streaming loads in flight per thread (the loop is HBM-latency bound otherwise)
+      for (; r + 7LL * RL < r1; r += 8LL * RL) {
+        float a[8], gv[8];
+#pragma unroll
+        for (int u = 0; u < 8; ++u) a[u] = __ldcs(ptr + (size_t)(r + (long long)u * RL) * ncol);
+#pragma unroll
+        for (int u = 0; u < 8; ++u) gv[u] = __ldg(gM + r + (long long)u * RL);
+#pragma unroll
+        for (int u = 0; u < 8; u += 2) {
+          acc = fmaf(gv[u], a[u], acc);
+          acc2 = fmaf(gv[u + 1], a[u + 1], acc2);
+        }
+      }
+      for (; r < r1; r += RL) acc = fmaf(__ldg(gM + r), __ldcs(ptr + (size_t)r * ncol), acc);
+      atomicAdd(&sacc[col], acc + acc2);
     }
     __syncthreads();
     if (t < ncol) atomicAdd(forces + (size_t)a0 * 3 + t, -sacc[t]);
@@ -96,7 +110,7 @@ int contract_dense(const float* g, const int32_t* mol_off, int32_t n_mol, int64_
   QMLL_CUDA_TRY(cudaMemsetAsync(forces, 0, (size_t)n_atoms * 3 * sizeof(float), st));
   if (n_mol == 0 || n_atoms == 0) return QMLL_OK;
   // enough blocks for ~8 per SM even with few molecules; rows of a molecule are split across blockIdx.y
-  const int want = device_sm_count() * 8;
+  const int want = device_sm_count() * 32;
   int splits = (want + n_mol - 1) / n_mol;
   if (splits < 1) splits = 1;
   if (splits > 64) splits = 64;

@@ -175,7 +175,7 @@ __device__ __forceinline__ float warp_sum(float v) {
 }
 
 template <typename S>
-__global__ void __launch_bounds__(kFwdThreads, (S::E >= 128 ? 3 : 4))
+__global__ void __launch_bounds__(kFwdThreads, (S::E >= 128 ? 2 : 4))
 sorf_backward_kernel(const float* __restrict__ x, const int32_t* __restrict__ elem,
                      const int32_t* __restrict__ mol_off, int n_atoms, int n_mol, int n_s, int T, float c_rev,
                      float c, const uint32_t* __restrict__ sign_bits, const float* __restrict__ bias_rev,

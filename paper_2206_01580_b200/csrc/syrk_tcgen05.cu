@@ -4,8 +4,8 @@
 // row dimension into chunks whose partial products are summed in fp32 round-to-nearest).
 //
 // Pipeline of one call (per panel of rows that fits the workspace):
-//   1. split_transpose_kernel: A[rows, D] -> At_hi, At_lo [D, R_pad] (K-major for the MMA: the contraction
-//      index `row` becomes the contiguous one), hi = tf32(a), lo = tf32(a - hi); Zty += A^T y rides along.
+//   1. split_transpose_kernel: A[rows, D] -> At_hi, At_lo [R_pad/32][D][32] (K-major for the MMA: the contraction
+//      index `row` is the contiguous one inside each 32-row block; one TMA box is 16 KB contiguous), hi = tf32(a), lo = tf32(a - hi); Zty += A^T y rides along.
 //   2. syrk_tcgen05_kernel: persistent, warp-specialised.  One CTA owns a 128 x 256 tile T = At[I,:] At[J,:]^T
 //      for ALL rows: TMA (SWIZZLE_128B) -> 2-stage smem ring -> tcgen05.mma kind::tf32 (hi*hi + hi*lo +
 //      lo*hi) into one of two 256-column TMEM accumulators; every 1024 rows the accumulator is drained by
@@ -138,11 +138,12 @@ split_transpose_kernel(const float* __restrict__ A, const float* __restrict__ y,
   for (int cc = 0; cc < 4; ++cc) {
     const int c = warp * 4 + cc;
     if (i0 + c < D) {
-      const size_t o = (size_t)(i0 + c) * R_pad + r0;
-      At_hi[o + lane] = thi[lane][c];
-      At_hi[o + lane + 32] = thi[lane + 32][c];
-      At_lo[o + lane] = tlo[lane][c];
-      At_lo[o + lane + 32] = tlo[lane + 32][c];
+      // k-block-major layout [R_pad/32][D][32]: the 128 features x 32 rows of one TMA box are 16 KB contiguous
+      const size_t o0 = ((size_t)(r0 / 32) * D + (i0 + c)) * 32, o1 = o0 + (size_t)D * 32;
+      At_hi[o0 + lane] = thi[lane][c];
+      At_hi[o1 + lane] = thi[lane + 32][c];
+      At_lo[o0 + lane] = tlo[lane][c];
+      At_lo[o1 + lane] = tlo[lane + 32][c];
     }
   }
   if (Zty != nullptr && y != nullptr && warp == 0 && i < D) {
@@ -208,13 +209,15 @@ syrk_tcgen05_kernel(const __grid_constant__ CUtensorMap map_hi, const __grid_con
           mbar_wait(&empty_bar[s], ph ^ 1);
           uint8_t* st = smem + s * kStageBytes;
           mbar_expect_tx(&full_bar[s], kStageBytes);
-          const int r = kb * kBK;
-          tma_load_2d(st, &map_hi, &full_bar[s], r, I0);
-          tma_load_2d(st + kTileABytes, &map_lo, &full_bar[s], r, I0);
-          tma_load_2d(st + 2 * kTileABytes, &map_hi, &full_bar[s], r, J0);
-          tma_load_2d(st + 2 * kTileABytes + kTileABytes, &map_hi, &full_bar[s], r, J0 + 128);
-          tma_load_2d(st + 2 * kTileABytes + kTileBBytes, &map_lo, &full_bar[s], r, J0);
-          tma_load_2d(st + 2 * kTileABytes + kTileBBytes + kTileABytes, &map_lo, &full_bar[s], r, J0 + 128);
+          // tensor = [n_kb * D][32]: box row index = kb * D + feature.  Features past D alias the next k-block
+          // (finite values; those accumulator rows / columns are masked at the store), past the end TMA fills zeros.
+          const int base = kb * D;
+          tma_load_2d(st, &map_hi, &full_bar[s], 0, base + I0);
+          tma_load_2d(st + kTileABytes, &map_lo, &full_bar[s], 0, base + I0);
+          tma_load_2d(st + 2 * kTileABytes, &map_hi, &full_bar[s], 0, base + J0);
+          tma_load_2d(st + 2 * kTileABytes + kTileABytes, &map_hi, &full_bar[s], 0, base + J0 + 128);
+          tma_load_2d(st + 2 * kTileABytes + kTileBBytes, &map_lo, &full_bar[s], 0, base + J0);
+          tma_load_2d(st + 2 * kTileABytes + kTileBBytes + kTileABytes, &map_lo, &full_bar[s], 0, base + J0 + 128);
         }
       }
     }
@@ -355,8 +358,8 @@ static EncodeTiledFn get_encode_fn() {
 static int make_map(CUtensorMap* map, float* base, int D, long long R_pad) {
   EncodeTiledFn fn = get_encode_fn();
   if (!fn) return QMLL_ERR_CUDA;
-  cuuint64_t dims[2] = {(cuuint64_t)R_pad, (cuuint64_t)D};
-  cuuint64_t strides[1] = {(cuuint64_t)R_pad * sizeof(float)};
+  cuuint64_t dims[2] = {(cuuint64_t)kBK, (cuuint64_t)D * (cuuint64_t)(R_pad / kBK)};
+  cuuint64_t strides[1] = {(cuuint64_t)kBK * sizeof(float)};
   cuuint32_t box[2] = {(cuuint32_t)kBK, 128u};
   cuuint32_t estr[2] = {1u, 1u};
   CUresult r = fn(map, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, base, dims, strides, box, estr,
