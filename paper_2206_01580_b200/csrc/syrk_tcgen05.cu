@@ -161,6 +161,30 @@ split_transpose_kernel(const float* __restrict__ A, const float* __restrict__ y,
 // it is needed iff 128 ti <= 256 tj + 255, i.e. ti <= 2 tj + 1.
 __host__ __device__ inline int tiles_in_row(int tj, int n_ti) { return (2 * tj + 2 < n_ti) ? 2 * tj + 2 : n_ti; }
 
+// Tile order.  The ~148 tiles in flight should touch as few distinct operand rows of A^T as possible (they are
+// re-read from L2, and from DRAM once per wave): tile rows are grouped in bands of kBandRows, and inside a band the
+// tiles run column by column, so a wave covers a roughly square patch (about 8 J-blocks x 18 I-blocks) instead of
+// two or three full-width rows.
+constexpr int kBandRows = 8;
+__host__ __device__ inline void tile_decode(int tile, int n_ti, int n_tj, int* tj_out, int* ti_out) {
+  int r0 = 0, r1 = 0;
+  for (r0 = 0; r0 < n_tj; r0 += kBandRows) {
+    r1 = r0 + kBandRows < n_tj ? r0 + kBandRows : n_tj;
+    int cnt = 0;
+    for (int tj = r0; tj < r1; ++tj) cnt += tiles_in_row(tj, n_ti);
+    if (tile < cnt) break;
+    tile -= cnt;
+  }
+  for (int ti = 0; ti < n_ti; ++ti) {
+    const int lo = (ti / 2 > r0) ? ti / 2 : r0;  // first tile row of the band that needs column ti
+    const int cnt = r1 - lo;
+    if (cnt <= 0) continue;
+    if (tile < cnt) { *tj_out = lo + tile; *ti_out = ti; return; }
+    tile -= cnt;
+  }
+  *tj_out = r1 - 1; *ti_out = 0;  // not reached for tile < n_tiles
+}
+
 __global__ void __launch_bounds__(kSyrkThreads, 1)
 syrk_tcgen05_kernel(const __grid_constant__ CUtensorMap map_hi, const __grid_constant__ CUtensorMap map_lo,
                     float* __restrict__ C, int D, int n_kb /* 32-row blocks in the panel */, int n_tiles,
@@ -175,7 +199,7 @@ syrk_tcgen05_kernel(const __grid_constant__ CUtensorMap map_hi, const __grid_con
   uint32_t* tmem_ptr_smem = reinterpret_cast<uint32_t*>(bars + 2 * kStages + 4);
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const int n_ti = (D + kBM - 1) / kBM;
+  const int n_ti = (D + kBM - 1) / kBM, n_tj = (D + kBN - 1) / kBN;
   const int n_chunks = (n_kb + kb_per_chunk - 1) / kb_per_chunk;
 
   if (threadIdx.x == 0) {
@@ -201,8 +225,8 @@ syrk_tcgen05_kernel(const __grid_constant__ CUtensorMap map_hi, const __grid_con
       asm volatile("prefetch.tensormap [%0];" ::"l"(&map_lo) : "memory");
       uint32_t kbc = 0;  // running k-block counter -> stage / phase
       for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
-        int tj = 0, rem = tile;
-        while (rem >= tiles_in_row(tj, n_ti)) { rem -= tiles_in_row(tj, n_ti); ++tj; }
+        int tj, rem;
+        tile_decode(tile, n_ti, n_tj, &tj, &rem);
         const int I0 = rem * kBM, J0 = tj * kBN;
         for (int kb = 0; kb < n_kb; ++kb, ++kbc) {
           const uint32_t s = kbc % kStages, ph = (kbc / kStages) & 1;
@@ -265,8 +289,8 @@ syrk_tcgen05_kernel(const __grid_constant__ CUtensorMap map_hi, const __grid_con
     const int i_loc = quarter * 32 + lane;
     uint32_t item = 0;
     for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
-      int tj = 0, rem = tile;
-      while (rem >= tiles_in_row(tj, n_ti)) { rem -= tiles_in_row(tj, n_ti); ++tj; }
+      int tj, rem;
+      tile_decode(tile, n_ti, n_tj, &tj, &rem);
       const int I0 = rem * kBM, J0 = tj * kBN + chalf * 128;
       const int col = I0 + i_loc;  // column of C this thread writes (transposed store)
       float acc[128];
