@@ -32,6 +32,8 @@ def parse():
     ap.add_argument("--D", type=int, default=None, help="shrink the workload (debug only)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--report-configs", action="store_true",
+                    help="time every call of all five BASELINE.json configs (one JSON line per config); not the bench line")
     return ap.parse_args()
 
 
@@ -339,9 +341,80 @@ def ours_arm(args):
         dist.destroy_process_group()
 
 
+def report_configs(args):
+    """Absolute numbers and roofline fractions for all five configs (north_star), device-resident inputs."""
+    import torch
+    import paper_2206_01580_b200 as pkg
+    from paper_2206_01580_b200 import workload_io
+    from workloads import make_workload
+    pk = peaks()
+    alu_peak = 148 * 128 * 1.965e9
+
+    def tm(f, n):
+        for _ in range(2):
+            f()
+        torch.cuda.synchronize()
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record()
+        for _ in range(n):
+            f()
+        b.record()
+        torch.cuda.synchronize()
+        return a.elapsed_time(b) / n
+
+    for name, part in (("c1", "train"), ("c2", "train"), ("c3", "train"), ("c4", "train"), ("c4", "infer"), ("c5", "train")):
+        w = make_workload(name, part=part)
+        dp = workload_io.device_problem(w)
+        p, m = dp.params, w.model
+        L, T, D, na, nm = m.d.bit_length() - 1, m.T, m.D, w.n_atoms, w.n_mol
+        out = {"config": w.name, "n_mol": nm, "n_atoms": na, "d": m.d, "D": D}
+        train = w.grad is not None and w.grad.layout == "dense" and part == "train"
+        if name == "c3" or train:
+            rows = nm + (3 * na if train else 0)
+            A = torch.empty((rows, D), dtype=torch.float32, device="cuda")
+            if train:
+                t = tm(lambda: pkg.qmll_sorf_forward(p, dp.x, dp.elem, dp.mol_off, dp.grad, Z=A[:nm], G=A[nm:]), args.steps)
+                cols = 3.0 * sum(int(c) ** 2 for c in (w.mol_off[1:] - w.mol_off[:-1]))
+                ops = cols * D * (T * L + 2) + na * D * (T * L + 3)
+            else:
+                t = tm(lambda: pkg.qmll_sorf_forward(p, dp.x, dp.elem, dp.mol_off, Z=A), args.steps)
+                ops = na * D * (T * L + 3)
+            out["forward_ms"] = t
+            out["forward_alu_frac"] = ops / (t * 1e-3) / alu_peak
+            out["forward_molecules_per_s"] = nm / (t * 1e-3)
+            ZtZ = torch.empty((D, D), dtype=torch.float32, device="cuda")
+            Zty = torch.empty((D,), dtype=torch.float32, device="cuda")
+            y = dp.y if dp.y is not None and dp.y.numel() == rows else torch.zeros(rows, device="cuda")
+            pkg.time_normal_equations_kernel(True)
+            pkg.collect_normal_equations_kernel_ms()
+            t = tm(lambda: pkg.qmll_normal_equations(A, y, ZtZ=ZtZ, Zty=Zty), max(1, args.steps // 2))
+            kms, kn = pkg.collect_normal_equations_kernel_ms()
+            pkg.time_normal_equations_kernel(False)
+            out["normal_equations_ms"] = t
+            out["ztz_kernel_ms"] = kms / max(kn, 1)
+            tf = rows * D * (D + 1.0) / (kms / max(kn, 1) * 1e-3) / 1e12
+            out["ztz_tflops_fp32eq_half"] = tf
+            out["ztz_frac_of_3xtf32_sustained"] = tf / (0.5 * pk["bf16_sustained"] / 3.0)
+            del A, ZtZ
+        if name != "c3":
+            E = torch.empty((nm,), dtype=torch.float32, device="cuda")
+            F = torch.empty((na, 3), dtype=torch.float32, device="cuda")
+            t = tm(lambda: pkg.qmll_predict(p, dp.x, dp.elem, dp.mol_off, dp.alpha, dp.grad, energies=E, forces=F), args.steps)
+            gbytes = (w.grad.dense.nbytes if w.grad.layout == "dense" else w.grad.nbr_val.nbytes)
+            out.update({"predict_ms": t, "predict_molecules_per_s": nm / (t * 1e-3), "predict_us_per_atom": t * 1e3 / na,
+                        "predict_alu_frac": na * D * (2 * T * L + 6) / (t * 1e-3) / alu_peak,
+                        "predict_gradient_stream_GBps_if_alone": gbytes / (t * 1e-3) / 1e9})
+        print(json.dumps(out), flush=True)
+        del dp, w
+        pkg.release_workspaces()
+        torch.cuda.empty_cache()
+
+
 if __name__ == "__main__":
     a = parse()
-    if a.impl == "reference":
+    if a.report_configs:
+        report_configs(a)
+    elif a.impl == "reference":
         reference_arm(a)
     else:
         ours_arm(a)

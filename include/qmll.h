@@ -109,12 +109,21 @@ int qmll_predict(const qmll_sorf_params* p, const float* x, const int32_t* elem,
                  int64_t n_atoms, int32_t n_mol, const float* alpha, const qmll_grad* grad, float* energies,
                  float* forces, void* workspace, size_t workspace_bytes, void* cuda_stream);
 
+/* NEXT step after the accumulation: alpha = (ZtZ + lambda I)^-1 Zty, the regularised
+ * normal equations of eq. 16-17 (L134-144; "solved by LU decomposition", L137 -- SPD, so a blocked Cholesky), in FP64.
+ *   ZtZ [D, D] fp32 symmetric (only the lower triangle is read), Zty [D] fp32, lambda >= 0, alpha [D] fp32 out,
+ *   info: device int32, LAPACK convention: 0 = success, k > 0 = leading minor of order k not positive definite
+ *   (alpha is then NaN-contaminated).  The inputs are not modified. */
+int qmll_solve(const float* ZtZ, const float* Zty, int32_t D, double lambda, float* alpha, int32_t* info,
+               void* workspace, size_t workspace_bytes, void* cuda_stream);
+
 enum {
   QMLL_CALL_FORWARD = 0,         /* qmll_sorf_forward without grad            */
   QMLL_CALL_FORWARD_GRAD = 1,    /* qmll_sorf_forward with grad and G         */
   QMLL_CALL_BACKWARD_FORCES = 2, /* qmll_sorf_backward_forces                 */
   QMLL_CALL_NORMAL_EQUATIONS = 3,/* qmll_normal_equations (uses rows and p->D; p->d may be 0) */
-  QMLL_CALL_PREDICT = 4          /* qmll_predict                              */
+  QMLL_CALL_PREDICT = 4,         /* qmll_predict                              */
+  QMLL_CALL_SOLVE = 5            /* qmll_solve (uses p->D only)               */
 };
 
 /* Scratch bytes the named call needs for these sizes (host-side arithmetic only, no CUDA call).

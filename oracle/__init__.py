@@ -156,6 +156,17 @@ def normal_equations(A, y):
     return ZtZ, Zty
 
 
+def solve(ZtZ, Zty, lam: float):
+    """(alpha[D] float64, info): (ZtZ + lam I) alpha = Zty by FP64 Cholesky (eq. 16-17)."""
+    ZtZ, Zty = _f32(ZtZ), _f32(Zty)
+    D = ZtZ.shape[0]
+    alpha = np.zeros(D, dtype=np.float64)
+    lib = _load()
+    lib.qo_solve.restype = ctypes.c_int
+    info = lib.qo_solve(_p(ZtZ), _p(Zty), _I(D), _D(lam), _p(alpha))
+    return alpha, int(info)
+
+
 def gram_entries(A, ii, jj) -> np.ndarray:
     A, ii, jj = _f32(A), _i32(ii), _i32(jj)
     out = np.empty(ii.shape[0], dtype=np.float64)

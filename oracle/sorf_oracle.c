@@ -313,3 +313,38 @@ void qo_gram_rows(const float* A, const float* y, int64_t rows, int D, const int
     }
   }
 }
+
+/* Regularised normal equations (eq. 16-17): alpha = (ZtZ + lambda I)^-1 Zty.  The paper solves by LU (L137);
+ * the matrix is symmetric positive definite, so this is the textbook (unblocked, row-by-row) Cholesky A = L L^T in
+ * FP64 followed by the two triangular solves.  Returns 0, or k > 0 if the leading minor of order k is not positive
+ * definite (LAPACK convention).  Pins: numpy.linalg.solve, residual, diagonal closed form, non-PD detection. */
+int qo_solve(const float* ZtZ, const float* Zty, int D, double lambda, double* alpha /* [D] */) {
+  double* L = (double*)malloc(sizeof(double) * (size_t)D * D);
+  int info = 0;
+  for (int i = 0; i < D && !info; ++i) {
+    for (int j = 0; j <= i; ++j) {
+      double s = (double)ZtZ[(size_t)i * D + j] + (i == j ? lambda : 0.0);
+      for (int m = 0; m < j; ++m) s -= L[(size_t)i * D + m] * L[(size_t)j * D + m];
+      if (i == j) {
+        if (!(s > 0.0)) { info = i + 1; break; }
+        L[(size_t)i * D + i] = sqrt(s);
+      } else {
+        L[(size_t)i * D + j] = s / L[(size_t)j * D + j];
+      }
+    }
+  }
+  if (!info) {
+    for (int i = 0; i < D; ++i) {          /* L y = b */
+      double s = (double)Zty[i];
+      for (int m = 0; m < i; ++m) s -= L[(size_t)i * D + m] * alpha[m];
+      alpha[i] = s / L[(size_t)i * D + i];
+    }
+    for (int i = D - 1; i >= 0; --i) {     /* L^T alpha = y */
+      double s = alpha[i];
+      for (int m = i + 1; m < D; ++m) s -= L[(size_t)m * D + i] * alpha[m];
+      alpha[i] = s / L[(size_t)i * D + i];
+    }
+  }
+  free(L);
+  return info;
+}

@@ -21,9 +21,9 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libqmll.so")
 
 QMLL_GRAD_DENSE, QMLL_GRAD_NEIGHBOR = 1, 2
-CALL_FORWARD, CALL_FORWARD_GRAD, CALL_BACKWARD_FORCES, CALL_NORMAL_EQUATIONS, CALL_PREDICT = range(5)
+CALL_FORWARD, CALL_FORWARD_GRAD, CALL_BACKWARD_FORCES, CALL_NORMAL_EQUATIONS, CALL_PREDICT, CALL_SOLVE = range(6)
 
-EXPORTS = ("qmll_sorf_forward", "qmll_sorf_backward_forces", "qmll_normal_equations", "qmll_predict",
+EXPORTS = ("qmll_solve", "qmll_sorf_forward", "qmll_sorf_backward_forces", "qmll_normal_equations", "qmll_predict",
            "qmll_workspace_bytes", "qmll_normal_equations_min_workspace", "qmll_status_string",
            "qmll_launch_count", "qmll_reset_launch_count", "qmll_time_normal_equations_kernel",
            "qmll_collect_normal_equations_kernel_ms")
@@ -67,6 +67,8 @@ def load_library() -> ctypes.CDLL:
     lib.qmll_predict.argtypes = [pp, vp, vp, vp, i64, i32, vp, gp, vp, vp, vp, sz, vp]
     for name in ("qmll_sorf_forward", "qmll_sorf_backward_forces", "qmll_normal_equations", "qmll_predict"):
         getattr(lib, name).restype = ctypes.c_int
+    lib.qmll_solve.argtypes = [vp, vp, i32, ctypes.c_double, vp, vp, vp, sz, vp]
+    lib.qmll_solve.restype = ctypes.c_int
     lib.qmll_workspace_bytes.argtypes = [ctypes.c_int, pp, i64, i32, i64]
     lib.qmll_workspace_bytes.restype = sz
     lib.qmll_normal_equations_min_workspace.argtypes = [i32]
@@ -251,6 +253,22 @@ def qmll_normal_equations(A, y=None, ZtZ=None, Zty=None, accumulate: bool = Fals
                                      _dev(Zty, torch.float32, "Zty"), ctypes.c_void_p(ws.data_ptr()),
                                      min(ws.numel(), nb), _stream()))
     return ZtZ, Zty
+
+
+def qmll_solve(ZtZ, Zty, lam: float, alpha=None):
+    """(alpha [D], info int32[1]) with (ZtZ + lam I) alpha = Zty: include/qmll.h qmll_solve (FP64 Cholesky)."""
+    lib = load_library()
+    D = int(ZtZ.shape[0])
+    if alpha is None:
+        alpha = torch.empty((D,), dtype=torch.float32, device=ZtZ.device)
+    info = torch.zeros((1,), dtype=torch.int32, device=ZtZ.device)
+    cp = _CParams(0, D, 0, 0, 0.0, None, None)
+    nb = int(lib.qmll_workspace_bytes(CALL_SOLVE, ctypes.byref(cp), 0, 0, 0))
+    ws = workspace(nb, ZtZ.device)
+    _check(lib.qmll_solve(_dev(ZtZ, torch.float32, "ZtZ"), _dev(Zty, torch.float32, "Zty"), D, float(lam),
+                          _dev(alpha, torch.float32, "alpha"), _dev(info, torch.int32, "info"),
+                          ctypes.c_void_p(ws.data_ptr()), ws.numel(), _stream()))
+    return alpha, info
 
 
 def launch_count() -> int:

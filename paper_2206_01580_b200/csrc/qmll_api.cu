@@ -119,6 +119,7 @@ size_t qmll_workspace_bytes(int which_call, const qmll_sorf_params* p, int64_t n
                             int64_t rows) {
   if (!p) return 0;
   if (which_call == QMLL_CALL_NORMAL_EQUATIONS) return p->D > 0 ? syrk_full_workspace(rows, p->D) : 0;
+  if (which_call == QMLL_CALL_SOLVE) return p->D > 0 ? solve_workspace_bytes(p->D) : 0;
   if (p->d <= 0 || p->D <= 0 || p->D % p->d != 0 || p->n_elem < 1 || p->n_transform < 1 || !sorf_supported_d(p->d))
     return 0;
   if (n_atoms < 0) n_atoms = 0;
@@ -200,6 +201,15 @@ int qmll_normal_equations(const float* A, const float* y, int64_t rows, int32_t 
   if (rc) return rc;
   return syrk_normal_equations(A, y, rows, D, accumulate, ZtZ, Zty, workspace, workspace_bytes,
                                static_cast<cudaStream_t>(cuda_stream));
+}
+
+int qmll_solve(const float* ZtZ, const float* Zty, int32_t D, double lambda, float* alpha, int32_t* info,
+               void* workspace, size_t workspace_bytes, void* cuda_stream) {
+  if (!ZtZ || !Zty || !alpha || !info || D <= 0 || !(lambda >= 0.0)) return QMLL_ERR_INVALID_ARG;
+  int rc = check_device();
+  if (rc) return rc;
+  return solve_normal_equations(ZtZ, Zty, D, lambda, alpha, info, workspace, workspace_bytes,
+                                static_cast<cudaStream_t>(cuda_stream));
 }
 
 const char* qmll_status_string(int status) {

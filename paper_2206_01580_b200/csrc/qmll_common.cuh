@@ -96,6 +96,11 @@ size_t syrk_full_workspace(int64_t rows, int32_t D);
 int syrk_normal_equations(const float* A, const float* y, int64_t rows, int32_t D, int accumulate, float* ZtZ,
                           float* Zty, void* ws, size_t ws_bytes, cudaStream_t st);
 
+// ---- solve (solve_kernels.cu) ------------------------------------------------------------------------------
+size_t solve_workspace_bytes(int32_t D);
+int solve_normal_equations(const float* ZtZ, const float* Zty, int32_t D, double lambda, float* alpha, int32_t* info,
+                           void* ws, size_t ws_bytes, cudaStream_t st);
+
 void syrk_set_timing(bool on);
 int syrk_collect_timing(double* total_ms, int* launches);
 

@@ -219,24 +219,37 @@ sorf_backward_kernel(const float* __restrict__ x, const int32_t* __restrict__ el
       const int gl = (valid ? s_raw : n_s - 1) * S::P + p;
       float v[S::E];
       load_row<S>(v, x + (size_t)a * S::d, p);
-      chain_forward<S>(v, sign_bits, e, T, n_gl, gl, p);
       const float4* b4 = bias4 + (size_t)e * S::E4 * n_gl + gl;
       const float4* al4 = alpha4 + gl;
+      // Forward chain, sin/cos, transposed chain as ONE loop over 2T+1 phases so that the unrolled butterfly and
+      // sign-flip code exist once (the straight-line version overflowed the instruction cache: 37 % no-instruction
+      // stalls).  Phase i < T: S_i then H.  Phase T: u -> (energy, q) then H.  Phase T < i < 2T: S_{2T-i} then H.
+      // Phase 2T: S_0 only.   [ (H S_{T-1} ... H S_0) x ;  S_0 H S_1 H ... S_{T-1} H q ]
+#pragma unroll 1
+      for (int i = 0; i <= 2 * T; ++i) {
+        if (i == T) {
 #pragma unroll
-      for (int q = 0; q < S::E4; ++q) {
-        const float4 b = __ldg(b4 + (size_t)q * n_gl);
-        float4 al = __ldg(al4 + (size_t)q * n_gl);
-        if (!valid) al = make_float4(0.f, 0.f, 0.f, 0.f);
-        const float f0 = frac_rev(fmaf(v[4 * q + 0], c_rev, b.x));
-        const float f1 = frac_rev(fmaf(v[4 * q + 1], c_rev, b.y));
-        const float f2 = frac_rev(fmaf(v[4 * q + 2], c_rev, b.z));
-        const float f3 = frac_rev(fmaf(v[4 * q + 3], c_rev, b.w));
-        epart = fmaf(al.x, cos_rev(f0), epart); epart = fmaf(al.y, cos_rev(f1), epart);
-        epart = fmaf(al.z, cos_rev(f2), epart); epart = fmaf(al.w, cos_rev(f3), epart);
-        v[4 * q + 0] = -al.x * sin_rev(f0); v[4 * q + 1] = -al.y * sin_rev(f1);
-        v[4 * q + 2] = -al.z * sin_rev(f2); v[4 * q + 3] = -al.w * sin_rev(f3);
+          for (int q = 0; q < S::E4; ++q) {
+            const float4 b = __ldg(b4 + (size_t)q * n_gl);
+            float4 al = __ldg(al4 + (size_t)q * n_gl);
+            if (!valid) al = make_float4(0.f, 0.f, 0.f, 0.f);
+            const float f0 = frac_rev(fmaf(v[4 * q + 0], c_rev, b.x));
+            const float f1 = frac_rev(fmaf(v[4 * q + 1], c_rev, b.y));
+            const float f2 = frac_rev(fmaf(v[4 * q + 2], c_rev, b.z));
+            const float f3 = frac_rev(fmaf(v[4 * q + 3], c_rev, b.w));
+            epart = fmaf(al.x, cos_rev(f0), epart); epart = fmaf(al.y, cos_rev(f1), epart);
+            epart = fmaf(al.z, cos_rev(f2), epart); epart = fmaf(al.w, cos_rev(f3), epart);
+            v[4 * q + 0] = -al.x * sin_rev(f0); v[4 * q + 1] = -al.y * sin_rev(f1);
+            v[4 * q + 2] = -al.z * sin_rev(f2); v[4 * q + 3] = -al.w * sin_rev(f3);
+          }
+        } else {
+          const int t = i < T ? i : 2 * T - i;
+          uint32_t w[S::EW];
+          load_sign_words<S>(w, sign_bits, e, t, T, n_gl, gl);
+          apply_signs<S>(v, w);
+        }
+        if (i < 2 * T) fwht<S>(v, p);
       }
-      chain_transposed<S>(v, sign_bits, e, T, n_gl, gl, p);
       SR::run(v, lane, jbase);
 #pragma unroll
       for (int i = 0; i < SR::R; ++i) gacc[i] += v[i];

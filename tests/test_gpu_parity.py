@@ -166,3 +166,43 @@ def test_error_codes(q):
     bad2 = pkg.SorfParams(d=64, D=128, n_transform=4, n_elem=3, sigma=1.0, signs=dp.params.signs, bias=dp.params.bias)
     with pytest.raises(pkg.QmllError):
         pkg.qmll_sorf_forward(bad2, dp.x, dp.elem, dp.mol_off)
+
+
+@pytest.mark.parametrize("D,rows", [(1, 4), (50, 300), (256, 448), (1000, 3000)])
+def test_solve_matches_oracle(q, D, rows):
+    """qmll_solve (blocked FP64 Cholesky) against the oracle's unblocked one on the same fp32 ZtZ / Zty."""
+    pkg, wio, torch = q
+    rng = np.random.default_rng(D)
+    A = rng.standard_normal((rows, D)).astype(np.float32)
+    y = rng.standard_normal(rows).astype(np.float32)
+    ZtZ = (A.astype(np.float64).T @ A.astype(np.float64)).astype(np.float32)
+    Zty = (A.astype(np.float64).T @ y.astype(np.float64)).astype(np.float32)
+    lam = 1e-2
+    alpha, info = pkg.qmll_solve(torch.from_numpy(ZtZ).cuda(), torch.from_numpy(Zty).cuda(), lam)
+    ao, io = oracle.solve(ZtZ, Zty, lam)
+    assert int(info.item()) == 0 and io == 0
+    assert rel(alpha.cpu().numpy(), ao) <= 1e-6          # fp32 output of an FP64 solve
+
+
+def test_solve_reports_non_positive_definite(q):
+    pkg, wio, torch = q
+    bad = torch.tensor([[1.0, 2.0], [2.0, 1.0]], device="cuda")
+    _, info = pkg.qmll_solve(bad, torch.ones(2, device="cuda"), 0.0)
+    assert int(info.item()) == 2
+
+
+def test_train_then_predict_recovers_targets(q):
+    """Closes the loop on config 1: y := [Z; G] alpha*, normal equations, solve, predict -> E, F reproduce y."""
+    pkg, wio, torch = q
+    w = make_workload("c1", D=256)
+    dp = wio.device_problem(w)
+    Z, G = pkg.qmll_sorf_forward(dp.params, dp.x, dp.elem, dp.mol_off, dp.grad)
+    A = torch.cat([Z, G]).contiguous()
+    y = (A.double() @ dp.alpha.double()).float()
+    ZtZ, Zty = pkg.qmll_normal_equations(A, y)
+    lam = 1e-9 * float(torch.trace(ZtZ)) / 256
+    alpha, info = pkg.qmll_solve(ZtZ, Zty, lam)
+    assert int(info.item()) == 0
+    E, F = pkg.qmll_predict(dp.params, dp.x, dp.elem, dp.mol_off, alpha, dp.grad)
+    pred = torch.cat([E, F.reshape(-1)]).cpu().numpy()
+    assert rel(pred, y.cpu().numpy()) <= 1e-3

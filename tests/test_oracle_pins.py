@@ -318,3 +318,31 @@ def test_c1_golden_regression():
     assert np.allclose(E[:4], gold["energy_first4"], rtol=1e-11, atol=1e-14)
     assert np.allclose(F[0], gold["forces_atom0"], rtol=1e-11, atol=1e-14)
     assert np.isclose(np.linalg.norm(F), gold["forces_fro"], rtol=1e-12)
+
+
+# ----------------------------------------------------------------------------- solve (NEXT #1; eq. 16-17)
+def test_solve_matches_numpy_and_residual():
+    rng = np.random.default_rng(11)
+    for D, rows in ((1, 3), (7, 20), (64, 200), (130, 400)):
+        A = rng.standard_normal((rows, D)).astype(np.float32)
+        y = rng.standard_normal(rows).astype(np.float32)
+        ZtZ = (A.astype(np.float64).T @ A.astype(np.float64)).astype(np.float32)
+        Zty = (A.astype(np.float64).T @ y.astype(np.float64)).astype(np.float32)
+        lam = 1e-3
+        alpha, info = oracle.solve(ZtZ, Zty, lam)
+        assert info == 0
+        M = ZtZ.astype(np.float64) + lam * np.eye(D)
+        assert np.allclose(alpha, np.linalg.solve(M, Zty.astype(np.float64)), rtol=1e-9, atol=1e-12)
+        assert np.linalg.norm(M @ alpha - Zty) <= 1e-10 * np.linalg.norm(Zty)
+
+
+def test_solve_closed_forms_and_failure():
+    d = np.array([1.0, 4.0, 0.25, 9.0], dtype=np.float32)
+    b = np.array([2.0, -8.0, 1.0, 3.0], dtype=np.float32)
+    alpha, info = oracle.solve(np.diag(d), b, 0.5)                      # diagonal: alpha_i = b_i / (d_i + lambda)
+    assert info == 0 and np.allclose(alpha, b.astype(np.float64) / (d.astype(np.float64) + 0.5), rtol=1e-14)
+    alpha, info = oracle.solve(np.zeros((3, 3), np.float32), np.ones(3, np.float32), 2.0)   # pure ridge: b / lambda
+    assert info == 0 and np.allclose(alpha, 0.5)
+    bad = np.array([[1.0, 2.0], [2.0, 1.0]], dtype=np.float32)          # indefinite: second minor fails
+    _, info = oracle.solve(bad, np.ones(2, np.float32), 0.0)
+    assert info == 2
