@@ -175,7 +175,7 @@ __device__ __forceinline__ float warp_sum(float v) {
 }
 
 template <typename S>
-__global__ void __launch_bounds__(kFwdThreads, (S::E >= 128 ? 2 : 4))
+__global__ void __launch_bounds__(kFwdThreads, (S::E >= 128 ? 3 : 4))
 sorf_backward_kernel(const float* __restrict__ x, const int32_t* __restrict__ elem,
                      const int32_t* __restrict__ mol_off, int n_atoms, int n_mol, int n_s, int T, float c_rev,
                      float c, const uint32_t* __restrict__ sign_bits, const float* __restrict__ bias_rev,
@@ -187,8 +187,9 @@ sorf_backward_kernel(const float* __restrict__ x, const int32_t* __restrict__ el
   if (task >= n_chunks) return;
   const int p = lane % S::P, sl = lane / S::P;
   const int n_gl = n_s * S::P;
-  const int a_begin = chunk_cut(mol_off, n_mol, n_atoms, (int)task, chunk);
-  const int a_end = chunk_cut(mol_off, n_mol, n_atoms, (int)task + 1, chunk);
+  // fixed-size atom chunks (equal work per warp); molecule changes inside a chunk only flush the energy partial
+  const int a_begin = (int)task * chunk;
+  const int a_end = a_begin + chunk < n_atoms ? a_begin + chunk : n_atoms;
   if (a_begin >= a_end) return;
 
   int mol = owner_molecule(mol_off, n_mol, a_begin);
@@ -446,7 +447,7 @@ struct SorfLaunch {
     const int n_s = p->D / p->d, n_sg = (n_s + S::SPW - 1) / S::SPW;
     const int n_atoms = (int)pr.n_atoms;
     if (n_atoms == 0 || pr.n_mol == 0) return QMLL_OK;
-    const int chunk = clampi((long long)n_atoms / (4LL * warp_slots()), 1, 16);
+    const int chunk = clampi((long long)n_atoms / (8LL * warp_slots()), 1, 8);
     const int n_chunks = (n_atoms + chunk - 1) / chunk;
     const unsigned grid = (unsigned)((n_chunks + kWarpsPerBlock - 1) / kWarpsPerBlock);
     const float c = c_of(p);
