@@ -6,7 +6,7 @@
 // therefore carries SPW = 32/P independent vectors, one per SORF stack s ("stack lane" sl = lane / P):
 // all of them are transforms of the SAME input row x_I with different sign diagonals, so x_I is a
 // broadcast load and no inter-lane traffic is needed for the log2(E) low butterfly stages.  The
-// log2(P) high stages (d > 128 only) are one shuffle + one FFMA per element.  For d <= 128 the whole
+// log2(P) high stages (d > 128 only) exchange through a small shared-memory scratch (see fwht).  For d <= 128 the whole
 // H*D3*H*D2*H*D1 chain of a stack is register-local.
 #pragma once
 #include <cuda_runtime.h>
@@ -36,9 +36,22 @@ struct Shape {
   static_assert(P_ >= 1 && P_ <= 16 && (P_ & (P_ - 1)) == 0, "P");
 };
 
-// v <- H_d v (unnormalised, natural order): any order of the butterfly stages gives the same matrix.
+// Per-warp shared-memory scratch for the cross-lane butterfly stages (P > 1): 32 elements per lane at a time.
+constexpr int kXchgFloat4PerWarp = 8 * kWarp;  // 4 KB
 template <typename S>
-__device__ __forceinline__ void fwht(float (&v)[S::E], int p) {
+struct Xchg {
+  static constexpr size_t kBytesPerWarp = S::P > 1 ? kXchgFloat4PerWarp * sizeof(float4) : 0;
+};
+
+// v <- H_d v (unnormalised, natural order): any order of the butterfly stages gives the same matrix.
+// The log2(E) low stages are register-local.  The log2(P) high stages pair lane p with lane p ^ h: the partner's
+// values come through the warp's shared-memory scratch as float4 (8 LDS.128 deliver 32 operands, which keeps the
+// FFMAs fed; one SHFL per element left them waiting on the shuffle latency -- 29 % short-scoreboard stalls).
+// kSmem selects the exchange path: the backward kernel (no other shared memory) uses it; the forward and force-row
+// kernels keep one SHFL + FFMA per element, because 16 KB more shared memory per block would cost them a resident
+// block per SM (their accumulators already take 64 KB).
+template <typename S, bool kSmem>
+__device__ __forceinline__ void fwht(float (&v)[S::E], int p, float4* xb, int lane) {
 #pragma unroll
   for (int h = 1; h < S::E; h <<= 1) {
 #pragma unroll
@@ -55,10 +68,30 @@ __device__ __forceinline__ void fwht(float (&v)[S::E], int p) {
 #pragma unroll
     for (int h = 1; h < S::P; h <<= 1) {
       const float sg = (p & h) ? -1.0f : 1.0f;  // upper partner holds (lower - upper)
+      if constexpr (!kSmem) {
 #pragma unroll
-      for (int j = 0; j < S::E; ++j) {
-        float o = __shfl_xor_sync(0xffffffffu, v[j], h);
-        v[j] = fmaf(v[j], sg, o);
+        for (int j = 0; j < S::E; ++j) {
+          float o = __shfl_xor_sync(0xffffffffu, v[j], h);
+          v[j] = fmaf(v[j], sg, o);
+        }
+        continue;
+      }
+      constexpr int kChunk = S::E < 32 ? S::E : 32;
+#pragma unroll
+      for (int c = 0; c < S::E; c += kChunk) {
+#pragma unroll
+        for (int q = 0; q < kChunk / 4; ++q)
+          xb[q * kWarp + lane] = make_float4(v[c + 4 * q], v[c + 4 * q + 1], v[c + 4 * q + 2], v[c + 4 * q + 3]);
+        __syncwarp();
+#pragma unroll
+        for (int q = 0; q < kChunk / 4; ++q) {
+          const float4 o = xb[q * kWarp + (lane ^ h)];
+          v[c + 4 * q + 0] = fmaf(v[c + 4 * q + 0], sg, o.x);
+          v[c + 4 * q + 1] = fmaf(v[c + 4 * q + 1], sg, o.y);
+          v[c + 4 * q + 2] = fmaf(v[c + 4 * q + 2], sg, o.z);
+          v[c + 4 * q + 3] = fmaf(v[c + 4 * q + 3], sg, o.w);
+        }
+        __syncwarp();
       }
     }
   }
@@ -95,23 +128,23 @@ __device__ __forceinline__ void load_row(float (&v)[S::E], const float* __restri
 // One stack of eq. 20 without the constant c:  v <- H S_{T-1} ... H S_0 v   (sign flip, then H: L268, A4)
 template <typename S>
 __device__ __forceinline__ void chain_forward(float (&v)[S::E], const uint32_t* __restrict__ sign_bits, int e,
-                                              int T, int n_gl, int gl, int p) {
+                                              int T, int n_gl, int gl, int p, float4* xb, int lane) {
   for (int t = 0; t < T; ++t) {
     uint32_t w[S::EW];
     load_sign_words<S>(w, sign_bits, e, t, T, n_gl, gl);
     apply_signs<S>(v, w);
-    fwht<S>(v, p);
+    fwht<S, false>(v, p, xb, lane);
   }
 }
 
 // Transposed stack: v <- S_0 H ... S_{T-1} H v   (H symmetric).
 template <typename S>
 __device__ __forceinline__ void chain_transposed(float (&v)[S::E], const uint32_t* __restrict__ sign_bits,
-                                                 int e, int T, int n_gl, int gl, int p) {
+                                                 int e, int T, int n_gl, int gl, int p, float4* xb, int lane) {
   for (int t = T - 1; t >= 0; --t) {
     uint32_t w[S::EW];
     load_sign_words<S>(w, sign_bits, e, t, T, n_gl, gl);
-    fwht<S>(v, p);
+    fwht<S, false>(v, p, xb, lane);
     apply_signs<S>(v, w);
   }
 }

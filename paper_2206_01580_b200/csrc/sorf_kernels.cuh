@@ -76,6 +76,7 @@ sorf_forward_kernel(const float* __restrict__ x, const int32_t* __restrict__ ele
   if (a_begin >= a_end) return;
 
   zero_acc<S>(acc, tid);
+  float4* xb = acc + S::E4 * kFwdThreads + warp * kXchgFloat4PerWarp;  // cross-lane scratch (P > 1 only)
   int mol = owner_molecule(mol_off, n_mol, a_begin);
   int mol_lo = __ldg(mol_off + mol), mol_hi = __ldg(mol_off + mol + 1);
   const float4* bias4 = reinterpret_cast<const float4*>(bias_rev);
@@ -92,7 +93,7 @@ sorf_forward_kernel(const float* __restrict__ x, const int32_t* __restrict__ ele
     const int e = __ldg(elem + a);
     float v[S::E];
     load_row<S>(v, x + (size_t)a * S::d, p);
-    chain_forward<S>(v, sign_bits, e, T, n_gl, gl, p);
+    chain_forward<S>(v, sign_bits, e, T, n_gl, gl, p, xb, lane);
     const float4* b4 = bias4 + (size_t)e * S::E4 * n_gl + gl;
     float4* zs4 = kWriteSin ? reinterpret_cast<float4*>(zs_out) + (size_t)a * S::E4 * n_gl + gl : nullptr;
 #pragma unroll
@@ -182,7 +183,9 @@ sorf_backward_kernel(const float* __restrict__ x, const int32_t* __restrict__ el
                      const float* __restrict__ alpha_s, float* __restrict__ g_out,
                      double* __restrict__ energy_acc, int chunk, int n_chunks, int n_sg) {
   using SR = StackReduce<S>;
+  extern __shared__ float4 xchg_smem[];
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  float4* xb = xchg_smem + warp * kXchgFloat4PerWarp;  // cross-lane scratch (P > 1 only)
   const long long task = (long long)blockIdx.x * (kFwdThreads / kWarp) + warp;
   if (task >= n_chunks) return;
   const int p = lane % S::P, sl = lane / S::P;
@@ -249,7 +252,7 @@ sorf_backward_kernel(const float* __restrict__ x, const int32_t* __restrict__ el
           load_sign_words<S>(w, sign_bits, e, t, T, n_gl, gl);
           apply_signs<S>(v, w);
         }
-        if (i < 2 * T) fwht<S>(v, p);
+        if (i < 2 * T) fwht<S, true>(v, p, xb, lane);
       }
       SR::run(v, lane, jbase);
 #pragma unroll
@@ -297,6 +300,8 @@ sorf_force_rows_dense_kernel(const int32_t* __restrict__ elem, const int32_t* __
   float* colbuf = reinterpret_cast<float*>(acc + S::E4 * kFwdThreads) + warp * 2 * CS::kBufFloats;
   uint64_t* bars = reinterpret_cast<uint64_t*>(reinterpret_cast<float*>(acc + S::E4 * kFwdThreads) +
                                                kWarps * 2 * CS::kBufFloats) + warp * 2;
+  float4* xb = reinterpret_cast<float4*>(reinterpret_cast<char*>(acc) + S::E * kFwdThreads * sizeof(float) +
+                                         CS::kBytes) + warp * kXchgFloat4PerWarp;  // cross-lane scratch (P > 1)
   const long long task = (long long)blockIdx.x * kWarps + warp;
   if (task >= 3LL * n_atoms * n_sg) return;
   const int sg = (int)(task % n_sg);
@@ -347,7 +352,7 @@ sorf_force_rows_dense_kernel(const int32_t* __restrict__ elem, const int32_t* __
       }
     }
     __syncwarp();
-    chain_forward<S>(v, sign_bits, e, T, n_gl, gl, p);
+    chain_forward<S>(v, sign_bits, e, T, n_gl, gl, p, xb, lane);
     const float4* z4 = zs4 + (size_t)(a0 + I) * S::E4 * n_gl + gl;
 #pragma unroll
     for (int q = 0; q < S::E4; ++q) {
@@ -369,7 +374,9 @@ sorf_force_rows_neighbor_kernel(const int32_t* __restrict__ elem, int n_atoms, i
                                 const uint32_t* __restrict__ sign_bits, const float* __restrict__ zs,
                                 const int32_t* __restrict__ nbr_idx, const float* __restrict__ nbr_val, int K,
                                 float* __restrict__ G, int n_sg) {
+  extern __shared__ float4 xchg_smem[];
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  float4* xb = xchg_smem + warp * kXchgFloat4PerWarp;  // cross-lane scratch (P > 1 only)
   const long long task = (long long)blockIdx.x * (kFwdThreads / kWarp) + warp;
   if (task >= (long long)n_atoms * K * n_sg) return;
   const int sg = (int)(task % n_sg);
@@ -390,7 +397,7 @@ sorf_force_rows_neighbor_kernel(const int32_t* __restrict__ elem, int n_atoms, i
     float v[S::E];
 #pragma unroll
     for (int j = 0; j < S::E; ++j) v[j] = __ldg(val + (size_t)(p * S::E + j) * 3 + k);
-    chain_forward<S>(v, sign_bits, e, T, n_gl, gl, p);
+    chain_forward<S>(v, sign_bits, e, T, n_gl, gl, p, xb, lane);
     if (valid) {
       float* dst = G + ((size_t)jg * 3 + k) * (size_t)n_s * S::d + (size_t)s_raw * S::d + p * S::E;
 #pragma unroll
@@ -414,6 +421,7 @@ template <typename S>
 struct SorfLaunch {
   static constexpr int kWarpsPerBlock = kFwdThreads / kWarp;
   static constexpr size_t kAccBytes = (size_t)S::E * kFwdThreads * sizeof(float);
+  static constexpr size_t kXchgBytes = kWarpsPerBlock * Xchg<S>::kBytesPerWarp;
 
   static float c_of(const qmll_sorf_params* p) {
     return (float)(sqrt((double)p->d) / (double)p->sigma * pow((double)p->d, -0.5 * p->n_transform));
@@ -452,7 +460,7 @@ struct SorfLaunch {
     const unsigned grid = (unsigned)((n_chunks + kWarpsPerBlock - 1) / kWarpsPerBlock);
     const float c = c_of(p);
     const float c_rev = (float)((double)c / (2.0 * M_PI));
-    sorf_backward_kernel<S><<<grid, kFwdThreads, 0, st>>>(pr.x, pr.elem, pr.mol_off, n_atoms, pr.n_mol, n_s,
+    sorf_backward_kernel<S><<<grid, kFwdThreads, kXchgBytes, st>>>(pr.x, pr.elem, pr.mol_off, n_atoms, pr.n_mol, n_s,
                                                           p->n_transform, c_rev, c, t.sign_bits, t.bias_rev,
                                                           t.alpha_s, g_out, energy_acc, chunk, n_chunks, n_sg);
     QMLL_LAUNCH_CHECK("sorf_backward_kernel");
