@@ -95,12 +95,25 @@ int qmll_sorf_backward_forces(const qmll_sorf_params* p, const float* x, const i
 
 /* Step a8: normal equations (eq. 16, eq. 17; FP32 round-off remark L351):
  *   ZtZ (+)= A^T A,  Zty (+)= A^T y   for a block of rows A [rows, D] fp32 (rows of Z and/or G), y [rows] fp32.
- * ZtZ [D, D] fp32 is stored full and exactly symmetric; Zty [D] fp32.  accumulate = 0 overwrites, 1 adds to the
- * existing (symmetric) content.  The product runs on the tensor cores in 3xTF32 with the row dimension cut
- * into chunks that are summed in fp32 round-to-nearest.  lambda*I and the solve are the caller's (A10).
- * rows == 0 is legal (accumulate = 0 then zeroes the outputs).  y and Zty may both be NULL (ZtZ only). */
+ * ZtZ [D, D] fp32 is stored full and exactly symmetric; Zty [D] fp32 (summed in fp64, deterministic).
+ * accumulate = 0 overwrites, 1 adds to the existing (symmetric) content.  The product runs on the tensor cores
+ * with every operand split into hi + lo parts of 11 significant bits each (hi*hi + hi*lo + lo*hi, fp32
+ * accumulate) and the row dimension cut into 128-row chunks that are summed in fp32 round-to-nearest.
+ * lambda*I and the solve are the caller's (A10).  rows == 0 is legal (accumulate = 0 then zeroes the outputs).
+ * y and Zty may both be NULL (ZtZ only).  Any D >= 1 is supported.
+ * qmll_normal_equations uses QMLL_NE_SPLIT_F16; qmll_normal_equations_mode selects the operand container:
+ *   QMLL_NE_SPLIT_F16   hi/lo in fp16 (same 11 significant bits as TF32, twice the MMA rate, half the bytes); one
+ *                       power-of-two scale per (128-row chunk, 128-column block) keeps the parts inside fp16's
+ *                       exponent range and is undone exactly.  Entries smaller than 2^-38 of the largest entry of
+ *                       their 128 x 128 block lose their low bits (irrelevant for the Frobenius-norm accuracy of
+ *                       a Gram matrix; use QMLL_NE_SPLIT_TF32 if single tiny entries matter).
+ *   QMLL_NE_SPLIT_TF32  hi/lo in TF32 (the 3xTF32 scheme): full fp32 exponent range, half the speed. */
+enum { QMLL_NE_SPLIT_F16 = 0, QMLL_NE_SPLIT_TF32 = 1 };
 int qmll_normal_equations(const float* A, const float* y, int64_t rows, int32_t D, int32_t accumulate,
                           float* ZtZ, float* Zty, void* workspace, size_t workspace_bytes, void* cuda_stream);
+int qmll_normal_equations_mode(const float* A, const float* y, int64_t rows, int32_t D, int32_t accumulate,
+                               float* ZtZ, float* Zty, void* workspace, size_t workspace_bytes, int32_t mode,
+                               void* cuda_stream);
 
 /* Steps a1-a6 composed: energies[M] = Z[M, :] . alpha (eq. 15) and, if grad != NULL, forces as in
  * qmll_sorf_backward_forces, from one pass that shares u between cos and sin; Z is never materialised.
@@ -133,22 +146,13 @@ enum {
 size_t qmll_workspace_bytes(int which_call, const qmll_sorf_params* p, int64_t n_atoms, int32_t n_mol,
                             int64_t rows);
 size_t qmll_normal_equations_min_workspace(int32_t D);
+/* The same two sizes for an explicit mode (qmll_workspace_bytes / _min_workspace answer for QMLL_NE_SPLIT_F16). */
+size_t qmll_normal_equations_workspace(int64_t rows, int32_t D, int32_t mode);
+size_t qmll_normal_equations_min_workspace_mode(int32_t D, int32_t mode);
 
 /* Static description of a status code; for QMLL_ERR_CUDA the text of the last CUDA error seen by this
  * thread is appended.  The returned pointer stays valid until the next call from the same thread. */
 const char* qmll_status_string(int status);
-
-/* Counters for benchmarks: number of kernel launches issued by this library since the last reset
- * (process-wide, host-side counter). */
-int64_t qmll_launch_count(void);
-void qmll_reset_launch_count(void);
-
-/* Measurement aid (bench.py roofline): when enabled, every launch of the tensor-core kernel inside
- * qmll_normal_equations is bracketed by CUDA events on the caller's stream.  The collect call waits for them,
- * returns the summed kernel time in ms and the number of launches since the last collect, and frees them
- * (at most 4096 launches are recorded between collects).  Not thread-safe. */
-void qmll_time_normal_equations_kernel(int enable);
-int qmll_collect_normal_equations_kernel_ms(double* total_ms, int* launches);
 
 #ifdef __cplusplus
 }

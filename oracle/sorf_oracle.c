@@ -267,48 +267,77 @@ void qo_force_rows_neighbor(const float* x, const int32_t* elem, int64_t n_atoms
 }
 
 /* Normal equations (eq. 16, eq. 17): ZtZ = A^T A, Zty = A^T y, the definition written out.
- * A is fp32 [rows, D] (what the GPU library is given), widened to double. */
+ * A is fp32 [rows, D] (what the GPU library is given), widened to double.  Every entry is the plain sum over
+ * r = 0 .. rows-1 in that order; the row loop is the outer one only so that A is read along its rows (a thread
+ * owns a block of rows i of ZtZ and visits A once). */
 void qo_normal_equations(const float* A, const float* y, int64_t rows, int D, double* ZtZ /* [D, D] */,
                          double* Zty /* [D] */) {
-#pragma omp parallel for schedule(dynamic, 8)
-  for (int i = 0; i < D; ++i) {
-    for (int j = 0; j < D; ++j) {
-      double acc = 0.0;
-      for (int64_t r = 0; r < rows; ++r) acc += (double)A[(size_t)r * D + i] * (double)A[(size_t)r * D + j];
-      ZtZ[(size_t)i * D + j] = acc;
+#pragma omp parallel
+  {
+    int nt = 1, tid = 0;
+#ifdef _OPENMP
+    nt = omp_get_num_threads(); tid = omp_get_thread_num();
+#endif
+    const int i0 = (int)((int64_t)D * tid / nt), i1 = (int)((int64_t)D * (tid + 1) / nt);
+    for (int i = i0; i < i1; ++i) {
+      for (int j = 0; j < D; ++j) ZtZ[(size_t)i * D + j] = 0.0;
+      Zty[i] = 0.0;
     }
-    double acc = 0.0;
-    for (int64_t r = 0; r < rows; ++r) acc += (double)A[(size_t)r * D + i] * (double)y[r];
-    Zty[i] = acc;
+    for (int64_t r = 0; r < rows; ++r) {
+      const float* Ar = A + (size_t)r * D;
+      for (int i = i0; i < i1; ++i) {
+        const double a = (double)Ar[i];
+        double* row = ZtZ + (size_t)i * D;
+        for (int j = 0; j < D; ++j) row[j] += a * (double)Ar[j];
+        Zty[i] += a * (double)y[r];
+      }
+    }
   }
 }
 
 /* Selected entries (i_k, j_k) of A^T A: the same definition, for sampled parity at full size. */
 void qo_gram_entries(const float* A, int64_t rows, int D, const int32_t* ii, const int32_t* jj, int64_t n,
                      double* out) {
-#pragma omp parallel for schedule(static)
-  for (int64_t k = 0; k < n; ++k) {
-    double acc = 0.0;
-    const int i = ii[k], j = jj[k];
-    for (int64_t r = 0; r < rows; ++r) acc += (double)A[(size_t)r * D + i] * (double)A[(size_t)r * D + j];
-    out[k] = acc;
+#pragma omp parallel
+  {
+    int nt = 1, tid = 0;
+#ifdef _OPENMP
+    nt = omp_get_num_threads(); tid = omp_get_thread_num();
+#endif
+    const int64_t k0 = n * tid / nt, k1 = n * (tid + 1) / nt;
+    for (int64_t k = k0; k < k1; ++k) out[k] = 0.0;
+    for (int64_t r = 0; r < rows; ++r) {
+      const float* Ar = A + (size_t)r * D;
+      for (int64_t k = k0; k < k1; ++k) out[k] += (double)Ar[ii[k]] * (double)Ar[jj[k]];
+    }
   }
 }
 
 /* Selected full rows i_k of A^T A (out[k, :]), plus A^T y if y != NULL (out_y[k]). */
 void qo_gram_rows(const float* A, const float* y, int64_t rows, int D, const int32_t* ii, int n,
                   double* out /* [n, D] */, double* out_y /* [n] or NULL */) {
-  for (int k = 0; k < n; ++k) {
-    const int i = ii[k];
-#pragma omp parallel for schedule(static)
-    for (int j = 0; j < D; ++j) {
-      double acc = 0.0;
-      for (int64_t r = 0; r < rows; ++r) acc += (double)A[(size_t)r * D + i] * (double)A[(size_t)r * D + j];
-      out[(size_t)k * D + j] = acc;
+#pragma omp parallel
+  {
+    int nt = 1, tid = 0;
+#ifdef _OPENMP
+    nt = omp_get_num_threads(); tid = omp_get_thread_num();
+#endif
+    const int j0 = (int)((int64_t)D * tid / nt), j1 = (int)((int64_t)D * (tid + 1) / nt);
+    for (int k = 0; k < n; ++k)
+      for (int j = j0; j < j1; ++j) out[(size_t)k * D + j] = 0.0;
+    for (int64_t r = 0; r < rows; ++r) {
+      const float* Ar = A + (size_t)r * D;
+      for (int k = 0; k < n; ++k) {
+        const double a = (double)Ar[ii[k]];
+        double* row = out + (size_t)k * D;
+        for (int j = j0; j < j1; ++j) row[j] += a * (double)Ar[j];
+      }
     }
-    if (y && out_y) {
+  }
+  if (y && out_y) {
+    for (int k = 0; k < n; ++k) {
       double acc = 0.0;
-      for (int64_t r = 0; r < rows; ++r) acc += (double)A[(size_t)r * D + i] * (double)y[r];
+      for (int64_t r = 0; r < rows; ++r) acc += (double)A[(size_t)r * D + ii[k]] * (double)y[r];
       out_y[k] = acc;
     }
   }

@@ -23,10 +23,13 @@ LIB_PATH = os.path.join(_HERE, "libqmll.so")
 QMLL_GRAD_DENSE, QMLL_GRAD_NEIGHBOR = 1, 2
 CALL_FORWARD, CALL_FORWARD_GRAD, CALL_BACKWARD_FORCES, CALL_NORMAL_EQUATIONS, CALL_PREDICT, CALL_SOLVE = range(6)
 
-EXPORTS = ("qmll_solve", "qmll_sorf_forward", "qmll_sorf_backward_forces", "qmll_normal_equations", "qmll_predict",
-           "qmll_workspace_bytes", "qmll_normal_equations_min_workspace", "qmll_status_string",
+NE_SPLIT_F16, NE_SPLIT_TF32 = 0, 1
+
+EXPORTS = ("qmll_solve", "qmll_sorf_forward", "qmll_sorf_backward_forces", "qmll_normal_equations",
+           "qmll_normal_equations_mode", "qmll_predict", "qmll_workspace_bytes", "qmll_normal_equations_min_workspace",
+           "qmll_normal_equations_workspace", "qmll_normal_equations_min_workspace_mode", "qmll_status_string",
            "qmll_launch_count", "qmll_reset_launch_count", "qmll_time_normal_equations_kernel",
-           "qmll_collect_normal_equations_kernel_ms")
+           "qmll_collect_normal_equations_kernel_ms", "qmll_microbench")
 
 
 class _CParams(ctypes.Structure):
@@ -64,6 +67,12 @@ def load_library() -> ctypes.CDLL:
     lib.qmll_sorf_forward.argtypes = [pp, vp, vp, vp, i64, i32, gp, vp, vp, vp, sz, vp]
     lib.qmll_sorf_backward_forces.argtypes = [pp, vp, vp, vp, i64, i32, vp, gp, vp, vp, sz, vp]
     lib.qmll_normal_equations.argtypes = [vp, vp, i64, i32, i32, vp, vp, vp, sz, vp]
+    lib.qmll_normal_equations_mode.argtypes = [vp, vp, i64, i32, i32, vp, vp, vp, sz, i32, vp]
+    lib.qmll_normal_equations_mode.restype = ctypes.c_int
+    lib.qmll_normal_equations_workspace.argtypes = [i64, i32, i32]
+    lib.qmll_normal_equations_workspace.restype = sz
+    lib.qmll_normal_equations_min_workspace_mode.argtypes = [i32, i32]
+    lib.qmll_normal_equations_min_workspace_mode.restype = sz
     lib.qmll_predict.argtypes = [pp, vp, vp, vp, i64, i32, vp, gp, vp, vp, vp, sz, vp]
     for name in ("qmll_sorf_forward", "qmll_sorf_backward_forces", "qmll_normal_equations", "qmll_predict"):
         getattr(lib, name).restype = ctypes.c_int
@@ -148,14 +157,19 @@ _workspaces: dict = {}
 
 
 def workspace(nbytes: int, device) -> torch.Tensor:
-    """A cached, grow-only scratch tensor per device (torch allocations are 512-byte aligned)."""
-    key = torch.device(device).index or 0
-    ws = _workspaces.get(key)
-    if ws is None or ws.numel() < nbytes:
-        _workspaces.pop(key, None)
-        ws = None
-        ws = torch.empty(max(int(nbytes), 256), dtype=torch.uint8, device=device)
-        _workspaces[key] = ws
+    """A cached, grow-only scratch tensor per (device, stream): the C-ABI is stateless but this cache is not, so
+    calls issued on different streams never share scratch.  A replaced tensor is handed back to torch's caching
+    allocator, which is keyed to the stream it was allocated on -- the only stream that ever used it."""
+    dev = torch.device(device)
+    index = dev.index if dev.index is not None else torch.cuda.current_device()
+    with torch.cuda.device(index):
+        key = (index, torch.cuda.current_stream().cuda_stream)
+        ws = _workspaces.get(key)
+        if ws is None or ws.numel() < nbytes:
+            _workspaces.pop(key, None)
+            ws = None
+            ws = torch.empty(max(int(nbytes), 256), dtype=torch.uint8, device=torch.device("cuda", index))
+            _workspaces[key] = ws
     return ws
 
 
@@ -231,8 +245,8 @@ def qmll_predict(p: SorfParams, x, elem, mol_off, alpha, grad: Optional[Grad] = 
 
 
 def qmll_normal_equations(A, y=None, ZtZ=None, Zty=None, accumulate: bool = False,
-                          workspace_limit: Optional[int] = None):
-    """(ZtZ [D, D], Zty [D] or None) (+)= (A^T A, A^T y): include/qmll.h qmll_normal_equations."""
+                          workspace_limit: Optional[int] = None, mode: int = NE_SPLIT_F16):
+    """(ZtZ [D, D], Zty [D] or None) (+)= (A^T A, A^T y): include/qmll.h qmll_normal_equations(_mode)."""
     lib = load_library()
     rows, D = int(A.shape[0]), int(A.shape[1])
     if ZtZ is None:
@@ -243,15 +257,14 @@ def qmll_normal_equations(A, y=None, ZtZ=None, Zty=None, accumulate: bool = Fals
         if accumulate:
             raise ValueError("accumulate=True needs Zty")
         Zty = torch.empty((D,), dtype=torch.float32, device=A.device)
-    cp = _CParams(0, D, 0, 0, 0.0, None, None)
-    nb = int(lib.qmll_workspace_bytes(CALL_NORMAL_EQUATIONS, ctypes.byref(cp), 0, 0, rows))
+    nb = int(lib.qmll_normal_equations_workspace(rows, D, mode))
     if workspace_limit is not None:
-        nb = max(min(nb, int(workspace_limit)), int(lib.qmll_normal_equations_min_workspace(D)))
+        nb = max(min(nb, int(workspace_limit)), int(lib.qmll_normal_equations_min_workspace_mode(D, mode)))
     ws = workspace(nb, A.device)
-    _check(lib.qmll_normal_equations(_dev(A, torch.float32, "A") if rows > 0 else None, _dev(y, torch.float32, "y"),
-                                     rows, D, 1 if accumulate else 0, _dev(ZtZ, torch.float32, "ZtZ"),
-                                     _dev(Zty, torch.float32, "Zty"), ctypes.c_void_p(ws.data_ptr()),
-                                     min(ws.numel(), nb), _stream()))
+    _check(lib.qmll_normal_equations_mode(_dev(A, torch.float32, "A") if rows > 0 else None,
+                                          _dev(y, torch.float32, "y"), rows, D, 1 if accumulate else 0,
+                                          _dev(ZtZ, torch.float32, "ZtZ"), _dev(Zty, torch.float32, "Zty"),
+                                          ctypes.c_void_p(ws.data_ptr()), min(ws.numel(), nb), mode, _stream()))
     return ZtZ, Zty
 
 

@@ -47,11 +47,12 @@ static int check_grad(const qmll_grad* g) {
 }
 
 static int check_device() {
-  int dev = 0, major = 0;
+  int dev = 0, major = 0, minor = 0;
   cudaError_t e = cudaGetDevice(&dev);
   if (e == cudaSuccess) e = cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev);
+  if (e == cudaSuccess) e = cudaDeviceGetAttribute(&minor, cudaDevAttrComputeCapabilityMinor, dev);
   if (e != cudaSuccess) { note_cuda_error(e, "cudaGetDevice"); return QMLL_ERR_CUDA; }
-  return major == 10 ? QMLL_OK : QMLL_ERR_UNSUPPORTED;
+  return (major == 10 && minor == 0) ? QMLL_OK : QMLL_ERR_UNSUPPORTED;  // the kernels are built for sm_100a only
 }
 
 static int check_ws(void* ws, size_t have, size_t need) {
@@ -113,12 +114,19 @@ using namespace qmll;
 
 extern "C" {
 
-size_t qmll_normal_equations_min_workspace(int32_t D) { return D > 0 ? syrk_min_workspace(D) : 0; }
+static bool valid_mode(int32_t mode) { return mode == QMLL_NE_SPLIT_F16 || mode == QMLL_NE_SPLIT_TF32; }
+size_t qmll_normal_equations_min_workspace(int32_t D) { return D > 0 ? syrk_min_workspace(D, QMLL_NE_SPLIT_F16) : 0; }
+size_t qmll_normal_equations_min_workspace_mode(int32_t D, int32_t mode) {
+  return (D > 0 && valid_mode(mode)) ? syrk_min_workspace(D, mode) : 0;
+}
+size_t qmll_normal_equations_workspace(int64_t rows, int32_t D, int32_t mode) {
+  return (D > 0 && valid_mode(mode)) ? syrk_full_workspace(rows, D, mode) : 0;
+}
 
 size_t qmll_workspace_bytes(int which_call, const qmll_sorf_params* p, int64_t n_atoms, int32_t n_mol,
                             int64_t rows) {
   if (!p) return 0;
-  if (which_call == QMLL_CALL_NORMAL_EQUATIONS) return p->D > 0 ? syrk_full_workspace(rows, p->D) : 0;
+  if (which_call == QMLL_CALL_NORMAL_EQUATIONS) return p->D > 0 ? syrk_full_workspace(rows, p->D, QMLL_NE_SPLIT_F16) : 0;
   if (which_call == QMLL_CALL_SOLVE) return p->D > 0 ? solve_workspace_bytes(p->D) : 0;
   if (p->d <= 0 || p->D <= 0 || p->D % p->d != 0 || p->n_elem < 1 || p->n_transform < 1 || !sorf_supported_d(p->d))
     return 0;
@@ -191,16 +199,22 @@ int qmll_predict(const qmll_sorf_params* p, const float* x, const int32_t* elem,
                        workspace_bytes, static_cast<cudaStream_t>(cuda_stream), QMLL_CALL_PREDICT);
 }
 
-int qmll_normal_equations(const float* A, const float* y, int64_t rows, int32_t D, int32_t accumulate, float* ZtZ,
-                          float* Zty, void* workspace, size_t workspace_bytes, void* cuda_stream) {
-  if (rows < 0 || D <= 0 || !ZtZ) return QMLL_ERR_INVALID_ARG;
+int qmll_normal_equations_mode(const float* A, const float* y, int64_t rows, int32_t D, int32_t accumulate,
+                               float* ZtZ, float* Zty, void* workspace, size_t workspace_bytes, int32_t mode,
+                               void* cuda_stream) {
+  if (rows < 0 || D <= 0 || !ZtZ || !valid_mode(mode)) return QMLL_ERR_INVALID_ARG;
   if (rows > 0 && !A) return QMLL_ERR_INVALID_ARG;
   if (rows > 0 && (y != nullptr) != (Zty != nullptr)) return QMLL_ERR_INVALID_ARG;
-  if (D % 4 != 0) return QMLL_ERR_UNSUPPORTED;  // TMA row pitch / 16-byte alignment of A rows
   int rc = check_device();
   if (rc) return rc;
-  return syrk_normal_equations(A, y, rows, D, accumulate, ZtZ, Zty, workspace, workspace_bytes,
+  return syrk_normal_equations(A, y, rows, D, accumulate, ZtZ, Zty, workspace, workspace_bytes, mode,
                                static_cast<cudaStream_t>(cuda_stream));
+}
+
+int qmll_normal_equations(const float* A, const float* y, int64_t rows, int32_t D, int32_t accumulate, float* ZtZ,
+                          float* Zty, void* workspace, size_t workspace_bytes, void* cuda_stream) {
+  return qmll_normal_equations_mode(A, y, rows, D, accumulate, ZtZ, Zty, workspace, workspace_bytes,
+                                    QMLL_NE_SPLIT_F16, cuda_stream);
 }
 
 int qmll_solve(const float* ZtZ, const float* Zty, int32_t D, double lambda, float* alpha, int32_t* info,

@@ -7,6 +7,7 @@
 #include <stddef.h>
 
 #include "../../include/qmll.h"
+#include "../../include/qmll_aux.h"
 
 namespace qmll {
 
@@ -91,10 +92,10 @@ int contract_neighbor(const float* g, int64_t n_atoms, int d, int K, const int32
                       const float* nbr_val, float* forces, cudaStream_t st);
 
 // ---- normal equations (syrk_tcgen05.cu) ----------------------------------------------------------------
-size_t syrk_min_workspace(int32_t D);
-size_t syrk_full_workspace(int64_t rows, int32_t D);
+size_t syrk_min_workspace(int32_t D, int mode);
+size_t syrk_full_workspace(int64_t rows, int32_t D, int mode);
 int syrk_normal_equations(const float* A, const float* y, int64_t rows, int32_t D, int accumulate, float* ZtZ,
-                          float* Zty, void* ws, size_t ws_bytes, cudaStream_t st);
+                          float* Zty, void* ws, size_t ws_bytes, int mode, cudaStream_t st);
 
 // ---- solve (solve_kernels.cu) ------------------------------------------------------------------------------
 size_t solve_workspace_bytes(int32_t D);

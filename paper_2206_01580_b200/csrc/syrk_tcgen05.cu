@@ -1,20 +1,29 @@
 // syrk_tcgen05.cu -- step a8: the normal equations ZtZ (+)= A^T A, Zty (+)= A^T y (eq. 16,
-// eq. 17) on the 5th-generation tensor cores in 3xTF32 (fp32-level accuracy; the paper's FP32
-// round-off remark L351 is answered by splitting every operand into TF32 hi + lo parts and by cutting the
-// row dimension into chunks whose partial products are summed in fp32 round-to-nearest).
+// eq. 17) on the 5th-generation tensor cores with fp32-level accuracy: every operand is split into a
+// high and a low part with 11 significant bits each, the product is hi*hi + hi*lo + lo*hi (three MMAs, small
+// terms first), and the row dimension is cut into 128-row chunks whose partial products are summed in fp32
+// round-to-nearest (the paper's FP32 round-off remark, L351, restated for a truncating TMEM accumulator).
+//
+// Two operand containers (qmll_normal_equations_mode):
+//   QMLL_NE_SPLIT_F16  (default)  hi/lo are fp16 (kind::f16, K = 16 per MMA).  fp16 and TF32 carry the same 11
+//       significant bits, so the split is as exact as 3xTF32, but the f16 MMA runs at twice the TF32 rate and the
+//       operands are half as large.  fp16's narrow exponent is handled by one power-of-two scale per
+//       (128-row chunk, 128-column block), measured by the split pass and undone exactly in the epilogue.
+//   QMLL_NE_SPLIT_TF32            hi/lo are TF32 in fp32 containers (kind::tf32, K = 8 per MMA): the 3xTF32 scheme.
 //
 // Pipeline of one call (per panel of rows that fits the workspace):
-//   1. split_transpose_kernel: A[rows, D] -> At_hi, At_lo [R_pad/32][D][32] (K-major for the MMA: the contraction
-//      index `row` is the contiguous one inside each 32-row block; one TMA box is 16 KB contiguous), hi = tf32(a), lo = tf32(a - hi); Zty += A^T y rides along.
+//   1. split_kernel: A[rows, D] -> At_hi, At_lo, k-block-major [R_pad/BK][D][BK] (the contraction index `row` is
+//      the contiguous one inside each BK-row block, BK*elem = 128 bytes: one TMA box = 16 KB contiguous); per-block
+//      partial sums of A^T y ride along and are reduced deterministically in fp64 by zty_reduce_kernel.
 //   2. syrk_tcgen05_kernel: persistent, warp-specialised.  One CTA owns a 128 x 256 tile T = At[I,:] At[J,:]^T
-//      for ALL rows: TMA (SWIZZLE_128B) -> 2-stage smem ring -> tcgen05.mma kind::tf32 (hi*hi + hi*lo +
-//      lo*hi) into one of two 256-column TMEM accumulators; every 1024 rows the accumulator is drained by
-//      4 epilogue warps (tcgen05.ld) and added into C in fp32 while the next chunk is already running.
-//      The tile is written transposed (C[J0+j, I0+i], coalesced along i); only tiles touching the lower
-//      triangle are computed.
+//      for ALL rows: TMA (SWIZZLE_128B) -> 2-stage smem ring -> tcgen05.mma (lo*hi + hi*lo + hi*hi) into one of
+//      two 256-column TMEM accumulators; every 128 rows the accumulator is drained by 8 epilogue warps
+//      (tcgen05.ld) and summed in registers in fp32 while the next chunk is already running.  The tile is written
+//      transposed (C[J0+j, I0+i], coalesced along i); only tiles touching the lower triangle are computed.
 //   3. mirror_lower_kernel: C[i, j] = C[j, i] for i < j  -> full, exactly symmetric matrix.
 #include <cuda.h>
-#include <stdlib.h>
+#include <cuda_fp16.h>
+#include <mutex>
 
 #include "qmll_common.cuh"
 #include "ptx_utils.cuh"
@@ -23,28 +32,31 @@ namespace qmll {
 
 constexpr int kBM = 128;          // tile extent along I (MMA M, TMEM lanes)
 constexpr int kBN = 256;          // tile extent along J (MMA N, TMEM columns)
-constexpr int kBK = 32;           // rows per pipeline stage = one 128-byte swizzle span of fp32
-constexpr int kUmmaK = 8;         // rows per tcgen05.mma kind::tf32 (32 bytes)
 constexpr int kStages = 2;
-constexpr int kChunkRows = 1024;  // panel granularity (rows); the TMEM drain interval is chunk_rows() <= this
 // Rows accumulated in TMEM before a drain.  The tensor core truncates (rounds toward zero) every accumulate, a
 // bias of ~2e-8 per MMA relative to the running sum, so long same-sign sums (Gram diagonals, coherent Z columns)
-// need short chunks; chunk partials are summed in fp32 round-to-nearest.  QMLL_CHUNK_ROWS overrides (tuning).
-static int chunk_rows() {
-  static int v = 0;
-  if (v == 0) {
-    v = 128;
-    const char* e = getenv("QMLL_CHUNK_ROWS");
-    if (e) { int t = atoi(e); if (t >= 32 && t <= 1024 && t % 32 == 0) v = t; }
-  }
-  return v;
-}
-constexpr int kRowPad = 64;       // panels are padded with zero rows to a multiple of this
+// need short chunks (measured: 1024 rows 1.0e-5, 128 rows 1.0e-6 relative); chunk partials are summed in fp32
+// round-to-nearest.  A compile-time constant: it is part of the numerics of the call.
+constexpr int kChunkRows = 128;
+constexpr int kPanelRows = 1024;  // panel granularity (rows) when the workspace cannot hold all rows
+constexpr int kColBlock = 128;    // column granularity of the fp16 scales and of the split pass
 constexpr int kSyrkThreads = 320; // warp 0 TMA producer, warp 1 MMA issuer, warps 2..9 epilogue
-constexpr uint32_t kTileABytes = kBM * kBK * 4;             // 16 KB
-constexpr uint32_t kTileBBytes = kBN * kBK * 4;             // 32 KB
+constexpr uint32_t kTileABytes = kBM * 128;                 // 128 features x 128 bytes of rows: 16 KB
+constexpr uint32_t kTileBBytes = kBN * 128;                 // 32 KB
 constexpr uint32_t kStageBytes = 2 * kTileABytes + 2 * kTileBBytes;  // hi + lo of both operands: 96 KB
 constexpr uint32_t kSmemBytes = kStages * kStageBytes + 256 + 1024;  // + barriers + alignment slack
+
+template <bool F16>
+struct SplitMode {
+  static constexpr int kElemBytes = F16 ? 2 : 4;
+  static constexpr int kBK = 128 / kElemBytes;      // rows per pipeline stage = one 128-byte swizzle span
+  static constexpr int kUmmaK = 32 / kElemBytes;    // rows per tcgen05.mma (32 bytes)
+  static constexpr int kTileRows = 2 * kBK;         // rows per block of the split pass (F16: one chunk)
+  static constexpr uint32_t kFmt = F16 ? 0u : 2u;   // instruction-descriptor operand format: 0 = F16, 2 = TF32
+  // Instruction descriptor: D fp32, A/B as kFmt, both K-major, N = 256, M = 128.
+  static constexpr uint32_t kIdesc = (1u << 4) | (kFmt << 7) | (kFmt << 10) | ((uint32_t)(kBN >> 3) << 17) |
+                                     ((uint32_t)(kBM >> 4) << 24);
+};
 
 // ---------------------------------------------------------------------------------------------------
 // PTX wrappers
@@ -61,17 +73,23 @@ __device__ __forceinline__ void tcgen05_commit(uint64_t* bar) {
   asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(smem_u32(bar))
                : "memory");
 }
-// D[tmem] (+)= A[smem desc] * B[smem desc]^T, kind::tf32, fp32 accumulate
-__device__ __forceinline__ void umma_tf32(uint32_t tmem_d, uint64_t desc_a, uint64_t desc_b, uint32_t idesc,
-                                          uint32_t accumulate) {
-  asm volatile(
-      "{\n"
-      ".reg .pred p;\n"
-      "setp.ne.b32 p, %4, 0;\n"
-      "tcgen05.mma.cta_group::1.kind::tf32 [%0], %1, %2, %3, p;\n"
-      "}\n" ::"r"(tmem_d),
-      "l"(desc_a), "l"(desc_b), "r"(idesc), "r"(accumulate)
-      : "memory");
+// D[tmem] (+)= A[smem desc] * B[smem desc]^T, fp32 accumulate
+template <bool F16>
+__device__ __forceinline__ void umma(uint32_t tmem_d, uint64_t desc_a, uint64_t desc_b, uint32_t idesc,
+                                     uint32_t accumulate) {
+  if constexpr (F16) {
+    asm volatile(
+        "{\n.reg .pred p;\nsetp.ne.b32 p, %4, 0;\n"
+        "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n}\n" ::"r"(tmem_d),
+        "l"(desc_a), "l"(desc_b), "r"(idesc), "r"(accumulate)
+        : "memory");
+  } else {
+    asm volatile(
+        "{\n.reg .pred p;\nsetp.ne.b32 p, %4, 0;\n"
+        "tcgen05.mma.cta_group::1.kind::tf32 [%0], %1, %2, %3, p;\n}\n" ::"r"(tmem_d),
+        "l"(desc_a), "l"(desc_b), "r"(idesc), "r"(accumulate)
+        : "memory");
+  }
 }
 __device__ __forceinline__ void tmem_ld_32x32b_x32(uint32_t taddr, uint32_t (&r)[32]) {
   asm volatile(
@@ -97,9 +115,6 @@ __device__ __forceinline__ uint64_t make_kmajor_sw128_desc(uint32_t smem_addr) {
   d |= (uint64_t)2 << 61;                        // layout type SWIZZLE_128B, bits [61,64)
   return d;
 }
-// Instruction descriptor: D fp32, A/B tf32, both K-major, N = 256, M = 128.
-constexpr uint32_t kIdesc = (1u << 4) | (2u << 7) | (2u << 10) | ((uint32_t)(kBN >> 3) << 17) |
-                            ((uint32_t)(kBM >> 4) << 24);
 
 __device__ __forceinline__ float to_tf32(float a) {
   uint32_t r;
@@ -108,50 +123,125 @@ __device__ __forceinline__ float to_tf32(float a) {
 }
 
 // ---------------------------------------------------------------------------------------------------
-// 1. split + transpose (+ A^T y).  Block: 32 features x 64 rows.
+// 1. split (+ scale) + transpose (+ partial A^T y).  Block: kTileRows rows x 128 features, 8 warps; a warp owns
+//    kTileRows/8 adjacent rows, a lane the features lane, lane+32, lane+64, lane+96 of the block (coalesced 128-byte
+//    loads whatever D is).  The hi/lo values of a feature for the warp's rows are 32 contiguous bytes of the output.
 // ---------------------------------------------------------------------------------------------------
+constexpr int kSplitColBytes = 256 + 16;  // shared-memory bytes per feature (two 128-byte k-blocks + pad: no conflicts)
+constexpr int kSplitSmem = 2 * kColBlock * kSplitColBytes;
+
+template <bool F16>
 __global__ void __launch_bounds__(256)
-split_transpose_kernel(const float* __restrict__ A, const float* __restrict__ y, long long rows, int D,
-                       long long R_pad, float* __restrict__ At_hi, float* __restrict__ At_lo,
-                       float* __restrict__ Zty) {
-  __shared__ float thi[64][33], tlo[64][33];
-  __shared__ float ysum[8][32];
+split_kernel(const float* __restrict__ A, const float* __restrict__ y, long long rows, int D,
+             uint8_t* __restrict__ At_hi, uint8_t* __restrict__ At_lo, float* __restrict__ inv_scale, int n_cb,
+             float* __restrict__ zty_part) {
+  using M = SplitMode<F16>;
+  constexpr int RPW = M::kTileRows / 8;   // rows per warp: 16 (F16) / 8 (TF32)
+  extern __shared__ __align__(16) uint8_t sm[];
+  __shared__ float red[8];
+  __shared__ float ysum[8][kColBlock];
+  uint8_t* sm_hi = sm;
+  uint8_t* sm_lo = sm + kColBlock * kSplitColBytes;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  const int i0 = blockIdx.x * 32;
-  const long long r0 = (long long)blockIdx.y * 64;
-  const int i = i0 + lane;
-  float zacc = 0.f;
+  const long long rb = blockIdx.x;
+  const int cb = blockIdx.y, c0 = cb * kColBlock;
+  const long long r0 = rb * M::kTileRows + warp * RPW;
+
+  float v[RPW][4];
+  float zacc[4] = {0.f, 0.f, 0.f, 0.f};
+  float amax = 0.f;
 #pragma unroll
-  for (int rr = warp; rr < 64; rr += 8) {
+  for (int rr = 0; rr < RPW; ++rr) {
     const long long r = r0 + rr;
-    float a = 0.f;
-    if (r < rows && i < D) a = __ldcs(A + (size_t)r * D + i);
-    const float hi = to_tf32(a);
-    const float lo = to_tf32(a - hi);
-    thi[rr][lane] = hi;
-    tlo[rr][lane] = lo;
-    if (y != nullptr && r < rows) zacc = fmaf(a, __ldg(y + r), zacc);
-  }
-  ysum[warp][lane] = zacc;
-  __syncthreads();
+    const float yv = (y != nullptr && r < rows) ? __ldg(y + r) : 0.f;
 #pragma unroll
-  for (int cc = 0; cc < 4; ++cc) {
-    const int c = warp * 4 + cc;
-    if (i0 + c < D) {
-      // k-block-major layout [R_pad/32][D][32]: the 128 features x 32 rows of one TMA box are 16 KB contiguous
-      const size_t o0 = ((size_t)(r0 / 32) * D + (i0 + c)) * 32, o1 = o0 + (size_t)D * 32;
-      At_hi[o0 + lane] = thi[lane][c];
-      At_hi[o1 + lane] = thi[lane + 32][c];
-      At_lo[o0 + lane] = tlo[lane][c];
-      At_lo[o1 + lane] = tlo[lane + 32][c];
+    for (int c = 0; c < 4; ++c) {
+      const int col = c0 + lane + 32 * c;
+      const float a = (r < rows && col < D) ? __ldcs(A + (size_t)r * D + col) : 0.f;
+      v[rr][c] = a;
+      amax = fmaxf(amax, fabsf(a));
+      zacc[c] = fmaf(a, yv, zacc[c]);
     }
   }
-  if (Zty != nullptr && y != nullptr && warp == 0 && i < D) {
-    float s = 0.f;
+  float s = 1.f;
+  if constexpr (F16) {
+    // one power-of-two scale per block: amax * s in [2^13, 2^14), undone exactly by the tcgen05 kernel's epilogue
 #pragma unroll
-    for (int w = 0; w < 8; ++w) s += ysum[w][lane];
-    atomicAdd(Zty + i, s);
+    for (int m = 16; m > 0; m >>= 1) amax = fmaxf(amax, __shfl_xor_sync(0xffffffffu, amax, m));
+    if (lane == 0) red[warp] = amax;
+    __syncthreads();
+    amax = red[0];
+#pragma unroll
+    for (int w = 1; w < 8; ++w) amax = fmaxf(amax, red[w]);
+    int e = (int)((__float_as_uint(amax) >> 23) & 0xffu) - 127;   // floor(log2 amax) for normal numbers
+    int sh = 13 - e;
+    if (amax == 0.f) sh = 0;
+    sh = sh < -100 ? -100 : (sh > 100 ? 100 : sh);
+    s = __uint_as_float((uint32_t)(127 + sh) << 23);
+    if (threadIdx.x == 0) inv_scale[rb * n_cb + cb] = __uint_as_float((uint32_t)(127 - sh) << 23);
   }
+#pragma unroll
+  for (int c = 0; c < 4; ++c) {
+    const int cl = lane + 32 * c;
+    uint4 h[2], l[2];
+    if constexpr (F16) {
+      __half hh[RPW], ll[RPW];
+#pragma unroll
+      for (int rr = 0; rr < RPW; ++rr) {
+        const float a = v[rr][c] * s;
+        hh[rr] = __float2half_rn(a);
+        ll[rr] = __float2half_rn(a - __half2float(hh[rr]));
+      }
+      memcpy(h, hh, 32);
+      memcpy(l, ll, 32);
+    } else {
+      float hh[RPW], ll[RPW];
+#pragma unroll
+      for (int rr = 0; rr < RPW; ++rr) {
+        hh[rr] = to_tf32(v[rr][c]);
+        ll[rr] = to_tf32(v[rr][c] - hh[rr]);
+      }
+      memcpy(h, hh, 32);
+      memcpy(l, ll, 32);
+    }
+    uint4* dh = reinterpret_cast<uint4*>(sm_hi + cl * kSplitColBytes + warp * 32);
+    uint4* dl = reinterpret_cast<uint4*>(sm_lo + cl * kSplitColBytes + warp * 32);
+    dh[0] = h[0]; dh[1] = h[1];
+    dl[0] = l[0]; dl[1] = l[1];
+    ysum[warp][cl] = zacc[c];
+  }
+  __syncthreads();
+  // k-block-major output [R_pad/BK][D][BK]: for one k-block the 128 features of this block are 16 KB contiguous
+  const int ncol = (D - c0 < kColBlock) ? D - c0 : kColBlock;
+#pragma unroll
+  for (int kb = 0; kb < 2; ++kb) {
+    const size_t obase = ((size_t)(rb * 2 + kb) * D + c0) * 128;
+#pragma unroll
+    for (int pass = 0; pass < 4; ++pass) {
+      const int piece = pass * 256 + threadIdx.x, cl = piece >> 3, part = piece & 7;
+      if (cl < ncol) {
+        const int so = cl * kSplitColBytes + kb * 128 + part * 16;
+        *reinterpret_cast<uint4*>(At_hi + obase + (size_t)piece * 16) = *reinterpret_cast<const uint4*>(sm_hi + so);
+        *reinterpret_cast<uint4*>(At_lo + obase + (size_t)piece * 16) = *reinterpret_cast<const uint4*>(sm_lo + so);
+      }
+    }
+  }
+  if (zty_part != nullptr && threadIdx.x < ncol) {
+    float t = 0.f;
+#pragma unroll
+    for (int w = 0; w < 8; ++w) t += ysum[w][threadIdx.x];
+    zty_part[(size_t)rb * D + c0 + threadIdx.x] = t;
+  }
+}
+
+// Zty[i] (+)= sum over row blocks of the partials, in fp64, fixed order: deterministic and independent of the grid.
+__global__ void __launch_bounds__(256)
+zty_reduce_kernel(const float* __restrict__ part, long long n_rb, int D, float* __restrict__ Zty, int accumulate) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= D) return;
+  double t = accumulate ? (double)Zty[i] : 0.0;
+  for (long long rb = 0; rb < n_rb; ++rb) t += (double)part[(size_t)rb * D + i];
+  Zty[i] = (float)t;
 }
 
 // ---------------------------------------------------------------------------------------------------
@@ -185,10 +275,13 @@ __host__ __device__ inline void tile_decode(int tile, int n_ti, int n_tj, int* t
   *tj_out = r1 - 1; *ti_out = 0;  // not reached for tile < n_tiles
 }
 
+template <bool F16>
 __global__ void __launch_bounds__(kSyrkThreads, 1)
 syrk_tcgen05_kernel(const __grid_constant__ CUtensorMap map_hi, const __grid_constant__ CUtensorMap map_lo,
-                    float* __restrict__ C, int D, int n_kb /* 32-row blocks in the panel */, int n_tiles,
-                    int first_store, int kb_per_chunk) {
+                    float* __restrict__ C, int D, int n_kb /* BK-row blocks in the panel */, int n_tiles,
+                    int first_store, const float* __restrict__ inv_scale /* [n_chunks][n_cb], F16 only */, int n_cb) {
+  using M = SplitMode<F16>;
+  constexpr int kb_per_chunk = kChunkRows / M::kBK;
   extern __shared__ uint8_t smem_raw[];
   uint8_t* smem = reinterpret_cast<uint8_t*>(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
   uint64_t* bars = reinterpret_cast<uint64_t*>(smem + kStages * kStageBytes);
@@ -233,7 +326,7 @@ syrk_tcgen05_kernel(const __grid_constant__ CUtensorMap map_hi, const __grid_con
           mbar_wait(&empty_bar[s], ph ^ 1);
           uint8_t* st = smem + s * kStageBytes;
           mbar_expect_tx(&full_bar[s], kStageBytes);
-          // tensor = [n_kb * D][32]: box row index = kb * D + feature.  Features past D alias the next k-block
+          // tensor = [n_kb * D][BK]: box row index = kb * D + feature.  Features past D alias the next k-block
           // (finite values; those accumulator rows / columns are masked at the store), past the end TMA fills zeros.
           const int base = kb * D;
           tma_load_2d(st, &map_hi, &full_bar[s], 0, base + I0);
@@ -266,12 +359,12 @@ syrk_tcgen05_kernel(const __grid_constant__ CUtensorMap map_hi, const __grid_con
             const uint64_t b_hi = make_kmajor_sw128_desc(base + 2 * kTileABytes);
             const uint64_t b_lo = make_kmajor_sw128_desc(base + 2 * kTileABytes + kTileBBytes);
 #pragma unroll
-            for (int kk = 0; kk < kBK / kUmmaK; ++kk) {
-              const uint64_t adv = (uint64_t)((kk * kUmmaK * 4) >> 4);  // +32 bytes per K step, in 16 B units
+            for (int kk = 0; kk < M::kBK / M::kUmmaK; ++kk) {
+              const uint64_t adv = (uint64_t)((kk * 32) >> 4);  // +32 bytes per K step, in 16 B units
               const uint32_t acc0 = (kb > ch * kb_per_chunk || kk > 0) ? 1u : 0u;
-              umma_tf32(tmem_d, a_lo + adv, b_hi + adv, kIdesc, acc0);   // small terms first
-              umma_tf32(tmem_d, a_hi + adv, b_lo + adv, kIdesc, 1u);
-              umma_tf32(tmem_d, a_hi + adv, b_hi + adv, kIdesc, 1u);
+              umma<F16>(tmem_d, a_lo + adv, b_hi + adv, M::kIdesc, acc0);   // small terms first
+              umma<F16>(tmem_d, a_hi + adv, b_lo + adv, M::kIdesc, 1u);
+              umma<F16>(tmem_d, a_hi + adv, b_hi + adv, M::kIdesc, 1u);
             }
             tcgen05_commit(&empty_bar[s]);  // smem stage reusable once these MMAs have read it
           }
@@ -282,8 +375,8 @@ syrk_tcgen05_kernel(const __grid_constant__ CUtensorMap map_hi, const __grid_con
   } else {
     // ===================== epilogue warps 2..9 =====================
     // Two warps per TMEM lane quarter; each owns half of the 256 accumulator columns.  Chunk partials are summed
-    // in REGISTERS (128 fp32 per thread, round-to-nearest) so that draining TMEM every few hundred rows costs only
-    // tcgen05.ld + FADD; C is touched once per tile.
+    // in REGISTERS (128 fp32 per thread, round-to-nearest) so that draining TMEM every 128 rows costs only
+    // tcgen05.ld + FADD (FFMA with the chunk's power-of-two scale in fp16 mode); C is touched once per tile.
     const int quarter = warp & 3;  // TMEM lanes [32 q, 32 q + 32) are the ones this warp may read
     const int chalf = (warp - 2) >> 2;  // 0: columns [0,128), 1: columns [128,256)
     const int i_loc = quarter * 32 + lane;
@@ -293,10 +386,14 @@ syrk_tcgen05_kernel(const __grid_constant__ CUtensorMap map_hi, const __grid_con
       tile_decode(tile, n_ti, n_tj, &tj, &rem);
       const int I0 = rem * kBM, J0 = tj * kBN + chalf * 128;
       const int col = I0 + i_loc;  // column of C this thread writes (transposed store)
+      const int cbI = rem, cbJ = 2 * tj + chalf;  // 128-column blocks of the two operands
       float acc[128];
 #pragma unroll
       for (int j = 0; j < 128; ++j) acc[j] = 0.f;
       for (int ch = 0; ch < n_chunks; ++ch, ++item) {
+        float f = 1.f;
+        if constexpr (F16)
+          f = __ldg(inv_scale + (size_t)ch * n_cb + cbI) * (cbJ < n_cb ? __ldg(inv_scale + (size_t)ch * n_cb + cbJ) : 1.f);
         const uint32_t buf = item & 1, tph = (item >> 1) & 1;
         mbar_wait(&tfull_bar[buf], tph);
         tcgen05_fence_after();
@@ -307,7 +404,10 @@ syrk_tcgen05_kernel(const __grid_constant__ CUtensorMap map_hi, const __grid_con
           tmem_ld_32x32b_x32(taddr + c0, r);
           tmem_ld_wait();
 #pragma unroll
-          for (int jj = 0; jj < 32; ++jj) acc[c0 + jj] += __uint_as_float(r[jj]);
+          for (int jj = 0; jj < 32; ++jj) {
+            if constexpr (F16) acc[c0 + jj] = fmaf(__uint_as_float(r[jj]), f, acc[c0 + jj]);
+            else acc[c0 + jj] += __uint_as_float(r[jj]);
+          }
         }
         tcgen05_fence_before();  // all TMEM reads of this warp are done: hand the accumulator back
         __syncwarp();
@@ -378,17 +478,19 @@ static EncodeTiledFn get_encode_fn() {
   return fn;
 }
 
-// At [D, R_pad] fp32, inner (contiguous) dimension = rows.  Box = 32 rows x 128 features, SWIZZLE_128B.
-static int make_map(CUtensorMap* map, float* base, int D, long long R_pad) {
+// At as [n_kb * D][BK] elements, inner (contiguous) dimension = the BK rows of a k-block (128 bytes).
+// Box = BK rows x 128 features, SWIZZLE_128B.
+static int make_map(CUtensorMap* map, void* base, int D, long long n_kb, bool f16) {
   EncodeTiledFn fn = get_encode_fn();
   if (!fn) return QMLL_ERR_CUDA;
-  cuuint64_t dims[2] = {(cuuint64_t)kBK, (cuuint64_t)D * (cuuint64_t)(R_pad / kBK)};
-  cuuint64_t strides[1] = {(cuuint64_t)kBK * sizeof(float)};
-  cuuint32_t box[2] = {(cuuint32_t)kBK, 128u};
+  const cuuint32_t bk = f16 ? 64u : 32u;
+  cuuint64_t dims[2] = {(cuuint64_t)bk, (cuuint64_t)D * (cuuint64_t)n_kb};
+  cuuint64_t strides[1] = {128};
+  cuuint32_t box[2] = {bk, 128u};
   cuuint32_t estr[2] = {1u, 1u};
-  CUresult r = fn(map, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, base, dims, strides, box, estr,
-                  CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
-                  CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  CUresult r = fn(map, f16 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT16 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, base, dims, strides,
+                  box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
+                  CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
   if (r != CUDA_SUCCESS) {
     note_cuda_error(cudaErrorInvalidValue, "cuTensorMapEncodeTiled");
     return QMLL_ERR_CUDA;
@@ -397,12 +499,17 @@ static int make_map(CUtensorMap* map, float* base, int D, long long R_pad) {
 }
 
 // Optional per-launch timing of the tcgen05 kernel (bench.py's roofline): events on the caller's stream.
+static std::mutex g_timing_mutex;
 static bool g_timing = false;
 struct TimedLaunch { cudaEvent_t a, b; };
 static TimedLaunch g_timed[4096];
 static int g_n_timed = 0;
-void syrk_set_timing(bool on) { g_timing = on; }
+void syrk_set_timing(bool on) {
+  std::lock_guard<std::mutex> lock(g_timing_mutex);
+  g_timing = on;
+}
 int syrk_collect_timing(double* total_ms, int* launches) {
+  std::lock_guard<std::mutex> lock(g_timing_mutex);
   double tot = 0.0;
   for (int i = 0; i < g_n_timed; ++i) {
     float ms = 0.f;
@@ -418,62 +525,98 @@ int syrk_collect_timing(double* total_ms, int* launches) {
   return QMLL_OK;
 }
 
-static long long pad_rows(long long r) { return (r + kRowPad - 1) / kRowPad * kRowPad; }
-
-size_t syrk_min_workspace(int32_t D) { return (size_t)2 * D * kChunkRows * sizeof(float) + 1024; }
-size_t syrk_full_workspace(int64_t rows, int32_t D) {
-  long long rp = pad_rows(rows < 1 ? 1 : rows);
-  if (rp < kChunkRows) rp = kChunkRows;
-  return (size_t)2 * D * rp * sizeof(float) + 1024;
+// Workspace layout of one panel of `rp` padded rows:  At_hi | At_lo | inv_scale [rp/128][n_cb] | zty_part [n_rb][D]
+struct PanelLayout {
+  size_t op_bytes, scale_bytes, part_bytes;
+  size_t total() const { return 2 * op_bytes + scale_bytes + part_bytes + 4 * 256; }
+};
+static long long tile_rows(int mode) { return mode == QMLL_NE_SPLIT_F16 ? 128 : 64; }
+static long long pad_rows(long long r, int mode) { return (r + tile_rows(mode) - 1) / tile_rows(mode) * tile_rows(mode); }
+static PanelLayout panel_layout(long long rp, int D, int mode) {
+  const int eb = mode == QMLL_NE_SPLIT_F16 ? 2 : 4;
+  const int n_cb = (D + kColBlock - 1) / kColBlock;
+  PanelLayout l;
+  l.op_bytes = align_up((size_t)D * rp * eb, 256);
+  l.scale_bytes = align_up((size_t)((rp + kChunkRows - 1) / kChunkRows) * n_cb * sizeof(float), 256);
+  l.part_bytes = align_up((size_t)(rp / tile_rows(mode)) * D * sizeof(float), 256);
+  return l;
 }
 
-int syrk_normal_equations(const float* A, const float* y, int64_t rows, int32_t D, int accumulate, float* ZtZ,
-                          float* Zty, void* ws, size_t ws_bytes, cudaStream_t st) {
-  if (!accumulate) {
-    if (Zty) QMLL_CUDA_TRY(cudaMemsetAsync(Zty, 0, (size_t)D * sizeof(float), st));
-    if (rows == 0) QMLL_CUDA_TRY(cudaMemsetAsync(ZtZ, 0, (size_t)D * D * sizeof(float), st));
+size_t syrk_min_workspace(int32_t D, int mode) { return panel_layout(kPanelRows, D, mode).total(); }
+size_t syrk_full_workspace(int64_t rows, int32_t D, int mode) {
+  long long rp = pad_rows(rows < 1 ? 1 : rows, mode);
+  if (rp < kPanelRows) rp = kPanelRows;
+  return panel_layout(rp, D, mode).total();
+}
+
+template <bool F16>
+static int syrk_impl(const float* A, const float* y, int64_t rows, int32_t D, int accumulate, float* ZtZ, float* Zty,
+                     void* ws, size_t ws_bytes, cudaStream_t st) {
+  using M = SplitMode<F16>;
+  constexpr int mode = F16 ? QMLL_NE_SPLIT_F16 : QMLL_NE_SPLIT_TF32;
+  // rows per panel: as many as the workspace holds, a multiple of kPanelRows unless everything fits
+  long long panel = pad_rows(rows, mode);
+  if (panel_layout(panel, D, mode).total() > ws_bytes) {
+    const size_t per_row = (size_t)2 * D * M::kElemBytes + (size_t)D * sizeof(float) / M::kTileRows +
+                           (size_t)((D + kColBlock - 1) / kColBlock) * sizeof(float) / kChunkRows + 1;
+    panel = (long long)((ws_bytes > 4096 ? ws_bytes - 4096 : 0) / per_row) / kPanelRows * kPanelRows;
+    while (panel >= kPanelRows && panel_layout(panel, D, mode).total() > ws_bytes) panel -= kPanelRows;
+    if (panel < kPanelRows) return QMLL_ERR_WORKSPACE;
   }
-  if (rows == 0) return QMLL_OK;
-  if (ws == nullptr || ((uintptr_t)ws & 255) != 0) return QMLL_ERR_WORKSPACE;
-  // rows per panel: as many as the workspace holds (two [D, R_pad] fp32 arrays), a multiple of the chunk
-  long long cap = (long long)((ws_bytes > 1024 ? ws_bytes - 1024 : 0) / ((size_t)2 * D * sizeof(float)));
-  long long panel = pad_rows(rows);
-  if (cap < panel) {
-    panel = cap / kChunkRows * kChunkRows;
-    if (panel < kChunkRows) return QMLL_ERR_WORKSPACE;
-  }
-  float* At_hi = static_cast<float*>(ws);
-  float* At_lo = At_hi + (size_t)D * panel;
+  // the split pass puts row blocks on grid.x (2^31-1 blocks), feature blocks on grid.y (D <= 65535 * 128)
+  const int n_cb = (D + kColBlock - 1) / kColBlock;
+  if (n_cb > 65535) return QMLL_ERR_UNSUPPORTED;
+  const PanelLayout lay = panel_layout(panel, D, mode);
+  Carver carve(ws, ws_bytes);
+  uint8_t* At_hi = carve.take<uint8_t>(lay.op_bytes);
+  uint8_t* At_lo = carve.take<uint8_t>(lay.op_bytes);
+  float* inv_scale = carve.take<float>(lay.scale_bytes / sizeof(float));
+  float* zty_part = carve.take<float>(lay.part_bytes / sizeof(float));
+  if (!carve.fits()) return QMLL_ERR_WORKSPACE;
 
   const int n_ti = (D + kBM - 1) / kBM, n_tj = (D + kBN - 1) / kBN;
   int n_tiles = 0;
   for (int tj = 0; tj < n_tj; ++tj) n_tiles += tiles_in_row(tj, n_ti);
   const int grid = n_tiles < device_sm_count() ? n_tiles : device_sm_count();
-  QMLL_CUDA_TRY(cudaFuncSetAttribute(syrk_tcgen05_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+  QMLL_CUDA_TRY(cudaFuncSetAttribute(syrk_tcgen05_kernel<F16>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                      (int)kSmemBytes));
+  QMLL_CUDA_TRY(cudaFuncSetAttribute(split_kernel<F16>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSplitSmem));
   int first_store = accumulate ? 0 : 1;
+  int zty_acc = accumulate ? 1 : 0;
   for (int64_t r0 = 0; r0 < rows; r0 += panel) {
     const long long pr = (rows - r0 < panel) ? rows - r0 : panel;
-    const long long rp = pad_rows(pr);
-    dim3 g1((unsigned)((D + 31) / 32), (unsigned)(rp / 64));
-    split_transpose_kernel<<<g1, 256, 0, st>>>(A + (size_t)r0 * D, y ? y + r0 : nullptr, pr, D, rp, At_hi, At_lo,
-                                              Zty);
-    QMLL_LAUNCH_CHECK("split_transpose_kernel");
-    CUtensorMap map_hi, map_lo;
-    int rc = make_map(&map_hi, At_hi, D, rp);
-    if (rc != QMLL_OK) return rc;
-    rc = make_map(&map_lo, At_lo, D, rp);
-    if (rc != QMLL_OK) return rc;
-    const bool timed = g_timing && g_n_timed < 4096;
-    if (timed) {
-      QMLL_CUDA_TRY(cudaEventCreate(&g_timed[g_n_timed].a));
-      QMLL_CUDA_TRY(cudaEventCreate(&g_timed[g_n_timed].b));
-      QMLL_CUDA_TRY(cudaEventRecord(g_timed[g_n_timed].a, st));
+    const long long rp = pad_rows(pr, mode);
+    const long long n_rb = rp / M::kTileRows;
+    dim3 g1((unsigned)n_rb, (unsigned)n_cb);
+    split_kernel<F16><<<g1, 256, kSplitSmem, st>>>(A + (size_t)r0 * D, y ? y + r0 : nullptr, pr, D, At_hi, At_lo,
+                                                  inv_scale, n_cb, (y && Zty) ? zty_part : nullptr);
+    QMLL_LAUNCH_CHECK("split_kernel");
+    if (y && Zty) {
+      zty_reduce_kernel<<<(D + 255) / 256, 256, 0, st>>>(zty_part, n_rb, D, Zty, zty_acc);
+      QMLL_LAUNCH_CHECK("zty_reduce_kernel");
+      zty_acc = 1;
     }
-    syrk_tcgen05_kernel<<<grid, kSyrkThreads, kSmemBytes, st>>>(map_hi, map_lo, ZtZ, D, (int)(rp / kBK), n_tiles,
-                                                              first_store, chunk_rows() / kBK);
+    CUtensorMap map_hi, map_lo;
+    const long long n_kb = rp / M::kBK;
+    int rc = make_map(&map_hi, At_hi, D, n_kb, F16);
+    if (rc != QMLL_OK) return rc;
+    rc = make_map(&map_lo, At_lo, D, n_kb, F16);
+    if (rc != QMLL_OK) return rc;
+    bool timed = false;
+    {
+      std::lock_guard<std::mutex> lock(g_timing_mutex);
+      timed = g_timing && g_n_timed < 4096;
+      if (timed) {
+        QMLL_CUDA_TRY(cudaEventCreate(&g_timed[g_n_timed].a));
+        QMLL_CUDA_TRY(cudaEventCreate(&g_timed[g_n_timed].b));
+        QMLL_CUDA_TRY(cudaEventRecord(g_timed[g_n_timed].a, st));
+      }
+    }
+    syrk_tcgen05_kernel<F16><<<grid, kSyrkThreads, kSmemBytes, st>>>(map_hi, map_lo, ZtZ, D, (int)n_kb, n_tiles,
+                                                                     first_store, inv_scale, n_cb);
     QMLL_LAUNCH_CHECK("syrk_tcgen05_kernel");
     if (timed) {
+      std::lock_guard<std::mutex> lock(g_timing_mutex);
       QMLL_CUDA_TRY(cudaEventRecord(g_timed[g_n_timed].b, st));
       ++g_n_timed;
     }
@@ -483,6 +626,18 @@ int syrk_normal_equations(const float* A, const float* y, int64_t rows, int32_t 
   mirror_lower_kernel<<<g3, 256, 0, st>>>(ZtZ, D);
   QMLL_LAUNCH_CHECK("mirror_lower_kernel");
   return QMLL_OK;
+}
+
+int syrk_normal_equations(const float* A, const float* y, int64_t rows, int32_t D, int accumulate, float* ZtZ,
+                          float* Zty, void* ws, size_t ws_bytes, int mode, cudaStream_t st) {
+  if (!accumulate) {
+    if (Zty) QMLL_CUDA_TRY(cudaMemsetAsync(Zty, 0, (size_t)D * sizeof(float), st));
+    if (rows == 0) QMLL_CUDA_TRY(cudaMemsetAsync(ZtZ, 0, (size_t)D * D * sizeof(float), st));
+  }
+  if (rows == 0) return QMLL_OK;
+  if (ws == nullptr || ((uintptr_t)ws & 255) != 0) return QMLL_ERR_WORKSPACE;
+  if (mode == QMLL_NE_SPLIT_F16) return syrk_impl<true>(A, y, rows, D, accumulate, ZtZ, Zty, ws, ws_bytes, st);
+  return syrk_impl<false>(A, y, rows, D, accumulate, ZtZ, Zty, ws, ws_bytes, st);
 }
 
 }  // namespace qmll

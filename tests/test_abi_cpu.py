@@ -18,9 +18,14 @@ def lib():
 
 
 def declared_symbols():
-    text = open(os.path.join(ROOT, "include", "qmll.h")).read()
-    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
-    return sorted(set(re.findall(r"\b(qmll_[a-z_0-9]+)\s*\(", text)))
+    names = set()
+    inc = os.path.join(ROOT, "include")
+    for h in sorted(os.listdir(inc)):
+        if h.endswith(".h"):
+            text = open(os.path.join(inc, h)).read()
+            text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+            names |= set(re.findall(r"\b(qmll_[a-z_0-9]+)\s*\(", text))
+    return sorted(names)
 
 
 def test_header_symbols_are_exported(lib):
@@ -49,8 +54,10 @@ def test_workspace_arithmetic(lib):
     assert fwdg - fwd >= 21000 * 8192 * 4                        # per-atom sin table for the force rows
     assert pred >= fwd + 21000 * 128 * 4 + 1000 * 8
     ne = l.qmll_workspace_bytes(pkg.CALL_NORMAL_EQUATIONS, ctypes.byref(p), 0, 0, 64000)
-    assert ne >= 2 * 8192 * 64000 * 4
+    assert ne >= 2 * 8192 * 64000 * 2                            # fp16 hi + lo copies of A^T
     assert 0 < l.qmll_normal_equations_min_workspace(8192) <= ne
+    assert l.qmll_normal_equations_workspace(64000, 8192, pkg.NE_SPLIT_TF32) >= 2 * 8192 * 64000 * 4
+    assert l.qmll_normal_equations_workspace(64000, 8192, 7) == 0
     bad = pkg._CParams(100, 8192, 3, 5, 8.0, None, None)          # d not a power of two
     assert l.qmll_workspace_bytes(pkg.CALL_FORWARD, ctypes.byref(bad), 10, 1, 0) == 0
 
@@ -60,6 +67,7 @@ def test_host_side_argument_checks_need_no_gpu(lib):
     # null parameter struct / invalid sizes are rejected before any CUDA call
     assert l.qmll_sorf_forward(None, None, None, None, 0, 0, None, None, None, None, 0, None) == -1
     assert l.qmll_normal_equations(None, None, -1, 256, 0, None, None, None, 0, None) == -1
+    assert l.qmll_normal_equations_mode(None, None, 4, 256, 0, None, None, None, 0, 9, None) == -1
     assert l.qmll_predict(None, None, None, None, 0, 0, None, None, None, None, None, 0, None) == -1
     assert l.qmll_sorf_backward_forces(None, None, None, None, 0, 0, None, None, None, None, 0, None) == -1
 

@@ -123,15 +123,16 @@ def test_empty_inputs(q):
     assert float(E.abs().max()) == 0.0
 
 
-@pytest.mark.parametrize("rows,D", [(1, 256), (777, 384), (1500, 128), (2500, 520), (4096, 1024)])
-def test_normal_equations_shapes(q, rows, D):
+@pytest.mark.parametrize("mode", [0, 1])      # QMLL_NE_SPLIT_F16, QMLL_NE_SPLIT_TF32
+@pytest.mark.parametrize("rows,D", [(1, 256), (777, 384), (1500, 128), (2500, 520), (4096, 1024), (300, 451), (130, 7)])
+def test_normal_equations_shapes(q, rows, D, mode):
     pkg, wio, torch = q
     rng = np.random.default_rng(rows + D)
     # correlated, non-zero-mean rows (like Z of near-identical molecules): the hard case for fp32 accumulation
     A = (0.7 + 0.3 * rng.standard_normal((rows, D))).astype(np.float32)
     y = rng.standard_normal(rows).astype(np.float32)
     Ad, yd = torch.from_numpy(A).cuda(), torch.from_numpy(y).cuda()
-    ZtZ, Zty = pkg.qmll_normal_equations(Ad, yd)
+    ZtZ, Zty = pkg.qmll_normal_equations(Ad, yd, mode=mode)
     ZtZo, Ztyo = oracle.normal_equations(A, y)
     assert rel(ZtZ.cpu().numpy(), ZtZo) <= TOL
     assert rel(Zty.cpu().numpy(), Ztyo) <= TOL
@@ -139,12 +140,37 @@ def test_normal_equations_shapes(q, rows, D):
     B = rng.standard_normal((rows, D)).astype(np.float32)
     yb = rng.standard_normal(rows).astype(np.float32)
     pkg.qmll_normal_equations(torch.from_numpy(B).cuda(), torch.from_numpy(yb).cuda(), ZtZ=ZtZ, Zty=Zty,
-                              accumulate=True, workspace_limit=0)
+                              accumulate=True, workspace_limit=0, mode=mode)
     ZtZo2, Ztyo2 = oracle.normal_equations(B, yb)
     Zn = ZtZ.cpu().numpy()
     assert rel(Zn, ZtZo + ZtZo2) <= TOL
     assert rel(Zty.cpu().numpy(), Ztyo + Ztyo2) <= TOL
     assert np.array_equal(Zn, Zn.T)
+
+
+def test_normal_equations_wide_dynamic_range(q):
+    """Rows whose magnitudes differ by 2^40 and columns by 2^20 (energy rows next to tiny force rows): the fp16
+    container's per-(chunk, column block) power-of-two scales must keep the relative Frobenius accuracy."""
+    pkg, wio, torch = q
+    rng = np.random.default_rng(99)
+    rows, D = 1000, 512
+    A = rng.standard_normal((rows, D))
+    A *= np.exp2(rng.integers(-20, 20, size=(rows // 125, 1)).repeat(125, axis=0))   # per 125-row group (straddles chunks)
+    A *= np.exp2(rng.integers(-10, 10, size=(1, D)))
+    A = A.astype(np.float32)
+    y = rng.standard_normal(rows).astype(np.float32)
+    ZtZo, Ztyo = oracle.normal_equations(A, y)
+    for mode in (0, 1):
+        ZtZ, Zty = pkg.qmll_normal_equations(torch.from_numpy(A).cuda(), torch.from_numpy(y).cuda(), mode=mode)
+        assert rel(ZtZ.cpu().numpy(), ZtZo) <= TOL
+        assert rel(Zty.cpu().numpy(), Ztyo) <= TOL
+    # every 128 x 128 block of the result individually (the scales are per block)
+    Zn = ZtZ.cpu().numpy()
+    ZtZ16, _ = pkg.qmll_normal_equations(torch.from_numpy(A).cuda(), torch.from_numpy(y).cuda(), mode=0)
+    Z16 = ZtZ16.cpu().numpy()
+    for i in range(0, D, 128):
+        for j in range(0, D, 128):
+            assert rel(Z16[i:i + 128, j:j + 128], ZtZo[i:i + 128, j:j + 128]) <= TOL
 
 
 def test_normal_equations_zero_rows(q):
@@ -168,7 +194,7 @@ def test_error_codes(q):
         pkg.qmll_sorf_forward(bad2, dp.x, dp.elem, dp.mol_off)
 
 
-@pytest.mark.parametrize("D,rows", [(1, 4), (50, 300), (256, 448), (1000, 3000)])
+@pytest.mark.parametrize("D,rows", [(1, 4), (50, 300), (256, 448), (1000, 3000), (4096, 6000)])
 def test_solve_matches_oracle(q, D, rows):
     """qmll_solve (blocked FP64 Cholesky) against the oracle's unblocked one on the same fp32 ZtZ / Zty."""
     pkg, wio, torch = q
