@@ -557,9 +557,8 @@ static int syrk_impl(const float* A, const float* y, int64_t rows, int32_t D, in
   // rows per panel: as many as the workspace holds, a multiple of kPanelRows unless everything fits
   long long panel = pad_rows(rows, mode);
   if (panel_layout(panel, D, mode).total() > ws_bytes) {
-    const size_t per_row = (size_t)2 * D * M::kElemBytes + (size_t)D * sizeof(float) / M::kTileRows +
-                           (size_t)((D + kColBlock - 1) / kColBlock) * sizeof(float) / kChunkRows + 1;
-    panel = (long long)((ws_bytes > 4096 ? ws_bytes - 4096 : 0) / per_row) / kPanelRows * kPanelRows;
+    const size_t per_row = (size_t)2 * D * M::kElemBytes;   // lower bound of the bytes one more row costs
+    panel = (long long)(ws_bytes / per_row) / kPanelRows * kPanelRows + kPanelRows;
     while (panel >= kPanelRows && panel_layout(panel, D, mode).total() > ws_bytes) panel -= kPanelRows;
     if (panel < kPanelRows) return QMLL_ERR_WORKSPACE;
   }
