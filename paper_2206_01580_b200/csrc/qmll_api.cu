@@ -62,18 +62,10 @@ static int check_ws(void* ws, size_t have, size_t need) {
 }
 
 static size_t zs_bytes(const qmll_sorf_params* p, int64_t n_atoms) {
-  return align_up((size_t)n_atoms * p->D * sizeof(float), 256) + 256;
+  return align_up(sorf_zs_floats(p, n_atoms) * sizeof(float), 256) + 256;
 }
-static size_t g_bytes(const qmll_sorf_params* p, int64_t n_atoms) {
-  return align_up((size_t)n_atoms * p->d * sizeof(float), 256) + 256;
-}
+static size_t grp_bytes(int32_t n_mol) { return align_up(((size_t)n_mol + 1) * sizeof(int32_t), 256) + 256; }
 static size_t e_bytes(int32_t n_mol) { return align_up((size_t)n_mol * sizeof(double), 256) + 256; }
-
-static int contract(const qmll_grad* grad, const float* g, const SorfProblem& pr, float* forces, cudaStream_t st) {
-  if (grad->layout == QMLL_GRAD_DENSE)
-    return contract_dense(g, pr.mol_off, pr.n_mol, pr.n_atoms, pr.p->d, grad->dense, grad->dense_off, forces, st);
-  return contract_neighbor(g, pr.n_atoms, pr.p->d, grad->K, grad->nbr_idx, grad->nbr_val, forces, st);
-}
 
 // shared body of qmll_sorf_backward_forces and qmll_predict
 static int backward_impl(const qmll_sorf_params* p, const float* x, const int32_t* elem, const int32_t* mol_off,
@@ -96,15 +88,14 @@ static int backward_impl(const qmll_sorf_params* p, const float* x, const int32_
   SorfTables t;
   rc = sorf_prepare_tables(p, alpha, ws, &t, st);
   if (rc) return rc;
-  float* g = forces ? ws.take<float>((size_t)n_atoms * p->d) : nullptr;
   double* eacc = energies ? ws.take<double>((size_t)n_mol) : nullptr;
   if (!ws.fits()) return QMLL_ERR_WORKSPACE;
   if (eacc && n_mol > 0) QMLL_CUDA_TRY(cudaMemsetAsync(eacc, 0, (size_t)n_mol * sizeof(double), st));
+  if (forces && n_atoms > 0) QMLL_CUDA_TRY(cudaMemsetAsync(forces, 0, (size_t)n_atoms * 3 * sizeof(float), st));
   SorfProblem pr{p, x, elem, mol_off, n_atoms, n_mol};
-  rc = sorf_launch_backward(pr, t, g, eacc, st);
+  rc = sorf_launch_predict(pr, t, forces ? grad : nullptr, forces, eacc, st);
   if (rc) return rc;
   if (energies) { rc = sorf_finish_energies(eacc, energies, n_mol, st); if (rc) return rc; }
-  if (forces) { rc = contract(grad, g, pr, forces, st); if (rc) return rc; }
   return QMLL_OK;
 }
 
@@ -135,9 +126,10 @@ size_t qmll_workspace_bytes(int which_call, const qmll_sorf_params* p, int64_t n
   switch (which_call) {
     case QMLL_CALL_FORWARD: return sorf_tables_bytes(p, false);
     case QMLL_CALL_FORWARD_GRAD:
-      return sorf_tables_bytes(p, false) + zs_bytes(p, n_atoms) + align_up((size_t)(rows > 0 ? rows : 0) * 4, 256) + 256;
-    case QMLL_CALL_BACKWARD_FORCES: return sorf_tables_bytes(p, true) + g_bytes(p, n_atoms);
-    case QMLL_CALL_PREDICT: return sorf_tables_bytes(p, true) + g_bytes(p, n_atoms) + e_bytes(n_mol);
+      return sorf_tables_bytes(p, false) + zs_bytes(p, n_atoms) + grp_bytes(n_mol) +
+             align_up((size_t)(rows > 0 ? rows : 0) * 4, 256) + 256;
+    case QMLL_CALL_BACKWARD_FORCES: return sorf_tables_bytes(p, true);
+    case QMLL_CALL_PREDICT: return sorf_tables_bytes(p, true) + e_bytes(n_mol);
     default: return 0;
   }
 }
@@ -163,7 +155,7 @@ int qmll_sorf_forward(const qmll_sorf_params* p, const float* x, const int32_t* 
   SorfTables t;
   rc = sorf_prepare_tables(p, nullptr, ws, &t, st);
   if (rc) return rc;
-  float* zs = grad ? ws.take<float>((size_t)n_atoms * p->D) : nullptr;
+  float* zs = grad ? ws.take<float>(sorf_zs_floats(p, n_atoms)) : nullptr;
   if (!ws.fits()) return QMLL_ERR_WORKSPACE;
   SorfProblem pr{p, x, elem, mol_off, n_atoms, n_mol};
   rc = sorf_launch_forward(pr, t, Z, zs, st);
@@ -171,10 +163,11 @@ int qmll_sorf_forward(const qmll_sorf_params* p, const float* x, const int32_t* 
   if (grad) {
     if (grad->layout == QMLL_GRAD_DENSE) {
       float* gt = ws.take<float>((size_t)grad->dense_floats);
+      int32_t* grp_off = ws.take<int32_t>((size_t)n_mol + 1);
       if (!ws.fits()) return QMLL_ERR_WORKSPACE;
       rc = sorf_transpose_dense(pr, grad->dense, grad->dense_off, gt, st);
       if (rc) return rc;
-      rc = sorf_launch_force_rows_dense(pr, t, zs, gt, grad->dense_off, G, st);
+      rc = sorf_launch_force_rows_dense(pr, t, zs, gt, grad->dense_off, grp_off, G, st);
     }
     else
       rc = sorf_launch_force_rows_neighbor(pr, t, zs, grad->nbr_idx, grad->nbr_val, grad->K, G, st);

@@ -62,21 +62,23 @@ struct SorfProblem {
   int32_t n_mol;
 };
 
-// Permuted / packed copies of the model tables living in the workspace (layouts in sorf_kernels.cu).
+// Lane-ordered copies of the model tables living in the workspace (layouts in sorf_device.cuh).
 struct SorfTables {
-  uint32_t* sign_bits;  // [E][T][EW][n_s*P]
-  float* bias_rev;      // [E][Ereg/4][n_s*P][4]   bias / (2 pi)
-  float* alpha_s;       // [Ereg/4][n_s*P][4]      alpha * sqrt(2/D)   (may be unused)
+  uint32_t* sign_bits;  // [n_elem][T][n_sg][EW][32]
+  float* bias_t;        // [n_elem][n_sg][E/4][32][4]   bias (radians)
+  float* alpha_s;       // [n_sg][E/4][32][4]           alpha * sqrt(2/D)   (may be unused)
 };
 
 size_t sorf_tables_bytes(const qmll_sorf_params* p, bool with_alpha);
 int sorf_prepare_tables(const qmll_sorf_params* p, const float* alpha, Carver& ws, SorfTables* t,
                         cudaStream_t st);
 int sorf_launch_forward(const SorfProblem& pr, const SorfTables& t, float* Z, float* zs_out, cudaStream_t st);
-int sorf_launch_backward(const SorfProblem& pr, const SorfTables& t, float* g_out, double* energy_acc,
-                         cudaStream_t st);
+int sorf_launch_predict(const SorfProblem& pr, const SorfTables& t, const qmll_grad* grad, float* forces,
+                        double* energy_acc, cudaStream_t st);
 int sorf_launch_force_rows_dense(const SorfProblem& pr, const SorfTables& t, const float* zs,
-                                 const float* dense, const int64_t* dense_off, float* G, cudaStream_t st);
+                                 const float* dense_t, const int64_t* dense_off, int32_t* grp_off, float* G,
+                                 cudaStream_t st);
+size_t sorf_zs_floats(const qmll_sorf_params* p, int64_t n_atoms);
 int sorf_launch_force_rows_neighbor(const SorfProblem& pr, const SorfTables& t, const float* zs,
                                     const int32_t* nbr_idx, const float* nbr_val, int K, float* G,
                                     cudaStream_t st);
@@ -84,12 +86,6 @@ int sorf_transpose_dense(const SorfProblem& pr, const float* dense, const int64_
                          cudaStream_t st);
 int sorf_finish_energies(const double* energy_acc, float* energies, int32_t n_mol, cudaStream_t st);
 bool sorf_supported_d(int d);
-
-// ---- gradient contraction (contract_kernels.cu) ------------------------------------------------------
-int contract_dense(const float* g, const int32_t* mol_off, int32_t n_mol, int64_t n_atoms, int d,
-                   const float* dense, const int64_t* dense_off, float* forces, cudaStream_t st);
-int contract_neighbor(const float* g, int64_t n_atoms, int d, int K, const int32_t* nbr_idx,
-                      const float* nbr_val, float* forces, cudaStream_t st);
 
 // ---- normal equations (syrk_tcgen05.cu) ----------------------------------------------------------------
 size_t syrk_min_workspace(int32_t D, int mode);

@@ -5,46 +5,46 @@
 namespace qmll {
 
 // ------------------------------------------------------------------------------------------------
-// Table packing.  gl = s*P + p is the "global lane" of stack s, sub-lane p; n_gl = n_s*P.
-//   sign_bits[((e*T + t)*EW + k)*n_gl + gl]  bit i  <->  S[e, s, t, p*E + 32k + i] == -1
-//   bias_rev [((e*E4 + j4)*n_gl + gl)*4 + i]        =   b[e, s*d + p*E + 4 j4 + i] / (2 pi)
-//   alpha_s  [(j4*n_gl + gl)*4 + i]                 =   alpha[s*d + p*E + 4 j4 + i] * sqrt(2/D)
-// so that a warp's loads of any of them are contiguous.
+// Table packing: the per-(element, stack group) lane-ordered layouts documented in sorf_device.cuh.
 // ------------------------------------------------------------------------------------------------
 __global__ void pack_signs_kernel(const int8_t* __restrict__ signs, uint32_t* __restrict__ out, int n_elem,
-                                  int n_s, int T, int d, int E, int P, int EW) {
-  const int n_gl = n_s * P;
-  const long long total = (long long)n_elem * T * EW * n_gl;
+                                  int n_s, int n_sg, int T, int d, int E, int P, int EW) {
+  const int spw = kWarp / P;
+  const long long total = (long long)n_elem * T * n_sg * EW * kWarp;
   for (long long idx = blockIdx.x * (long long)blockDim.x + threadIdx.x; idx < total;
        idx += (long long)gridDim.x * blockDim.x) {
-    int gl = (int)(idx % n_gl);
-    long long r = idx / n_gl;
-    int k = (int)(r % EW); r /= EW;
-    int t = (int)(r % T);
-    int e = (int)(r / T);
-    int s = gl / P, p = gl % P;
-    const int8_t* src = signs + (((size_t)e * n_s + s) * T + t) * d + p * E + 32 * k;
-    int nb = E - 32 * k < 32 ? E - 32 * k : 32;
+    const int lane = (int)(idx % kWarp);
+    long long r = idx / kWarp;
+    const int k = (int)(r % EW); r /= EW;
+    const int sg = (int)(r % n_sg); r /= n_sg;
+    const int t = (int)(r % T);
+    const int e = (int)(r / T);
+    const int s = sg * spw + lane / P, p = lane % P;
     uint32_t w = 0;
-    for (int i = 0; i < nb; ++i) w |= (src[i] < 0 ? 1u : 0u) << i;
+    if (s < n_s) {
+      const int8_t* src = signs + (((size_t)e * n_s + s) * T + t) * d + p * E + 32 * k;
+      const int nb = E - 32 * k < 32 ? E - 32 * k : 32;
+      for (int i = 0; i < nb; ++i) w |= (src[i] < 0 ? 1u : 0u) << i;
+    }
     out[idx] = w;
   }
 }
 
 __global__ void permute_table_kernel(const float* __restrict__ in /* [rows, D] */, float* __restrict__ out,
-                                     int rows, int n_s, int d, int E, int P, float scale) {
-  const int n_gl = n_s * P, E4 = E / 4;
+                                     int rows, int n_s, int n_sg, int d, int E, int P, float scale) {
+  const int E4 = E / 4, spw = kWarp / P;
   const long long D = (long long)n_s * d;
-  const long long total = (long long)rows * E4 * n_gl * 4;
+  const long long total = (long long)rows * n_sg * E4 * kWarp * 4;
   for (long long idx = blockIdx.x * (long long)blockDim.x + threadIdx.x; idx < total;
        idx += (long long)gridDim.x * blockDim.x) {
-    int i = (int)(idx & 3);
+    const int i = (int)(idx & 3);
     long long r = idx >> 2;
-    int gl = (int)(r % n_gl); r /= n_gl;
-    int j4 = (int)(r % E4);
-    int e = (int)(r / E4);
-    int s = gl / P, p = gl % P;
-    out[idx] = in[e * D + (long long)s * d + p * E + 4 * j4 + i] * scale;
+    const int lane = (int)(r % kWarp); r /= kWarp;
+    const int q = (int)(r % E4); r /= E4;
+    const int sg = (int)(r % n_sg);
+    const int e = (int)(r / n_sg);
+    const int s = sg * spw + lane / P, p = lane % P;
+    out[idx] = s < n_s ? in[e * D + (long long)s * d + p * E + 4 * q + i] * scale : 0.f;
   }
 }
 
@@ -111,13 +111,21 @@ static void shape_of(int d, int* E, int* P) {
   *P = shape_P(d);
 }
 
+// floats of the per-atom sin table written by the forward kernel: [n_atoms][n_sg][E*32]
+size_t sorf_zs_floats(const qmll_sorf_params* p, int64_t n_atoms) {
+  int E, P;
+  shape_of(p->d, &E, &P);
+  const int spw = kWarp / P, n_s = p->D / p->d, n_sg = (n_s + spw - 1) / spw;
+  return (size_t)n_atoms * n_sg * E * kWarp;
+}
+
 size_t sorf_tables_bytes(const qmll_sorf_params* p, bool with_alpha) {
   int E, P;
   shape_of(p->d, &E, &P);
-  const size_t n_gl = (size_t)(p->D / p->d) * P, EW = (E + 31) / 32;
-  size_t b = align_up((size_t)p->n_elem * p->n_transform * EW * n_gl * 4, 256);
-  b += align_up((size_t)p->n_elem * p->D * 4, 256);
-  if (with_alpha) b += align_up((size_t)p->D * 4, 256);
+  const size_t spw = kWarp / P, n_s = p->D / p->d, n_sg = (n_s + spw - 1) / spw, EW = (E + 31) / 32;
+  size_t b = align_up((size_t)p->n_elem * p->n_transform * n_sg * EW * kWarp * 4, 256);
+  b += align_up((size_t)p->n_elem * n_sg * E * kWarp * 4, 256);
+  if (with_alpha) b += align_up(n_sg * E * kWarp * 4, 256);
   return b + 256;
 }
 
@@ -125,23 +133,24 @@ int sorf_prepare_tables(const qmll_sorf_params* p, const float* alpha, Carver& w
                         cudaStream_t st) {
   int E, P;
   shape_of(p->d, &E, &P);
-  const int n_s = p->D / p->d, EW = (E + 31) / 32;
-  const size_t n_gl = (size_t)n_s * P;
-  t->sign_bits = ws.take<uint32_t>((size_t)p->n_elem * p->n_transform * EW * n_gl);
-  t->bias_rev = ws.take<float>((size_t)p->n_elem * p->D);
-  t->alpha_s = alpha ? ws.take<float>((size_t)p->D) : nullptr;
+  const int spw = kWarp / P, n_s = p->D / p->d, n_sg = (n_s + spw - 1) / spw, EW = (E + 31) / 32;
+  const size_t n_sign = (size_t)p->n_elem * p->n_transform * n_sg * EW * kWarp;
+  const size_t n_tab = (size_t)n_sg * E * kWarp;
+  t->sign_bits = ws.take<uint32_t>(n_sign);
+  t->bias_t = ws.take<float>((size_t)p->n_elem * n_tab);
+  t->alpha_s = alpha ? ws.take<float>(n_tab) : nullptr;
   if (!ws.fits()) return QMLL_ERR_WORKSPACE;
   const int threads = 256;
   auto blocks = [&](size_t n) { size_t b = (n + threads - 1) / threads; return (unsigned)(b > 65535 ? 65535 : (b ? b : 1)); };
-  pack_signs_kernel<<<blocks((size_t)p->n_elem * p->n_transform * EW * n_gl), threads, 0, st>>>(
-      p->signs, t->sign_bits, p->n_elem, n_s, p->n_transform, p->d, E, P, EW);
+  pack_signs_kernel<<<blocks(n_sign), threads, 0, st>>>(p->signs, t->sign_bits, p->n_elem, n_s, n_sg, p->n_transform,
+                                                        p->d, E, P, EW);
   QMLL_LAUNCH_CHECK("pack_signs_kernel");
-  permute_table_kernel<<<blocks((size_t)p->n_elem * p->D), threads, 0, st>>>(
-      p->bias, t->bias_rev, p->n_elem, n_s, p->d, E, P, (float)(1.0 / (2.0 * M_PI)));
+  permute_table_kernel<<<blocks((size_t)p->n_elem * n_tab), threads, 0, st>>>(p->bias, t->bias_t, p->n_elem, n_s, n_sg,
+                                                                              p->d, E, P, 1.0f);
   QMLL_LAUNCH_CHECK("permute_table_kernel(bias)");
   if (alpha) {
-    permute_table_kernel<<<blocks((size_t)p->D), threads, 0, st>>>(alpha, t->alpha_s, 1, n_s, p->d, E, P,
-                                                                   (float)sqrt(2.0 / (double)p->D));
+    permute_table_kernel<<<blocks(n_tab), threads, 0, st>>>(alpha, t->alpha_s, 1, n_s, n_sg, p->d, E, P,
+                                                            (float)sqrt(2.0 / (double)p->D));
     QMLL_LAUNCH_CHECK("permute_table_kernel(alpha)");
   }
   return QMLL_OK;
@@ -164,15 +173,18 @@ int sorf_launch_forward(const SorfProblem& pr, const SorfTables& t, float* Z, fl
   QMLL_SWITCH_D(pr.p->d, CALL)
 #undef CALL
 }
-int sorf_launch_backward(const SorfProblem& pr, const SorfTables& t, float* g_out, double* energy_acc,
-                         cudaStream_t st) {
-#define CALL(TAG) sorf_backward_##TAG(pr, t, g_out, energy_acc, st)
+int sorf_launch_predict(const SorfProblem& pr, const SorfTables& t, const qmll_grad* grad, float* forces,
+                        double* energy_acc, cudaStream_t st) {
+  GradView gv{QMLL_GRAD_NONE, nullptr, nullptr, nullptr, nullptr, 0};
+  if (grad) gv = GradView{grad->layout, grad->dense, grad->dense_off, grad->nbr_idx, grad->nbr_val, grad->K};
+#define CALL(TAG) sorf_predict_##TAG(pr, t, gv, forces, energy_acc, st)
   QMLL_SWITCH_D(pr.p->d, CALL)
 #undef CALL
 }
 int sorf_launch_force_rows_dense(const SorfProblem& pr, const SorfTables& t, const float* zs,
-                                 const float* dense, const int64_t* dense_off, float* G, cudaStream_t st) {
-#define CALL(TAG) sorf_force_rows_dense_##TAG(pr, t, zs, dense, dense_off, G, st)
+                                 const float* dense_t, const int64_t* dense_off, int32_t* grp_off, float* G,
+                                 cudaStream_t st) {
+#define CALL(TAG) sorf_force_rows_dense_##TAG(pr, t, zs, dense_t, dense_off, grp_off, G, st)
   QMLL_SWITCH_D(pr.p->d, CALL)
 #undef CALL
 }
