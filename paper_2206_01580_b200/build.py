@@ -20,8 +20,6 @@ INCLUDE = os.path.join(os.path.dirname(HERE), "include")
 
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "-I", INCLUDE]
-if os.environ.get("QMLL_MAX_E"):          # tuning experiment: elements per lane (see csrc/sorf_device.cuh)
-    NVCC_FLAGS += [f"-DQMLL_MAX_E={int(os.environ['QMLL_MAX_E'])}"]
 
 
 def _nvcc() -> str:

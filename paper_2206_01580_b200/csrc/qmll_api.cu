@@ -64,7 +64,6 @@ static int check_ws(void* ws, size_t have, size_t need) {
 static size_t zs_bytes(const qmll_sorf_params* p, int64_t n_atoms) {
   return align_up(sorf_zs_floats(p, n_atoms) * sizeof(float), 256) + 256;
 }
-static size_t grp_bytes(int32_t n_mol) { return align_up(((size_t)n_mol + 1) * sizeof(int32_t), 256) + 256; }
 static size_t e_bytes(int32_t n_mol) { return align_up((size_t)n_mol * sizeof(double), 256) + 256; }
 
 // shared body of qmll_sorf_backward_forces and qmll_predict
@@ -126,8 +125,7 @@ size_t qmll_workspace_bytes(int which_call, const qmll_sorf_params* p, int64_t n
   switch (which_call) {
     case QMLL_CALL_FORWARD: return sorf_tables_bytes(p, false);
     case QMLL_CALL_FORWARD_GRAD:
-      return sorf_tables_bytes(p, false) + zs_bytes(p, n_atoms) + grp_bytes(n_mol) +
-             align_up((size_t)(rows > 0 ? rows : 0) * 4, 256) + 256;
+      return sorf_tables_bytes(p, false) + zs_bytes(p, n_atoms) + align_up((size_t)(rows > 0 ? rows : 0) * 4, 256) + 256;
     case QMLL_CALL_BACKWARD_FORCES: return sorf_tables_bytes(p, true);
     case QMLL_CALL_PREDICT: return sorf_tables_bytes(p, true) + e_bytes(n_mol);
     default: return 0;
@@ -163,11 +161,10 @@ int qmll_sorf_forward(const qmll_sorf_params* p, const float* x, const int32_t* 
   if (grad) {
     if (grad->layout == QMLL_GRAD_DENSE) {
       float* gt = ws.take<float>((size_t)grad->dense_floats);
-      int32_t* grp_off = ws.take<int32_t>((size_t)n_mol + 1);
       if (!ws.fits()) return QMLL_ERR_WORKSPACE;
       rc = sorf_transpose_dense(pr, grad->dense, grad->dense_off, gt, st);
       if (rc) return rc;
-      rc = sorf_launch_force_rows_dense(pr, t, zs, gt, grad->dense_off, grp_off, G, st);
+      rc = sorf_launch_force_rows_dense(pr, t, zs, gt, grad->dense_off, G, st);
     }
     else
       rc = sorf_launch_force_rows_neighbor(pr, t, zs, grad->nbr_idx, grad->nbr_val, grad->K, G, st);

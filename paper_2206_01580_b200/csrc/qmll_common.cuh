@@ -76,8 +76,7 @@ int sorf_launch_forward(const SorfProblem& pr, const SorfTables& t, float* Z, fl
 int sorf_launch_predict(const SorfProblem& pr, const SorfTables& t, const qmll_grad* grad, float* forces,
                         double* energy_acc, cudaStream_t st);
 int sorf_launch_force_rows_dense(const SorfProblem& pr, const SorfTables& t, const float* zs,
-                                 const float* dense_t, const int64_t* dense_off, int32_t* grp_off, float* G,
-                                 cudaStream_t st);
+                                 const float* dense_t, const int64_t* dense_off, float* G, cudaStream_t st);
 size_t sorf_zs_floats(const qmll_sorf_params* p, int64_t n_atoms);
 int sorf_launch_force_rows_neighbor(const SorfProblem& pr, const SorfTables& t, const float* zs,
                                     const int32_t* nbr_idx, const float* nbr_val, int K, float* G,

@@ -182,9 +182,8 @@ int sorf_launch_predict(const SorfProblem& pr, const SorfTables& t, const qmll_g
 #undef CALL
 }
 int sorf_launch_force_rows_dense(const SorfProblem& pr, const SorfTables& t, const float* zs,
-                                 const float* dense_t, const int64_t* dense_off, int32_t* grp_off, float* G,
-                                 cudaStream_t st) {
-#define CALL(TAG) sorf_force_rows_dense_##TAG(pr, t, zs, dense_t, dense_off, grp_off, G, st)
+                                 const float* dense_t, const int64_t* dense_off, float* G, cudaStream_t st) {
+#define CALL(TAG) sorf_force_rows_dense_##TAG(pr, t, zs, dense_t, dense_off, G, st)
   QMLL_SWITCH_D(pr.p->d, CALL)
 #undef CALL
 }

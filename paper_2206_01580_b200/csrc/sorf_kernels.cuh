@@ -14,8 +14,8 @@
 namespace qmll {
 
 constexpr int kFwdThreads = 128;  // forward: 4 warps; smem accumulators: E * 128 * 4 B (64 KB at E = 128)
-constexpr int kPredThreads = 256; // predict: 8 warps, one block per SM (the chain + accumulators want ~200 registers)
-constexpr int kRowsMaxWarps = 10; // force rows: up to 10 warps (rows of one molecule) share one staged sin table
+constexpr int kPredThreads = 256; // predict with forces: 8 warps, one block per SM (chain + stream want ~250 registers)
+constexpr int kEnergyThreads = 384; // energies only: 12 warps (no transposed chain, no accumulators: 168 registers)
 
 // ------------------------------------------------------------------------------------------------
 // Forward (a1-a3).  Warp task = (atom chunk, stack group of SPW stacks).  The warp walks the atoms of its
@@ -119,8 +119,8 @@ sorf_forward_kernel(const float* __restrict__ x, const int32_t* __restrict__ ele
 // stack lanes once per atom:  gbuf = c * sum_s W_{e,s}^T q_s = -dE/dx_I.  The warp then streams the atom's block of
 // the descriptor gradient exactly once and adds  F[j, k] += sum_m gbuf[m] * dx_I[m]/dr_{j,k}  (F = -dE/dr, eq. 5/10)
 // with one float atomic per (atom, column) -- the ALU-bound chain of some warps overlaps the HBM-bound gradient
-// stream of others, and g never leaves the SM.  The block's warps step through the stack groups together
-// (__syncthreads per group) so that the group's bias / alpha / sign tables stay resident in L1.
+// stream of others, and g never leaves the SM.  The block's warps step through the stack groups
+// without a barrier (measured: forcing them onto the same group with __syncthreads costs 5-8 %).
 // energy_acc[mol] (double, pre-zeroed) receives one atomicAdd per atom.
 // ------------------------------------------------------------------------------------------------
 __device__ __forceinline__ float warp_sum(float v) {
@@ -138,76 +138,101 @@ struct GradView {          // qmll_grad flattened for the device
   int K;
 };
 
-// F[a0 + j, k] += sum_m gbuf[m] * dx[Il][m][3 j + k]   (dense layout, A12): lane = column, rows streamed 16 deep.
+// F[a0 + j, k] += sum_m gbuf[m] * dx[Il][m][3 j + k]   (dense layout, A12): lane = up to three columns (col, col + 32,
+// col + 64), rows streamed 16 deep, i.e. up to 48 independent loads in flight per lane: the stream is latency-bound
+// per warp, and the warp holds no chain state while it runs (its 128 vector registers are free).
 template <typename S>
 __device__ __forceinline__ void contract_dense_atom(const float* __restrict__ gbuf, const float* __restrict__ blk,
                                                     int ncol, float* __restrict__ Fmol, int lane) {
-  for (int c0 = 0; c0 < ncol; c0 += kWarp) {
-    const int col = c0 + lane;
-    const bool ok = col < ncol;
-    const float* ptr = blk + (ok ? col : 0);
-    float s0 = 0.f, s1 = 0.f;
+  for (int c0 = 0; c0 < ncol; c0 += 3 * kWarp) {
+    const int col0 = c0 + lane, col1 = col0 + kWarp, col2 = col1 + kWarp;
+    const bool ok0 = col0 < ncol, ok1 = col1 < ncol, ok2 = col2 < ncol;
+    const float* p0 = blk + (ok0 ? col0 : 0);
+    const float* p1 = blk + (ok1 ? col1 : 0);
+    const float* p2 = blk + (ok2 ? col2 : 0);
+    float s0 = 0.f, s1 = 0.f, s2 = 0.f;
 #pragma unroll 1
     for (int m = 0; m < S::d; m += 16) {
-      float a[16];
+      float a[16], b[16], c[16];
 #pragma unroll
-      for (int u = 0; u < 16; ++u) a[u] = __ldcs(ptr + (size_t)(m + u) * ncol);
+      for (int u = 0; u < 16; ++u) {
+        a[u] = __ldcs(p0 + (size_t)(m + u) * ncol);
+        b[u] = __ldcs(p1 + (size_t)(m + u) * ncol);
+        c[u] = __ldcs(p2 + (size_t)(m + u) * ncol);
+      }
 #pragma unroll
       for (int u = 0; u < 16; u += 4) {
         const float4 g = *reinterpret_cast<const float4*>(gbuf + m + u);
-        s0 = fmaf(g.x, a[u], s0); s1 = fmaf(g.y, a[u + 1], s1);
-        s0 = fmaf(g.z, a[u + 2], s0); s1 = fmaf(g.w, a[u + 3], s1);
+        s0 = fmaf(g.x, a[u], s0); s1 = fmaf(g.x, b[u], s1); s2 = fmaf(g.x, c[u], s2);
+        s0 = fmaf(g.y, a[u + 1], s0); s1 = fmaf(g.y, b[u + 1], s1); s2 = fmaf(g.y, c[u + 1], s2);
+        s0 = fmaf(g.z, a[u + 2], s0); s1 = fmaf(g.z, b[u + 2], s1); s2 = fmaf(g.z, c[u + 2], s2);
+        s0 = fmaf(g.w, a[u + 3], s0); s1 = fmaf(g.w, b[u + 3], s1); s2 = fmaf(g.w, c[u + 3], s2);
       }
     }
-    if (ok) atomicAdd(Fmol + col, s0 + s1);
+    if (ok0) atomicAdd(Fmol + col0, s0);
+    if (ok1) atomicAdd(Fmol + col1, s1);
+    if (ok2) atomicAdd(Fmol + col2, s2);
   }
 }
 
 // F[j, k] += sum_m gbuf[m] * val[q][m][k], j = nbr_idx[a, q]   (neighbour layout, A13; duplicates and self add,
-// -1 = padding): each [d, 3] block is 3d contiguous floats; a lane takes 12 of them (4 values of m) per step.
+// -1 = padding): each [d, 3] block is 3d contiguous floats; a lane takes 12 of them (4 values of m) per step, and
+// kNbrBatch neighbour blocks are in flight at once (the stream is latency-bound per warp).
+constexpr int kNbrBatch = 4;
 template <typename S>
 __device__ __forceinline__ void contract_neighbor_atom(const float* __restrict__ gbuf, const int32_t* __restrict__ idx,
                                                        const float* __restrict__ val, int K, float* __restrict__ F,
                                                        int lane) {
   constexpr int G = S::d / 4;                          // groups of 12 floats per block
   constexpr int GPL = (G + kWarp - 1) / kWarp;         // groups per lane
+  constexpr int NB = GPL <= 2 ? kNbrBatch : (GPL <= 4 ? 2 : 1);
   const float4* g4 = reinterpret_cast<const float4*>(gbuf);
-#pragma unroll 1
-  for (int q = 0; q < K; ++q) {
-    const int j = __ldg(idx + q);
-    if (j < 0) continue;
-    const float4* v4 = reinterpret_cast<const float4*>(val + (size_t)q * S::d * 3);
-    float4 f[GPL][3];
+  float4 gv[GPL];
 #pragma unroll
-    for (int t = 0; t < GPL; ++t) {
-      const int grp = lane + kWarp * t;
-      if (G % kWarp == 0 || grp < G) {
-        f[t][0] = __ldcs(v4 + 3 * grp); f[t][1] = __ldcs(v4 + 3 * grp + 1); f[t][2] = __ldcs(v4 + 3 * grp + 2);
-      } else {
-        f[t][0] = f[t][1] = f[t][2] = make_float4(0.f, 0.f, 0.f, 0.f);
+  for (int t = 0; t < GPL; ++t) {
+    const int grp = lane + kWarp * t;
+    gv[t] = (G % kWarp == 0 || grp < G) ? g4[grp] : make_float4(0.f, 0.f, 0.f, 0.f);
+  }
+#pragma unroll 1
+  for (int q0 = 0; q0 < K; q0 += NB) {
+    int j[NB];
+    float4 f[NB][GPL][3];
+#pragma unroll
+    for (int b = 0; b < NB; ++b) {
+      j[b] = (q0 + b < K) ? __ldg(idx + q0 + b) : -1;
+      const float4* v4 = reinterpret_cast<const float4*>(val + (size_t)(q0 + b) * S::d * 3);
+#pragma unroll
+      for (int t = 0; t < GPL; ++t) {
+        const int grp = lane + kWarp * t;
+        if (j[b] >= 0 && (G % kWarp == 0 || grp < G)) {
+          f[b][t][0] = __ldcs(v4 + 3 * grp); f[b][t][1] = __ldcs(v4 + 3 * grp + 1); f[b][t][2] = __ldcs(v4 + 3 * grp + 2);
+        } else {
+          f[b][t][0] = f[b][t][1] = f[b][t][2] = make_float4(0.f, 0.f, 0.f, 0.f);
+        }
       }
     }
-    float ax = 0.f, ay = 0.f, az = 0.f;
 #pragma unroll
-    for (int t = 0; t < GPL; ++t) {
-      const int grp = lane + kWarp * t;
-      const float4 gv = (G % kWarp == 0 || grp < G) ? g4[grp] : make_float4(0.f, 0.f, 0.f, 0.f);
-      const float4 f0 = f[t][0], f1 = f[t][1], f2 = f[t][2];
-      ax = fmaf(gv.x, f0.x, ax); ay = fmaf(gv.x, f0.y, ay); az = fmaf(gv.x, f0.z, az);
-      ax = fmaf(gv.y, f0.w, ax); ay = fmaf(gv.y, f1.x, ay); az = fmaf(gv.y, f1.y, az);
-      ax = fmaf(gv.z, f1.z, ax); ay = fmaf(gv.z, f1.w, ay); az = fmaf(gv.z, f2.x, az);
-      ax = fmaf(gv.w, f2.y, ax); ay = fmaf(gv.w, f2.z, ay); az = fmaf(gv.w, f2.w, az);
-    }
+    for (int b = 0; b < NB; ++b) {
+      float ax = 0.f, ay = 0.f, az = 0.f;
 #pragma unroll
-    for (int m = 16; m > 0; m >>= 1) {
-      ax += __shfl_xor_sync(0xffffffffu, ax, m);
-      ay += __shfl_xor_sync(0xffffffffu, ay, m);
-      az += __shfl_xor_sync(0xffffffffu, az, m);
-    }
-    if (lane == 0) {
-      atomicAdd(F + (size_t)j * 3 + 0, ax);
-      atomicAdd(F + (size_t)j * 3 + 1, ay);
-      atomicAdd(F + (size_t)j * 3 + 2, az);
+      for (int t = 0; t < GPL; ++t) {
+        const float4 g = gv[t], f0 = f[b][t][0], f1 = f[b][t][1], f2 = f[b][t][2];
+        ax = fmaf(g.x, f0.x, ax); ay = fmaf(g.x, f0.y, ay); az = fmaf(g.x, f0.z, az);
+        ax = fmaf(g.y, f0.w, ax); ay = fmaf(g.y, f1.x, ay); az = fmaf(g.y, f1.y, az);
+        ax = fmaf(g.z, f1.z, ax); ay = fmaf(g.z, f1.w, ay); az = fmaf(g.z, f2.x, az);
+        ax = fmaf(g.w, f2.y, ax); ay = fmaf(g.w, f2.z, ay); az = fmaf(g.w, f2.w, az);
+      }
+#pragma unroll
+      for (int m = 16; m > 0; m >>= 1) {
+        ax += __shfl_xor_sync(0xffffffffu, ax, m);
+        ay += __shfl_xor_sync(0xffffffffu, ay, m);
+        az += __shfl_xor_sync(0xffffffffu, az, m);
+      }
+      if (lane == 0 && j[b] >= 0) {
+        atomicAdd(F + (size_t)j[b] * 3 + 0, ax);
+        atomicAdd(F + (size_t)j[b] * 3 + 1, ay);
+        atomicAdd(F + (size_t)j[b] * 3 + 2, az);
+      }
     }
   }
 }
@@ -219,15 +244,15 @@ struct PredSmem {
   static constexpr size_t kBytes = kWarps * (kAccBytes + S::d * sizeof(float));   // + gbuf[d] per warp
 };
 
-template <typename S, bool kNeedG>
-__global__ void __launch_bounds__(kPredThreads, 1)
+template <typename S, bool kNeedG, int kThreads>
+__global__ void __launch_bounds__(kThreads, 1)
 sorf_predict_kernel(const float* __restrict__ x, const int32_t* __restrict__ elem,
                     const int32_t* __restrict__ mol_off, int n_atoms, int n_mol, int n_s, int T, float c,
                     const uint32_t* __restrict__ sign_bits, const float* __restrict__ bias_t,
                     const float* __restrict__ alpha_s, GradView grad, float* __restrict__ forces,
                     double* __restrict__ energy_acc, int atoms_per_block, int n_sg) {
   extern __shared__ float4 smem4[];
-  constexpr int kWarps = kPredThreads / kWarp;
+  constexpr int kWarps = kThreads / kWarp;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   float4* acc = smem4 + warp * (S::E4 * kWarp);                                           // [E4][32]
   float* gbuf = reinterpret_cast<float*>(smem4 + kWarps * (S::E4 * kWarp)) + warp * S::d;  // [d]
@@ -250,7 +275,6 @@ sorf_predict_kernel(const float* __restrict__ x, const int32_t* __restrict__ ele
     }
 #pragma unroll 1
     for (int sg = 0; sg < n_sg; ++sg) {
-      __syncthreads();  // the block's warps stay on the same stack group: its tables are L1-resident
       if (!have) continue;
       f32x2 v[S::E2];
       load_row<S>(v, x + (size_t)a * S::d, p);
@@ -287,7 +311,7 @@ sorf_predict_kernel(const float* __restrict__ x, const int32_t* __restrict__ ele
           const int t = i < T ? i : 2 * T - i;
           load_sign_words<S>(w, sign_bits, e, t, T, n_sg, sg, lane);
         }
-        sign_fwht<S, true>(v, w, p);
+        sign_fwht<S>(v, w, p);
       }
       if (kNeedG) {
         uint32_t w[S::EW];
@@ -352,152 +376,105 @@ sorf_predict_kernel(const float* __restrict__ x, const int32_t* __restrict__ ele
 }
 
 // ------------------------------------------------------------------------------------------------
-// Force rows (a7), dense gradient.  Block task = (a group of up to W rows r = 3*j + k of ONE molecule, stack group);
-// warp w owns one row.  All warps loop together over the atoms I of the molecule: the gradient column
-// dx_I[:, j, k] of the warp's row goes through the same chain as x (JVP of a linear map = the map itself), is
-// weighted by sqrt(2/D) sin(u_I + b) of that (atom, stack group) and summed over I in the warp's shared-memory
-// accumulators; the finished [SPW, d] slab of G row r is then written once.
+// Force rows (a7), dense gradient.  Warp task = (row r = 3*j + k, stack group); the four warps of a block take
+// four consecutive rows of the same stack group.  The warp loops over the atoms I of the molecule that owns
+// atom j: the gradient column dx_I[:, j, k] goes through the same chain as x (JVP of a linear map = the map
+// itself), is weighted by sqrt(2/D) sin(u_I + b) of that (atom, stack group) and summed over I in the warp's
+// shared-memory accumulators; the finished [SPW, d] slab of G row r is then written once.
 //   G[r, l] = c * sum_I zs_I[l] * (H S_T ... H S_1 dx_I[:, j, k])[l]
-// The sin table of (I, stack group) -- E*128 bytes, written by the forward kernel -- is staged ONCE per block and
-// atom by a TMA bulk copy into a 2-slot ring (full / empty mbarriers) and read by all W warps, so it crosses L2
-// once per W rows; every warp stages its own gradient column the same way (2-slot ring, 1-D bulk copies of the
-// column made contiguous by transpose_dense_kernel).
+// `gt` is the gradient with each column made contiguous ([n, n, 3, d] = (I, j, k, m) per molecule, written by
+// transpose_dense_kernel); the column of the next atom is staged in shared memory by a 1-D TMA bulk copy while
+// the current one runs through the chain (2-slot ring per warp, one mbarrier per slot).  The sin table of
+// (I, stack group) -- E*128 bytes, written by the forward kernel -- is read through L1: every warp prefetches the
+// table of the NEXT atom into L1 before it starts the chain of the current one, and the warps of a block (same
+// molecule, same stack group) find each other's lines there.  The warps are independent (no block-level barrier):
+// measured, coupling them through a shared staged table put their shared-memory phases in lockstep and cost 15 %.
 // ------------------------------------------------------------------------------------------------
 template <typename S>
-struct RowsSmem {
+struct ColStage {
   static constexpr int kSlice = S::E + 4;                 // floats per lane slice (+16 B: no bank conflicts for P > 1)
-  static constexpr int kColFloats = S::P * kSlice;        // one staged column
-  static constexpr size_t kAccBytes = (size_t)S::E * kWarp * sizeof(float);   // per warp [E4][32] float4
-  static constexpr size_t kZsBytes = kAccBytes;                               // one (atom, stack group) sin table
-  static size_t bytes(int W) {
-    return (size_t)W * kAccBytes + 2 * kZsBytes + (size_t)W * 2 * kColFloats * sizeof(float) +
-           (size_t)(4 + 2 * W) * sizeof(uint64_t);
-  }
+  static constexpr int kBufFloats = S::P * kSlice;        // one staged column
+  static constexpr size_t kBytes = (size_t)(kFwdThreads / kWarp) * 2 * (kBufFloats * sizeof(float) + sizeof(uint64_t));
 };
 
 template <typename S>
-__global__ void __launch_bounds__(kRowsMaxWarps * kWarp, 1)
+__global__ void __launch_bounds__(kFwdThreads, (S::E >= 128 ? 3 : 4))
 sorf_force_rows_dense_kernel(const int32_t* __restrict__ elem, const int32_t* __restrict__ mol_off, int n_atoms,
                              int n_mol, int n_s, int T, float c, const uint32_t* __restrict__ sign_bits,
                              const float* __restrict__ zs, const float* __restrict__ gt,
-                             const int64_t* __restrict__ dense_off, const int32_t* __restrict__ grp_off,
-                             float* __restrict__ G, int n_sg, int W) {
-  extern __shared__ float4 smem4[];
-  using RS = RowsSmem<S>;
+                             const int64_t* __restrict__ dense_off, float* __restrict__ G, int n_sg) {
+  extern __shared__ float4 acc[];
+  using CS = ColStage<S>;
+  constexpr int kWarps = kFwdThreads / kWarp;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  float4* acc = smem4 + warp * (S::E4 * kWarp);
-  float4* zsbuf = smem4 + W * (S::E4 * kWarp);                       // [2][E4][32]
-  float* colbuf = reinterpret_cast<float*>(zsbuf + 2 * (S::E4 * kWarp)) + warp * 2 * RS::kColFloats;
-  uint64_t* bars = reinterpret_cast<uint64_t*>(reinterpret_cast<float*>(zsbuf + 2 * (S::E4 * kWarp)) +
-                                               W * 2 * RS::kColFloats);
-  uint64_t* zs_full = bars;          // [2]
-  uint64_t* zs_empty = bars + 2;     // [2]
-  uint64_t* col_bar = bars + 4 + 2 * warp;  // [2] per warp
-
-  // block -> (molecule M, row group rg, stack group sg); grp_off[M] = number of row groups before molecule M
+  float* colbuf = reinterpret_cast<float*>(acc + S::E4 * kFwdThreads) + warp * 2 * CS::kBufFloats;
+  uint64_t* bars = reinterpret_cast<uint64_t*>(reinterpret_cast<float*>(acc + S::E4 * kFwdThreads) +
+                                               kWarps * 2 * CS::kBufFloats) + warp * 2;
+  // block -> (group of kWarps consecutive rows, stack group); warp -> row
   const int sg = blockIdx.x % n_sg;
-  const int g = blockIdx.x / n_sg;
-  if (g >= __ldg(grp_off + n_mol)) return;
-  int lo = 0, hi = n_mol - 1;
-  while (lo < hi) { const int mid = (lo + hi) >> 1; if (__ldg(grp_off + mid + 1) > g) hi = mid; else lo = mid + 1; }
-  const int M = lo, rg = g - __ldg(grp_off + M), n_grp = __ldg(grp_off + M + 1) - __ldg(grp_off + M);
-  const int a0 = __ldg(mol_off + M), n = __ldg(mol_off + M + 1) - a0;
-  const int r_lo = (int)((long long)3 * n * rg / n_grp), r_hi = (int)((long long)3 * n * (rg + 1) / n_grp);
-  const int n_rows = r_hi - r_lo;    // <= W active warps
+  const long long r = (long long)(blockIdx.x / n_sg) * kWarps + warp;
+  if (r >= 3LL * n_atoms) return;
+  const int jg = (int)(r / 3);
   const int p = lane % S::P;
 
-  if (tid == 0) {
-    mbar_init(&zs_full[0], 1); mbar_init(&zs_full[1], 1);
-    mbar_init(&zs_empty[0], n_rows); mbar_init(&zs_empty[1], n_rows);
-    for (int w = 0; w < W; ++w) { mbar_init(bars + 4 + 2 * w, 1); mbar_init(bars + 5 + 2 * w, 1); }
-    fence_mbarrier_init();
-  }
-  __syncthreads();
-  if (warp >= n_rows) return;
-
-  const int rl = r_lo + warp;                     // local row 3*jl + k of molecule M
-  const long long r = (long long)3 * a0 + rl;     // global row of G
+  const int M = owner_molecule(mol_off, n_mol, jg);
+  const int a0 = __ldg(mol_off + M), n = __ldg(mol_off + M + 1) - a0;
+  const int rl = (int)(r - 3LL * a0);             // local row 3*jl + k of molecule M
   // column (I, jl, k) of molecule M: d contiguous floats of gt; consecutive I are 3*n*d floats apart
   const float* col0 = gt + __ldg(dense_off + M) + (size_t)rl * S::d;
   const size_t istride = (size_t)3 * n * S::d;
-  const float* zs_src = zs + ((size_t)a0 * n_sg + sg) * (S::E * kWarp);   // + I * n_sg * E*32 floats
-  const size_t zs_stride = (size_t)n_sg * S::E * kWarp;
+  const float4* zs4 = reinterpret_cast<const float4*>(zs) + ((size_t)a0 * n_sg + sg) * (S::E4 * kWarp) + lane;
+  const size_t zs_stride = (size_t)n_sg * (S::E4 * kWarp);   // float4 per atom
 
-  auto stage_col = [&](int I) {  // lane 0 of each warp
-    uint64_t* bar = &col_bar[I & 1];
-    float* dst = colbuf + (I & 1) * RS::kColFloats;
+  if (lane == 0) {
+    mbar_init(&bars[0], 1);
+    mbar_init(&bars[1], 1);
+    fence_mbarrier_init();
+  }
+  __syncwarp();
+  auto stage = [&](int I) {  // lane 0 only
+    uint64_t* bar = &bars[I & 1];
+    float* dst = colbuf + (I & 1) * CS::kBufFloats;
     mbar_expect_tx(bar, S::d * sizeof(float));
 #pragma unroll
     for (int pp = 0; pp < S::P; ++pp)
-      bulk_copy_g2s(dst + pp * RS::kSlice, col0 + (size_t)I * istride + pp * S::E, S::E * sizeof(float), bar);
+      bulk_copy_g2s(dst + pp * CS::kSlice, col0 + (size_t)I * istride + pp * S::E, S::E * sizeof(float), bar);
   };
-  auto stage_zs = [&](int I) {   // thread 0 of the block
-    const int slot = I & 1, use = I >> 1;
-    if (use > 0) mbar_wait(&zs_empty[slot], (uint32_t)((use - 1) & 1));   // all warps are done with the previous tenant
-    mbar_expect_tx(&zs_full[slot], (uint32_t)RS::kZsBytes);
-    bulk_copy_g2s(zsbuf + slot * (S::E4 * kWarp), zs_src + (size_t)I * zs_stride, (uint32_t)RS::kZsBytes,
-                  &zs_full[slot]);
-  };
-  if (tid == 0) stage_zs(0);
-  if (lane == 0) stage_col(0);
-
+  auto prefetch_zs = [&](int I) {  // the (atom, stack group) table is E*128 contiguous bytes = E lines of 128 B
+    const char* base = reinterpret_cast<const char*>(zs4 - lane + (size_t)I * zs_stride);
 #pragma unroll
-  for (int q = 0; q < S::E4; ++q) acc[q * kWarp + lane] = make_float4(0.f, 0.f, 0.f, 0.f);
+    for (int k = 0; k < S::E / kWarp; ++k)
+      asm volatile("prefetch.global.L1 [%0];" ::"l"(base + (size_t)(k * kWarp + lane) * 128));
+  };
+  if (lane == 0) stage(0);
+  prefetch_zs(0);
+
+  zero_acc<S, kFwdThreads>(acc, tid);
 #pragma unroll 1
   for (int I = 0; I < n; ++I) {
     if (I + 1 < n) {
-      if (tid == 0) stage_zs(I + 1);
-      if (lane == 0) stage_col(I + 1);   // slot (I+1)&1 was last read in iteration I-1 (warp-synced below)
+      if (lane == 0) stage(I + 1);  // slot (I+1)&1 was last read in iteration I-1 (warp-synced below)
+      prefetch_zs(I + 1);
     }
     const int e = __ldg(elem + a0 + I);
-    mbar_wait(&col_bar[I & 1], (uint32_t)((I >> 1) & 1));
+    mbar_wait(&bars[I & 1], (uint32_t)((I >> 1) & 1));
     f32x2 v[S::E2];
-    load_row<S>(v, colbuf + (I & 1) * RS::kColFloats + p * 4, p);   // slices are kSlice = E + 4 floats apart
+    load_row<S>(v, colbuf + (I & 1) * CS::kBufFloats + p * 4, p);   // slices are kSlice = E + 4 floats apart
     __syncwarp();
     chain_forward<S>(v, sign_bits, e, T, n_sg, sg, lane);
-    mbar_wait(&zs_full[I & 1], (uint32_t)((I >> 1) & 1));
-    const float4* z4 = zsbuf + (I & 1) * (S::E4 * kWarp) + lane;
+    const float4* z4 = zs4 + (size_t)I * zs_stride;
 #pragma unroll
     for (int q = 0; q < S::E4; ++q) {
-      const float4 z = z4[q * kWarp];
-      float4 ac = acc[q * kWarp + lane];
+      const float4 z = __ldg(z4 + q * kWarp);
+      float4 ac = acc[q * kFwdThreads + tid];
       f32x2 a01 = fma2(pk(z.x, z.y), v[2 * q], pk(ac.x, ac.y));
       f32x2 a23 = fma2(pk(z.z, z.w), v[2 * q + 1], pk(ac.z, ac.w));
       upk(a01, ac.x, ac.y);
       upk(a23, ac.z, ac.w);
-      acc[q * kWarp + lane] = ac;
+      acc[q * kFwdThreads + tid] = ac;
     }
-    __syncwarp();
-    if (lane == 0) mbar_arrive(&zs_empty[I & 1]);
   }
-  flush_slab<S, kWarp>(acc, 0, lane, G + (size_t)r * (size_t)n_s * S::d, sg, n_s, c, false);
-}
-
-// Number of row groups of every molecule: grp_off[M] = sum_{M' < M} ceil(3 n_M' / W)  (one block, serial scan over
-// chunks of 1024 molecules; n_mol is at most a few hundred thousand).
-static __global__ void __launch_bounds__(1024)
-row_group_offsets_kernel(const int32_t* __restrict__ mol_off, int n_mol, int W, int32_t* __restrict__ grp_off) {
-  __shared__ int part[1024];
-  __shared__ int carry;
-  if (threadIdx.x == 0) carry = 0;
-  __syncthreads();
-  for (int base = 0; base < n_mol; base += 1024) {
-    const int M = base + threadIdx.x;
-    const int cnt = M < n_mol ? (3 * (__ldg(mol_off + M + 1) - __ldg(mol_off + M)) + W - 1) / W : 0;
-    part[threadIdx.x] = cnt;
-    __syncthreads();
-    for (int off = 1; off < 1024; off <<= 1) {   // inclusive scan
-      const int t = threadIdx.x >= off ? part[threadIdx.x - off] : 0;
-      __syncthreads();
-      part[threadIdx.x] += t;
-      __syncthreads();
-    }
-    if (M < n_mol) grp_off[M] = carry + part[threadIdx.x] - cnt;
-    __syncthreads();
-    if (threadIdx.x == 1023) carry += part[1023];
-    __syncthreads();
-  }
-  if (threadIdx.x == 0) grp_off[n_mol] = carry;
+  flush_slab<S, kFwdThreads>(acc, warp * kWarp, lane, G + (size_t)r * (size_t)n_s * S::d, sg, n_s, c, false);
 }
 
 // Force rows, neighbour-sparse gradient (A13): rows of different atoms collide, so contributions are added
@@ -588,53 +565,34 @@ struct SorfLaunch {
     const int n_s = p->D / p->d, n_sg = (n_s + S::SPW - 1) / S::SPW;
     const int n_atoms = (int)pr.n_atoms;
     if (n_atoms == 0 || pr.n_mol == 0) return QMLL_OK;
-    constexpr int kWarps = kPredThreads / kWarp;
+    const int threads = forces ? kPredThreads : kEnergyThreads, n_warps = threads / kWarp;
     const int n_sm = device_sm_count();
     int apb = (n_atoms + n_sm - 1) / n_sm;
-    apb = (apb + kWarps - 1) / kWarps * kWarps;
+    apb = (apb + n_warps - 1) / n_warps * n_warps;
     const unsigned grid = (unsigned)((n_atoms + apb - 1) / apb);
-    auto kern = forces ? sorf_predict_kernel<S, true> : sorf_predict_kernel<S, false>;
-    const size_t smem = PredSmem<S>::kBytes;
+    auto kern = forces ? sorf_predict_kernel<S, true, kPredThreads> : sorf_predict_kernel<S, false, kEnergyThreads>;
+    const size_t smem = forces ? PredSmem<S>::kBytes : 0;
     QMLL_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    kern<<<grid, kPredThreads, smem, st>>>(pr.x, pr.elem, pr.mol_off, n_atoms, pr.n_mol, n_s, p->n_transform,
+    kern<<<grid, threads, smem, st>>>(pr.x, pr.elem, pr.mol_off, n_atoms, pr.n_mol, n_s, p->n_transform,
                                            c_of(p), t.sign_bits, t.bias_t, t.alpha_s, gv, forces, energy_acc, apb,
                                            n_sg);
     QMLL_LAUNCH_CHECK("sorf_predict_kernel");
     return QMLL_OK;
   }
 
-  // rows-per-block W: as many as shared memory and registers allow, then the value that wastes the fewest warps
-  // for molecules of the average size (exact when all molecules have the same number of atoms)
-  static int rows_per_block(long long n_atoms, int n_mol) {
-    int w_max = kRowsMaxWarps;
-    while (w_max > 1 && RowsSmem<S>::bytes(w_max) > 220 * 1024) --w_max;
-    const long long rows = n_mol > 0 ? (3 * n_atoms + n_mol - 1) / n_mol : 3;
-    int best = w_max;
-    double best_eff = 0.0;
-    for (int w = w_max; w >= (w_max + 1) / 2; --w) {
-      const double eff = (double)rows / (double)(((rows + w - 1) / w) * w);
-      if (eff > best_eff + 1e-9) { best_eff = eff; best = w; }
-    }
-    return best;
-  }
-
   static int force_rows_dense(const SorfProblem& pr, const SorfTables& t, const float* zs, const float* dense_t,
-                              const int64_t* dense_off, int32_t* grp_off, float* G, cudaStream_t st) {
+                              const int64_t* dense_off, float* G, cudaStream_t st) {
     const qmll_sorf_params* p = pr.p;
     const int n_s = p->D / p->d, n_sg = (n_s + S::SPW - 1) / S::SPW;
     const long long n_atoms = pr.n_atoms;
     if (n_atoms == 0) return QMLL_OK;
-    const int W = rows_per_block(n_atoms, pr.n_mol);
-    row_group_offsets_kernel<<<1, 1024, 0, st>>>(pr.mol_off, pr.n_mol, W, grp_off);
-    QMLL_LAUNCH_CHECK("row_group_offsets_kernel");
-    const long long groups_max = (3 * n_atoms + W - 1) / W + pr.n_mol;   // >= sum_M ceil(3 n_M / W)
-    const long long grid = groups_max * n_sg;
+    const long long grid = (3 * n_atoms + kWarpsPerBlock - 1) / kWarpsPerBlock * n_sg;
     if (grid > 0x7fffffffLL) return QMLL_ERR_UNSUPPORTED;
     auto kern = sorf_force_rows_dense_kernel<S>;
-    const size_t smem = RowsSmem<S>::bytes(W);
+    const size_t smem = kAccBytes + ColStage<S>::kBytes;
     QMLL_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    kern<<<(unsigned)grid, W * kWarp, smem, st>>>(pr.elem, pr.mol_off, (int)n_atoms, pr.n_mol, n_s, p->n_transform,
-                                                  c_of(p), t.sign_bits, zs, dense_t, dense_off, grp_off, G, n_sg, W);
+    kern<<<(unsigned)grid, kFwdThreads, smem, st>>>(pr.elem, pr.mol_off, (int)n_atoms, pr.n_mol, n_s, p->n_transform,
+                                                    c_of(p), t.sign_bits, zs, dense_t, dense_off, G, n_sg);
     QMLL_LAUNCH_CHECK("sorf_force_rows_dense_kernel");
     return QMLL_OK;
   }
@@ -662,7 +620,7 @@ struct SorfLaunch {
   int sorf_forward_##TAG(const SorfProblem&, const SorfTables&, float*, float*, cudaStream_t);                 \
   int sorf_predict_##TAG(const SorfProblem&, const SorfTables&, const GradView&, float*, double*, cudaStream_t); \
   int sorf_force_rows_dense_##TAG(const SorfProblem&, const SorfTables&, const float*, const float*,           \
-                                  const int64_t*, int32_t*, float*, cudaStream_t);                             \
+                                  const int64_t*, float*, cudaStream_t);                                       \
   int sorf_force_rows_neighbor_##TAG(const SorfProblem&, const SorfTables&, const float*, const int32_t*,      \
                                      const float*, int, float*, cudaStream_t);
 
@@ -676,9 +634,8 @@ struct SorfLaunch {
     return SorfLaunch<Shape<E_, P_>>::predict(pr, t, gv, f, en, st);                                           \
   }                                                                                                            \
   int sorf_force_rows_dense_##TAG(const SorfProblem& pr, const SorfTables& t, const float* zs,                 \
-                                  const float* dense, const int64_t* off, int32_t* grp, float* G,              \
-                                  cudaStream_t st) {                                                           \
-    return SorfLaunch<Shape<E_, P_>>::force_rows_dense(pr, t, zs, dense, off, grp, G, st);                     \
+                                  const float* dense, const int64_t* off, float* G, cudaStream_t st) {         \
+    return SorfLaunch<Shape<E_, P_>>::force_rows_dense(pr, t, zs, dense, off, G, st);                          \
   }                                                                                                            \
   int sorf_force_rows_neighbor_##TAG(const SorfProblem& pr, const SorfTables& t, const float* zs,              \
                                      const int32_t* idx, const float* val, int K, float* G, cudaStream_t st) { \
