@@ -1,10 +1,12 @@
-"""bench.py -- one "step" = one pass of the whole SORF hot path over one
-batch of synthetic input shaped like BASELINE.json:configs[1] (MD-trajectory-like: 1000 x 21 atoms, d = 128,
-D = 8192, E+F training rows + E+F prediction):
-    qmll_sorf_forward (+G)  ->  qmll_normal_equations on [Z; G]  ->  qmll_predict (E + F)
-Prints ONE JSON line (contract in the task statement; extra keys: roofline, cpu_baseline, e2e, clocks).
+"""bench.py -- one "step" = one pass of the whole SORF hot path over one batch of
+synthetic input shaped like BASELINE.json:configs[3] (drug-like flexible molecule, the largest single-GPU config that
+exercises every call):
+    qmll_sorf_forward (+G) on the 500 training configurations  ->  qmll_normal_equations on [Z; G] (41 000 rows,
+    D = 16384)  ->  qmll_predict (E + F) on the 2000 inference configurations
+Prints ONE JSON line (contract in the task statement; extra keys: roofline, sorf_rooflines, configs, cpu_baseline,
+e2e, clocks).
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--n-mol M] [--D D]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
 """
 import argparse
 import json
@@ -19,6 +21,9 @@ sys.path.insert(0, ROOT)
 
 METRIC = "SORF molecules/s (energy+forces), ZtZ TFLOPS, % of HBM/tensor roofline"
 UNIT = "molecules/s"
+WORKLOAD = ("c4: {nt} training + {ni} inference configurations of a 27-atom C12H12N2O molecule per GPU, d=256, D=16384, "
+            "T=3, sigma=16, dense gradient (27,256,27,3); step = forward+force rows -> normal equations on {rows} rows "
+            "-> predict E+F on the inference set; molecules per step = {nt} + {ni}")
 
 
 def parse():
@@ -27,68 +32,95 @@ def parse():
     ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--config", default="c2")
-    ap.add_argument("--n-mol", type=int, default=None, help="shrink the workload (debug only; invalid as a bench)")
+    ap.add_argument("--n-train", type=int, default=None, help="shrink the workload (debug only; invalid as a bench)")
+    ap.add_argument("--n-infer", type=int, default=None, help="shrink the workload (debug only; invalid as a bench)")
     ap.add_argument("--D", type=int, default=None, help="shrink the workload (debug only)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
-    ap.add_argument("--report-configs", action="store_true",
-                    help="time every call of all five BASELINE.json configs (one JSON line per config); not the bench line")
+    ap.add_argument("--no-configs", action="store_true", help="skip the per-config block (C2, C3, C5)")
     return ap.parse_args()
 
 
 def peaks():
+    """Roofline denominators: the driver's MEASURED_PEAKS.json (HBM copy, cuBLAS bf16) and this repo's own
+    measurement of what that file lacks (profiles/peaks_r2.json: FADD issue rate, TF32 GEMM)."""
+    out = {"hbm_gbs": 6650.0, "bf16_burst": 1590.0, "bf16_sustained": 1400.0, "source": "fallback",
+           "fadd_per_s": 148 * 128 * 1.965e9, "fadd_source": "nominal 148 SM x 128 lanes x 1.965 GHz",
+           "tf32_burst": None, "tf32_sustained": None}
     path = os.path.join(ROOT, "MEASURED_PEAKS.json")
     if os.path.exists(path):
         with open(path) as f:
             p = json.load(f)
-        return {"hbm_gbs": p["hbm_gbs"], "bf16_burst": p["bf16_tflops"], "bf16_sustained": p["bf16_tflops_sustained"],
-                "source": "measured"}
-    return {"hbm_gbs": 6650.0, "bf16_burst": 1590.0, "bf16_sustained": 1400.0, "source": "fallback"}
+        out.update({"hbm_gbs": p["hbm_gbs"], "bf16_burst": p["bf16_tflops"], "bf16_sustained": p["bf16_tflops_sustained"],
+                    "source": "measured"})
+    path = os.path.join(ROOT, "profiles", "peaks_r2.json")
+    if os.path.exists(path):
+        with open(path) as f:
+            p = json.load(f)
+        out.update({"fadd_per_s": p["alu"]["0"]["per_s"], "fadd_source": "measured (profiles/peaks_r2.json, FADD loop on all SMs)",
+                    "tf32_burst": p["tensor"]["tf32_tflops_burst"], "tf32_sustained": p["tensor"]["tf32_tflops_sustained"]})
+    return out
 
 
 # ------------------------------------------------------------------------------------------------ oracle arm
-def oracle_sample_step(w):
-    """The whole path on workload w with the FP64 oracle as it stands (never tuned)."""
+def oracle_stages(wt, wi):
+    """Seconds the FP64 oracle, as it stands, needs for each stage of the step on the sample workloads."""
     import numpy as np
     import oracle
-    Z = oracle.forward_w(w)
-    G = oracle.force_rows_w(w)
+    t0 = time.perf_counter()
+    Z = oracle.forward_w(wt)
+    G = oracle.force_rows_w(wt)
+    t1 = time.perf_counter()
     A = np.concatenate([Z, G]).astype(np.float32)
-    oracle.normal_equations(A, w.y)
-    oracle.predict_w(w)
+    oracle.normal_equations(A, wt.y)
+    t2 = time.perf_counter()
+    oracle.predict_w(wi)
+    t3 = time.perf_counter()
+    return {"forward_force_rows_s": t1 - t0, "normal_equations_s": t2 - t1, "predict_s": t3 - t2}
 
 
-def time_oracle(cfg, D, sample_mol, steps, warmup):
+def oracle_sample(D, n_train=1, n_infer=2):
     import oracle
     from workloads import make_workload
-    w = make_workload(cfg, n_mol=sample_mol, D=D)
     oracle.build()
-    for _ in range(warmup):
-        oracle_sample_step(w)
-    t0 = time.perf_counter()
-    for _ in range(steps):
-        oracle_sample_step(w)
-    dt = (time.perf_counter() - t0) / steps
-    return dt, oracle.num_threads(), w
+    wt = make_workload("c4", n_mol=n_train, D=D)
+    wi = make_workload("c4", n_mol=n_infer, D=D, part="infer")
+    return wt, wi, oracle.num_threads()
+
+
+def describe_sample(wt, wi, D):
+    return (f"{wt.n_mol} of 500 training + {wi.n_mol} of 2000 inference configurations of c4 at full D={D}: forward + "
+            f"force rows, FP64 A^T A on their {wt.n_mol + 3 * wt.n_atoms} rows, predict E+F")
+
+
+def extrapolate(st, wt, wi, n_train=500, n_infer=2000):
+    """Linear extrapolation of the sampled stage times to the full step (every stage is linear in its row count)."""
+    return (st["forward_force_rows_s"] * n_train / wt.n_mol + st["normal_equations_s"] * n_train / wt.n_mol +
+            st["predict_s"] * n_infer / wi.n_mol)
 
 
 def reference_arm(args):
-    rank = int(os.environ.get("RANK", "0"))
-    if rank != 0:
+    if int(os.environ.get("RANK", "0")) != 0:
         return
-    sample_mol = 2
-    full_D = args.D or 8192
-    dt, cores, w = time_oracle(args.config, full_D, sample_mol, args.steps, min(args.warmup, 1))
-    val = sample_mol / dt
-    sample = (f"{sample_mol} of 1000 molecules of {args.config} at full D={full_D}: forward + force rows + FP64 A^T A "
-              f"on its {w.n_mol + 3 * w.n_atoms} rows + predict E+F, per step")
+    D = args.D or 16384
+    wt, wi, cores = oracle_sample(D)
+    for _ in range(min(args.warmup, 1)):
+        oracle_stages(wt, wi)
+    tot, st = 0.0, None
+    for _ in range(args.steps):
+        st = oracle_stages(wt, wi)
+        tot += sum(st.values())
+    dt = tot / args.steps
+    val = (wt.n_mol + wi.n_mol) / dt
+    sample = describe_sample(wt, wi, D)
     line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt * 1e3, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": "c2: 1000 x C9H8O4 (21 atoms), d=128, D=8192, T=3, dense gradient; oracle on a sample",
+            "config": {"workload": WORKLOAD.format(nt=500, ni=2000, rows=41000) + "; oracle arm: a bounded sample per step",
                        "sample": sample},
-            "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+            "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample,
+                             "stage_seconds_on_sample": st,
+                             "extrapolated_full_step_s": extrapolate(st, wt, wi), "extrapolation": "linear in rows, labelled"},
             "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
     print(json.dumps(line))
@@ -138,6 +170,47 @@ class ClockSampler:
         return out
 
 
+# ------------------------------------------------------------------------------------------------ roofline arithmetic
+def sorf_ops(w, train):
+    """Algorithmic fp32 lane-operations: forward D*(T*log2 d + 3) per atom, force rows
+    D*(T*log2 d + 2) per gradient column, predict D*(2*T*log2 d + 6) per atom."""
+    m = w.model
+    L, T, D = m.d.bit_length() - 1, m.T, m.D
+    fwd = w.n_atoms * D * (T * L + 3.0)
+    cols = 3.0 * sum(int(c) ** 2 for c in (w.mol_off[1:] - w.mol_off[:-1])) if train else 0.0
+    return fwd, cols * D * (T * L + 2.0), w.n_atoms * D * (2.0 * T * L + 6.0)
+
+
+def ne_roofline(rows, D, kern_ms, ms_step, pk, traffic):
+    alg_flops = float(rows) * D * (D + 1)            # symmetric half, fp32-equivalent (SURVEY.md 8(d), a8)
+    achieved = alg_flops / (kern_ms * 1e-3) / 1e12 if kern_ms > 0 else 0.0
+    peak = pk["bf16_sustained"] / 3.0                # three f16 MMAs (hi*hi, hi*lo, lo*hi) per fp32-equivalent product
+    r = {"kernel": "syrk_tcgen05_kernel<f16 split>", "bound": "tensor", "achieved": achieved, "peak": peak,
+         "unit": "TFLOP/s", "frac": achieved / peak, "traffic": traffic,
+         "algorithmic_bytes": 4.0 * rows * D + 2.0 * D * (D + 1),
+         "frac_of_burst_peak": achieved / (pk["bf16_burst"] / 3.0),
+         "note": (f"achieved = rows*D*(D+1) fp32-equivalent flops per launch / CUDA-event time of the kernel "
+                  f"({kern_ms:.3f} ms avg, events on the launch stream inside the library); peak = cuBLAS bf16 "
+                  f"SUSTAINED ({pk['source']}: the kernel is timed inside a long step) / 3 -- f16 and bf16 MMAs run at "
+                  f"the same rate; against the burst figure the fraction is frac_of_burst_peak; share of step = "
+                  f"{kern_ms / ms_step:.3f}"),
+         "full_gemm_equiv_tflops": 2.0 * rows * D * D / (kern_ms * 1e-3) / 1e12 if kern_ms > 0 else 0.0}
+    if pk["tf32_sustained"]:
+        r["vs_3xtf32_peak_measured"] = achieved / (pk["tf32_sustained"] / 3.0)   # what north_star's 3xTF32 scheme could reach
+    if r["frac"] > 1.05:
+        r["warning"] = "fraction above 1: the denominator is a cuBLAS measurement under the power cap, not the pipe peak"
+    return r
+
+
+def load_traffic():
+    try:
+        with open(os.path.join(ROOT, "profiles", "r2_traffic.json")) as f:
+            t = json.load(f)
+        return t["syrk_tcgen05_kernel"]["dram_bytes_per_launch"]
+    except Exception:
+        return None
+
+
 # ------------------------------------------------------------------------------------------------ our arm
 def ours_arm(args):
     import numpy as np
@@ -156,32 +229,37 @@ def ours_arm(args):
         dist.init_process_group("nccl", device_id=dev)
     pkg.load_library()  # fails loudly if the CUDA library is missing: there is no fallback
 
-    # weak scaling: every rank owns its own batch of molecules (same shapes, rank-dependent seed not needed:
-    # throughput does not depend on the values); the normal equations are summed over ranks each step.
-    w = make_workload(args.config, n_mol=args.n_mol, D=args.D)
-    dp = workload_io.device_problem(w, dev)
-    p, D, n_mol, n_atoms = dp.params, w.model.D, w.n_mol, w.n_atoms
-    rows = n_mol + 3 * n_atoms
+    # weak scaling: every rank owns its own batch of configurations (same shapes; throughput does not depend on the
+    # values); the normal equations are summed over ranks each step (packed lower triangle, NCCL).
+    wt = make_workload("c4", n_mol=args.n_train, D=args.D)
+    wi = make_workload("c4", n_mol=args.n_infer, D=args.D, part="infer")
+    dt_, di_ = workload_io.device_problem(wt, dev), workload_io.device_problem(wi, dev)
+    p, D = dt_.params, wt.model.D
+    n_train, n_infer = wt.n_mol, wi.n_mol
+    rows = n_train + 3 * wt.n_atoms
     A = torch.empty((rows, D), dtype=torch.float32, device=dev)
-    Z, G = A[:n_mol], A[n_mol:]
+    Z, G = A[:n_train], A[n_train:]
     ZtZ = torch.empty((D, D), dtype=torch.float32, device=dev)
     Zty = torch.empty((D,), dtype=torch.float32, device=dev)
-    E = torch.empty((n_mol,), dtype=torch.float32, device=dev)
-    F = torch.empty((n_atoms, 3), dtype=torch.float32, device=dev)
+    E = torch.empty((n_infer,), dtype=torch.float32, device=dev)
+    F = torch.empty((wi.n_atoms, 3), dtype=torch.float32, device=dev)
+    reducer = qdist.NormalEquationsReducer(D, dev) if world > 1 else None
 
-    def step(d):
-        pkg.qmll_sorf_forward(p, d.x, d.elem, d.mol_off, d.grad, Z=Z, G=G)
-        pkg.qmll_normal_equations(A, d.y, ZtZ=ZtZ, Zty=Zty)
-        qdist.allreduce_normal_equations(ZtZ, Zty)
-        pkg.qmll_predict(p, d.x, d.elem, d.mol_off, d.alpha, d.grad, energies=E, forces=F)
+    def step(tr, inf, ZtZ_, Zty_, E_, F_):
+        pkg.qmll_sorf_forward(p, tr.x, tr.elem, tr.mol_off, tr.grad, Z=Z, G=G)
+        pkg.qmll_normal_equations(A, tr.y, ZtZ=ZtZ_, Zty=Zty_)
+        if reducer is not None:
+            reducer.allreduce(ZtZ_, Zty_)
+        pkg.qmll_predict(p, inf.x, inf.elem, inf.mol_off, inf.alpha, inf.grad, energies=E_, forces=F_)
 
     def barrier():
         if world > 1:
             dist.barrier()
         torch.cuda.synchronize()
 
-    for _ in range(max(args.warmup, 3)):
-        step(dp)
+    warm = max(args.warmup, 3)
+    for _ in range(warm):
+        step(dt_, di_, ZtZ, Zty, E, F)
     barrier()
 
     # ---- device-resident timing (value) --------------------------------------------------------------
@@ -195,12 +273,13 @@ def ours_arm(args):
     e0.record()
     for k in range(args.steps):
         parts[k][0].record()
-        pkg.qmll_sorf_forward(p, dp.x, dp.elem, dp.mol_off, dp.grad, Z=Z, G=G)
+        pkg.qmll_sorf_forward(p, dt_.x, dt_.elem, dt_.mol_off, dt_.grad, Z=Z, G=G)
         parts[k][1].record()
-        pkg.qmll_normal_equations(A, dp.y, ZtZ=ZtZ, Zty=Zty)
-        qdist.allreduce_normal_equations(ZtZ, Zty)
+        pkg.qmll_normal_equations(A, dt_.y, ZtZ=ZtZ, Zty=Zty)
+        if reducer is not None:
+            reducer.allreduce(ZtZ, Zty)
         parts[k][2].record()
-        pkg.qmll_predict(p, dp.x, dp.elem, dp.mol_off, dp.alpha, dp.grad, energies=E, forces=F)
+        pkg.qmll_predict(p, di_.x, di_.elem, di_.mol_off, di_.alpha, di_.grad, energies=E, forces=F)
         parts[k][3].record()
     e1.record()
     barrier()
@@ -220,14 +299,16 @@ def ours_arm(args):
         # Steps are pipelined the way a training loop would be: while step k computes, the copy stream uploads the
         # inputs of step k+1 into the other device buffer set and a third stream downloads the results of step k-1.
         # Every step still uploads ALL its inputs from pinned host memory and downloads ALL its results.
-        host = {k: torch.from_numpy(v).pin_memory() for k, v in workload_io.host_arrays(w).items()}
-        dbuf = [{k: torch.empty_like(v, device=dev) for k, v in host.items()} for _ in range(2)]
+        host_t = {k: torch.from_numpy(v).pin_memory() for k, v in workload_io.host_arrays(wt).items()}
+        host_i = {k: torch.from_numpy(v).pin_memory() for k, v in workload_io.host_arrays(wi).items()}
+        dbuf_t = [{k: torch.empty_like(v, device=dev) for k, v in host_t.items()} for _ in range(2)]
+        dbuf_i = [{k: torch.empty_like(v, device=dev) for k, v in host_i.items()} for _ in range(2)]
         outs = [{"ZtZ": torch.empty((D, D), dtype=torch.float32, device=dev),
                  "Zty": torch.empty((D,), dtype=torch.float32, device=dev),
-                 "E": torch.empty((n_mol,), dtype=torch.float32, device=dev),
-                 "F": torch.empty((n_atoms, 3), dtype=torch.float32, device=dev)} for _ in range(2)]
+                 "E": torch.empty((n_infer,), dtype=torch.float32, device=dev),
+                 "F": torch.empty((wi.n_atoms, 3), dtype=torch.float32, device=dev)} for _ in range(2)]
         out_host = {k: torch.empty(v.shape, dtype=v.dtype).pin_memory() for k, v in outs[0].items()}
-        h2d = sum(v.numel() * v.element_size() for v in host.values())
+        h2d = sum(v.numel() * v.element_size() for v in list(host_t.values()) + list(host_i.values()))
         d2h = sum(v.numel() * v.element_size() for v in out_host.values())
         s_in, s_out, s_main = torch.cuda.Stream(), torch.cuda.Stream(), torch.cuda.current_stream()
         ev_in = [torch.cuda.Event() for _ in range(2)]       # inputs of buffer b uploaded
@@ -240,18 +321,21 @@ def ours_arm(args):
                 with torch.cuda.stream(s_in):
                     if k >= 2:
                         s_in.wait_event(ev_done[b])           # step k-2 no longer reads this input set
-                    for name, v in host.items():
-                        dbuf[b][name].copy_(v, non_blocking=True)
+                    for name, v in host_t.items():
+                        dbuf_t[b][name].copy_(v, non_blocking=True)
+                    for name, v in host_i.items():
+                        dbuf_i[b][name].copy_(v, non_blocking=True)
                     ev_in[b].record(s_in)
                 s_main.wait_event(ev_in[b])
                 if k >= 2:
                     s_main.wait_event(ev_out[b])              # results of step k-2 have left this output set
-                db, o = dbuf[b], outs[b]
-                g = workload_io.device_grad(db, dev)
-                pkg.qmll_sorf_forward(p, db["x"], db["elem"], db["mol_off"], g, Z=Z, G=G)
-                pkg.qmll_normal_equations(A, db["y"], ZtZ=o["ZtZ"], Zty=o["Zty"])
-                qdist.allreduce_normal_equations(o["ZtZ"], o["Zty"])
-                pkg.qmll_predict(p, db["x"], db["elem"], db["mol_off"], dp.alpha, g, energies=o["E"], forces=o["F"])
+                tb, ib, o = dbuf_t[b], dbuf_i[b], outs[b]
+                gt_, gi_ = workload_io.device_grad(tb, dev), workload_io.device_grad(ib, dev)
+                pkg.qmll_sorf_forward(p, tb["x"], tb["elem"], tb["mol_off"], gt_, Z=Z, G=G)
+                pkg.qmll_normal_equations(A, tb["y"], ZtZ=o["ZtZ"], Zty=o["Zty"])
+                if reducer is not None:
+                    reducer.allreduce(o["ZtZ"], o["Zty"])
+                pkg.qmll_predict(p, ib["x"], ib["elem"], ib["mol_off"], di_.alpha, gi_, energies=o["E"], forces=o["F"])
                 ev_done[b].record(s_main)
                 with torch.cuda.stream(s_out):
                     s_out.wait_event(ev_done[b])
@@ -269,152 +353,154 @@ def ours_arm(args):
         t1.record()
         barrier()
         e2e_ms = qdist.max_over_ranks(t0.elapsed_time(t1), dev) / args.steps
-        e2e = {"value": world * n_mol / (e2e_ms * 1e-3), "unit": UNIT, "ms_per_step": e2e_ms,
+        e2e = {"value": world * (n_train + n_infer) / (e2e_ms * 1e-3), "unit": UNIT, "ms_per_step": e2e_ms,
                "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
-               "note": "public API on pinned HOST buffers; uploads/downloads of neighbouring steps overlap compute"}
+               "h2d_GBps": h2d / (e2e_ms * 1e-3) / 1e9,
+               "note": "public API on pinned HOST buffers; uploads/downloads of neighbouring steps overlap compute; "
+                       "the 5.6 GB of descriptor gradients per step make this PCIe-bound"}
+        del dbuf_t, dbuf_i, outs, host_t, host_i
+        torch.cuda.empty_cache()
 
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
         return
 
-    # ---- roofline of the dominant kernel (tcgen05 3xTF32 A^T A) ---------------------------------------
+    # ---- rooflines -----------------------------------------------------------------------------------------------
     pk = peaks()
-    alg_flops = float(rows) * D * (D + 1)            # symmetric half, fp32-equivalent
     kern_ms = syrk_ms / max(syrk_n, 1)
-    achieved = alg_flops / (kern_ms * 1e-3) / 1e12 if kern_ms > 0 else 0.0
-    tf32_peak = 0.5 * pk["bf16_sustained"]           # nominal tf32 : bf16 = 1 : 2 (profiling guide)
-    peak3 = tf32_peak / 3.0                          # three TF32 MMAs per fp32-equivalent product
-    roofline = {"kernel": "syrk_tcgen05_kernel", "bound": "tensor", "achieved": achieved, "peak": peak3,
-                "unit": "TFLOP/s", "frac": achieved / peak3, "traffic": None,
-                "note": (f"achieved = rows*D*(D+1) fp32-equivalent flops per launch / CUDA-event time of the kernel "
-                         f"({kern_ms:.3f} ms avg over {syrk_n} launches); peak = bf16 sustained "
-                         f"({pk['source']}) x 0.5 (tf32) / 3 (3xTF32); share of step = {kern_ms / ms_step:.3f}"),
-                "full_gemm_equiv_tflops": 2.0 * rows * D * D / (kern_ms * 1e-3) / 1e12 if kern_ms > 0 else 0.0}
-
-    # traffic of that kernel from the committed ncu --set full capture (profiles/), per launch
-    try:
-        with open(os.path.join(ROOT, "profiles", "r1_traffic.json")) as f:
-            roofline["traffic"] = json.load(f)["syrk_tcgen05_kernel"]["dram_bytes_per_launch"]
-    except Exception:
-        roofline["traffic"] = None
-    roofline["algorithmic_bytes"] = 2.0 * 4 * rows * D + 4.0 * D * (D + 1) / 2   # hi+lo operands once + half of C
-    # the SORF kernels are bound by plain fp32 ALU issue: lane-ops / s against 148 SM x 128 x clock
-    L = (w.model.d).bit_length() - 1
-    T = w.model.T
-    alu_peak = 148 * 128 * 1.965e9
-    cols = 3.0 * sum(int(c) ** 2 for c in (w.mol_off[1:] - w.mol_off[:-1]))
-    fr_ops = cols * D * (T * L + 2) + n_atoms * D * (T * L + 3)
-    pr_ops = n_atoms * D * (2 * T * L + 6)
+    roofline = ne_roofline(rows, D, kern_ms, ms_step, pk, load_traffic())
+    fwd_ops, fr_ops, _ = sorf_ops(wt, True)
+    _, _, pr_ops = sorf_ops(wi, False)
+    sm_mhz = (clocks or {}).get("sm_mhz") or 0.0
+    fadd = pk["fadd_per_s"]
     sorf_rooflines = {
-        "forward_plus_force_rows": {"bound": "alu", "achieved": fr_ops / (fwd_ms * 1e-3) / 1e12, "peak": alu_peak / 1e12,
-                                    "unit": "T lane-ops/s", "frac": fr_ops / (fwd_ms * 1e-3) / alu_peak,
-                                    "note": "algorithmic fp32 lane-ops D*(T*log2 d + 2) per gradient column + forward; "
-                                            "time = whole qmll_sorf_forward call (CUDA events)"},
-        "predict": {"bound": "alu", "achieved": pr_ops / (pred_ms * 1e-3) / 1e12, "peak": alu_peak / 1e12,
-                    "unit": "T lane-ops/s", "frac": pr_ops / (pred_ms * 1e-3) / alu_peak,
-                    "note": "D*(2*T*log2 d + 6) lane-ops per atom; whole qmll_predict call incl. the HBM-bound contraction"}}
+        "forward_plus_force_rows": {"bound": "alu", "achieved": (fwd_ops + fr_ops) / (fwd_ms * 1e-3) / 1e12,
+                                    "peak": fadd / 1e12, "unit": "T lane-ops/s", "frac": (fwd_ops + fr_ops) / (fwd_ms * 1e-3) / fadd,
+                                    "note": "algorithmic fp32 lane-ops D*(T*log2 d + 2) per gradient column + forward; time = whole "
+                                            "qmll_sorf_forward call (CUDA events) incl. the gradient transpose; peak = " + pk["fadd_source"]},
+        "predict": {"bound": "alu", "achieved": pr_ops / (pred_ms * 1e-3) / 1e12, "peak": fadd / 1e12,
+                    "unit": "T lane-ops/s", "frac": pr_ops / (pred_ms * 1e-3) / fadd,
+                    "gradient_stream_GBps": wi.grad.dense.nbytes / (pred_ms * 1e-3) / 1e9,
+                    "note": "D*(2*T*log2 d + 6) lane-ops per atom; whole qmll_predict call: the fused kernel also streams the "
+                            "descriptor gradient once (gradient_stream_GBps, against hbm_gbs below)"},
+        "hbm_gbs_peak": pk["hbm_gbs"], "sm_mhz_during_run": sm_mhz}
 
-    line = {"metric": METRIC, "value": world * n_mol / (ms_step * 1e-3), "unit": UNIT, "n_gpus": world,
-            "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": ms_step, "higher_is_better": True,
-            "scaling": "weak", "vs_baseline": None, "dtype": "f32 (SORF), 3xTF32 with fp32 accumulate (ZtZ)",
+    n_mol_step = n_train + n_infer
+    line = {"metric": METRIC, "value": world * n_mol_step / (ms_step * 1e-3), "unit": UNIT, "n_gpus": world,
+            "steps": args.steps, "warmup": warm, "ms_per_step": ms_step, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None,
+            "dtype": "f32 (SORF), f16 hi/lo split tensor MMA with fp32 accumulate (ZtZ, fp32-level accuracy)",
             "data": "synthetic",
-            "config": {"workload": f"{w.name}: {n_mol} x 21-atom C9H8O4 configurations per GPU, d={w.model.d}, "
-                                   f"D={D}, T={w.model.T}, sigma={w.model.sigma}, dense gradient (21,128,21,3); "
-                                   f"train rows {rows} + predict E+F",
-                       "l2": "inputs larger than L2 (gradient 677 MB, A 2.1 GB); no explicit flush",
-                       "parallelism": f"dp{world} (molecules sharded, one all-reduce of ZtZ/Zty per step)"},
+            "config": {"workload": WORKLOAD.format(nt=n_train, ni=n_infer, rows=rows),
+                       "l2": "inputs larger than L2 (gradients 1.1 + 4.5 GB, A 2.7 GB); no explicit flush",
+                       "parallelism": f"dp{world} (configurations sharded, one all-reduce of the packed lower triangle of ZtZ + Zty per step)"},
             "breakdown_ms": {"forward_and_force_rows": fwd_ms, "normal_equations": ne_ms, "predict": pred_ms,
                              "syrk_kernel": kern_ms},
-            "ztz_tflops_fp32_equiv_half": achieved, "us_per_atom_predict": pred_ms * 1e3 / n_atoms,
-            "roofline": roofline, "sorf_rooflines": sorf_rooflines, "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks}
+            "ztz_tflops_fp32_equiv_half": roofline["achieved"], "us_per_atom_predict": pred_ms * 1e3 / wi.n_atoms,
+            "roofline": roofline, "sorf_rooflines": sorf_rooflines, "e2e": e2e, "gpu_launches": int(launches),
+            "clocks": clocks}
 
+    del A, ZtZ, dt_, di_
+    pkg.release_workspaces()
+    torch.cuda.empty_cache()
+    if not args.no_configs and world == 1:
+        line["configs"] = other_configs(pk, max(2, args.steps // 2))
     if not args.no_cpu_baseline and world == 1:
-        sample_mol = min(8, n_mol)
-        dt, cores, ws = time_oracle(args.config, D, sample_mol, 1, 0)
-        line["cpu_baseline"] = {"value": sample_mol / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
-                                "sample": f"{sample_mol} of {n_mol} molecules at full D={D}: forward + force rows + "
-                                          f"FP64 A^T A on its {ws.n_mol + 3 * ws.n_atoms} rows + predict, "
-                                          f"{dt:.1f} s of CPU work"}
+        st_wt, st_wi, cores = oracle_sample(D)
+        st = oracle_stages(st_wt, st_wi)
+        tot = sum(st.values())
+        line["cpu_baseline"] = {"value": (st_wt.n_mol + st_wi.n_mol) / tot, "unit": UNIT, "cores": cores, "kind": "oracle",
+                                "sample": describe_sample(st_wt, st_wi, D) + f", {tot:.1f} s of CPU work",
+                                "stage_seconds_on_sample": st,
+                                "extrapolated_full_step_s": extrapolate(st, st_wt, st_wi),
+                                "extrapolation": "linear in rows (every stage is), labelled; not measured"}
     print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()
 
 
-def report_configs(args):
-    """Absolute numbers and roofline fractions for all five configs (north_star), device-resident inputs."""
+def other_configs(pk, reps):
+    """Absolute numbers and the binding roofline fraction for the other timed configs (north_star): C2, C3, C5."""
     import torch
     import paper_2206_01580_b200 as pkg
     from paper_2206_01580_b200 import workload_io
     from workloads import make_workload
-    pk = peaks()
-    alu_peak = 148 * 128 * 1.965e9
+    fadd = pk["fadd_per_s"]
 
-    def tm(f, n):
+    def tm(f):
         for _ in range(2):
             f()
         torch.cuda.synchronize()
         a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         a.record()
-        for _ in range(n):
+        for _ in range(reps):
             f()
         b.record()
         torch.cuda.synchronize()
-        return a.elapsed_time(b) / n
+        return a.elapsed_time(b) / reps
 
-    for name, part in (("c1", "train"), ("c2", "train"), ("c3", "train"), ("c4", "train"), ("c4", "infer"), ("c5", "train")):
-        w = make_workload(name, part=part)
+    out = {}
+    for name in ("c2", "c3", "c5"):
+        w = make_workload(name)
         dp = workload_io.device_problem(w)
         p, m = dp.params, w.model
-        L, T, D, na, nm = m.d.bit_length() - 1, m.T, m.D, w.n_atoms, w.n_mol
-        out = {"config": w.name, "n_mol": nm, "n_atoms": na, "d": m.d, "D": D}
-        train = w.grad is not None and w.grad.layout == "dense" and part == "train"
-        if name == "c3" or train:
+        D, na, nm = m.D, w.n_atoms, w.n_mol
+        train = name == "c2"
+        fwd_ops, fr_ops, pr_ops = sorf_ops(w, train)
+        o = {"n_mol": nm, "n_atoms": na, "d": m.d, "D": D}
+        if name in ("c2", "c3"):
             rows = nm + (3 * na if train else 0)
             A = torch.empty((rows, D), dtype=torch.float32, device="cuda")
             if train:
-                t = tm(lambda: pkg.qmll_sorf_forward(p, dp.x, dp.elem, dp.mol_off, dp.grad, Z=A[:nm], G=A[nm:]), args.steps)
-                cols = 3.0 * sum(int(c) ** 2 for c in (w.mol_off[1:] - w.mol_off[:-1]))
-                ops = cols * D * (T * L + 2) + na * D * (T * L + 3)
+                t = tm(lambda: pkg.qmll_sorf_forward(p, dp.x, dp.elem, dp.mol_off, dp.grad, Z=A[:nm], G=A[nm:]))
             else:
-                t = tm(lambda: pkg.qmll_sorf_forward(p, dp.x, dp.elem, dp.mol_off, Z=A), args.steps)
-                ops = na * D * (T * L + 3)
-            out["forward_ms"] = t
-            out["forward_alu_frac"] = ops / (t * 1e-3) / alu_peak
-            out["forward_molecules_per_s"] = nm / (t * 1e-3)
+                t = tm(lambda: pkg.qmll_sorf_forward(p, dp.x, dp.elem, dp.mol_off, Z=A))
+            o.update({"forward_ms": t, "forward_molecules_per_s": nm / (t * 1e-3),
+                      "forward_alu_frac": (fwd_ops + fr_ops) / (t * 1e-3) / fadd})
             ZtZ = torch.empty((D, D), dtype=torch.float32, device="cuda")
             Zty = torch.empty((D,), dtype=torch.float32, device="cuda")
-            y = dp.y if dp.y is not None and dp.y.numel() == rows else torch.zeros(rows, device="cuda")
             pkg.time_normal_equations_kernel(True)
             pkg.collect_normal_equations_kernel_ms()
-            t = tm(lambda: pkg.qmll_normal_equations(A, y, ZtZ=ZtZ, Zty=Zty), max(1, args.steps // 2))
+            t = tm(lambda: pkg.qmll_normal_equations(A, dp.y, ZtZ=ZtZ, Zty=Zty))
             kms, kn = pkg.collect_normal_equations_kernel_ms()
             pkg.time_normal_equations_kernel(False)
-            out["normal_equations_ms"] = t
-            out["ztz_kernel_ms"] = kms / max(kn, 1)
             tf = rows * D * (D + 1.0) / (kms / max(kn, 1) * 1e-3) / 1e12
-            out["ztz_tflops_fp32eq_half"] = tf
-            out["ztz_frac_of_3xtf32_sustained"] = tf / (0.5 * pk["bf16_sustained"] / 3.0)
+            o.update({"normal_equations_ms": t, "ztz_kernel_ms": kms / max(kn, 1), "ztz_tflops_fp32eq_half": tf,
+                      "ztz_tensor_frac": tf / (pk["bf16_sustained"] / 3.0)})
             del A, ZtZ
         if name != "c3":
             E = torch.empty((nm,), dtype=torch.float32, device="cuda")
             F = torch.empty((na, 3), dtype=torch.float32, device="cuda")
-            t = tm(lambda: pkg.qmll_predict(p, dp.x, dp.elem, dp.mol_off, dp.alpha, dp.grad, energies=E, forces=F), args.steps)
-            gbytes = (w.grad.dense.nbytes if w.grad.layout == "dense" else w.grad.nbr_val.nbytes)
-            out.update({"predict_ms": t, "predict_molecules_per_s": nm / (t * 1e-3), "predict_us_per_atom": t * 1e3 / na,
-                        "predict_alu_frac": na * D * (2 * T * L + 6) / (t * 1e-3) / alu_peak,
-                        "predict_gradient_stream_GBps_if_alone": gbytes / (t * 1e-3) / 1e9})
-        print(json.dumps(out), flush=True)
+            t = tm(lambda: pkg.qmll_predict(p, dp.x, dp.elem, dp.mol_off, dp.alpha, dp.grad, energies=E, forces=F))
+            gbytes = w.grad.dense.nbytes if w.grad.layout == "dense" else w.grad.nbr_val.nbytes
+            o.update({"predict_ms": t, "predict_molecules_per_s": nm / (t * 1e-3), "predict_us_per_atom": t * 1e3 / na,
+                      "predict_alu_frac": pr_ops / (t * 1e-3) / fadd,
+                      "predict_gradient_stream_frac_of_hbm": gbytes / (t * 1e-3) / 1e9 / pk["hbm_gbs"]})
+        else:
+            E = torch.empty((nm,), dtype=torch.float32, device="cuda")
+            t = tm(lambda: pkg.qmll_predict(p, dp.x, dp.elem, dp.mol_off, dp.alpha, energies=E))
+            o.update({"predict_energies_ms": t, "predict_molecules_per_s": nm / (t * 1e-3)})
+        out[name] = o
         del dp, w
         pkg.release_workspaces()
         torch.cuda.empty_cache()
+    return out
+
+
+def spawn_ranks(args):
+    """`python bench.py --gpus N` without a launcher: start N ranks of this script under torch.distributed.run."""
+    argv = [a for a in sys.argv[1:]]
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+           "--master-addr", "127.0.0.1", "--master-port", str(29500 + os.getpid() % 2000), os.path.abspath(__file__)] + argv
+    sys.exit(subprocess.call(cmd))
 
 
 if __name__ == "__main__":
     a = parse()
-    if a.report_configs:
-        report_configs(a)
-    elif a.impl == "reference":
+    if a.impl == "reference":
         reference_arm(a)
+    elif a.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        spawn_ranks(a)
     else:
         ours_arm(a)

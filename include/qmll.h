@@ -115,6 +115,13 @@ int qmll_normal_equations_mode(const float* A, const float* y, int64_t rows, int
                                float* ZtZ, float* Zty, void* workspace, size_t workspace_bytes, int32_t mode,
                                void* cuda_stream);
 
+/* Exchange step of data-parallel training: the normal equations are sums over rows, so
+ * ranks that own different molecules add their ZtZ / Zty.  ZtZ is symmetric: pack its lower triangle row by row
+ * (row i holds i + 1 entries at offset i (i + 1) / 2; D (D + 1) / 2 floats), all-reduce the packed buffer, unpack
+ * (writes both triangles: exactly symmetric).  D <= 65535. */
+int qmll_pack_lower(const float* ZtZ, int32_t D, float* packed, void* cuda_stream);
+int qmll_unpack_lower(const float* packed, int32_t D, float* ZtZ, void* cuda_stream);
+
 /* Steps a1-a6 composed: energies[M] = Z[M, :] . alpha (eq. 15) and, if grad != NULL, forces as in
  * qmll_sorf_backward_forces, from one pass that shares u between cos and sin; Z is never materialised.
  *   energies [n_mol] fp32, overwritten;  forces [n_atoms, 3] fp32 or NULL (then grad must be NULL). */

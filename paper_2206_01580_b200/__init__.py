@@ -29,7 +29,7 @@ EXPORTS = ("qmll_solve", "qmll_sorf_forward", "qmll_sorf_backward_forces", "qmll
            "qmll_normal_equations_mode", "qmll_predict", "qmll_workspace_bytes", "qmll_normal_equations_min_workspace",
            "qmll_normal_equations_workspace", "qmll_normal_equations_min_workspace_mode", "qmll_status_string",
            "qmll_launch_count", "qmll_reset_launch_count", "qmll_time_normal_equations_kernel",
-           "qmll_collect_normal_equations_kernel_ms", "qmll_microbench")
+           "qmll_collect_normal_equations_kernel_ms", "qmll_microbench", "qmll_pack_lower", "qmll_unpack_lower")
 
 
 class _CParams(ctypes.Structure):
@@ -74,6 +74,10 @@ def load_library() -> ctypes.CDLL:
     lib.qmll_normal_equations_min_workspace_mode.argtypes = [i32, i32]
     lib.qmll_normal_equations_min_workspace_mode.restype = sz
     lib.qmll_predict.argtypes = [pp, vp, vp, vp, i64, i32, vp, gp, vp, vp, vp, sz, vp]
+    lib.qmll_pack_lower.argtypes = [vp, i32, vp, vp]
+    lib.qmll_pack_lower.restype = ctypes.c_int
+    lib.qmll_unpack_lower.argtypes = [vp, i32, vp, vp]
+    lib.qmll_unpack_lower.restype = ctypes.c_int
     for name in ("qmll_sorf_forward", "qmll_sorf_backward_forces", "qmll_normal_equations", "qmll_predict"):
         getattr(lib, name).restype = ctypes.c_int
     lib.qmll_solve.argtypes = [vp, vp, i32, ctypes.c_double, vp, vp, vp, sz, vp]
@@ -266,6 +270,24 @@ def qmll_normal_equations(A, y=None, ZtZ=None, Zty=None, accumulate: bool = Fals
                                           _dev(ZtZ, torch.float32, "ZtZ"), _dev(Zty, torch.float32, "Zty"),
                                           ctypes.c_void_p(ws.data_ptr()), min(ws.numel(), nb), mode, _stream()))
     return ZtZ, Zty
+
+
+def qmll_pack_lower(ZtZ, packed=None):
+    """Row-packed lower triangle of ZtZ [D (D + 1) / 2]: include/qmll.h qmll_pack_lower."""
+    D = int(ZtZ.shape[0])
+    if packed is None:
+        packed = torch.empty((D * (D + 1) // 2,), dtype=torch.float32, device=ZtZ.device)
+    _check(load_library().qmll_pack_lower(_dev(ZtZ, torch.float32, "ZtZ"), D, _dev(packed, torch.float32, "packed"),
+                                          _stream()))
+    return packed
+
+
+def qmll_unpack_lower(packed, ZtZ):
+    """ZtZ (both triangles) from its row-packed lower triangle: include/qmll.h qmll_unpack_lower."""
+    D = int(ZtZ.shape[0])
+    _check(load_library().qmll_unpack_lower(_dev(packed, torch.float32, "packed"), D, _dev(ZtZ, torch.float32, "ZtZ"),
+                                            _stream()))
+    return ZtZ
 
 
 def qmll_solve(ZtZ, Zty, lam: float, alpha=None):

@@ -207,6 +207,19 @@ int qmll_normal_equations(const float* A, const float* y, int64_t rows, int32_t 
                                     QMLL_NE_SPLIT_F16, cuda_stream);
 }
 
+int qmll_pack_lower(const float* ZtZ, int32_t D, float* packed, void* cuda_stream) {
+  if (!ZtZ || !packed || D <= 0 || D > 65535) return QMLL_ERR_INVALID_ARG;
+  int rc = check_device();
+  if (rc) return rc;
+  return syrk_pack_lower(ZtZ, D, packed, static_cast<cudaStream_t>(cuda_stream));
+}
+int qmll_unpack_lower(const float* packed, int32_t D, float* ZtZ, void* cuda_stream) {
+  if (!ZtZ || !packed || D <= 0 || D > 65535) return QMLL_ERR_INVALID_ARG;
+  int rc = check_device();
+  if (rc) return rc;
+  return syrk_unpack_lower(packed, D, ZtZ, static_cast<cudaStream_t>(cuda_stream));
+}
+
 int qmll_solve(const float* ZtZ, const float* Zty, int32_t D, double lambda, float* alpha, int32_t* info,
                void* workspace, size_t workspace_bytes, void* cuda_stream) {
   if (!ZtZ || !Zty || !alpha || !info || D <= 0 || !(lambda >= 0.0)) return QMLL_ERR_INVALID_ARG;

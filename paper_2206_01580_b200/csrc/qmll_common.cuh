@@ -92,6 +92,9 @@ size_t syrk_full_workspace(int64_t rows, int32_t D, int mode);
 int syrk_normal_equations(const float* A, const float* y, int64_t rows, int32_t D, int accumulate, float* ZtZ,
                           float* Zty, void* ws, size_t ws_bytes, int mode, cudaStream_t st);
 
+int syrk_pack_lower(const float* C, int32_t D, float* packed, cudaStream_t st);
+int syrk_unpack_lower(const float* packed, int32_t D, float* C, cudaStream_t st);
+
 // ---- solve (solve_kernels.cu) ------------------------------------------------------------------------------
 size_t solve_workspace_bytes(int32_t D);
 int solve_normal_equations(const float* ZtZ, const float* Zty, int32_t D, double lambda, float* alpha, int32_t* info,

@@ -456,6 +456,51 @@ mirror_lower_kernel(float* __restrict__ C, int D) {
 }
 
 // ---------------------------------------------------------------------------------------------------
+// 4. multi-GPU exchange helpers: the lower triangle of ZtZ packed row by row (row i: i + 1 entries at offset
+//    i (i + 1) / 2), so that the one all-reduce of the data-parallel training step moves D (D + 1) / 2 values
+//    instead of D^2; unpack writes both triangles (exactly symmetric again).
+// ---------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256)
+pack_lower_kernel(const float* __restrict__ C, int D, float* __restrict__ packed) {
+  const int i = blockIdx.y;
+  const int j = blockIdx.x * blockDim.x + threadIdx.x;
+  if (j <= i) packed[(size_t)i * (i + 1) / 2 + j] = C[(size_t)i * D + j];
+}
+__global__ void __launch_bounds__(256)
+unpack_lower_kernel(const float* __restrict__ packed, int D, float* __restrict__ C) {
+  __shared__ float t[32][33];
+  const int bi = blockIdx.y, bj = blockIdx.x;  // lower-triangle source block: rows 32 bi, cols 32 bj, bj <= bi
+  if (bj > bi) return;
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  for (int rr = warp; rr < 32; rr += 8) {
+    const int i = bi * 32 + rr, j = bj * 32 + lane;
+    float v = 0.f;
+    if (i < D && j <= i) {
+      v = packed[(size_t)i * (i + 1) / 2 + j];
+      C[(size_t)i * D + j] = v;
+    }
+    t[rr][lane] = v;
+  }
+  __syncthreads();
+  for (int rr = warp; rr < 32; rr += 8) {      // mirrored block: rows 32 bj + rr, cols 32 bi + lane
+    const int i = bj * 32 + rr, j = bi * 32 + lane;
+    if (i < D && j < D && i < j) C[(size_t)i * D + j] = t[lane][rr];
+  }
+}
+int syrk_pack_lower(const float* C, int32_t D, float* packed, cudaStream_t st) {
+  dim3 g((unsigned)((D + 255) / 256), (unsigned)D);
+  pack_lower_kernel<<<g, 256, 0, st>>>(C, D, packed);
+  QMLL_LAUNCH_CHECK("pack_lower_kernel");
+  return QMLL_OK;
+}
+int syrk_unpack_lower(const float* packed, int32_t D, float* C, cudaStream_t st) {
+  dim3 g((unsigned)((D + 31) / 32), (unsigned)((D + 31) / 32));
+  unpack_lower_kernel<<<g, 256, 0, st>>>(packed, D, C);
+  QMLL_LAUNCH_CHECK("unpack_lower_kernel");
+  return QMLL_OK;
+}
+
+// ---------------------------------------------------------------------------------------------------
 // Host side
 // ---------------------------------------------------------------------------------------------------
 int device_sm_count();

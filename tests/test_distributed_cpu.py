@@ -10,7 +10,9 @@ import torch
 import torch.distributed as dist
 import torch.multiprocessing as mp
 
-from paper_2206_01580_b200.distributed import shard_range, allreduce_normal_equations, max_over_ranks
+from paper_2206_01580_b200.distributed import (shard_range, allreduce_normal_equations, max_over_ranks,
+                                                NormalEquationsReducer, pack_lower_reference, unpack_lower_reference,
+                                                allreduce_forces)
 
 
 def test_shard_range_partitions():
@@ -21,6 +23,18 @@ def test_shard_range_partitions():
             assert all(got[i][1] == got[i + 1][0] for i in range(world - 1))
             sizes = [b - a for a, b in got]
             assert max(sizes) - min(sizes) <= 1
+
+
+def test_pack_lower_roundtrip():
+    rng = np.random.default_rng(0)
+    for D in (1, 2, 7, 33):
+        A = rng.standard_normal((D + 3, D)).astype(np.float32)
+        S = torch.from_numpy(A.T @ A)
+        p = pack_lower_reference(S)
+        assert p.numel() == D * (D + 1) // 2
+        for i in range(D):                       # row i holds i + 1 entries at offset i (i + 1) / 2
+            assert torch.equal(p[i * (i + 1) // 2: i * (i + 1) // 2 + i + 1], S[i, : i + 1])
+        assert torch.equal(unpack_lower_reference(p, D), S)
 
 
 def _worker(rank, world, port, ret):
@@ -35,7 +49,17 @@ def _worker(rank, world, port, ret):
     allreduce_normal_equations(ZtZ, Zty)
     t = max_over_ranks(float(rank + 1), "cpu")
     ok = (np.allclose(ZtZ.numpy(), A.T @ A, rtol=1e-5, atol=1e-5) and np.allclose(Zty.numpy(), A.T @ y, rtol=1e-5, atol=1e-5)
-          and t == float(world))
+          and t == float(world) and np.array_equal(ZtZ.numpy(), ZtZ.numpy().T))
+    # persistent reducer, ZtZ only, twice in a row (buffer reuse)
+    red = NormalEquationsReducer(16, "cpu")
+    for _ in range(2):
+        Z2 = torch.from_numpy(A[lo:hi].T @ A[lo:hi])
+        red.allreduce(Z2, None)
+        ok = ok and np.allclose(Z2.numpy(), A.T @ A, rtol=1e-5, atol=1e-5)
+    # inference sharded over atoms: forces scattered by every rank are summed
+    F = torch.zeros((37, 3)); F[lo:hi] = 1.0; F[(lo + 5) % 37] += 2.0
+    allreduce_forces(F)
+    ok = ok and abs(float(F.sum()) - (37 * 3 + 2.0 * 3 * world)) < 1e-4
     ret[rank] = bool(ok)
     dist.destroy_process_group()
 

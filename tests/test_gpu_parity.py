@@ -173,6 +173,21 @@ def test_normal_equations_wide_dynamic_range(q):
             assert rel(Z16[i:i + 128, j:j + 128], ZtZo[i:i + 128, j:j + 128]) <= TOL
 
 
+@pytest.mark.parametrize("D", [1, 33, 520, 2048])
+def test_pack_unpack_lower_triangle(q, D):
+    """The multi-GPU exchange helpers: row-packed lower triangle and its symmetric unpack (bit-exact data movement)."""
+    pkg, wio, torch = q
+    from paper_2206_01580_b200.distributed import pack_lower_reference
+    g = torch.Generator(device="cuda").manual_seed(D)
+    S = torch.randn((D, D), device="cuda", generator=g)
+    S = (S + S.T).contiguous()
+    packed = pkg.qmll_pack_lower(S)
+    assert torch.equal(packed, pack_lower_reference(S))
+    out = torch.full((D, D), float("nan"), device="cuda")
+    pkg.qmll_unpack_lower(packed, out)
+    assert torch.equal(out, S)
+
+
 def test_normal_equations_zero_rows(q):
     pkg, wio, torch = q
     A = torch.empty((0, 256), dtype=torch.float32, device="cuda")
