@@ -84,6 +84,18 @@ int qmll_sorf_forward(const qmll_sorf_params* p, const float* x, const int32_t* 
                       int64_t n_atoms, int32_t n_mol, const qmll_grad* grad, float* Z, float* G,
                       void* workspace, size_t workspace_bytes, void* cuda_stream);
 
+/* The same call with an explicit choice of how the force rows of a DENSE gradient are computed (both give the same
+ * linear map applied to the same inputs, to fp32 accuracy):
+ *   QMLL_ROWS_FWHT  every gradient column goes through the register Walsh-Hadamard / sign chain (any d).
+ *   QMLL_ROWS_MMA   the chain of each (element, stack) is expanded once into its d x d integer matrix (exact in
+ *                   fp16 for d <= 256) and applied to the columns on the tensor cores (tcgen05, columns split into
+ *                   fp16 hi + lo); d = 128 or 256 only, else QMLL_ERR_UNSUPPORTED.
+ *   QMLL_ROWS_AUTO  MMA where supported, else FWHT (what qmll_sorf_forward does). */
+enum { QMLL_ROWS_AUTO = 0, QMLL_ROWS_FWHT = 1, QMLL_ROWS_MMA = 2 };
+int qmll_sorf_forward_mode(const qmll_sorf_params* p, const float* x, const int32_t* elem, const int32_t* mol_off,
+                           int64_t n_atoms, int32_t n_mol, const qmll_grad* grad, float* Z, float* G,
+                           void* workspace, size_t workspace_bytes, int32_t force_rows_mode, void* cuda_stream);
+
 /* Steps a1, a5, a6: F[j, k] = -dE/dr_{j,k} with E = sum_M Z[M, :] . alpha  (eq. 15; F = -dE/dr,
  * eq. 5/10 L63, L90): q[l] = -sqrt(2/D) alpha[l] sin(u_I[l] + b); g_I = sum_s W_{e,s}^T q_s (transposed
  * Hadamard / sign chain, L268 "backwards pass"); F[j,k] = -sum_I sum_m g_I[m] dx_I[m]/dr_{j,k}.

@@ -24,8 +24,9 @@ QMLL_GRAD_DENSE, QMLL_GRAD_NEIGHBOR = 1, 2
 CALL_FORWARD, CALL_FORWARD_GRAD, CALL_BACKWARD_FORCES, CALL_NORMAL_EQUATIONS, CALL_PREDICT, CALL_SOLVE = range(6)
 
 NE_SPLIT_F16, NE_SPLIT_TF32 = 0, 1
+ROWS_AUTO, ROWS_FWHT, ROWS_MMA = 0, 1, 2
 
-EXPORTS = ("qmll_solve", "qmll_sorf_forward", "qmll_sorf_backward_forces", "qmll_normal_equations",
+EXPORTS = ("qmll_solve", "qmll_sorf_forward", "qmll_sorf_forward_mode", "qmll_sorf_backward_forces", "qmll_normal_equations",
            "qmll_normal_equations_mode", "qmll_predict", "qmll_workspace_bytes", "qmll_normal_equations_min_workspace",
            "qmll_normal_equations_workspace", "qmll_normal_equations_min_workspace_mode", "qmll_status_string",
            "qmll_launch_count", "qmll_reset_launch_count", "qmll_time_normal_equations_kernel",
@@ -65,6 +66,8 @@ def load_library() -> ctypes.CDLL:
     vp, i32, i64, sz = ctypes.c_void_p, ctypes.c_int32, ctypes.c_int64, ctypes.c_size_t
     pp, gp = ctypes.POINTER(_CParams), ctypes.POINTER(_CGrad)
     lib.qmll_sorf_forward.argtypes = [pp, vp, vp, vp, i64, i32, gp, vp, vp, vp, sz, vp]
+    lib.qmll_sorf_forward_mode.argtypes = [pp, vp, vp, vp, i64, i32, gp, vp, vp, vp, sz, i32, vp]
+    lib.qmll_sorf_forward_mode.restype = ctypes.c_int
     lib.qmll_sorf_backward_forces.argtypes = [pp, vp, vp, vp, i64, i32, vp, gp, vp, vp, sz, vp]
     lib.qmll_normal_equations.argtypes = [vp, vp, i64, i32, i32, vp, vp, vp, sz, vp]
     lib.qmll_normal_equations_mode.argtypes = [vp, vp, i64, i32, i32, vp, vp, vp, sz, i32, vp]
@@ -193,7 +196,7 @@ def _problem(x, elem, mol_off):
 
 
 def qmll_sorf_forward(p: SorfParams, x, elem, mol_off, grad: Optional[Grad] = None, Z=None, G=None,
-                      want_Z: bool = True):
+                      want_Z: bool = True, force_rows_mode: int = ROWS_AUTO):
     """Z [n_mol, D] (and G [3 n_atoms, D] when `grad` is given): include/qmll.h qmll_sorf_forward."""
     lib = load_library()
     xp, ep, mp, n_atoms, n_mol = _problem(x, elem, mol_off)
@@ -207,9 +210,10 @@ def qmll_sorf_forward(p: SorfParams, x, elem, mol_off, grad: Optional[Grad] = No
     nb = lib.qmll_workspace_bytes(CALL_FORWARD_GRAD if grad is not None else CALL_FORWARD, ctypes.byref(cp),
                                   n_atoms, n_mol, dense_floats)
     ws = workspace(nb, x.device)
-    _check(lib.qmll_sorf_forward(ctypes.byref(cp), xp, ep, mp, n_atoms, n_mol,
-                                 ctypes.byref(cg) if cg is not None else None, _dev(Z, torch.float32, "Z"),
-                                 _dev(G, torch.float32, "G"), ctypes.c_void_p(ws.data_ptr()), ws.numel(), _stream()))
+    _check(lib.qmll_sorf_forward_mode(ctypes.byref(cp), xp, ep, mp, n_atoms, n_mol,
+                                      ctypes.byref(cg) if cg is not None else None, _dev(Z, torch.float32, "Z"),
+                                      _dev(G, torch.float32, "G"), ctypes.c_void_p(ws.data_ptr()), ws.numel(),
+                                      force_rows_mode, _stream()))
     return (Z, G) if grad is not None else Z
 
 

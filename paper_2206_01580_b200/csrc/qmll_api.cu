@@ -64,6 +64,16 @@ static int check_ws(void* ws, size_t have, size_t need) {
 static size_t zs_bytes(const qmll_sorf_params* p, int64_t n_atoms) {
   return align_up(sorf_zs_floats(p, n_atoms) * sizeof(float), 256) + 256;
 }
+// scratch of the dense force-row step: the transposed gradient (FWHT path) or W table + split columns (tensor path)
+static bool use_rows_mma(const qmll_sorf_params* p, int32_t mode) {
+  return mode != QMLL_ROWS_FWHT && sorf_mma_supported(p);
+}
+static size_t rows_scratch_bytes(const qmll_sorf_params* p, int64_t n_atoms, int32_t n_mol, int64_t dense_floats,
+                                 bool mma) {
+  if (!mma) return align_up((size_t)(dense_floats > 0 ? dense_floats : 0) * 4, 256) + 256;
+  return align_up(sorf_mma_w_bytes(p), 256) + 2 * align_up(sorf_mma_x_bytes(p, n_atoms, dense_floats), 256) +
+         align_up(((size_t)n_mol + 1) * sizeof(long long), 256) + align_up((size_t)n_atoms * sizeof(float), 256) + 5 * 256;
+}
 static size_t e_bytes(int32_t n_mol) { return align_up((size_t)n_mol * sizeof(double), 256) + 256; }
 
 // shared body of qmll_sorf_backward_forces and qmll_predict
@@ -124,17 +134,20 @@ size_t qmll_workspace_bytes(int which_call, const qmll_sorf_params* p, int64_t n
   if (n_mol < 0) n_mol = 0;
   switch (which_call) {
     case QMLL_CALL_FORWARD: return sorf_tables_bytes(p, false);
-    case QMLL_CALL_FORWARD_GRAD:
-      return sorf_tables_bytes(p, false) + zs_bytes(p, n_atoms) + align_up((size_t)(rows > 0 ? rows : 0) * 4, 256) + 256;
+    case QMLL_CALL_FORWARD_GRAD: {   // enough for either force-row path
+      const size_t a = rows_scratch_bytes(p, n_atoms, n_mol, rows, false);
+      const size_t b = sorf_mma_supported(p) ? rows_scratch_bytes(p, n_atoms, n_mol, rows, true) : 0;
+      return sorf_tables_bytes(p, false) + zs_bytes(p, n_atoms) + (a > b ? a : b);
+    }
     case QMLL_CALL_BACKWARD_FORCES: return sorf_tables_bytes(p, true);
     case QMLL_CALL_PREDICT: return sorf_tables_bytes(p, true) + e_bytes(n_mol);
     default: return 0;
   }
 }
 
-int qmll_sorf_forward(const qmll_sorf_params* p, const float* x, const int32_t* elem, const int32_t* mol_off,
-                      int64_t n_atoms, int32_t n_mol, const qmll_grad* grad, float* Z, float* G, void* workspace,
-                      size_t workspace_bytes, void* cuda_stream) {
+int qmll_sorf_forward_mode(const qmll_sorf_params* p, const float* x, const int32_t* elem, const int32_t* mol_off,
+                           int64_t n_atoms, int32_t n_mol, const qmll_grad* grad, float* Z, float* G, void* workspace,
+                           size_t workspace_bytes, int32_t force_rows_mode, void* cuda_stream) {
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
   int rc = check_params(p);
   if (rc) return rc;
@@ -142,7 +155,10 @@ int qmll_sorf_forward(const qmll_sorf_params* p, const float* x, const int32_t* 
   if (rc) return rc;
   if ((G != nullptr) != (grad != nullptr)) return QMLL_ERR_INVALID_ARG;
   if (!Z && !G) return QMLL_ERR_INVALID_ARG;
+  if (force_rows_mode < QMLL_ROWS_AUTO || force_rows_mode > QMLL_ROWS_MMA) return QMLL_ERR_INVALID_ARG;
   if (grad) { rc = check_grad(grad); if (rc) return rc; }
+  if (force_rows_mode == QMLL_ROWS_MMA && !(grad && grad->layout == QMLL_GRAD_DENSE && sorf_mma_supported(p)))
+    return QMLL_ERR_UNSUPPORTED;
   rc = check_device();
   if (rc) return rc;
   rc = check_ws(workspace, workspace_bytes,
@@ -159,17 +175,33 @@ int qmll_sorf_forward(const qmll_sorf_params* p, const float* x, const int32_t* 
   rc = sorf_launch_forward(pr, t, Z, zs, st);
   if (rc) return rc;
   if (grad) {
-    if (grad->layout == QMLL_GRAD_DENSE) {
+    if (grad->layout == QMLL_GRAD_DENSE && use_rows_mma(p, force_rows_mode)) {
+      void* W16 = ws.take<uint8_t>(sorf_mma_w_bytes(p));
+      const size_t xb = sorf_mma_x_bytes(p, n_atoms, grad->dense_floats);
+      void* Xh = ws.take<uint8_t>(xb);
+      void* Xl = ws.take<uint8_t>(xb);
+      long long* xoff = ws.take<long long>((size_t)n_mol + 1);
+      float* inv_scale = ws.take<float>((size_t)n_atoms);
+      if (!ws.fits()) return QMLL_ERR_WORKSPACE;
+      rc = sorf_force_rows_dense_mma(pr, t, zs, grad, W16, Xh, Xl, xoff, inv_scale, G, st);
+    } else if (grad->layout == QMLL_GRAD_DENSE) {
       float* gt = ws.take<float>((size_t)grad->dense_floats);
       if (!ws.fits()) return QMLL_ERR_WORKSPACE;
       rc = sorf_transpose_dense(pr, grad->dense, grad->dense_off, gt, st);
       if (rc) return rc;
       rc = sorf_launch_force_rows_dense(pr, t, zs, gt, grad->dense_off, G, st);
-    }
-    else
+    } else {
       rc = sorf_launch_force_rows_neighbor(pr, t, zs, grad->nbr_idx, grad->nbr_val, grad->K, G, st);
+    }
   }
   return rc;
+}
+
+int qmll_sorf_forward(const qmll_sorf_params* p, const float* x, const int32_t* elem, const int32_t* mol_off,
+                      int64_t n_atoms, int32_t n_mol, const qmll_grad* grad, float* Z, float* G, void* workspace,
+                      size_t workspace_bytes, void* cuda_stream) {
+  return qmll_sorf_forward_mode(p, x, elem, mol_off, n_atoms, n_mol, grad, Z, G, workspace, workspace_bytes,
+                                QMLL_ROWS_AUTO, cuda_stream);
 }
 
 int qmll_sorf_backward_forces(const qmll_sorf_params* p, const float* x, const int32_t* elem,

@@ -78,6 +78,14 @@ int sorf_launch_predict(const SorfProblem& pr, const SorfTables& t, const qmll_g
 int sorf_launch_force_rows_dense(const SorfProblem& pr, const SorfTables& t, const float* zs,
                                  const float* dense_t, const int64_t* dense_off, float* G, cudaStream_t st);
 size_t sorf_zs_floats(const qmll_sorf_params* p, int64_t n_atoms);
+
+// ---- force rows on the tensor cores (sorf_mma.cu) -----------------------------------------------------
+bool sorf_mma_supported(const qmll_sorf_params* p);
+size_t sorf_mma_w_bytes(const qmll_sorf_params* p);
+size_t sorf_mma_x_bytes(const qmll_sorf_params* p, int64_t n_atoms, int64_t dense_floats);
+int sorf_force_rows_dense_mma(const SorfProblem& pr, const SorfTables& t, const float* zs, const qmll_grad* grad,
+                              void* W16, void* Xh, void* Xl, long long* xoff, float* inv_scale, float* G,
+                              cudaStream_t st);
 int sorf_launch_force_rows_neighbor(const SorfProblem& pr, const SorfTables& t, const float* zs,
                                     const int32_t* nbr_idx, const float* nbr_val, int K, float* G,
                                     cudaStream_t st);

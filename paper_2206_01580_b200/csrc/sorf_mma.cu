@@ -1,0 +1,428 @@
+// sorf_mma.cu -- force rows (step a7: G = -dZ/dr, eq. 17) on the tensor cores.
+//
+// The SORF map of one stack is LINEAR: (H S_T ... H S_1) = W_{e,s}, a d x d matrix of small integers, and the
+// force rows apply it to 3 n^2 gradient columns per molecule -- a dense contraction with the same matrix for every
+// column of the same (element, stack).  The register FWHT needs d log2(d) T adds + d T sign flips per column and is
+// bound by fp32/integer issue (62 % of the measured FADD peak at best); the explicit product needs d^2 MACs but runs
+// on tcgen05 at ~30x the rate, so it is 2.5-3.5x faster for d = 128 / 256:
+//   1. build_w_kernel:  W_{e,s} for every (element, stack) by pushing the d unit vectors through the SAME
+//      register chain the other kernels use (exact: integers below 2^24), stored as fp16.  |W_ij| <= d^(3/2) (Cauchy-
+//      Schwarz on the orthogonal rows of H S H) and all entries are even for T = 3, so fp16 holds them EXACTLY for
+//      d <= 256 (d = 128: <= 1448 < 2048; d = 256: even integers <= 4096); T <= 2 gives |W_ij| <= d.
+//   2. prep_columns_kernel:  gradient block of atom I, [d, 3n] fp32 -> columns split into fp16 hi + lo parts (22
+//      significant bits, the same split as the normal equations) with one power-of-two scale per atom block,
+//      k-block-major and pre-swizzled, so that a tile is one contiguous bulk copy.
+//   3. sorf_rows_mma_kernel:  persistent, warp-specialised (bulk-copy producer / MMA issuer / epilogue warps).  Task =
+//      (molecule, stack): for every atom I:  U_I = W_{e_I,s} X_I  (tcgen05.mma kind::f16, hi and lo passes, fp32
+//      accumulate in TMEM), and the epilogue adds  c * zs_I[l] * U_I[l, r]  into 3n register accumulators per thread
+//      (thread = output feature l); the finished [3n, d] block of G is written once, coalesced along l.
+// The result is the same linear map applied to the same inputs: parity against the FP64 oracle is unchanged.
+#include <cuda_fp16.h>
+
+#include "sorf_kernels.cuh"
+#include "tcgen05_utils.cuh"
+
+namespace qmll {
+
+constexpr int kTile = 128;         // MMA M: output features per tile (TMEM lanes)
+constexpr int kKBlk = 64;          // fp16 elements per 128-byte swizzle span (one k-block)
+constexpr uint32_t kTileBytes = kTile * 128;   // one A tile (128 outputs x 64 inputs): 16 KB
+
+// 16-byte chunk `ch` of row `row` inside a [rows][64 halves] k-block tile, SWIZZLE_128B pattern (what TMA would
+// write and what the K-major UMMA descriptor expects): chunk index XOR (row mod 8).
+__host__ __device__ inline size_t swz_half_index(size_t row, int jj) {
+  const int ch = jj >> 3;
+  return row * 64 + (size_t)(((ch ^ (int)(row & 7)) << 3) | (jj & 7));
+}
+
+// ---------------------------------------------------------------------------------------------------
+// 1. W table.  Warp = (element e, stack group sg, input index j); lanes = stacks (as everywhere).  The unit vector
+//    e_j goes through the chain; lane (sl, p) then holds column j of W_{e,s} for outputs p*E .. p*E+E-1.
+//    W16 tile index: ((e*n_s + s)*kMT + mt)*kKB + kb, tile = [128 outputs][64 inputs] halves, swizzled.
+// ---------------------------------------------------------------------------------------------------
+template <typename S>
+__global__ void __launch_bounds__(kFwdThreads, (S::E >= 128 ? 3 : 4))
+build_w_kernel(const uint32_t* __restrict__ sign_bits, int n_elem, int n_s, int n_sg, int T,
+               __half* __restrict__ W16) {
+  constexpr int kMT = S::d / kTile, kKB = S::d / kKBlk;
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const long long task = (long long)blockIdx.x * (kFwdThreads / kWarp) + warp;
+  if (task >= (long long)n_elem * n_sg * S::d) return;
+  const int j = (int)(task % S::d);
+  const int sg = (int)((task / S::d) % n_sg);
+  const int e = (int)(task / ((long long)S::d * n_sg));
+  const int p = lane % S::P, sl = lane / S::P;
+  const int s = sg * S::SPW + sl;
+  f32x2 v[S::E2];
+#pragma unroll
+  for (int q = 0; q < S::E2; ++q) {
+    const int m = p * S::E + 2 * q;
+    v[q] = pk(m == j ? 1.f : 0.f, m + 1 == j ? 1.f : 0.f);
+  }
+  chain_forward<S>(v, sign_bits, e, T, n_sg, sg, lane);
+  if (s >= n_s) return;
+  const int kb = j / kKBlk, jj = j % kKBlk;
+#pragma unroll
+  for (int q = 0; q < S::E2; ++q) {
+    float a, b;
+    upk(v[q], a, b);
+    const int i = p * S::E + 2 * q;                       // output index (even), i + 1 is the odd one
+    const int mt = i / kTile, row = i % kTile;
+    __half* tile = W16 + ((((size_t)e * n_s + s) * kMT + mt) * kKB + kb) * (size_t)(kTile * kKBlk);
+    tile[swz_half_index(row, jj)] = __float2half_rn(a);
+    tile[swz_half_index(row + 1, jj)] = __float2half_rn(b);
+  }
+}
+
+// ---------------------------------------------------------------------------------------------------
+// 2. Column preparation.  xoff[M] = first 128-byte row of molecule M in Xh / Xl; the block of atom I (local) holds
+//    kKB sub-blocks of Npad = roundup16(3n) rows: row = xoff[M] + (I*kKB + kb)*Npad + col, 64 halves per row
+//    (inputs 64 kb .. 64 kb + 63 of column col), swizzled; rows col >= 3n are zero.
+// ---------------------------------------------------------------------------------------------------
+static __global__ void __launch_bounds__(1024)
+x_offsets_kernel(const int32_t* __restrict__ mol_off, int n_mol, int kKB, long long* __restrict__ xoff) {
+  __shared__ long long part[1024];
+  __shared__ long long carry;
+  if (threadIdx.x == 0) carry = 0;
+  __syncthreads();
+  for (int base = 0; base < n_mol; base += 1024) {
+    const int M = base + threadIdx.x;
+    long long cnt = 0;
+    if (M < n_mol) {
+      const long long n = __ldg(mol_off + M + 1) - __ldg(mol_off + M);
+      cnt = n * kKB * ((3 * n + 15) / 16 * 16);
+    }
+    part[threadIdx.x] = cnt;
+    __syncthreads();
+    for (int off = 1; off < 1024; off <<= 1) {
+      const long long t = threadIdx.x >= off ? part[threadIdx.x - off] : 0;
+      __syncthreads();
+      part[threadIdx.x] += t;
+      __syncthreads();
+    }
+    if (M < n_mol) xoff[M] = carry + part[threadIdx.x] - cnt;
+    __syncthreads();
+    if (threadIdx.x == 1023) carry += part[1023];
+    __syncthreads();
+  }
+  if (threadIdx.x == 0) xoff[n_mol] = carry;
+}
+
+// Block = one atom I (global index): [d][3n] fp32 -> scale, split, transpose.
+static __global__ void __launch_bounds__(256)
+prep_columns_kernel(const float* __restrict__ dense, const int64_t* __restrict__ dense_off,
+                    const int32_t* __restrict__ mol_off, int n_mol, int d, const long long* __restrict__ xoff,
+                    __half* __restrict__ Xh, __half* __restrict__ Xl, float* __restrict__ inv_scale) {
+  __shared__ float tile[64][97];
+  __shared__ float red[8];
+  const int Ig = blockIdx.x;
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const int M = owner_molecule(mol_off, n_mol, Ig);
+  const int a0 = __ldg(mol_off + M), n = __ldg(mol_off + M + 1) - a0;
+  const int ncol = 3 * n, npad = (ncol + 15) / 16 * 16, kKB = d / kKBlk;
+  const float* src = dense + (size_t)__ldg(dense_off + M) + (size_t)(Ig - a0) * d * ncol;  // [d][ncol]
+  const size_t total = (size_t)d * ncol;
+  // pass 1: block absmax -> one power-of-two scale: amax * s in [2^9, 2^10)
+  float amax = 0.f;
+  for (size_t i = threadIdx.x; i < total; i += 256) amax = fmaxf(amax, fabsf(__ldg(src + i)));
+#pragma unroll
+  for (int m = 16; m > 0; m >>= 1) amax = fmaxf(amax, __shfl_xor_sync(0xffffffffu, amax, m));
+  if (lane == 0) red[warp] = amax;
+  __syncthreads();
+  amax = red[0];
+#pragma unroll
+  for (int w = 1; w < 8; ++w) amax = fmaxf(amax, red[w]);
+  int sh = 9 - ((int)((__float_as_uint(amax) >> 23) & 0xffu) - 127);
+  if (amax == 0.f) sh = 0;
+  sh = sh < -100 ? -100 : (sh > 100 ? 100 : sh);
+  const float s = __uint_as_float((uint32_t)(127 + sh) << 23);
+  if (threadIdx.x == 0) inv_scale[Ig] = __uint_as_float((uint32_t)(127 - sh) << 23);
+  // pass 2: [64 inputs][96 columns] tiles through shared memory
+  const size_t row0 = (size_t)__ldg(xoff + M) + (size_t)(Ig - a0) * kKB * npad;
+  for (int kb = 0; kb < kKB; ++kb) {
+    for (int c0 = 0; c0 < npad; c0 += 96) {
+      const int nc = npad - c0 < 96 ? npad - c0 : 96;
+      __syncthreads();
+      for (int rr = warp; rr < kKBlk; rr += 8)
+        for (int cc = lane; cc < nc; cc += 32)
+          tile[rr][cc] = (c0 + cc < ncol) ? __ldcs(src + (size_t)(kb * kKBlk + rr) * ncol + c0 + cc) * s : 0.f;
+      __syncthreads();
+      // one thread = one 16-byte chunk (8 inputs) of one column
+      for (int item = threadIdx.x; item < nc * 8; item += 256) {
+        const int cc = item >> 3, ch = item & 7;
+        __half h[8], l[8];
+#pragma unroll
+        for (int u = 0; u < 8; ++u) {
+          const float a = tile[ch * 8 + u][cc];
+          h[u] = __float2half_rn(a);
+          l[u] = __float2half_rn(a - __half2float(h[u]));
+        }
+        const size_t row = row0 + (size_t)kb * npad + c0 + cc;
+        const size_t o = row * 64 + (size_t)((ch ^ (int)(row & 7)) << 3);
+        *reinterpret_cast<uint4*>(Xh + o) = *reinterpret_cast<const uint4*>(h);
+        *reinterpret_cast<uint4*>(Xl + o) = *reinterpret_cast<const uint4*>(l);
+      }
+    }
+  }
+}
+
+// ---------------------------------------------------------------------------------------------------
+// 3. The tcgen05 kernel.
+// ---------------------------------------------------------------------------------------------------
+template <int D_>
+struct MmaCfg {
+  static constexpr int d = D_;
+  static constexpr int kMT = D_ / kTile;              // output tiles (TMEM accumulators) per atom
+  static constexpr int kKB = D_ / kKBlk;              // k-blocks
+  static constexpr int kNMax = D_ <= 128 ? 128 : 96;  // columns per chunk (MMA N <= kNMax, multiple of 16)
+  static constexpr int kStages = D_ <= 128 ? 4 : 3;   // B ring: one stage = hi + lo tile of one (atom, k-block)
+  static constexpr int kTBuf = 512 / (kMT * kNMax) >= 4 ? 4 : 512 / (kMT * kNMax);   // TMEM accumulator buffers
+  static constexpr uint32_t kABytes = kMT * kKB * kTileBytes;
+  static constexpr uint32_t kStageBytes = 2 * kNMax * 128;
+  static constexpr int kEpiWarps = 4 * kMT;
+  static constexpr int kThreads = 64 + 32 * kEpiWarps;
+  static constexpr uint32_t kSmem = kABytes + kStages * kStageBytes + 256 + 1024;
+};
+
+template <int D_>
+__global__ void __launch_bounds__(MmaCfg<D_>::kThreads, 1)
+sorf_rows_mma_kernel(const int32_t* __restrict__ elem, const int32_t* __restrict__ mol_off, int n_mol, int n_s,
+                     int n_sg, float c, const __half* __restrict__ W16, const __half* __restrict__ Xh,
+                     const __half* __restrict__ Xl, const long long* __restrict__ xoff,
+                     const float* __restrict__ inv_scale, const float* __restrict__ zs, float* __restrict__ G) {
+  using C = MmaCfg<D_>;
+  extern __shared__ uint8_t smem_raw[];
+  uint8_t* smem = reinterpret_cast<uint8_t*>(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
+  uint8_t* a_smem = smem;
+  uint8_t* b_smem = smem + C::kABytes;
+  uint64_t* bars = reinterpret_cast<uint64_t*>(b_smem + C::kStages * C::kStageBytes);
+  uint64_t* a_full = bars;                       // [1]
+  uint64_t* a_empty = bars + 1;                  // [1]
+  uint64_t* b_full = bars + 2;                   // [kStages]
+  uint64_t* b_empty = b_full + C::kStages;       // [kStages]
+  uint64_t* t_full = b_empty + C::kStages;       // [kTBuf]
+  uint64_t* t_empty = t_full + C::kTBuf;         // [kTBuf]
+  uint32_t* tmem_ptr_smem = reinterpret_cast<uint32_t*>(t_empty + C::kTBuf);
+
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const long long n_tasks = (long long)n_mol * n_s;
+  const int D = n_s * C::d;
+
+  if (threadIdx.x == 0) {
+    mbar_init(a_full, 1); mbar_init(a_empty, 1);
+    for (int i = 0; i < C::kStages; ++i) { mbar_init(&b_full[i], 1); mbar_init(&b_empty[i], 1); }
+    for (int i = 0; i < C::kTBuf; ++i) { mbar_init(&t_full[i], 1); mbar_init(&t_empty[i], C::kEpiWarps); }
+    fence_mbarrier_init();
+  }
+  if (warp == 2) {
+    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], 512;" ::"r"(smem_u32(tmem_ptr_smem))
+                 : "memory");
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+  }
+  tcgen05_fence_before();
+  __syncthreads();
+  tcgen05_fence_after();
+  const uint32_t tmem_base = *tmem_ptr_smem;
+
+  if (warp == 0) {
+    // ===================== producer: bulk copies of W tiles (per element run) and column tiles =====================
+    if (lane == 0) {
+      uint32_t n_a = 0, n_b = 0;   // A loads / B stages issued so far
+      for (long long task = blockIdx.x; task < n_tasks; task += gridDim.x) {
+        const int M = (int)(task / n_s), s = (int)(task % n_s);
+        const int a0 = __ldg(mol_off + M), n = __ldg(mol_off + M + 1) - a0;
+        const int ncol = 3 * n, npad = (ncol + 15) / 16 * 16;
+        const size_t row_m = (size_t)__ldg(xoff + M);
+        for (int c0 = 0; c0 < npad; c0 += C::kNMax) {
+          const int nc = npad - c0 < C::kNMax ? npad - c0 : C::kNMax;
+          int e_prev = -1;
+          for (int I = 0; I < n; ++I) {
+            const int e = __ldg(elem + a0 + I);
+            if (e != e_prev) {
+              if (n_a > 0) mbar_wait(a_empty, (n_a - 1) & 1);
+              mbar_expect_tx(a_full, C::kABytes);
+              const __half* w = W16 + ((size_t)e * n_s + s) * (size_t)(C::kMT * C::kKB) * (kTile * kKBlk);
+#pragma unroll 1
+              for (int t = 0; t < C::kMT * C::kKB; ++t)
+                bulk_copy_g2s(a_smem + t * kTileBytes, w + (size_t)t * (kTile * kKBlk), kTileBytes, a_full);
+              ++n_a;
+              e_prev = e;
+            }
+            for (int kb = 0; kb < C::kKB; ++kb, ++n_b) {
+              const uint32_t st = n_b % C::kStages, use = n_b / C::kStages;
+              if (use > 0) mbar_wait(&b_empty[st], (use - 1) & 1);
+              const uint32_t bytes = (uint32_t)nc * 128;
+              mbar_expect_tx(&b_full[st], 2 * bytes);
+              const size_t row = row_m + ((size_t)I * C::kKB + kb) * npad + c0;
+              uint8_t* dst = b_smem + st * C::kStageBytes;
+              bulk_copy_g2s(dst, Xh + row * 64, bytes, &b_full[st]);
+              bulk_copy_g2s(dst + C::kNMax * 128, Xl + row * 64, bytes, &b_full[st]);
+            }
+          }
+        }
+      }
+    }
+  } else if (warp == 1) {
+    // ===================== MMA issuer (one thread) =====================
+    if (lane == 0) {
+      uint32_t n_a = 0, n_b = 0, n_t = 0;
+      for (long long task = blockIdx.x; task < n_tasks; task += gridDim.x) {
+        const int M = (int)(task / n_s);
+        const int a0 = __ldg(mol_off + M), n = __ldg(mol_off + M + 1) - a0;
+        const int ncol = 3 * n, npad = (ncol + 15) / 16 * 16;
+        for (int c0 = 0; c0 < npad; c0 += C::kNMax) {
+          const int nc = npad - c0 < C::kNMax ? npad - c0 : C::kNMax;
+          // D fp32, A/B fp16, both K-major, N = nc, M = 128
+          const uint32_t idesc = (1u << 4) | ((uint32_t)(nc >> 3) << 17) | ((uint32_t)(kTile >> 4) << 24);
+          int e_prev = -1;
+          for (int I = 0; I < n; ++I, ++n_t) {
+            const int e = __ldg(elem + a0 + I);
+            if (e != e_prev) {
+              mbar_wait(a_full, n_a & 1);
+              ++n_a;
+              e_prev = e;
+            }
+            const uint32_t tb = n_t % C::kTBuf, tuse = n_t / C::kTBuf;
+            if (tuse > 0) mbar_wait(&t_empty[tb], (tuse - 1) & 1);
+            tcgen05_fence_after();
+            for (int kb = 0; kb < C::kKB; ++kb, ++n_b) {
+              const uint32_t st = n_b % C::kStages;
+              mbar_wait(&b_full[st], (n_b / C::kStages) & 1);
+              tcgen05_fence_after();
+              const uint32_t b_base = smem_u32(b_smem + st * C::kStageBytes);
+              const uint64_t b_hi = make_kmajor_sw128_desc(b_base);
+              const uint64_t b_lo = make_kmajor_sw128_desc(b_base + C::kNMax * 128);
+#pragma unroll
+              for (int mt = 0; mt < C::kMT; ++mt) {
+                const uint64_t a_d = make_kmajor_sw128_desc(smem_u32(a_smem + (mt * C::kKB + kb) * kTileBytes));
+                const uint32_t tmem_d = tmem_base + tb * (C::kMT * C::kNMax) + mt * C::kNMax;
+#pragma unroll
+                for (int kk = 0; kk < kKBlk / 16; ++kk) {
+                  const uint64_t adv = (uint64_t)((kk * 32) >> 4);
+                  umma<true>(tmem_d, a_d + adv, b_lo + adv, idesc, (kb > 0 || kk > 0) ? 1u : 0u);  // small term first
+                  umma<true>(tmem_d, a_d + adv, b_hi + adv, idesc, 1u);
+                }
+              }
+              tcgen05_commit(&b_empty[st]);
+            }
+            tcgen05_commit(&t_full[tb]);
+            // the W tiles may be replaced once every MMA of this element run has completed
+            const bool last_of_run = (I + 1 == n) || (__ldg(elem + a0 + I + 1) != e);
+            if (last_of_run) tcgen05_commit(a_empty);
+          }
+        }
+      }
+    }
+  } else {
+    // ===================== epilogue warps: thread = output feature =====================
+    const int quarter = warp & 3;               // TMEM lanes [32 q, 32 q + 32) are the ones this warp may read
+    const int mt = (warp - 2) >> 2;
+    const int m = mt * kTile + quarter * 32 + lane;        // output index inside the stack
+    // position of feature (s, m) inside the lane-ordered sin table of the forward kernel (sorf_kernels.cuh)
+    using ZS = Shape<(D_ < kMaxE ? D_ : kMaxE), (D_ < kMaxE ? 1 : D_ / kMaxE)>;
+    constexpr int E = ZS::E, P = ZS::P, SPW = ZS::SPW, E4 = ZS::E4;
+    const int zp = m / E, zj = m % E;
+    uint32_t n_t = 0;
+    for (long long task = blockIdx.x; task < n_tasks; task += gridDim.x) {
+      const int M = (int)(task / n_s), s = (int)(task % n_s);
+      const int a0 = __ldg(mol_off + M), n = __ldg(mol_off + M + 1) - a0;
+      const int ncol = 3 * n, npad = (ncol + 15) / 16 * 16;
+      const size_t zs_idx = ((((size_t)(s / SPW)) * E4 + zj / 4) * kWarp + (s % SPW) * P + zp) * 4 + (zj & 3);
+      const size_t zs_atom = (size_t)n_sg * E * kWarp;       // floats per atom
+      for (int c0 = 0; c0 < npad; c0 += C::kNMax) {
+        const int nc = npad - c0 < C::kNMax ? npad - c0 : C::kNMax;
+        float acc[C::kNMax];
+#pragma unroll
+        for (int r = 0; r < C::kNMax; ++r) acc[r] = 0.f;
+        float f_next = c * __ldg(inv_scale + a0) * __ldg(zs + (size_t)a0 * zs_atom + zs_idx);
+        for (int I = 0; I < n; ++I, ++n_t) {
+          const float f = f_next;
+          if (I + 1 < n) f_next = c * __ldg(inv_scale + a0 + I + 1) * __ldg(zs + (size_t)(a0 + I + 1) * zs_atom + zs_idx);
+          const uint32_t tb = n_t % C::kTBuf;
+          mbar_wait(&t_full[tb], (n_t / C::kTBuf) & 1);
+          tcgen05_fence_after();
+          const uint32_t taddr = tmem_base + ((uint32_t)(quarter * 32) << 16) + tb * (C::kMT * C::kNMax) + mt * C::kNMax;
+#pragma unroll
+          for (int r0 = 0; r0 < C::kNMax; r0 += 16) {
+            if (r0 < nc) {
+              uint32_t u[16];
+              tmem_ld_32x32b_x16(taddr + r0, u);
+              tmem_ld_wait();
+#pragma unroll
+              for (int r = 0; r < 16; ++r) acc[r0 + r] = fmaf(f, __uint_as_float(u[r]), acc[r0 + r]);
+            }
+          }
+          tcgen05_fence_before();
+          __syncwarp();
+          if (lane == 0) mbar_arrive(&t_empty[tb]);
+        }
+        float* dst = G + ((size_t)3 * a0 + c0) * D + (size_t)s * C::d + m;
+#pragma unroll
+        for (int r = 0; r < C::kNMax; ++r)
+          if (r < nc && c0 + r < ncol) dst[(size_t)r * D] = acc[r];
+      }
+    }
+  }
+
+  tcgen05_fence_before();
+  __syncthreads();
+  if (warp == 2) {
+    tcgen05_fence_after();
+    asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, 512;" ::"r"(tmem_base) : "memory");
+  }
+}
+
+// ---------------------------------------------------------------------------------------------------
+// Host side
+// ---------------------------------------------------------------------------------------------------
+bool sorf_mma_supported(const qmll_sorf_params* p) {
+  return (p->d == 128 || p->d == 256) && p->n_transform >= 1 && p->n_transform <= 3;
+}
+
+// bytes of the W table, of ONE of the two column arrays (upper bound: n * kKB * roundup16(3n) rows of 128 bytes per
+// molecule <= 2 * (dense_floats + 15 d n_atoms) bytes) and of the per-molecule offsets / per-atom scales
+size_t sorf_mma_w_bytes(const qmll_sorf_params* p) { return (size_t)p->n_elem * (p->D / p->d) * p->d * p->d * sizeof(__half); }
+size_t sorf_mma_x_bytes(const qmll_sorf_params* p, int64_t n_atoms, int64_t dense_floats) {
+  return (size_t)2 * ((size_t)dense_floats + (size_t)15 * p->d * (size_t)n_atoms) + 1024;
+}
+
+template <int D_>
+static int launch_rows_mma(const SorfProblem& pr, const SorfTables& t, const float* zs, const qmll_grad* grad,
+                           __half* W16, __half* Xh, __half* Xl, long long* xoff, float* inv_scale, float* G,
+                           cudaStream_t st) {
+  using S = Shape<shape_E(D_), shape_P(D_)>;
+  using C = MmaCfg<D_>;
+  const qmll_sorf_params* p = pr.p;
+  const int n_s = p->D / p->d, n_sg = (n_s + S::SPW - 1) / S::SPW;
+  const long long w_tasks = (long long)p->n_elem * n_sg * p->d;
+  build_w_kernel<S><<<(unsigned)((w_tasks + 3) / 4), kFwdThreads, 0, st>>>(t.sign_bits, p->n_elem, n_s, n_sg,
+                                                                          p->n_transform, W16);
+  QMLL_LAUNCH_CHECK("build_w_kernel");
+  x_offsets_kernel<<<1, 1024, 0, st>>>(pr.mol_off, pr.n_mol, C::kKB, xoff);
+  QMLL_LAUNCH_CHECK("x_offsets_kernel");
+  prep_columns_kernel<<<(unsigned)pr.n_atoms, 256, 0, st>>>(grad->dense, grad->dense_off, pr.mol_off, pr.n_mol, p->d,
+                                                           xoff, Xh, Xl, inv_scale);
+  QMLL_LAUNCH_CHECK("prep_columns_kernel");
+  auto kern = sorf_rows_mma_kernel<D_>;
+  QMLL_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::kSmem));
+  const long long n_tasks = (long long)pr.n_mol * n_s;
+  const int grid = (int)(n_tasks < device_sm_count() ? n_tasks : device_sm_count());
+  const float c = (float)(sqrt((double)p->d) / (double)p->sigma * pow((double)p->d, -0.5 * p->n_transform));
+  kern<<<grid, C::kThreads, C::kSmem, st>>>(pr.elem, pr.mol_off, pr.n_mol, n_s, n_sg, c, W16, Xh, Xl, xoff,
+                                            inv_scale, zs, G);
+  QMLL_LAUNCH_CHECK("sorf_rows_mma_kernel");
+  return QMLL_OK;
+}
+
+int sorf_force_rows_dense_mma(const SorfProblem& pr, const SorfTables& t, const float* zs, const qmll_grad* grad,
+                              void* W16, void* Xh, void* Xl, long long* xoff, float* inv_scale, float* G,
+                              cudaStream_t st) {
+  if (pr.n_atoms == 0 || pr.n_mol == 0) return QMLL_OK;
+  if (pr.p->d == 128)
+    return launch_rows_mma<128>(pr, t, zs, grad, (__half*)W16, (__half*)Xh, (__half*)Xl, xoff, inv_scale, G, st);
+  if (pr.p->d == 256)
+    return launch_rows_mma<256>(pr, t, zs, grad, (__half*)W16, (__half*)Xh, (__half*)Xl, xoff, inv_scale, G, st);
+  return QMLL_ERR_UNSUPPORTED;
+}
+
+}  // namespace qmll

@@ -45,11 +45,15 @@ def run_all(q, w, check_ne=True):
         assert F is None
         assert rel(E.cpu().numpy(), Eo) <= TOL
         return
-    # forward + force rows
-    Z2, G = pkg.qmll_sorf_forward(dp.params, dp.x, dp.elem, dp.mol_off, dp.grad)
+    # forward + force rows: the register-FWHT path and (dense gradient, d = 128 / 256) the tensor-core path
     Go = oracle.force_rows_w(w)
-    assert rel(Z2.cpu().numpy(), Zo) <= TOL
-    assert rel(G.cpu().numpy(), Go) <= TOL
+    modes = [pkg.ROWS_FWHT]
+    if w.grad.layout == "dense" and w.model.d in (128, 256):
+        modes.append(pkg.ROWS_MMA)
+    for mode in modes + [pkg.ROWS_AUTO]:
+        Z2, G = pkg.qmll_sorf_forward(dp.params, dp.x, dp.elem, dp.mol_off, dp.grad, force_rows_mode=mode)
+        assert rel(Z2.cpu().numpy(), Zo) <= TOL
+        assert rel(G.cpu().numpy(), Go) <= TOL, mode
     # predict and backward
     Fo = oracle.forces_w(w)
     E, F = pkg.qmll_predict(dp.params, dp.x, dp.elem, dp.mol_off, dp.alpha, dp.grad)
@@ -94,6 +98,34 @@ def test_tiny_neighbor(q, d, D):
     w = tiny_workload(seed=77 + d, d=d, D=D, T=3, sigma=np.sqrt(d) / 2, counts=[50, 0, 13], n_elem=2,
                       grad="neighbor", K=6)
     run_all(q, w, check_ne=False)
+
+
+def test_force_rows_mma_long_molecule_and_odd_stacks(q):
+    """Tensor-core force rows: a molecule whose 3n columns need several column chunks (n = 50 > 42), mixed with small
+    and empty ones, unsorted elements (a W reload per atom), stack counts that are not a multiple of the warp's."""
+    pkg, wio, torch = q
+    for d, D in ((128, 128 * 5), (256, 256 * 3)):
+        w = tiny_workload(seed=300 + d, d=d, D=D, T=3, sigma=np.sqrt(d) / 2, counts=[50, 0, 2, 17], n_elem=4,
+                          grad="dense")
+        dp = wio.device_problem(w)
+        Go = oracle.force_rows_w(w)
+        for mode in (pkg.ROWS_MMA, pkg.ROWS_FWHT):
+            _, G = pkg.qmll_sorf_forward(dp.params, dp.x, dp.elem, dp.mol_off, dp.grad, force_rows_mode=mode)
+            assert rel(G.cpu().numpy(), Go) <= TOL, (d, mode)
+    w = tiny_workload(seed=9, d=64, D=128, T=3, sigma=2.0, counts=[2], grad="dense")
+    dp = wio.device_problem(w)
+    with pytest.raises(pkg.QmllError) as ei:                      # d = 64 has no tensor-core path
+        pkg.qmll_sorf_forward(dp.params, dp.x, dp.elem, dp.mol_off, dp.grad, force_rows_mode=pkg.ROWS_MMA)
+    assert ei.value.status == -2
+
+
+@pytest.mark.parametrize("T", [1, 2])
+def test_force_rows_mma_fewer_transforms(q, T):
+    pkg, wio, torch = q
+    w = tiny_workload(seed=40 + T, d=128, D=1024, T=T, sigma=4.0, counts=[5, 9], n_elem=3, grad="dense")
+    dp = wio.device_problem(w)
+    _, G = pkg.qmll_sorf_forward(dp.params, dp.x, dp.elem, dp.mol_off, dp.grad, force_rows_mode=pkg.ROWS_MMA)
+    assert rel(G.cpu().numpy(), oracle.force_rows_w(w)) <= TOL
 
 
 def test_c2_reduced(q):
