@@ -168,21 +168,43 @@ prep_columns_kernel(const float* __restrict__ dense, const int64_t* __restrict__
 
 // ---------------------------------------------------------------------------------------------------
 // 3. The tcgen05 kernel.
+//    What bounds it: every (atom, stack) needs the atom's column tiles (hi + lo: 4 d N bytes) from L2, and one SM
+//    can pull ~20 B per clock from L2 when all SMs do (measured 5.5 TB/s; multicast in clusters of 4 does not help,
+//    L2 already merges up to ~4 identical requests).  The columns are therefore re-used from shared memory for kSPT
+//    stacks per CTA: as many as the W tiles of kSPT stacks leave room for (d = 128: 4 stacks = 128 KB of W; d = 256:
+//    1 stack = 128 KB).  Measured tensor-pipe activity: see DESIGN.md.
 // ---------------------------------------------------------------------------------------------------
 template <int D_>
 struct MmaCfg {
   static constexpr int d = D_;
-  static constexpr int kMT = D_ / kTile;              // output tiles (TMEM accumulators) per atom
+  static constexpr int kTPS = D_ / kTile;             // 128-row output tiles per stack
+  static constexpr int kSPT = D_ <= 128 ? 4 : 1;      // stacks per task (CTA)
+  static constexpr int kMT = kTPS * kSPT;             // output tiles (TMEM accumulators) per atom
   static constexpr int kKB = D_ / kKBlk;              // k-blocks
-  static constexpr int kNMax = D_ <= 128 ? 128 : 96;  // columns per chunk (MMA N <= kNMax, multiple of 16)
+  static constexpr int kNMax = D_ <= 128 ? 64 : 96;   // columns per chunk (MMA N <= kNMax, multiple of 16)
   static constexpr int kStages = D_ <= 128 ? 4 : 3;   // B ring: one stage = hi + lo tile of one (atom, k-block)
-  static constexpr int kTBuf = 512 / (kMT * kNMax) >= 4 ? 4 : 512 / (kMT * kNMax);   // TMEM accumulator buffers
-  static constexpr uint32_t kABytes = kMT * kKB * kTileBytes;
+  static constexpr int kTBuf = 512 / (kMT * kNMax);   // TMEM accumulator buffers (2)
+  static constexpr uint32_t kABytes = kMT * kKB * kTileBytes;   // W tiles of one (element, stack group): 128 KB
   static constexpr uint32_t kStageBytes = 2 * kNMax * 128;
-  static constexpr int kEpiWarps = 4 * kMT;
+  static constexpr int kEpiWarps = 8;
+  static constexpr int kTPW = kMT / 2;                // output tiles per epilogue warp (2 warp groups of 4 quarters)
   static constexpr int kThreads = 64 + 32 * kEpiWarps;
-  static constexpr uint32_t kSmem = kABytes + kStages * kStageBytes + 256 + 1024;
+  static constexpr uint32_t kSmem = kABytes + kStages * kStageBytes + 512 + 1024;
+  static_assert(kTBuf >= 2 && kMT % 2 == 0, "TMEM double buffering / epilogue split");
 };
+
+// Task order: molecules in groups of kMolGroup, inside a group the molecule index runs fastest, so that the CTAs that
+// run at the same time read different molecules' column tiles while a molecule's tiles stay in L2 between its stacks.
+constexpr int kMolGroup = 16;
+__device__ __forceinline__ void task_decode(long long task, int n_mol, int n_units, int* M, int* unit) {
+  const long long per_group = (long long)kMolGroup * n_units;
+  const long long g = task / per_group;
+  const int m0 = (int)(g * kMolGroup);
+  const int gm = n_mol - m0 < kMolGroup ? n_mol - m0 : kMolGroup;   // molecules in this group
+  const long long r = task - g * per_group;
+  *M = m0 + (int)(r % gm);
+  *unit = (int)(r / gm);
+}
 
 template <int D_>
 __global__ void __launch_bounds__(MmaCfg<D_>::kThreads, 1)
@@ -193,23 +215,24 @@ sorf_rows_mma_kernel(const int32_t* __restrict__ elem, const int32_t* __restrict
   using C = MmaCfg<D_>;
   extern __shared__ uint8_t smem_raw[];
   uint8_t* smem = reinterpret_cast<uint8_t*>(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
-  uint8_t* a_smem = smem;
+  uint8_t* a_smem = smem;                        // [kMT][kKB] tiles of 16 KB
   uint8_t* b_smem = smem + C::kABytes;
   uint64_t* bars = reinterpret_cast<uint64_t*>(b_smem + C::kStages * C::kStageBytes);
-  uint64_t* a_full = bars;                       // [1]
-  uint64_t* a_empty = bars + 1;                  // [1]
-  uint64_t* b_full = bars + 2;                   // [kStages]
+  uint64_t* a_full = bars;                       // [kKB]   one barrier pair per k-block of the W tiles: the next
+  uint64_t* a_empty = bars + C::kKB;             // [kKB]   element's tiles load k-block by k-block behind the last atom
+  uint64_t* b_full = bars + 2 * C::kKB;          // [kStages]
   uint64_t* b_empty = b_full + C::kStages;       // [kStages]
   uint64_t* t_full = b_empty + C::kStages;       // [kTBuf]
   uint64_t* t_empty = t_full + C::kTBuf;         // [kTBuf]
   uint32_t* tmem_ptr_smem = reinterpret_cast<uint32_t*>(t_empty + C::kTBuf);
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const long long n_tasks = (long long)n_mol * n_s;
+  const int n_grp = (n_s + C::kSPT - 1) / C::kSPT;          // stack groups per molecule
+  const long long n_tasks = (long long)n_mol * n_grp;
   const int D = n_s * C::d;
 
   if (threadIdx.x == 0) {
-    mbar_init(a_full, 1); mbar_init(a_empty, 1);
+    for (int i = 0; i < C::kKB; ++i) { mbar_init(&a_full[i], 1); mbar_init(&a_empty[i], 1); }
     for (int i = 0; i < C::kStages; ++i) { mbar_init(&b_full[i], 1); mbar_init(&b_empty[i], 1); }
     for (int i = 0; i < C::kTBuf; ++i) { mbar_init(&t_full[i], 1); mbar_init(&t_empty[i], C::kEpiWarps); }
     fence_mbarrier_init();
@@ -227,9 +250,12 @@ sorf_rows_mma_kernel(const int32_t* __restrict__ elem, const int32_t* __restrict
   if (warp == 0) {
     // ===================== producer: bulk copies of W tiles (per element run) and column tiles =====================
     if (lane == 0) {
-      uint32_t n_a = 0, n_b = 0;   // A loads / B stages issued so far
+      uint32_t n_a = 0, n_b = 0;   // element runs (W loads) / B stages issued so far
       for (long long task = blockIdx.x; task < n_tasks; task += gridDim.x) {
-        const int M = (int)(task / n_s), s = (int)(task % n_s);
+        int M, grp;
+        task_decode(task, n_mol, n_grp, &M, &grp);
+        const int s0 = grp * C::kSPT;
+        const int n_st = n_s - s0 < C::kSPT ? n_s - s0 : C::kSPT;      // stacks of this task (tail group: fewer)
         const int a0 = __ldg(mol_off + M), n = __ldg(mol_off + M + 1) - a0;
         const int ncol = 3 * n, npad = (ncol + 15) / 16 * 16;
         const size_t row_m = (size_t)__ldg(xoff + M);
@@ -238,13 +264,16 @@ sorf_rows_mma_kernel(const int32_t* __restrict__ elem, const int32_t* __restrict
           int e_prev = -1;
           for (int I = 0; I < n; ++I) {
             const int e = __ldg(elem + a0 + I);
-            if (e != e_prev) {
-              if (n_a > 0) mbar_wait(a_empty, (n_a - 1) & 1);
-              mbar_expect_tx(a_full, C::kABytes);
-              const __half* w = W16 + ((size_t)e * n_s + s) * (size_t)(C::kMT * C::kKB) * (kTile * kKBlk);
+            if (e != e_prev) {   // new element run: W tiles of (e, s0 .. s0 + n_st - 1), k-block by k-block
+              const __half* w = W16 + ((size_t)e * n_s + s0) * (size_t)(C::kTPS * C::kKB) * (kTile * kKBlk);
 #pragma unroll 1
-              for (int t = 0; t < C::kMT * C::kKB; ++t)
-                bulk_copy_g2s(a_smem + t * kTileBytes, w + (size_t)t * (kTile * kKBlk), kTileBytes, a_full);
+              for (int kb = 0; kb < C::kKB; ++kb) {
+                if (n_a > 0) mbar_wait(&a_empty[kb], (n_a - 1) & 1);
+                mbar_expect_tx(&a_full[kb], (uint32_t)(n_st * C::kTPS) * kTileBytes);
+                for (int t = 0; t < n_st * C::kTPS; ++t)   // tile t = stack t / kTPS, output tile t % kTPS
+                  bulk_copy_g2s(a_smem + (t * C::kKB + kb) * kTileBytes,
+                                w + (size_t)(t * C::kKB + kb) * (kTile * kKBlk), kTileBytes, &a_full[kb]);
+              }
               ++n_a;
               e_prev = e;
             }
@@ -264,10 +293,24 @@ sorf_rows_mma_kernel(const int32_t* __restrict__ elem, const int32_t* __restrict
     }
   } else if (warp == 1) {
     // ===================== MMA issuer (one thread) =====================
+    // The MMAs are short (N <= 64: 32 clocks each), so the issue loop is kept lean: all descriptors are formed once
+    // (the W tiles and the ring stages never move), the tile loop is unrolled.
     if (lane == 0) {
+      uint64_t a_desc[C::kMT][C::kKB], b_desc[C::kStages];
+#pragma unroll
+      for (int t = 0; t < C::kMT; ++t)
+#pragma unroll
+        for (int kb = 0; kb < C::kKB; ++kb)
+          a_desc[t][kb] = make_kmajor_sw128_desc(smem_u32(a_smem + (t * C::kKB + kb) * kTileBytes));
+#pragma unroll
+      for (int st = 0; st < C::kStages; ++st) b_desc[st] = make_kmajor_sw128_desc(smem_u32(b_smem + st * C::kStageBytes));
+      constexpr uint64_t kLoOff = (uint64_t)((C::kNMax * 128) >> 4);   // lo tile behind the hi tile, in 16-byte units
       uint32_t n_a = 0, n_b = 0, n_t = 0;
       for (long long task = blockIdx.x; task < n_tasks; task += gridDim.x) {
-        const int M = (int)(task / n_s);
+        int M, grp;
+        task_decode(task, n_mol, n_grp, &M, &grp);
+        const int s0 = grp * C::kSPT;
+        const int n_tiles = (n_s - s0 < C::kSPT ? n_s - s0 : C::kSPT) * C::kTPS;
         const int a0 = __ldg(mol_off + M), n = __ldg(mol_off + M + 1) - a0;
         const int ncol = 3 * n, npad = (ncol + 15) / 16 * 16;
         for (int c0 = 0; c0 < npad; c0 += C::kNMax) {
@@ -275,91 +318,135 @@ sorf_rows_mma_kernel(const int32_t* __restrict__ elem, const int32_t* __restrict
           // D fp32, A/B fp16, both K-major, N = nc, M = 128
           const uint32_t idesc = (1u << 4) | ((uint32_t)(nc >> 3) << 17) | ((uint32_t)(kTile >> 4) << 24);
           int e_prev = -1;
+          int e_next = __ldg(elem + a0);
           for (int I = 0; I < n; ++I, ++n_t) {
-            const int e = __ldg(elem + a0 + I);
-            if (e != e_prev) {
-              mbar_wait(a_full, n_a & 1);
-              ++n_a;
-              e_prev = e;
-            }
+            const int e = e_next;
+            e_next = (I + 1 < n) ? __ldg(elem + a0 + I + 1) : -1;
+            const bool first_of_run = e != e_prev;
+            if (first_of_run) { ++n_a; e_prev = e; }
+            const bool last_of_run = e_next != e;
             const uint32_t tb = n_t % C::kTBuf, tuse = n_t / C::kTBuf;
             if (tuse > 0) mbar_wait(&t_empty[tb], (tuse - 1) & 1);
             tcgen05_fence_after();
+            const uint32_t tmem_atom = tmem_base + tb * (C::kMT * C::kNMax);
+#pragma unroll
             for (int kb = 0; kb < C::kKB; ++kb, ++n_b) {
               const uint32_t st = n_b % C::kStages;
+              if (first_of_run) mbar_wait(&a_full[kb], (n_a - 1) & 1);
               mbar_wait(&b_full[st], (n_b / C::kStages) & 1);
               tcgen05_fence_after();
-              const uint32_t b_base = smem_u32(b_smem + st * C::kStageBytes);
-              const uint64_t b_hi = make_kmajor_sw128_desc(b_base);
-              const uint64_t b_lo = make_kmajor_sw128_desc(b_base + C::kNMax * 128);
+              uint64_t b_hi = b_desc[0];
 #pragma unroll
-              for (int mt = 0; mt < C::kMT; ++mt) {
-                const uint64_t a_d = make_kmajor_sw128_desc(smem_u32(a_smem + (mt * C::kKB + kb) * kTileBytes));
-                const uint32_t tmem_d = tmem_base + tb * (C::kMT * C::kNMax) + mt * C::kNMax;
+              for (int q = 1; q < C::kStages; ++q) b_hi = (st == (uint32_t)q) ? b_desc[q] : b_hi;
+              // Consecutive MMAs go to DIFFERENT accumulators: an MMA that accumulates into the tile its predecessor
+              // wrote waits for it (~96 clocks measured, three times the 32 clocks an N = 64 MMA takes).
 #pragma unroll
-                for (int kk = 0; kk < kKBlk / 16; ++kk) {
-                  const uint64_t adv = (uint64_t)((kk * 32) >> 4);
-                  umma<true>(tmem_d, a_d + adv, b_lo + adv, idesc, (kb > 0 || kk > 0) ? 1u : 0u);  // small term first
-                  umma<true>(tmem_d, a_d + adv, b_hi + adv, idesc, 1u);
-                }
+              for (int kk = 0; kk < kKBlk / 16; ++kk) {
+                const uint64_t adv = (uint64_t)((kk * 32) >> 4);
+#pragma unroll
+                for (int t = 0; t < C::kMT; ++t)
+                  if (t < n_tiles)
+                    umma<true>(tmem_atom + t * C::kNMax, a_desc[t][kb] + adv, b_hi + kLoOff + adv, idesc,
+                               (kb > 0 || kk > 0) ? 1u : 0u);   // small term first
+#pragma unroll
+                for (int t = 0; t < C::kMT; ++t)
+                  if (t < n_tiles) umma<true>(tmem_atom + t * C::kNMax, a_desc[t][kb] + adv, b_hi + adv, idesc, 1u);
               }
               tcgen05_commit(&b_empty[st]);
+              // the W tiles of this k-block may be replaced once the run's last MMAs on them have completed
+              if (last_of_run) tcgen05_commit(&a_empty[kb]);
             }
             tcgen05_commit(&t_full[tb]);
-            // the W tiles may be replaced once every MMA of this element run has completed
-            const bool last_of_run = (I + 1 == n) || (__ldg(elem + a0 + I + 1) != e);
-            if (last_of_run) tcgen05_commit(a_empty);
           }
         }
       }
     }
   } else {
-    // ===================== epilogue warps: thread = output feature =====================
+    // ===================== epilogue warps: thread = output feature of kTPW tiles =====================
     const int quarter = warp & 3;               // TMEM lanes [32 q, 32 q + 32) are the ones this warp may read
-    const int mt = (warp - 2) >> 2;
-    const int m = mt * kTile + quarter * 32 + lane;        // output index inside the stack
+    const int half = (warp - 2) >> 2;           // tiles [half * kTPW, half * kTPW + kTPW)
+    const int row = quarter * 32 + lane;        // output row inside a tile
     // position of feature (s, m) inside the lane-ordered sin table of the forward kernel (sorf_kernels.cuh)
     using ZS = Shape<(D_ < kMaxE ? D_ : kMaxE), (D_ < kMaxE ? 1 : D_ / kMaxE)>;
     constexpr int E = ZS::E, P = ZS::P, SPW = ZS::SPW, E4 = ZS::E4;
-    const int zp = m / E, zj = m % E;
+    const size_t zs_atom = (size_t)n_sg * E * kWarp;       // floats per atom
     uint32_t n_t = 0;
     for (long long task = blockIdx.x; task < n_tasks; task += gridDim.x) {
-      const int M = (int)(task / n_s), s = (int)(task % n_s);
+      int M, grp;
+      task_decode(task, n_mol, n_grp, &M, &grp);
+      const int s0 = grp * C::kSPT;
       const int a0 = __ldg(mol_off + M), n = __ldg(mol_off + M + 1) - a0;
       const int ncol = 3 * n, npad = (ncol + 15) / 16 * 16;
-      const size_t zs_idx = ((((size_t)(s / SPW)) * E4 + zj / 4) * kWarp + (s % SPW) * P + zp) * 4 + (zj & 3);
-      const size_t zs_atom = (size_t)n_sg * E * kWarp;       // floats per atom
+      size_t zs_idx[C::kTPW];
+      bool live[C::kTPW];
+      int feat[C::kTPW];
+#pragma unroll
+      for (int w = 0; w < C::kTPW; ++w) {
+        const int t = half * C::kTPW + w;
+        const int s = s0 + t / C::kTPS, m = (t % C::kTPS) * kTile + row;    // stack, output index inside the stack
+        live[w] = s < n_s;
+        const int sc = live[w] ? s : n_s - 1;
+        const int zp = m / E, zj = m % E;
+        zs_idx[w] = ((((size_t)(sc / SPW)) * E4 + zj / 4) * kWarp + (sc % SPW) * P + zp) * 4 + (zj & 3);
+        feat[w] = sc * C::d + m;
+      }
       for (int c0 = 0; c0 < npad; c0 += C::kNMax) {
         const int nc = npad - c0 < C::kNMax ? npad - c0 : C::kNMax;
-        float acc[C::kNMax];
+        float acc[C::kTPW][C::kNMax];
 #pragma unroll
-        for (int r = 0; r < C::kNMax; ++r) acc[r] = 0.f;
-        float f_next = c * __ldg(inv_scale + a0) * __ldg(zs + (size_t)a0 * zs_atom + zs_idx);
+        for (int w = 0; w < C::kTPW; ++w)
+#pragma unroll
+          for (int r = 0; r < C::kNMax; ++r) acc[w][r] = 0.f;
+        float f_next[C::kTPW];
+#pragma unroll
+        for (int w = 0; w < C::kTPW; ++w)
+          f_next[w] = c * __ldg(inv_scale + a0) * __ldg(zs + (size_t)a0 * zs_atom + zs_idx[w]);
         for (int I = 0; I < n; ++I, ++n_t) {
-          const float f = f_next;
-          if (I + 1 < n) f_next = c * __ldg(inv_scale + a0 + I + 1) * __ldg(zs + (size_t)(a0 + I + 1) * zs_atom + zs_idx);
+          float f[C::kTPW];
+#pragma unroll
+          for (int w = 0; w < C::kTPW; ++w) {
+            f[w] = f_next[w];
+            if (I + 1 < n)
+              f_next[w] = c * __ldg(inv_scale + a0 + I + 1) * __ldg(zs + (size_t)(a0 + I + 1) * zs_atom + zs_idx[w]);
+          }
           const uint32_t tb = n_t % C::kTBuf;
           mbar_wait(&t_full[tb], (n_t / C::kTBuf) & 1);
           tcgen05_fence_after();
-          const uint32_t taddr = tmem_base + ((uint32_t)(quarter * 32) << 16) + tb * (C::kMT * C::kNMax) + mt * C::kNMax;
 #pragma unroll
-          for (int r0 = 0; r0 < C::kNMax; r0 += 16) {
-            if (r0 < nc) {
-              uint32_t u[16];
-              tmem_ld_32x32b_x16(taddr + r0, u);
-              tmem_ld_wait();
+          for (int w = 0; w < C::kTPW; ++w) {
+            const uint32_t taddr = tmem_base + ((uint32_t)(quarter * 32) << 16) + tb * (C::kMT * C::kNMax) +
+                                   (half * C::kTPW + w) * C::kNMax;
+            if (live[w]) {
 #pragma unroll
-              for (int r = 0; r < 16; ++r) acc[r0 + r] = fmaf(f, __uint_as_float(u[r]), acc[r0 + r]);
+              for (int r0 = 0; r0 < C::kNMax; r0 += 32) {   // nc is a multiple of 16: pieces of 32 with a 16 tail
+                if (r0 + 32 <= nc) {
+                  uint32_t u[32];
+                  tmem_ld_32x32b_x32(taddr + r0, u);
+                  tmem_ld_wait();
+#pragma unroll
+                  for (int r = 0; r < 32; ++r) acc[w][r0 + r] = fmaf(f[w], __uint_as_float(u[r]), acc[w][r0 + r]);
+                } else if (r0 < nc) {
+                  uint32_t u[16];
+                  tmem_ld_32x32b_x16(taddr + r0, u);
+                  tmem_ld_wait();
+#pragma unroll
+                  for (int r = 0; r < 16; ++r) acc[w][r0 + r] = fmaf(f[w], __uint_as_float(u[r]), acc[w][r0 + r]);
+                }
+              }
             }
           }
           tcgen05_fence_before();
           __syncwarp();
           if (lane == 0) mbar_arrive(&t_empty[tb]);
         }
-        float* dst = G + ((size_t)3 * a0 + c0) * D + (size_t)s * C::d + m;
 #pragma unroll
-        for (int r = 0; r < C::kNMax; ++r)
-          if (r < nc && c0 + r < ncol) dst[(size_t)r * D] = acc[r];
+        for (int w = 0; w < C::kTPW; ++w) {
+          if (!live[w]) continue;
+          float* dst = G + ((size_t)3 * a0 + c0) * D + feat[w];
+#pragma unroll
+          for (int r = 0; r < C::kNMax; ++r)
+            if (r < nc && c0 + r < ncol) dst[(size_t)r * D] = acc[w][r];
+        }
       }
     }
   }
@@ -405,7 +492,7 @@ static int launch_rows_mma(const SorfProblem& pr, const SorfTables& t, const flo
   QMLL_LAUNCH_CHECK("prep_columns_kernel");
   auto kern = sorf_rows_mma_kernel<D_>;
   QMLL_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::kSmem));
-  const long long n_tasks = (long long)pr.n_mol * n_s;
+  const long long n_tasks = (long long)pr.n_mol * ((n_s + C::kSPT - 1) / C::kSPT);
   const int grid = (int)(n_tasks < device_sm_count() ? n_tasks : device_sm_count());
   const float c = (float)(sqrt((double)p->d) / (double)p->sigma * pow((double)p->d, -0.5 * p->n_transform));
   kern<<<grid, C::kThreads, C::kSmem, st>>>(pr.elem, pr.mol_off, pr.n_mol, n_s, n_sg, c, W16, Xh, Xl, xoff,
