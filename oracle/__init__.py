@@ -183,6 +183,28 @@ def gram_rows(A, y, ii):
     return out, out_y
 
 
+def project(rho, elem, U) -> np.ndarray:
+    """x [n_atoms, d] = rho_I^T U_e (eq. 22): rho [n_atoms, rep] fp32, U [n_elem, rep, d] fp32."""
+    rho, elem, U = _f32(rho), _i32(elem), _f32(U)
+    n_atoms, rep = rho.shape
+    d = U.shape[2]
+    x = np.empty((n_atoms, d), dtype=np.float64)
+    _load().qo_project(_p(rho), _p(elem), _L(n_atoms), _I(rep), _I(d), _p(U), _p(x))
+    return x
+
+
+def project_gradient(gin, in_off, elem, mol_off, U, out_off) -> np.ndarray:
+    """Dense gradient [n, rep, n, 3] per molecule -> [n, d, n, 3] per molecule (flat float64, offsets out_off)."""
+    gin, elem, mol_off, U = _f32(gin), _i32(elem), _i32(mol_off), _f32(U)
+    in_off = np.ascontiguousarray(in_off, dtype=np.int64)
+    out_off = np.ascontiguousarray(out_off, dtype=np.int64)
+    rep, d = U.shape[1], U.shape[2]
+    gout = np.zeros(int(out_off[-1]), dtype=np.float64)
+    _load().qo_project_gradient(_p(gin), _p(in_off), _p(elem), _p(mol_off), _I(mol_off.shape[0] - 1), _I(rep), _I(d),
+                                _p(U), _p(out_off), _p(gout))
+    return gout
+
+
 # ---- conveniences over a workloads.Workload-shaped object (attribute access only; no import) ----
 
 def _m(w):

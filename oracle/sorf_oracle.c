@@ -27,7 +27,9 @@
  * all-plus-signs closed form, the per-stack norm invariant, Monte-Carlo convergence to the
  * Gaussian kernel, a dense-W brute force of eq. 14/15, finite-difference forces, G*alpha = F,
  * finite differences of Z against G, Gram-matrix identities and a BLAS cross-check, and
- * sparse == scattered-dense gradients.  No function here is "parity unpinned".
+ * sparse == scattered-dense gradients; qo_project: numpy matmul, the identity U^T U = I (columns of U_e project
+ * onto unit vectors), the norm inequality |x| <= |rho| with equality on the span, and finite differences of a
+ * smooth rho(r) for the projected gradient.  No function here is "parity unpinned".
  */
 #include <math.h>
 #include <stdint.h>
@@ -376,4 +378,42 @@ int qo_solve(const float* ZtZ, const float* Zty, int D, double lambda, double* a
   }
   free(L);
   return info;
+}
+
+/* Per-element PCA projection (eq. 22): rho_I^proj = rho_I^T U_e^{N_PCA}, U_e^{N_PCA} = the first
+ * N_PCA = d columns of the left singular vectors of eq. 21 for the element of atom I ("each element has its own
+ * projection matrix").  U is [n_elem, rep, d] (the d kept columns), rho is [n_atoms, rep]:
+ *   x[I, m] = sum_k rho[I, k] * U[e_I, k, m]. */
+void qo_project(const float* rho, const int32_t* elem, int64_t n_atoms, int rep, int d, const float* U,
+                double* x /* [n_atoms, d] */) {
+#pragma omp parallel for schedule(static)
+  for (int64_t I = 0; I < n_atoms; ++I) {
+    const float* Ue = U + (size_t)elem[I] * rep * d;
+    for (int m = 0; m < d; ++m) {
+      double acc = 0.0;
+      for (int k = 0; k < rep; ++k) acc += (double)rho[(size_t)I * rep + k] * (double)Ue[(size_t)k * d + m];
+      x[(size_t)I * d + m] = acc;
+    }
+  }
+}
+
+/* The same projection applied to a dense descriptor gradient (U is constant, so d x_I / d r = (d rho_I / d r)^T U_e):
+ * molecule M with n atoms holds [n, rep, n, 3] = (I, k, j, c) on input and [n, d, n, 3] = (I, m, j, c) on output
+ * (layout A12 with rep resp. d as the descriptor length); in_off / out_off are the per-molecule float offsets. */
+void qo_project_gradient(const float* gin, const int64_t* in_off, const int32_t* elem, const int32_t* mol_off,
+                         int n_mol, int rep, int d, const float* U, const int64_t* out_off, double* gout) {
+  for (int M = 0; M < n_mol; ++M) {
+    const int a0 = mol_off[M], n = mol_off[M + 1] - a0, ncol = 3 * n;
+    for (int I = 0; I < n; ++I) {
+      const float* Ue = U + (size_t)elem[a0 + I] * rep * d;
+      const float* src = gin + in_off[M] + (size_t)I * rep * ncol;
+      double* dst = gout + out_off[M] + (size_t)I * d * ncol;
+      for (int m = 0; m < d; ++m)
+        for (int c = 0; c < ncol; ++c) {
+          double acc = 0.0;
+          for (int k = 0; k < rep; ++k) acc += (double)src[(size_t)k * ncol + c] * (double)Ue[(size_t)k * d + m];
+          dst[(size_t)m * ncol + c] = acc;
+        }
+    }
+  }
 }

@@ -346,3 +346,70 @@ def test_solve_closed_forms_and_failure():
     bad = np.array([[1.0, 2.0], [2.0, 1.0]], dtype=np.float32)          # indefinite: second minor fails
     _, info = oracle.solve(bad, np.ones(2, np.float32), 0.0)
     assert info == 2
+
+
+# ---------------------------------------------------------------------------------------------------
+# Per-element PCA projection (eq. 21-22): oracle.project / project_gradient
+# ---------------------------------------------------------------------------------------------------
+def test_project_matches_definition_and_picks_the_element_matrix():
+    """x_I = rho_I^T U_e with the matrix of the atom's OWN element (a shared matrix or a transposed one fails)."""
+    from workloads import projection_inputs
+    pi = projection_inputs(seed=5, counts=[4, 0, 7, 1], rep=37, d=16, n_elem=3)
+    x = oracle.project(pi.rho, pi.elem, pi.U)
+    for I in range(pi.rho.shape[0]):
+        ref = pi.rho[I].astype(np.float64) @ pi.U[pi.elem[I]].astype(np.float64)
+        assert np.allclose(x[I], ref, rtol=0, atol=1e-12)
+    wrong = pi.rho.astype(np.float64) @ pi.U[0].astype(np.float64)
+    assert not np.allclose(x[pi.elem != 0], wrong[pi.elem != 0], atol=1e-3)
+
+
+def test_project_orthonormal_columns_identities():
+    """U_e^T U_e = I: a kept singular vector projects onto a unit vector, vectors in the span keep their norm, and
+    every other vector gets shorter (Bessel)."""
+    from workloads import projection_inputs
+    pi = projection_inputs(seed=6, counts=[8], rep=40, d=8, n_elem=2)
+    for e in range(2):
+        Ue = pi.U[e].astype(np.float64)
+        cols = np.ascontiguousarray(Ue.T).astype(np.float32)             # the 8 kept columns as "atoms"
+        x = oracle.project(cols, np.full(8, e, np.int32), pi.U)
+        assert np.allclose(x, np.eye(8), atol=1e-6)
+        coeff = np.random.default_rng(e).standard_normal((5, 8))
+        inspan = (coeff @ Ue.T).astype(np.float32)
+        xs = oracle.project(inspan, np.full(5, e, np.int32), pi.U)
+        assert np.allclose(np.linalg.norm(xs, axis=1), np.linalg.norm(inspan.astype(np.float64), axis=1), rtol=1e-6)
+    x = oracle.project(pi.rho, pi.elem, pi.U)
+    assert np.all(np.linalg.norm(x, axis=1) <= np.linalg.norm(pi.rho.astype(np.float64), axis=1) * (1 + 1e-6))
+    assert np.any(np.linalg.norm(x, axis=1) < 0.9 * np.linalg.norm(pi.rho.astype(np.float64), axis=1))
+
+
+def test_project_gradient_is_the_jacobian_of_the_projected_descriptor():
+    """Finite differences: rho_I(r) = sum_j tanh(A_I r_j + b) is a smooth made-up descriptor whose Jacobian the test
+    writes by hand; the projected gradient must equal d(rho_I^T U_e)/dr (layout (I, m, j, c), A12)."""
+    from workloads import projection_inputs
+    n, rep, d = 3, 10, 4
+    pi = projection_inputs(seed=7, counts=[n], rep=rep, d=d, n_elem=2, with_grad=True)
+    rng = np.random.default_rng(70)
+    A = rng.standard_normal((n, rep, 3)); b = rng.standard_normal((n, rep))
+    r0 = rng.standard_normal((n, 3))
+
+    def rho_of(r):
+        return np.stack([np.sum(np.tanh(np.einsum("kc,jc->jk", A[I], r) + b[I]), axis=0) for I in range(n)])
+
+    drho = np.zeros((n, rep, n, 3))
+    for I in range(n):
+        t = np.tanh(np.einsum("kc,jc->jk", A[I], r0) + b[I])               # [j, k]
+        drho[I] = np.einsum("jk,kc->kjc", 1.0 - t * t, A[I])
+    gout = oracle.project_gradient(drho.astype(np.float32).ravel(), pi.drho_off, pi.elem, pi.mol_off, pi.U, pi.dx_off)
+    gout = gout.reshape(n, d, n, 3)
+    h = 2e-3                     # central differences: O(h^2) truncation, fp32 rounding of rho / h ~ 3e-5
+    for j in range(n):
+        for c in range(3):
+            rp, rm = r0.copy(), r0.copy()
+            rp[j, c] += h; rm[j, c] -= h
+            xp = oracle.project(rho_of(rp).astype(np.float32), pi.elem, pi.U)
+            xm = oracle.project(rho_of(rm).astype(np.float32), pi.elem, pi.U)
+            fd = (xp - xm) / (2 * h)                                         # [I, m]
+            assert np.allclose(gout[:, :, j, c], fd, atol=2e-3 * np.abs(fd).max() + 1e-5)
+    ref = np.einsum("ikjc,ikm->imjc", drho.astype(np.float32).astype(np.float64),
+                    pi.U[pi.elem].astype(np.float64))
+    assert np.allclose(gout, ref, atol=1e-10)

@@ -14,4 +14,6 @@ from .configs import (  # noqa: F401
     make_workload,
     tiny_workload,
     CONFIG_NAMES,
+    ProjectionInputs,
+    projection_inputs,
 )

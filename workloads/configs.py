@@ -261,3 +261,45 @@ def tiny_workload(seed: int, d: int, D: int, T: int, sigma: float, counts, n_ele
     return Workload(name=f"tiny-{seed}", model=model, elem=elem, mol_off=mol_off, x=x,
                     alpha=_normal_f32(seed, TAG_ALPHA, (D,), std=float(1.0 / np.sqrt(D))),
                     y=_y(seed, rows), grad=g, meta={"seed": seed})
+
+
+TAG_RHO, TAG_U, TAG_DRHO = 10, 11, 12
+
+
+@dataclass
+class ProjectionInputs:
+    """Inputs of the per-element PCA projection (eq. 21-22): raw representations rho, the kept
+    columns of every element's U_e, and (optionally) the dense gradient of rho.  Synthetic stand-ins for FCHL19
+    vectors (rep of a few hundred, L179-230); U_e has orthonormal columns, as the left singular vectors of eq. 21."""
+    rep: int
+    d: int
+    elem: np.ndarray                 # int32 [n_atoms]
+    mol_off: np.ndarray              # int32 [n_mol + 1]
+    rho: np.ndarray                  # float32 [n_atoms, rep]
+    U: np.ndarray                    # float32 [n_elem, rep, d]
+    drho: Optional[np.ndarray] = None        # float32 flat: molecule M holds [n, rep, n, 3]
+    drho_off: Optional[np.ndarray] = None    # int64 [n_mol + 1]
+    dx_off: Optional[np.ndarray] = None      # int64 [n_mol + 1]: offsets of the projected gradient [n, d, n, 3]
+
+
+def projection_inputs(seed: int, counts, rep: int, d: int, n_elem: int = N_ELEM, with_grad: bool = False,
+                      rho_std: float = 1.0, grad_std: float = 0.05) -> ProjectionInputs:
+    counts = np.asarray(counts, dtype=np.int32)
+    mol_off = np.zeros(counts.shape[0] + 1, dtype=np.int32)
+    np.cumsum(counts, out=mol_off[1:])
+    na = int(mol_off[-1])
+    elem = _rng(seed, TAG_TOPO).integers(0, n_elem, size=na).astype(np.int32)
+    rho = _normal_f32(seed, TAG_RHO, (na, rep), std=rho_std)
+    U = np.empty((n_elem, rep, d), dtype=np.float32)
+    for e in range(n_elem):        # orthonormal columns: QR of a Gaussian matrix (input generation, not the method)
+        q, _ = np.linalg.qr(_rng(seed, TAG_U, e).standard_normal((rep, d)))
+        U[e] = q.astype(np.float32)
+    out = ProjectionInputs(rep=rep, d=d, elem=elem, mol_off=mol_off, rho=rho, U=U)
+    if with_grad:
+        c2 = counts.astype(np.int64) ** 2
+        out.drho_off = np.zeros(counts.shape[0] + 1, dtype=np.int64)
+        np.cumsum(3 * rep * c2, out=out.drho_off[1:])
+        out.dx_off = np.zeros(counts.shape[0] + 1, dtype=np.int64)
+        np.cumsum(3 * d * c2, out=out.dx_off[1:])
+        out.drho = _normal_f32(seed, TAG_DRHO, (int(out.drho_off[-1]),), std=grad_std)
+    return out
