@@ -103,7 +103,7 @@ def reference_arm(args):
     if int(os.environ.get("RANK", "0")) != 0:
         return
     D = args.D or 16384
-    wt, wi, cores = oracle_sample(D)
+    wt, wi, cores = oracle_sample(D, 2, 8)
     for _ in range(min(args.warmup, 1)):
         oracle_stages(wt, wi)
     tot, st = 0.0, None
@@ -135,7 +135,7 @@ class ClockSampler:
         self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
         try:
             self.p = subprocess.Popen(["nvidia-smi", "-i", str(index), f"--query-gpu={self.Q}",
-                                       "--format=csv,noheader,nounits", "-lms", "100"], stdout=self.f,
+                                       "--format=csv,noheader,nounits", "-lms", "20"], stdout=self.f,
                                       stderr=subprocess.DEVNULL)
         except Exception:
             self.p = None
@@ -374,11 +374,20 @@ def ours_arm(args):
     _, _, pr_ops = sorf_ops(wi, False)
     sm_mhz = (clocks or {}).get("sm_mhz") or 0.0
     fadd = pk["fadd_per_s"]
+    cols = 3.0 * sum(int(c) ** 2 for c in (wt.mol_off[1:] - wt.mol_off[:-1]))
+    mma_flops = 2.0 * 2.0 * wt.model.d * D * cols        # W (d x d per stack) x columns, hi + lo passes, 2 flop per MAC
     sorf_rooflines = {
+        "force_rows_tensor": {"bound": "tensor", "achieved": mma_flops / (fwd_ms * 1e-3) / 1e12, "peak": pk["bf16_sustained"],
+                              "unit": "TFLOP/s", "frac": mma_flops / (fwd_ms * 1e-3) / 1e12 / pk["bf16_sustained"],
+                              "note": "the force rows run on tcgen05 (explicit W of every (element, stack) x fp16 hi/lo columns): "
+                                      "useful f16 flops 2*2*d*D per gradient column (column padding to 16 not counted) / the whole "
+                                      "qmll_sorf_forward call (CUDA events, incl. forward, W build and column split); peak = cuBLAS "
+                                      "bf16 sustained (" + pk["source"] + ")"},
         "forward_plus_force_rows": {"bound": "alu", "achieved": (fwd_ops + fr_ops) / (fwd_ms * 1e-3) / 1e12,
                                     "peak": fadd / 1e12, "unit": "T lane-ops/s", "frac": (fwd_ops + fr_ops) / (fwd_ms * 1e-3) / fadd,
-                                    "note": "algorithmic fp32 lane-ops D*(T*log2 d + 2) per gradient column + forward; time = whole "
-                                            "qmll_sorf_forward call (CUDA events) incl. the gradient transpose; peak = " + pk["fadd_source"]},
+                                    "note": "FWHT-EQUIVALENT rate: the fp32 lane-ops the register chain would need, D*(T*log2 d + 2) per "
+                                            "gradient column + forward, / the same call time; peak = " + pk["fadd_source"] +
+                                            ".  The tensor-core path is not bound by this roofline (it can exceed 1)"},
         "predict": {"bound": "alu", "achieved": pr_ops / (pred_ms * 1e-3) / 1e12, "peak": fadd / 1e12,
                     "unit": "T lane-ops/s", "frac": pr_ops / (pred_ms * 1e-3) / fadd,
                     "gradient_stream_GBps": wi.grad.dense.nbytes / (pred_ms * 1e-3) / 1e9,
@@ -407,7 +416,7 @@ def ours_arm(args):
     if not args.no_configs and world == 1:
         line["configs"] = other_configs(pk, max(2, args.steps // 2))
     if not args.no_cpu_baseline and world == 1:
-        st_wt, st_wi, cores = oracle_sample(D)
+        st_wt, st_wi, cores = oracle_sample(D, 3, 16)
         st = oracle_stages(st_wt, st_wi)
         tot = sum(st.values())
         line["cpu_baseline"] = {"value": (st_wt.n_mol + st_wi.n_mol) / tot, "unit": UNIT, "cores": cores, "kind": "oracle",

@@ -126,8 +126,9 @@ microbench_kernel(float* __restrict__ out, int iters, unsigned long long* __rest
 #pragma unroll
       for (int i = 0; i < kMbUnroll; ++i) {
         float4 v;
-        const uint32_t addr = (uint32_t)__cvta_generic_to_shared(&sm[(tid + 32 * i) & (2 * kMbThreads - 1)]);
-        asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(addr));
+        const uint32_t addr = (uint32_t)__cvta_generic_to_shared(&sm[(tid + 32 * i + it) & (2 * kMbThreads - 1)]);
+        asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];"
+                     : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(addr) : "memory");
         f[i] += v.x + v.w;
       }
     } else if constexpr (KIND == kMbShfl) {

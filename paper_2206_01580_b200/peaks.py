@@ -5,8 +5,9 @@ GPU and prints them as one JSON object:
 
   * plain-ALU issue rates through libqmll.so's `qmll_microbench` (register-only loops on every SM): FADD, FADD2
     (add.f32x2), FFMA, FFMA2, LOP3, SHF, the sign-flip + butterfly mixes of the SORF kernels, MUFU.COS, SHFL, and the
-    shared-memory LDS.128 bandwidth -- each as lane-operations per SM clock (clock64 inside the kernel) and per
-    second (CUDA events; the SM clock under that load is the ratio of the two);
+    shared-memory LDS.128 bandwidth -- each as lane-operations per second (CUDA events, the figure the rooflines use)
+    and per clock64 tick and SM (on this part clock64 advances at about half the SM clock, so that column is only
+    good for ratios between kinds);
   * the TF32 tensor-core GEMM rate (torch.matmul with TF32 allowed, 8192^3): best of 10 (burst) and back to back for
     4 s (sustained), the method MEASURED_PEAKS.json states for its bf16 figure.
 """
@@ -58,8 +59,8 @@ def microbench(kind: int, iters: int = 4096, blocks_per_sm: int = 4, reps: int =
     per_block = ops.value / nb.value
     per_clk_sm = per_block * blocks_per_sm / cyc          # all blocks of an SM are co-resident (4 x 256 threads)
     per_s = ops.value / (best_ms * 1e-3)
-    return {"what": KINDS[kind], "per_clk_per_sm": per_clk_sm, "per_s": per_s,
-            "implied_sm_mhz": per_s / (per_clk_sm * n_sm) / 1e6, "ms": best_ms}
+    return {"what": KINDS[kind], "per_s": per_s, "per_sm_per_clock_at_1965mhz": per_s / n_sm / 1.965e9,
+            "per_clock64_tick_per_sm": per_clk_sm, "ms": best_ms}
 
 
 def tf32_gemm(n: int = 8192, sustained_s: float = 4.0) -> dict:
