@@ -127,6 +127,22 @@ int qmll_normal_equations_mode(const float* A, const float* y, int64_t rows, int
                                float* ZtZ, float* Zty, void* workspace, size_t workspace_bytes, int32_t mode,
                                void* cuda_stream);
 
+/* NEXT row f2: the per-element PCA projection that produces the SORF input from the raw
+ * representation (eq. 21-22; "each element ... has its own projection matrix", L264):
+ *   x[I, m] = sum_k rho[I, k] U[e_I, k, m]                      rho_I^T U_e^{N_PCA},  N_PCA = d
+ * and, if grad_out != NULL, the same projection of a dense descriptor gradient (U is constant):
+ *   grad_out (I, m, j, c) = sum_k grad_in (I, k, j, c) U[e_I, k, m]
+ *   rho      [n_atoms, rep] fp32 (may be NULL if x is NULL)      elem [n_atoms] int32 in [0, n_elem)
+ *   U        [n_elem, rep, d] fp32: the first d columns of every element's U_e (eq. 21); d a multiple of 4
+ *   x        [n_atoms, d] fp32 out (may be NULL)
+ *   grad_in  dense layout A12 with rep as the descriptor length: molecule M (n atoms) holds [n, rep, n, 3] at float
+ *            offset grad_in_off[M]; grad_out holds [n, d, n, 3] at grad_out_off[M] (= the `dense` / `dense_off` of
+ *            qmll_grad); mol_off as in qmll_sorf_forward (needed only with a gradient).
+ * Plain fp32 FMAs (accuracy of an fp32 dot product of length rep); no workspace. */
+int qmll_project(const float* rho, const int32_t* elem, const int32_t* mol_off, int64_t n_atoms, int32_t n_mol,
+                 int32_t rep, int32_t d, int32_t n_elem, const float* U, float* x, const float* grad_in,
+                 const int64_t* grad_in_off, float* grad_out, const int64_t* grad_out_off, void* cuda_stream);
+
 /* Exchange step of data-parallel training: the normal equations are sums over rows, so
  * ranks that own different molecules add their ZtZ / Zty.  ZtZ is symmetric: pack its lower triangle row by row
  * (row i holds i + 1 entries at offset i (i + 1) / 2; D (D + 1) / 2 floats), all-reduce the packed buffer, unpack

@@ -30,7 +30,7 @@ EXPORTS = ("qmll_solve", "qmll_sorf_forward", "qmll_sorf_forward_mode", "qmll_so
            "qmll_normal_equations_mode", "qmll_predict", "qmll_workspace_bytes", "qmll_normal_equations_min_workspace",
            "qmll_normal_equations_workspace", "qmll_normal_equations_min_workspace_mode", "qmll_status_string",
            "qmll_launch_count", "qmll_reset_launch_count", "qmll_time_normal_equations_kernel",
-           "qmll_collect_normal_equations_kernel_ms", "qmll_microbench", "qmll_pack_lower", "qmll_unpack_lower")
+           "qmll_collect_normal_equations_kernel_ms", "qmll_microbench", "qmll_pack_lower", "qmll_unpack_lower", "qmll_project")
 
 
 class _CParams(ctypes.Structure):
@@ -77,6 +77,8 @@ def load_library() -> ctypes.CDLL:
     lib.qmll_normal_equations_min_workspace_mode.argtypes = [i32, i32]
     lib.qmll_normal_equations_min_workspace_mode.restype = sz
     lib.qmll_predict.argtypes = [pp, vp, vp, vp, i64, i32, vp, gp, vp, vp, vp, sz, vp]
+    lib.qmll_project.argtypes = [vp, vp, vp, i64, i32, i32, i32, i32, vp, vp, vp, vp, vp, vp, vp]
+    lib.qmll_project.restype = ctypes.c_int
     lib.qmll_pack_lower.argtypes = [vp, i32, vp, vp]
     lib.qmll_pack_lower.restype = ctypes.c_int
     lib.qmll_unpack_lower.argtypes = [vp, i32, vp, vp]
@@ -274,6 +276,26 @@ def qmll_normal_equations(A, y=None, ZtZ=None, Zty=None, accumulate: bool = Fals
                                           _dev(ZtZ, torch.float32, "ZtZ"), _dev(Zty, torch.float32, "Zty"),
                                           ctypes.c_void_p(ws.data_ptr()), min(ws.numel(), nb), mode, _stream()))
     return ZtZ, Zty
+
+
+def qmll_project(rho, elem, U, mol_off=None, grad_in=None, grad_in_off=None, grad_out_off=None, want_x: bool = True):
+    """(x [n_atoms, d], projected dense gradient or None): include/qmll.h qmll_project (eq. 21-22)."""
+    n_elem, rep, d = (int(v) for v in U.shape)
+    n_atoms = int(elem.shape[0])
+    x = torch.empty((n_atoms, d), dtype=torch.float32, device=U.device) if want_x else None
+    gout = None
+    n_mol = 0
+    if grad_in is not None:
+        n_mol = int(mol_off.shape[0]) - 1
+        total = int(grad_out_off[-1].item()) if grad_out_off.numel() else 0
+        gout = torch.empty((total,), dtype=torch.float32, device=U.device)
+    _check(load_library().qmll_project(_dev(rho, torch.float32, "rho"), _dev(elem, torch.int32, "elem"),
+                                       _dev(mol_off, torch.int32, "mol_off"), n_atoms, n_mol, rep, d, n_elem,
+                                       _dev(U, torch.float32, "U"), _dev(x, torch.float32, "x"),
+                                       _dev(grad_in, torch.float32, "grad_in"), _dev(grad_in_off, torch.int64, "grad_in_off"),
+                                       _dev(gout, torch.float32, "grad_out"), _dev(grad_out_off, torch.int64, "grad_out_off"),
+                                       _stream()))
+    return x, gout
 
 
 def qmll_pack_lower(ZtZ, packed=None):

@@ -1,0 +1,146 @@
+// project_kernels.cu -- NEXT row f2 of SURVEY.md section 8(f): the per-element PCA projection in front of the SORF map,
+//   x_I[m] = sum_k rho_I[k] U[e_I, k, m]                       (rho_I^T U_e^{N_PCA}, eq. 21-22)
+// and the same projection of a dense descriptor gradient (U is constant: d x_I / d r = (d rho_I / d r)^T U_e),
+//   dx_I[m, j, c] = sum_k drho_I[k, j, c] U[e_I, k, m].
+// Both are small grouped GEMMs [d x rep] x [rep x C] per atom (C = 1 resp. 3n) in plain fp32 FMAs: the work is
+// n_atoms * rep * d * C MACs (config 4: 1.1e11 for the gradient, a few ms; 5e9 for x), the accuracy is that of an fp32
+// dot product of length rep (~1e-6 relative), and the result feeds qmll_sorf_forward / qmll_predict unchanged.
+// Mapping: lane = column (an atom for x, a (j, c) column for the gradient), warp = a range of outputs m; the lane
+// keeps 32 accumulators in registers, its input value comes from a shared-memory tile, the U values of a k are the
+// same for the whole warp (broadcast float4 loads through L1).
+#include "qmll_common.cuh"
+#include "sorf_device.cuh"
+
+namespace qmll {
+
+constexpr int kProjThreads = 256;   // 8 warps
+constexpr int kProjK = 64;          // k-chunk staged in shared memory
+constexpr int kProjM = 32;          // outputs per warp pass (register accumulators)
+
+// acc[mm] += U[k][m0 + mm] * a  for k in the staged chunk; tile[k][lane] holds the lane's input values
+__device__ __forceinline__ void proj_accumulate(float (&acc)[kProjM], const float (*tile)[33], int kc, int lane,
+                                                const float* __restrict__ Uk /* U_e + k0*d + m0 */, int d) {
+#pragma unroll 4
+  for (int k = 0; k < kc; ++k) {
+    const float a = tile[k][lane];
+    const float4* u4 = reinterpret_cast<const float4*>(Uk + (size_t)k * d);
+#pragma unroll
+    for (int q = 0; q < kProjM / 4; ++q) {
+      const float4 u = __ldg(u4 + q);
+      acc[4 * q + 0] = fmaf(u.x, a, acc[4 * q + 0]); acc[4 * q + 1] = fmaf(u.y, a, acc[4 * q + 1]);
+      acc[4 * q + 2] = fmaf(u.z, a, acc[4 * q + 2]); acc[4 * q + 3] = fmaf(u.w, a, acc[4 * q + 3]);
+    }
+  }
+}
+
+// x: block = 32 consecutive atoms (lane = atom).  Atoms of different elements use different matrices: the block
+// runs once per element present in its tile, lanes of other elements are masked out.
+__global__ void __launch_bounds__(kProjThreads)
+project_x_kernel(const float* __restrict__ rho, const int32_t* __restrict__ elem, long long n_atoms, int rep, int d,
+                 int n_elem, const float* __restrict__ U, float* __restrict__ x) {
+  __shared__ float tile[kProjK][33];
+  __shared__ int present[64];
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const long long a = (long long)blockIdx.x * 32 + lane;
+  const int e_lane = a < n_atoms ? __ldg(elem + a) : -1;
+  for (int i = threadIdx.x; i < 64; i += kProjThreads) present[i] = 0;
+  __syncthreads();
+  if (warp == 0 && e_lane >= 0) present[e_lane & 63] = 1;   // n_elem <= 64 handled exactly; beyond that all are tried
+  __syncthreads();
+  for (int e = 0; e < n_elem; ++e) {
+    if (n_elem <= 64 && !present[e]) continue;
+    const float* Ue = U + (size_t)e * rep * d;
+    // every warp makes the same number of passes (it helps staging the tile even if it owns no outputs in a pass)
+    for (int mp = 0; mp < d; mp += (kProjThreads / 32) * kProjM) {
+      const int m0 = mp + warp * kProjM;
+      const int mw = m0 >= d ? 0 : (d - m0 < kProjM ? d - m0 : kProjM);
+      float acc[kProjM];
+#pragma unroll
+      for (int i = 0; i < kProjM; ++i) acc[i] = 0.f;
+      for (int k0 = 0; k0 < rep; k0 += kProjK) {
+        const int kc = rep - k0 < kProjK ? rep - k0 : kProjK;
+        __syncthreads();
+        // stage rho[atom][k0 .. k0 + kc) transposed: coalesced along k, one atom per warp pass
+        for (int at = warp; at < 32; at += kProjThreads / 32) {
+          const long long aa = (long long)blockIdx.x * 32 + at;
+          for (int k = lane; k < kc; k += 32) tile[k][at] = aa < n_atoms ? __ldg(rho + (size_t)aa * rep + k0 + k) : 0.f;
+        }
+        __syncthreads();
+        if (mw == kProjM) proj_accumulate(acc, tile, kc, lane, Ue + (size_t)k0 * d + m0, d);
+        else if (mw > 0) {
+          for (int k = 0; k < kc; ++k) {
+            const float av = tile[k][lane];
+            for (int i = 0; i < mw; ++i) acc[i] = fmaf(__ldg(Ue + (size_t)(k0 + k) * d + m0 + i), av, acc[i]);
+          }
+        }
+      }
+      if (e_lane == e) {
+#pragma unroll
+        for (int i = 0; i < kProjM; ++i)
+          if (i < mw) x[(size_t)a * d + m0 + i] = acc[i];
+      }
+    }
+  }
+}
+
+// gradient: block = one atom I; its [rep][3n] block is projected to [d][3n], 32 columns at a time (lane = column).
+__global__ void __launch_bounds__(kProjThreads)
+project_grad_kernel(const float* __restrict__ gin, const int64_t* __restrict__ in_off, const int32_t* __restrict__ elem,
+                    const int32_t* __restrict__ mol_off, int n_mol, int rep, int d, const float* __restrict__ U,
+                    const int64_t* __restrict__ out_off, float* __restrict__ gout) {
+  __shared__ float tile[kProjK][33];
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const int Ig = blockIdx.x;
+  const int M = owner_molecule(mol_off, n_mol, Ig);
+  const int a0 = __ldg(mol_off + M), n = __ldg(mol_off + M + 1) - a0, ncol = 3 * n;
+  const float* src = gin + __ldg(in_off + M) + (size_t)(Ig - a0) * rep * ncol;    // [rep][ncol]
+  float* dst = gout + __ldg(out_off + M) + (size_t)(Ig - a0) * d * ncol;           // [d][ncol]
+  const float* Ue = U + (size_t)__ldg(elem + Ig) * rep * d;
+  for (int c0 = 0; c0 < ncol; c0 += 32) {
+    const int col = c0 + lane;
+    for (int mp = 0; mp < d; mp += (kProjThreads / 32) * kProjM) {
+      const int m0 = mp + warp * kProjM;
+      const int mw = m0 >= d ? 0 : (d - m0 < kProjM ? d - m0 : kProjM);
+      float acc[kProjM];
+#pragma unroll
+      for (int i = 0; i < kProjM; ++i) acc[i] = 0.f;
+      for (int k0 = 0; k0 < rep; k0 += kProjK) {
+        const int kc = rep - k0 < kProjK ? rep - k0 : kProjK;
+        __syncthreads();
+        for (int k = warp; k < kc; k += kProjThreads / 32)
+          tile[k][lane] = col < ncol ? __ldg(src + (size_t)(k0 + k) * ncol + col) : 0.f;
+        __syncthreads();
+        if (mw == kProjM) proj_accumulate(acc, tile, kc, lane, Ue + (size_t)k0 * d + m0, d);
+        else if (mw > 0) {
+          for (int k = 0; k < kc; ++k) {
+            const float av = tile[k][lane];
+            for (int i = 0; i < mw; ++i) acc[i] = fmaf(__ldg(Ue + (size_t)(k0 + k) * d + m0 + i), av, acc[i]);
+          }
+        }
+      }
+      if (col < ncol) {
+#pragma unroll
+        for (int i = 0; i < kProjM; ++i)
+          if (i < mw) dst[(size_t)(m0 + i) * ncol + col] = acc[i];
+      }
+    }
+  }
+}
+
+int project_launch(const float* rho, const int32_t* elem, const int32_t* mol_off, int64_t n_atoms, int32_t n_mol,
+                   int32_t rep, int32_t d, int32_t n_elem, const float* U, float* x, const float* gin,
+                   const int64_t* in_off, float* gout, const int64_t* out_off, cudaStream_t st) {
+  if (n_atoms == 0) return QMLL_OK;
+  if (x) {
+    project_x_kernel<<<(unsigned)((n_atoms + 31) / 32), kProjThreads, 0, st>>>(rho, elem, n_atoms, rep, d, n_elem, U, x);
+    QMLL_LAUNCH_CHECK("project_x_kernel");
+  }
+  if (gout) {
+    project_grad_kernel<<<(unsigned)n_atoms, kProjThreads, 0, st>>>(gin, in_off, elem, mol_off, n_mol, rep, d, U,
+                                                                   out_off, gout);
+    QMLL_LAUNCH_CHECK("project_grad_kernel");
+  }
+  return QMLL_OK;
+}
+
+}  // namespace qmll

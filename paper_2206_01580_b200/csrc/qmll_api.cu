@@ -239,6 +239,20 @@ int qmll_normal_equations(const float* A, const float* y, int64_t rows, int32_t 
                                     QMLL_NE_SPLIT_F16, cuda_stream);
 }
 
+int qmll_project(const float* rho, const int32_t* elem, const int32_t* mol_off, int64_t n_atoms, int32_t n_mol,
+                 int32_t rep, int32_t d, int32_t n_elem, const float* U, float* x, const float* grad_in,
+                 const int64_t* grad_in_off, float* grad_out, const int64_t* grad_out_off, void* cuda_stream) {
+  if (n_atoms < 0 || n_mol < 0 || rep <= 0 || d <= 0 || d % 4 != 0 || n_elem < 1 || !U) return QMLL_ERR_INVALID_ARG;
+  if (!x && !grad_out) return QMLL_ERR_INVALID_ARG;
+  if (n_atoms > 0 && (!elem || (x && !rho))) return QMLL_ERR_INVALID_ARG;
+  if (grad_out && (!grad_in || !grad_in_off || !grad_out_off || !mol_off || n_atoms > 0x7fffff00LL))
+    return QMLL_ERR_INVALID_ARG;
+  int rc = check_device();
+  if (rc) return rc;
+  return project_launch(rho, elem, mol_off, n_atoms, n_mol, rep, d, n_elem, U, x, grad_in, grad_in_off, grad_out,
+                        grad_out_off, static_cast<cudaStream_t>(cuda_stream));
+}
+
 int qmll_pack_lower(const float* ZtZ, int32_t D, float* packed, void* cuda_stream) {
   if (!ZtZ || !packed || D <= 0 || D > 65535) return QMLL_ERR_INVALID_ARG;
   int rc = check_device();

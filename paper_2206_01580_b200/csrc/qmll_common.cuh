@@ -108,6 +108,11 @@ size_t solve_workspace_bytes(int32_t D);
 int solve_normal_equations(const float* ZtZ, const float* Zty, int32_t D, double lambda, float* alpha, int32_t* info,
                            void* ws, size_t ws_bytes, cudaStream_t st);
 
+// ---- per-element PCA projection (project_kernels.cu) ------------------------------------------------------
+int project_launch(const float* rho, const int32_t* elem, const int32_t* mol_off, int64_t n_atoms, int32_t n_mol,
+                   int32_t rep, int32_t d, int32_t n_elem, const float* U, float* x, const float* gin,
+                   const int64_t* in_off, float* gout, const int64_t* out_off, cudaStream_t st);
+
 void syrk_set_timing(bool on);
 int syrk_collect_timing(double* total_ms, int* launches);
 

@@ -128,6 +128,42 @@ def test_force_rows_mma_fewer_transforms(q, T):
     assert rel(G.cpu().numpy(), oracle.force_rows_w(w)) <= TOL
 
 
+@pytest.mark.parametrize("rep,d,counts,n_elem", [(37, 16, [4, 0, 7, 1], 3), (384, 128, [21] * 6, 3), (431, 256, [27, 3, 40], 5),
+                                                 (100, 64, [70], 2)])
+def test_project_matches_oracle(q, rep, d, counts, n_elem):
+    """Per-element PCA projection (eq. 21-22) of descriptors and of a dense gradient: odd rep, ragged molecules, more
+    than 32 columns per atom, several elements inside one 32-atom tile."""
+    pkg, wio, torch = q
+    from workloads import projection_inputs
+    pi = projection_inputs(seed=rep + d, counts=counts, rep=rep, d=d, n_elem=n_elem, with_grad=True)
+    t = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
+    x, g = pkg.qmll_project(t(pi.rho), t(pi.elem), t(pi.U), t(pi.mol_off), t(pi.drho), t(pi.drho_off), t(pi.dx_off))
+    assert rel(x.cpu().numpy(), oracle.project(pi.rho, pi.elem, pi.U)) <= TOL
+    go = oracle.project_gradient(pi.drho, pi.drho_off, pi.elem, pi.mol_off, pi.U, pi.dx_off)
+    assert rel(g.cpu().numpy(), go) <= TOL
+    x2, none = pkg.qmll_project(t(pi.rho), t(pi.elem), t(pi.U))
+    assert none is None and torch.equal(x2, x)
+
+
+def test_project_then_sorf_forward(q):
+    """The projected descriptor and gradient feed the SORF path unchanged: Z, G from raw representations."""
+    pkg, wio, torch = q
+    from workloads import projection_inputs
+    w = tiny_workload(seed=77, d=128, D=512, T=3, sigma=3.0, counts=[5, 8], n_elem=3, grad="dense")
+    pi = projection_inputs(seed=78, counts=[5, 8], rep=200, d=128, n_elem=3, with_grad=True)
+    t = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
+    x, g = pkg.qmll_project(t(pi.rho), t(w.elem), t(pi.U), t(w.mol_off), t(pi.drho), t(pi.drho_off), t(pi.dx_off))
+    dp = wio.device_problem(w)
+    Z, G = pkg.qmll_sorf_forward(dp.params, x, dp.elem, dp.mol_off, pkg.Grad.make_dense(g, t(pi.dx_off)))
+    xo = oracle.project(pi.rho, w.elem, pi.U).astype(np.float32)
+    go = oracle.project_gradient(pi.drho, pi.drho_off, w.elem, w.mol_off, pi.U, pi.dx_off).astype(np.float32)
+    m = w.model
+    Zo = oracle.forward(xo, w.elem, w.mol_off, m.d, m.D, m.T, m.sigma, m.signs, m.bias)
+    Go = oracle.force_rows_dense(xo, w.elem, w.mol_off, m.d, m.D, m.T, m.sigma, m.signs, m.bias, go, pi.dx_off)
+    assert rel(Z.cpu().numpy(), Zo) <= 2 * TOL          # two fp32 stages chained (projection, then SORF)
+    assert rel(G.cpu().numpy(), Go) <= 2 * TOL
+
+
 def test_c2_reduced(q):
     run_all(q, make_workload("c2", n_mol=12, D=2048))
 
