@@ -38,6 +38,8 @@ def parse():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-configs", action="store_true", help="skip the per-config block (C2, C3, C5)")
+    ap.add_argument("--force-rows", default="auto", choices=["auto", "fwht", "mma"],
+                    help="how the force rows are computed (qmll_sorf_forward_mode); the bench line uses auto")
     return ap.parse_args()
 
 
@@ -245,8 +247,10 @@ def ours_arm(args):
     F = torch.empty((wi.n_atoms, 3), dtype=torch.float32, device=dev)
     reducer = qdist.NormalEquationsReducer(D, dev) if world > 1 else None
 
+    rows_mode = {"auto": pkg.ROWS_AUTO, "fwht": pkg.ROWS_FWHT, "mma": pkg.ROWS_MMA}[args.force_rows]
+
     def step(tr, inf, ZtZ_, Zty_, E_, F_):
-        pkg.qmll_sorf_forward(p, tr.x, tr.elem, tr.mol_off, tr.grad, Z=Z, G=G)
+        pkg.qmll_sorf_forward(p, tr.x, tr.elem, tr.mol_off, tr.grad, Z=Z, G=G, force_rows_mode=rows_mode)
         pkg.qmll_normal_equations(A, tr.y, ZtZ=ZtZ_, Zty=Zty_)
         if reducer is not None:
             reducer.allreduce(ZtZ_, Zty_)
@@ -273,7 +277,7 @@ def ours_arm(args):
     e0.record()
     for k in range(args.steps):
         parts[k][0].record()
-        pkg.qmll_sorf_forward(p, dt_.x, dt_.elem, dt_.mol_off, dt_.grad, Z=Z, G=G)
+        pkg.qmll_sorf_forward(p, dt_.x, dt_.elem, dt_.mol_off, dt_.grad, Z=Z, G=G, force_rows_mode=rows_mode)
         parts[k][1].record()
         pkg.qmll_normal_equations(A, dt_.y, ZtZ=ZtZ, Zty=Zty)
         if reducer is not None:
@@ -331,7 +335,7 @@ def ours_arm(args):
                     s_main.wait_event(ev_out[b])              # results of step k-2 have left this output set
                 tb, ib, o = dbuf_t[b], dbuf_i[b], outs[b]
                 gt_, gi_ = workload_io.device_grad(tb, dev), workload_io.device_grad(ib, dev)
-                pkg.qmll_sorf_forward(p, tb["x"], tb["elem"], tb["mol_off"], gt_, Z=Z, G=G)
+                pkg.qmll_sorf_forward(p, tb["x"], tb["elem"], tb["mol_off"], gt_, Z=Z, G=G, force_rows_mode=rows_mode)
                 pkg.qmll_normal_equations(A, tb["y"], ZtZ=o["ZtZ"], Zty=o["Zty"])
                 if reducer is not None:
                     reducer.allreduce(o["ZtZ"], o["Zty"])
@@ -401,7 +405,7 @@ def ours_arm(args):
             "scaling": "weak", "vs_baseline": None,
             "dtype": "f32 (SORF), f16 hi/lo split tensor MMA with fp32 accumulate (ZtZ, fp32-level accuracy)",
             "data": "synthetic",
-            "config": {"workload": WORKLOAD.format(nt=n_train, ni=n_infer, rows=rows),
+            "config": {"workload": WORKLOAD.format(nt=n_train, ni=n_infer, rows=rows), "force_rows": args.force_rows,
                        "l2": "inputs larger than L2 (gradients 1.1 + 4.5 GB, A 2.7 GB); no explicit flush",
                        "parallelism": f"dp{world} (configurations sharded, one all-reduce of the packed lower triangle of ZtZ + Zty per step)"},
             "breakdown_ms": {"forward_and_force_rows": fwd_ms, "normal_equations": ne_ms, "predict": pred_ms,
@@ -414,7 +418,7 @@ def ours_arm(args):
     pkg.release_workspaces()
     torch.cuda.empty_cache()
     if not args.no_configs and world == 1:
-        line["configs"] = other_configs(pk, max(2, args.steps // 2))
+        line["configs"] = other_configs(pk, max(2, args.steps // 2), rows_mode)
     if not args.no_cpu_baseline and world == 1:
         st_wt, st_wi, cores = oracle_sample(D, 3, 16)
         st = oracle_stages(st_wt, st_wi)
@@ -429,7 +433,7 @@ def ours_arm(args):
         dist.destroy_process_group()
 
 
-def other_configs(pk, reps):
+def other_configs(pk, reps, rows_mode=0):
     """Absolute numbers and the binding roofline fraction for the other timed configs (north_star): C2, C3, C5."""
     import torch
     import paper_2206_01580_b200 as pkg
@@ -462,7 +466,8 @@ def other_configs(pk, reps):
             rows = nm + (3 * na if train else 0)
             A = torch.empty((rows, D), dtype=torch.float32, device="cuda")
             if train:
-                t = tm(lambda: pkg.qmll_sorf_forward(p, dp.x, dp.elem, dp.mol_off, dp.grad, Z=A[:nm], G=A[nm:]))
+                t = tm(lambda: pkg.qmll_sorf_forward(p, dp.x, dp.elem, dp.mol_off, dp.grad, Z=A[:nm], G=A[nm:],
+                                                     force_rows_mode=rows_mode))
             else:
                 t = tm(lambda: pkg.qmll_sorf_forward(p, dp.x, dp.elem, dp.mol_off, Z=A))
             o.update({"forward_ms": t, "forward_molecules_per_s": nm / (t * 1e-3),
