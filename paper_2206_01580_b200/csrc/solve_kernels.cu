@@ -1,16 +1,18 @@
 // solve_kernels.cu -- NEXT #1 of SURVEY.md section 8(f): alpha = (ZtZ + lambda I)^-1 Zty  (eq. 16-17;
 // "solved by LU decomposition", L137 -- the matrix is symmetric positive definite, so Cholesky).  FP64 throughout: the
 // Gram matrix of random features is ill-conditioned (the paper's FP32 round-off remark, L351), and the O(D^3/3) solve
-// is small beside the O(rows D^2) accumulation.  Blocked right-looking Cholesky (64-wide panels):
-//   potrf_diag_kernel (one CTA, diagonal block in shared memory)  ->  trsm_panel_kernel (thread per row)
-//   ->  syrk_update_kernel (64 x 64 x 64 DFMA tiles over the lower triangle of the trailing matrix),
+// is small beside the O(rows D^2) accumulation.  Two-level blocked right-looking Cholesky:
+//   potrf_diag_kernel (one CTA, 64 x 64 diagonal block in shared memory)  ->  trsm_panel_kernel (thread per row)
+//   ->  syrk_update_kernel on the 256-wide panel's own columns; after the panel one rank-256 syrk_update_kernel of
+//   the trailing matrix (128 x 128 tiles, 8 x 8 DFMA register tiles),
 // then forward / backward substitution by blocks.  `info` (device int) follows LAPACK: 0 = success, k > 0 = the
 // leading minor of order k is not positive definite (the factorisation then carries NaNs).
 #include "qmll_common.cuh"
 
 namespace qmll {
 
-constexpr int kNB = 64;
+constexpr int kNB = 64;     // inner step: diagonal block factorised in shared memory
+constexpr int kNB2 = 256;   // outer panel: one trailing update per 256 columns
 
 __global__ void solve_prepare_kernel(const float* __restrict__ ZtZ, const float* __restrict__ Zty, int D, double lambda,
                                      double* __restrict__ M, double* __restrict__ rhs, int* __restrict__ info) {
@@ -80,40 +82,63 @@ __global__ void __launch_bounds__(128) trsm_panel_kernel(double* __restrict__ M,
     if (c < nb) row[c] = x[c];
 }
 
-// Trailing update A22 -= L21 L21^T on the lower triangle: CTA (ti, tj), tj <= ti, computes a 64 x 64 tile.
-__global__ void __launch_bounds__(256) syrk_update_kernel(double* __restrict__ M, int D, int k0, int nb) {
-  if (blockIdx.y > blockIdx.x) return;
-  __shared__ double li[64][33], lj[64][33];  // one half of the 64-wide panel at a time (static smem <= 48 KB)
-  const int base = k0 + nb;
-  const int i0 = base + blockIdx.x * 64, j0 = base + blockIdx.y * 64;
-  const int t = threadIdx.x;
-  const int tr = (t / 16) * 4, tc = (t % 16) * 4;  // 4 x 4 outputs per thread
-  double acc[4][4] = {};
-  for (int mh = 0; mh < kNB; mh += 32) {
-    __syncthreads();
-    for (int idx = t; idx < 64 * 32; idx += 256) {
-      const int r = idx / 32, m = mh + idx % 32;
-      li[r][idx % 32] = (i0 + r < D && m < nb) ? M[(size_t)(i0 + r) * D + k0 + m] : 0.0;
-      lj[r][idx % 32] = (j0 + r < D && m < nb) ? M[(size_t)(j0 + r) * D + k0 + m] : 0.0;
+// Symmetric rank-kn update on the lower triangle:  C[i][j] -= sum_{m < kn} M[i][k0 + m] * M[j][k0 + m]  for rows
+// i >= r0, columns c0 <= j < c1, j <= i.  CTA = 128 x 128 tile (blockIdx.x: row tile from r0, blockIdx.y: column tile
+// from c0), thread = 8 x 8 outputs (rows ty + 16 u, columns tx + 16 v: shared-memory reads are broadcasts or
+// conflict-free, the write-back is coalesced), k in chunks of 16 through shared memory.  64 DFMA per 16 LDS.64: the
+// FP64 pipe, not shared memory, bounds it.
+constexpr int kUT = 128;   // tile
+constexpr int kUK = 16;    // k chunk
+__global__ void __launch_bounds__(256) syrk_update_kernel(double* __restrict__ M, int D, int r0, int c0, int c1, int k0,
+                                                          int kn) {
+  const int i0 = r0 + blockIdx.x * kUT, j0 = c0 + blockIdx.y * kUT;
+  if (j0 >= c1 || j0 > i0 + kUT - 1) return;          // tile entirely above the diagonal or outside the column range
+  __shared__ double li[kUK][kUT + 2], lj[kUK][kUT + 2];
+  const int t = threadIdx.x, tx = t & 15, ty = t >> 4;
+  double acc[8][8];
+#pragma unroll
+  for (int u = 0; u < 8; ++u)
+#pragma unroll
+    for (int v = 0; v < 8; ++v) acc[u][v] = 0.0;
+  // 128 rows x 16 k doubles per operand and chunk: thread t owns row t / 2, k half t % 2 (8 doubles = 64 contiguous
+  // bytes).  The next chunk is fetched into registers while the current one is multiplied (software pipeline).
+  const int lr = t >> 1, lkh = (t & 1) * 8;
+  const bool oki = i0 + lr < D, okj = j0 + lr < D;
+  const double* pi = M + (size_t)(oki ? i0 + lr : 0) * D + k0 + lkh;
+  const double* pj = M + (size_t)(okj ? j0 + lr : 0) * D + k0 + lkh;
+  double ni[8], nj[8];
+  auto fetch = [&](int m0) {
+#pragma unroll
+    for (int q = 0; q < 8; ++q) {
+      const bool okm = m0 + lkh + q < kn;
+      ni[q] = (oki && okm) ? pi[m0 + q] : 0.0;
+      nj[q] = (okj && okm) ? pj[m0 + q] : 0.0;
     }
+  };
+  fetch(0);
+  for (int m0 = 0; m0 < kn; m0 += kUK) {
     __syncthreads();
-#pragma unroll 8
-    for (int m = 0; m < 32; ++m) {
-      double a[4], b[4];
 #pragma unroll
-      for (int u = 0; u < 4; ++u) { a[u] = li[tr + u][m]; b[u] = lj[tc + u][m]; }
+    for (int q = 0; q < 8; ++q) { li[lkh + q][lr] = ni[q]; lj[lkh + q][lr] = nj[q]; }
+    __syncthreads();
+    if (m0 + kUK < kn) fetch(m0 + kUK);
 #pragma unroll
-      for (int u = 0; u < 4; ++u)
+    for (int m = 0; m < kUK; ++m) {
+      double a[8], b[8];
 #pragma unroll
-        for (int v = 0; v < 4; ++v) acc[u][v] = fma(a[u], b[v], acc[u][v]);
+      for (int u = 0; u < 8; ++u) { a[u] = li[m][ty + 16 * u]; b[u] = lj[m][tx + 16 * u]; }
+#pragma unroll
+      for (int u = 0; u < 8; ++u)
+#pragma unroll
+        for (int v = 0; v < 8; ++v) acc[u][v] = fma(a[u], b[v], acc[u][v]);
     }
   }
 #pragma unroll
-  for (int u = 0; u < 4; ++u)
+  for (int u = 0; u < 8; ++u)
 #pragma unroll
-    for (int v = 0; v < 4; ++v) {
-      const int i = i0 + tr + u, j = j0 + tc + v;
-      if (i < D && j <= i) M[(size_t)i * D + j] -= acc[u][v];
+    for (int v = 0; v < 8; ++v) {
+      const int i = i0 + ty + 16 * u, j = j0 + tx + 16 * v;
+      if (i < D && j < c1 && j <= i) M[(size_t)i * D + j] -= acc[u][v];
     }
 }
 
@@ -182,17 +207,31 @@ int solve_normal_equations(const float* ZtZ, const float* Zty, int32_t D, double
   if (!ws_ptr || ((uintptr_t)ws_ptr & 255) != 0 || !ws.fits()) return QMLL_ERR_WORKSPACE;
   solve_prepare_kernel<<<1184, 256, 0, st>>>(ZtZ, Zty, D, lambda, M, rhs, info);
   QMLL_LAUNCH_CHECK("solve_prepare_kernel");
-  for (int k0 = 0; k0 < D; k0 += kNB) {
-    const int nb = D - k0 < kNB ? D - k0 : kNB;
-    potrf_diag_kernel<<<1, 256, 0, st>>>(M, D, k0, nb, info);
-    QMLL_LAUNCH_CHECK("potrf_diag_kernel");
-    const int rest = D - k0 - nb;
-    if (rest > 0) {
-      trsm_panel_kernel<<<(rest + 127) / 128, 128, 0, st>>>(M, D, k0, nb);
-      QMLL_LAUNCH_CHECK("trsm_panel_kernel");
-      const unsigned nt = (unsigned)((rest + 63) / 64);
-      syrk_update_kernel<<<dim3(nt, nt), 256, 0, st>>>(M, D, k0, nb);
-      QMLL_LAUNCH_CHECK("syrk_update_kernel");
+  // Two levels: 64-wide steps factor a 256-wide panel (their updates touch the panel's own columns only), then ONE
+  // rank-256 update of the trailing matrix: the trailing matrix is read and written D / 256 times instead of D / 64.
+  for (int K0 = 0; K0 < D; K0 += kNB2) {
+    const int nb2 = D - K0 < kNB2 ? D - K0 : kNB2;
+    for (int k0 = K0; k0 < K0 + nb2; k0 += kNB) {
+      const int nb = K0 + nb2 - k0 < kNB ? K0 + nb2 - k0 : kNB;
+      potrf_diag_kernel<<<1, 256, 0, st>>>(M, D, k0, nb, info);
+      QMLL_LAUNCH_CHECK("potrf_diag_kernel");
+      const int rest = D - k0 - nb;
+      if (rest > 0) {
+        trsm_panel_kernel<<<(rest + 127) / 128, 128, 0, st>>>(M, D, k0, nb);
+        QMLL_LAUNCH_CHECK("trsm_panel_kernel");
+        const int c0 = k0 + nb, c1 = K0 + nb2;             // the panel's remaining columns
+        if (c1 > c0) {
+          dim3 g((unsigned)((D - c0 + kUT - 1) / kUT), (unsigned)((c1 - c0 + kUT - 1) / kUT));
+          syrk_update_kernel<<<g, 256, 0, st>>>(M, D, c0, c0, c1, k0, nb);
+          QMLL_LAUNCH_CHECK("syrk_update_kernel(panel)");
+        }
+      }
+    }
+    const int t0 = K0 + nb2;                                // trailing matrix
+    if (t0 < D) {
+      const unsigned nt = (unsigned)((D - t0 + kUT - 1) / kUT);
+      syrk_update_kernel<<<dim3(nt, nt), 256, 0, st>>>(M, D, t0, t0, D, K0, nb2);
+      QMLL_LAUNCH_CHECK("syrk_update_kernel(trailing)");
     }
   }
   for (int k0 = 0; k0 < D; k0 += kNB) {  // L y = b
