@@ -191,8 +191,8 @@ def ne_roofline(rows, D, kern_ms, ms_step, pk, traffic):
          "unit": "TFLOP/s", "frac": achieved / peak, "traffic": traffic,
          "algorithmic_bytes": 4.0 * rows * D + 2.0 * D * (D + 1),
          "frac_of_burst_peak": achieved / (pk["bf16_burst"] / 3.0),
-         "note": (f"achieved = rows*D*(D+1) fp32-equivalent flops per launch / CUDA-event time of the kernel "
-                  f"({kern_ms:.3f} ms avg, events on the launch stream inside the library); peak = cuBLAS bf16 "
+         "note": (f"achieved = rows*D*(D+1) fp32-equivalent flops per call / CUDA-event time of the tcgen05 kernel per call "
+                  f"({kern_ms:.3f} ms, summed over its row panels, events on the launch stream inside the library); peak = cuBLAS bf16 "
                   f"SUSTAINED ({pk['source']}: the kernel is timed inside a long step) / 3 -- f16 and bf16 MMAs run at "
                   f"the same rate; against the burst figure the fraction is frac_of_burst_peak; share of step = "
                   f"{kern_ms / ms_step:.3f}"),
@@ -372,7 +372,7 @@ def ours_arm(args):
 
     # ---- rooflines -----------------------------------------------------------------------------------------------
     pk = peaks()
-    kern_ms = syrk_ms / max(syrk_n, 1)
+    kern_ms = syrk_ms / args.steps          # per CALL: a call runs one tcgen05 launch per panel of <= 32768 rows
     roofline = ne_roofline(rows, D, kern_ms, ms_step, pk, load_traffic())
     fwd_ops, fr_ops, _ = sorf_ops(wt, True)
     _, _, pr_ops = sorf_ops(wi, False)
@@ -479,8 +479,10 @@ def other_configs(pk, reps, rows_mode=0):
             t = tm(lambda: pkg.qmll_normal_equations(A, dp.y, ZtZ=ZtZ, Zty=Zty))
             kms, kn = pkg.collect_normal_equations_kernel_ms()
             pkg.time_normal_equations_kernel(False)
-            tf = rows * D * (D + 1.0) / (kms / max(kn, 1) * 1e-3) / 1e12
-            o.update({"normal_equations_ms": t, "ztz_kernel_ms": kms / max(kn, 1), "ztz_tflops_fp32eq_half": tf,
+            kcall = kms / (2 + reps)             # tm() makes 2 warm-up + reps calls; a call = one launch per row panel
+            tf = rows * D * (D + 1.0) / (kcall * 1e-3) / 1e12
+            o.update({"normal_equations_ms": t, "ztz_kernel_ms": kcall, "ztz_launches_per_call": kn // (2 + reps),
+                      "ztz_tflops_fp32eq_half": tf,
                       "ztz_tensor_frac": tf / (pk["bf16_sustained"] / 3.0)})
             del A, ZtZ
         if name != "c3":

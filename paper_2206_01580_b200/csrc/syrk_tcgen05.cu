@@ -40,6 +40,7 @@ constexpr int kStages = 2;
 // round-to-nearest.  A compile-time constant: it is part of the numerics of the call.
 constexpr int kChunkRows = 128;
 constexpr int kPanelRows = 1024;  // panel granularity (rows) when the workspace cannot hold all rows
+constexpr long long kMaxPanelRows = 32768;  // see syrk_impl (measured: 100 000 x 16384 in 4 panels 68.7 ms, in one 85.0 ms)
 constexpr int kColBlock = 128;    // column granularity of the fp16 scales and of the split pass
 constexpr int kSyrkThreads = 320; // warp 0 TMA producer, warp 1 MMA issuer, warps 2..9 epilogue
 constexpr uint32_t kTileABytes = kBM * 128;                 // 128 features x 128 bytes of rows: 16 KB
@@ -551,8 +552,15 @@ static int syrk_impl(const float* A, const float* y, int64_t rows, int32_t D, in
                      void* ws, size_t ws_bytes, cudaStream_t st) {
   using M = SplitMode<F16>;
   constexpr int mode = F16 ? QMLL_NE_SPLIT_F16 : QMLL_NE_SPLIT_TF32;
-  // rows per panel: as many as the workspace holds, a multiple of kPanelRows unless everything fits
+  // rows per panel: as many as the workspace holds, a multiple of kPanelRows unless everything fits -- but never more
+  // than kMaxPanelRows: the CTAs of the persistent kernel drift apart along the rows, and once the operand rows they
+  // are reading no longer fit L2 together every CTA streams from DRAM on its own (config 3, 100 000 rows: 0.76 of the
+  // tensor peak in one panel).  Panels re-synchronise them; ZtZ is read-modify-written once per extra panel.
   long long panel = pad_rows(rows, mode);
+  if (panel > kMaxPanelRows) {
+    const long long n_pan = (panel + kMaxPanelRows - 1) / kMaxPanelRows;
+    panel = ((panel + n_pan - 1) / n_pan + kPanelRows - 1) / kPanelRows * kPanelRows;
+  }
   if (panel_layout(panel, D, mode).total() > ws_bytes) {
     const size_t per_row = (size_t)2 * D * M::kElemBytes;   // lower bound of the bytes one more row costs
     panel = (long long)(ws_bytes / per_row) / kPanelRows * kPanelRows + kPanelRows;
