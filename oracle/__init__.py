@@ -18,15 +18,16 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "sorf_oracle.c")
+_SRCS = [_SRC, os.path.join(_HERE, "fchl19_oracle.c")]
 _LIB = os.path.join(_HERE, "libsorf_oracle.so")
 _lib = None
 
 
 def build(force: bool = False) -> str:
-    """Compile sorf_oracle.c with gcc (-O2, no fast-math, OpenMP)."""
-    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+    """Compile sorf_oracle.c and fchl19_oracle.c with gcc (-O2, no fast-math, OpenMP)."""
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < max(os.path.getmtime(s) for s in _SRCS):
         tmp = _LIB + f".tmp{os.getpid()}"
-        subprocess.check_call(["gcc", "-O2", "-std=c99", "-fopenmp", "-fPIC", "-shared", _SRC, "-o", tmp, "-lm"])
+        subprocess.check_call(["gcc", "-O2", "-std=c99", "-fopenmp", "-fPIC", "-shared"] + _SRCS + ["-o", tmp, "-lm"])
         os.replace(tmp, _LIB)
     return _LIB
 
@@ -203,6 +204,63 @@ def project_gradient(gin, in_off, elem, mol_off, U, out_off) -> np.ndarray:
     _load().qo_project_gradient(_p(gin), _p(in_off), _p(elem), _p(mol_off), _I(mol_off.shape[0] - 1), _I(rep), _I(d),
                                 _p(U), _p(out_off), _p(gout))
     return gout
+
+
+# ---- FCHL19 representation and its Jacobian (fchl19_oracle.c; eq. 23-33) ----
+
+def _fchl_args(fp):
+    """fp: any object with n_elem, n2, n3, eta2, eta3, N2, N3, c3, zeta, r_cut (attribute access only)."""
+    return [_I(fp.n_elem), _I(fp.n2), _I(fp.n3), _D(fp.eta2), _D(fp.eta3), _D(fp.N2), _D(fp.N3), _D(fp.c3),
+            _D(fp.zeta), _D(fp.r_cut)]
+
+
+def fchl19_rep_size(fp) -> int:
+    return int(_load().qo_fchl19_rep_size(_I(fp.n_elem), _I(fp.n2), _I(fp.n3)))
+
+
+def fchl19(fp, r, elem, nbr_idx, nbr_shift=None) -> np.ndarray:
+    """rho [n_atoms, rep]: the FCHL19 representation of every atom from its neighbour images (readings B1-B8)."""
+    r, elem, nbr_idx = _f32(r), _i32(elem), _i32(nbr_idx)
+    nbr_shift = None if nbr_shift is None else _f32(nbr_shift)
+    n_atoms, K = nbr_idx.shape
+    rho = np.empty((n_atoms, fchl19_rep_size(fp)), dtype=np.float64)
+    _load().qo_fchl19(_p(r), _p(elem), _L(n_atoms), _p(nbr_idx), _p(nbr_shift), _I(K), *_fchl_args(fp), _p(rho))
+    return rho
+
+
+def fchl19_jacobian(fp, r, elem, nbr_idx, nbr_shift=None, atoms=None) -> np.ndarray:
+    """jac [n_sel, K + 1, rep, 3] for the atoms in `atoms` (default: all): slot 0 = the atom itself, slot 1 + q =
+    neighbour slot q (reading B9); complex-step derivative of the representation."""
+    r, elem, nbr_idx = _f32(r), _i32(elem), _i32(nbr_idx)
+    nbr_shift = None if nbr_shift is None else _f32(nbr_shift)
+    n_atoms, K = nbr_idx.shape
+    atoms = np.arange(n_atoms, dtype=np.int64) if atoms is None else np.ascontiguousarray(atoms, dtype=np.int64)
+    jac = np.empty((atoms.shape[0], K + 1, fchl19_rep_size(fp), 3), dtype=np.float64)
+    _load().qo_fchl19_jacobian(_p(r), _p(elem), _p(nbr_idx), _p(nbr_shift), _I(K), _p(atoms), _L(atoms.shape[0]),
+                               *_fchl_args(fp), _p(jac))
+    return jac
+
+
+def fchl19_atom(fp, centre, img, img_elem, jacobian: bool = False):
+    """rho [rep] (and jac [nn + 1, rep, 3]) of one atom from FP64 positions: centre [3], img [nn, 3]."""
+    centre = np.ascontiguousarray(centre, dtype=np.float64)
+    img = np.ascontiguousarray(img, dtype=np.float64).reshape(-1, 3)
+    img_elem = _i32(img_elem)
+    nn, rep = img.shape[0], fchl19_rep_size(fp)
+    rho = np.empty(rep, dtype=np.float64)
+    jac = np.empty((nn + 1, rep, 3), dtype=np.float64) if jacobian else None
+    _load().qo_fchl19_atom_f64(_p(centre), _p(img), _p(img_elem), _I(nn), *_fchl_args(fp), _p(rho), _p(jac))
+    return (rho, jac) if jacobian else rho
+
+
+def project_neighbor_gradient(gin, elem, U) -> np.ndarray:
+    """[n_atoms, S, rep, 3] fp32 -> [n_atoms, S, d, 3] float64 with every atom's own U_e (eq. 21-22)."""
+    gin, elem, U = _f32(gin), _i32(elem), _f32(U)
+    n_atoms, S, rep, _ = gin.shape
+    d = U.shape[2]
+    out = np.empty((n_atoms, S, d, 3), dtype=np.float64)
+    _load().qo_project_neighbor_gradient(_p(gin), _p(elem), _L(n_atoms), _I(S), _I(rep), _I(d), _p(U), _p(out))
+    return out
 
 
 # ---- conveniences over a workloads.Workload-shaped object (attribute access only; no import) ----

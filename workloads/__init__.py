@@ -17,3 +17,4 @@ from .configs import (  # noqa: F401
     ProjectionInputs,
     projection_inputs,
 )
+from .geometry import FchlParams, FCHL_E, Geometry, molecules_geometry, cell_geometry  # noqa: F401
