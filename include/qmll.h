@@ -143,6 +143,59 @@ int qmll_project(const float* rho, const int32_t* elem, const int32_t* mol_off, 
                  int32_t rep, int32_t d, int32_t n_elem, const float* U, float* x, const float* grad_in,
                  const int64_t* grad_in_off, float* grad_out, const int64_t* grad_out_off, void* cuda_stream);
 
+/* NEXT row f3: the FCHL19 atomic representation (section E, eq. 23-33;
+ * Table I) and its Jacobian with respect to the atomic positions, which make the path start from
+ * coordinates: qmll_fchl19 -> qmll_project / qmll_project_neighbor -> qmll_sorf_forward / qmll_predict.
+ *   two-body  (eq. 24-27): rho_i[X, s] = sum_{j: Z_j = X} f_cut(r_ij) r_ij^-N2 LogNormal(R_s; mu(r_ij), sigma(r_ij))
+ *   three-body (eq. 28-33): rho_i[{X,Y}, s, a] = sum_{j<k, {Z_j, Z_k} = {X, Y}} xi_3 G_radial,s G_angular,a
+ *                                                 f_cut(r_ij) f_cut(r_ik) f_cut(r_jk),  a = cos, sin (n = 1)
+ * Readings (B1-B9): R_s = r_cut (s + 1) / n; f_cut = 0 beyond r_cut; unordered neighbour pairs; layout of
+ * rho_i = [X][s] for X < n_elem, then [pair p(X <= Y) = X E - X (X - 1) / 2 + (Y - X)][s][cos, sin]:
+ *   rep = n_elem n2 + n_elem (n_elem + 1) n3. */
+typedef struct {
+  int32_t n_elem;          /* element classes E, 1..16                                                         */
+  int32_t n2, n3;          /* radial grid points of the two- and three-body terms, 1..32 (Table I: 23/24, 22/20) */
+  float eta2, eta3;        /* widths (eq. 25-26, eq. 29)                                                       */
+  float two_body_decay;    /* N_2 (eq. 24)                                                                     */
+  float three_body_decay;  /* N_3 (eq. 30)                                                                     */
+  float three_body_weight; /* c_3 (eq. 30)                                                                     */
+  float zeta;              /* angular width (eq. 32-33); Table I: pi                                           */
+  float r_cut;             /* cut-off radius > 0 (eq. 27); Table I: 6.0                                        */
+} qmll_fchl19_params;
+
+#define QMLL_FCHL19_MAX_NEIGHBOURS 160 /* neighbours INSIDE r_cut per atom the kernel holds on chip */
+
+/* Length of rho_i for these parameters (host arithmetic). */
+int32_t qmll_fchl19_rep_size(const qmll_fchl19_params* fp);
+
+/*   r        [n_atoms, 3] fp32 positions;  elem [n_atoms] int32 in [0, n_elem)
+ *   nbr_idx  [n_atoms, K] int32: candidate neighbours of atom i (global index j, -1 = padding); slot q stands for the
+ *            image r[j] + nbr_shift[i, q, :] (nbr_shift [n_atoms, K, 3] fp32, NULL = no shifts: isolated molecules).
+ *            The list is the caller's (neighbour search / periodic images are not part of this library); entries at
+ *            or beyond r_cut contribute nothing; an atom must not list itself with a zero shift.
+ *   rho      [n_atoms, rep] fp32 out
+ *   jac_idx  [n_atoms, K + 1] int32 out, jac_val [n_atoms, K + 1, rep, 3] fp32 out, both NULL = representation only:
+ *            slot 0 is the atom itself (jac_idx = i), slot 1 + q the image of neighbour slot q (jac_idx = j, or -1 and
+ *            a zero block if that slot is padding or outside r_cut);
+ *            jac_val[i, slot, k, c] = d rho_i[k] / d (position of that slot's atom)_c.  This is the NEIGHBOR layout of
+ *            qmll_grad with descriptor length rep and K + 1 neighbours (images are independent variables; qmll_predict
+ *            adds their contributions into the force on atom j).
+ *   info     device int32 out: 0, or 1 + index of an atom with more than QMLL_FCHL19_MAX_NEIGHBOURS neighbours inside
+ *            r_cut (its result is then incomplete).
+ * Collinear triplets (sin theta = 0) have an unbounded d sin theta / d r; the kernel clamps sin theta at 1e-6 there.
+ * fp32 arithmetic; no workspace. */
+int qmll_fchl19(const qmll_fchl19_params* fp, const float* r, const int32_t* elem, int64_t n_atoms,
+                const int32_t* nbr_idx, const float* nbr_shift, int32_t K, float* rho, int32_t* jac_idx,
+                float* jac_val, int32_t* info, void* cuda_stream);
+
+/* The per-element projection (qmll_project) of a NEIGHBOR-layout gradient, e.g. the Jacobian of qmll_fchl19:
+ *   grad_out[I, q, m, c] = sum_k grad_in[I, q, k, c] U[e_I, k, m]
+ *   grad_in [n_atoms, S, rep, 3] fp32, grad_out [n_atoms, S, d, 3] fp32, U [n_elem, rep, d] fp32, d % 4 == 0.
+ * idx [n_atoms, S] int32 (may be NULL): blocks whose idx is negative are not read and are written as zeros. */
+int qmll_project_neighbor(const float* grad_in, const int32_t* idx, const int32_t* elem, int64_t n_atoms, int32_t S,
+                          int32_t rep, int32_t d, int32_t n_elem, const float* U, float* grad_out,
+                          void* cuda_stream);
+
 /* Exchange step of data-parallel training: the normal equations are sums over rows, so
  * ranks that own different molecules add their ZtZ / Zty.  ZtZ is symmetric: pack its lower triangle row by row
  * (row i holds i + 1 entries at offset i (i + 1) / 2; D (D + 1) / 2 floats), all-reduce the packed buffer, unpack

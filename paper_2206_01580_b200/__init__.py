@@ -30,7 +30,8 @@ EXPORTS = ("qmll_solve", "qmll_sorf_forward", "qmll_sorf_forward_mode", "qmll_so
            "qmll_normal_equations_mode", "qmll_predict", "qmll_workspace_bytes", "qmll_normal_equations_min_workspace",
            "qmll_normal_equations_workspace", "qmll_normal_equations_min_workspace_mode", "qmll_status_string",
            "qmll_launch_count", "qmll_reset_launch_count", "qmll_time_normal_equations_kernel",
-           "qmll_collect_normal_equations_kernel_ms", "qmll_microbench", "qmll_pack_lower", "qmll_unpack_lower", "qmll_project")
+           "qmll_collect_normal_equations_kernel_ms", "qmll_microbench", "qmll_pack_lower", "qmll_unpack_lower", "qmll_project",
+           "qmll_project_neighbor", "qmll_fchl19", "qmll_fchl19_rep_size")
 
 
 class _CParams(ctypes.Structure):
@@ -43,6 +44,12 @@ class _CGrad(ctypes.Structure):
     _fields_ = [("layout", ctypes.c_int32), ("dense", ctypes.c_void_p), ("dense_off", ctypes.c_void_p),
                 ("nbr_idx", ctypes.c_void_p), ("nbr_val", ctypes.c_void_p), ("K", ctypes.c_int32),
                 ("dense_floats", ctypes.c_int64)]
+
+
+class _CFchl(ctypes.Structure):
+    _fields_ = [("n_elem", ctypes.c_int32), ("n2", ctypes.c_int32), ("n3", ctypes.c_int32), ("eta2", ctypes.c_float),
+                ("eta3", ctypes.c_float), ("two_body_decay", ctypes.c_float), ("three_body_decay", ctypes.c_float),
+                ("three_body_weight", ctypes.c_float), ("zeta", ctypes.c_float), ("r_cut", ctypes.c_float)]
 
 
 class QmllError(RuntimeError):
@@ -79,6 +86,12 @@ def load_library() -> ctypes.CDLL:
     lib.qmll_predict.argtypes = [pp, vp, vp, vp, i64, i32, vp, gp, vp, vp, vp, sz, vp]
     lib.qmll_project.argtypes = [vp, vp, vp, i64, i32, i32, i32, i32, vp, vp, vp, vp, vp, vp, vp]
     lib.qmll_project.restype = ctypes.c_int
+    lib.qmll_project_neighbor.argtypes = [vp, vp, vp, i64, i32, i32, i32, i32, vp, vp, vp]
+    lib.qmll_project_neighbor.restype = ctypes.c_int
+    lib.qmll_fchl19.argtypes = [ctypes.POINTER(_CFchl), vp, vp, i64, vp, vp, i32, vp, vp, vp, vp, vp]
+    lib.qmll_fchl19.restype = ctypes.c_int
+    lib.qmll_fchl19_rep_size.argtypes = [ctypes.POINTER(_CFchl)]
+    lib.qmll_fchl19_rep_size.restype = i32
     lib.qmll_pack_lower.argtypes = [vp, i32, vp, vp]
     lib.qmll_pack_lower.restype = ctypes.c_int
     lib.qmll_unpack_lower.argtypes = [vp, i32, vp, vp]
@@ -296,6 +309,64 @@ def qmll_project(rho, elem, U, mol_off=None, grad_in=None, grad_in_off=None, gra
                                        _dev(gout, torch.float32, "grad_out"), _dev(grad_out_off, torch.int64, "grad_out_off"),
                                        _stream()))
     return x, gout
+
+
+@dataclass
+class Fchl19Params:
+    """qmll_fchl19_params (Table I; defaults = column E + F)."""
+    n_elem: int = 5
+    n2: int = 24
+    n3: int = 20
+    eta2: float = 0.32
+    eta3: float = 2.7
+    two_body_decay: float = 1.8
+    three_body_decay: float = 0.57
+    three_body_weight: float = 13.4
+    zeta: float = 3.141592653589793
+    r_cut: float = 6.0
+
+    def c(self) -> _CFchl:
+        return _CFchl(self.n_elem, self.n2, self.n3, self.eta2, self.eta3, self.two_body_decay, self.three_body_decay,
+                      self.three_body_weight, self.zeta, self.r_cut)
+
+    @property
+    def rep(self) -> int:
+        cp = self.c()
+        return int(load_library().qmll_fchl19_rep_size(ctypes.byref(cp)))
+
+
+def qmll_fchl19(fp: Fchl19Params, r, elem, nbr_idx, nbr_shift=None, jacobian: bool = False, want_rho: bool = True):
+    """(rho [n_atoms, rep], jac_idx [n_atoms, K + 1] | None, jac_val [n_atoms, K + 1, rep, 3] | None, info int32[1]):
+    include/qmll.h qmll_fchl19 (eq. 23-33).  (jac_idx, jac_val) is a NEIGHBOR-layout gradient of length rep."""
+    n_atoms, K = int(nbr_idx.shape[0]), int(nbr_idx.shape[1])
+    rep = fp.rep
+    if rep < 0:
+        raise QmllError(-1, "qmll_fchl19_params invalid or outside the supported range (include/qmll.h)")
+    dev = r.device
+    rho = torch.empty((n_atoms, rep), dtype=torch.float32, device=dev) if want_rho else None
+    jac_idx = torch.empty((n_atoms, K + 1), dtype=torch.int32, device=dev) if jacobian else None
+    jac_val = torch.empty((n_atoms, K + 1, rep, 3), dtype=torch.float32, device=dev) if jacobian else None
+    info = torch.zeros((1,), dtype=torch.int32, device=dev)
+    cp = fp.c()
+    _check(load_library().qmll_fchl19(ctypes.byref(cp), _dev(r, torch.float32, "r"), _dev(elem, torch.int32, "elem"),
+                                      n_atoms, _dev(nbr_idx, torch.int32, "nbr_idx"),
+                                      _dev(nbr_shift, torch.float32, "nbr_shift"), K, _dev(rho, torch.float32, "rho"),
+                                      _dev(jac_idx, torch.int32, "jac_idx"), _dev(jac_val, torch.float32, "jac_val"),
+                                      _dev(info, torch.int32, "info"), _stream()))
+    return rho, jac_idx, jac_val, info
+
+
+def qmll_project_neighbor(grad_in, elem, U, idx=None, grad_out=None):
+    """[n_atoms, S, rep, 3] -> [n_atoms, S, d, 3] with every atom's own U_e: include/qmll.h qmll_project_neighbor."""
+    n_elem, rep, d = (int(v) for v in U.shape)
+    n_atoms, S = int(grad_in.shape[0]), int(grad_in.shape[1])
+    if grad_out is None:
+        grad_out = torch.empty((n_atoms, S, d, 3), dtype=torch.float32, device=U.device)
+    _check(load_library().qmll_project_neighbor(_dev(grad_in, torch.float32, "grad_in"), _dev(idx, torch.int32, "idx"),
+                                                _dev(elem, torch.int32, "elem"), n_atoms, S, rep, d, n_elem,
+                                                _dev(U, torch.float32, "U"), _dev(grad_out, torch.float32, "grad_out"),
+                                                _stream()))
+    return grad_out
 
 
 def qmll_pack_lower(ZtZ, packed=None):

@@ -127,6 +127,75 @@ project_grad_kernel(const float* __restrict__ gin, const int64_t* __restrict__ i
   }
 }
 
+// NEIGHBOR layout (the Jacobian of qmll_fchl19): block = one atom I; its S blocks [rep][3] are projected to [d][3], ten
+// slots (30 columns, lane = (slot, c)) at a time.  Input chunks are staged with coalesced reads (a slot's [64 k][3] piece
+// is 192 contiguous floats), outputs go through a per-warp shared-memory tile so that every slot's [32 m][3] piece is
+// written as 96 contiguous floats.  Slots whose idx is negative are skipped (zero blocks).
+constexpr int kNbrSlots = 10;
+__global__ void __launch_bounds__(kProjThreads)
+project_nbr_kernel(const float* __restrict__ gin, const int32_t* __restrict__ idx, const int32_t* __restrict__ elem,
+                   int S, int rep, int d, const float* __restrict__ U, float* __restrict__ gout) {
+  __shared__ float tile[kProjK][33];
+  __shared__ float otile[kProjThreads / 32][kProjM][33];
+  __shared__ int live[kNbrSlots];
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const size_t I = blockIdx.x;
+  const float* Ue = U + (size_t)__ldg(elem + I) * rep * d;
+  for (int q0 = 0; q0 < S; q0 += kNbrSlots) {
+    const int nq = S - q0 < kNbrSlots ? S - q0 : kNbrSlots;
+    __syncthreads();
+    if (threadIdx.x < kNbrSlots)
+      live[threadIdx.x] = threadIdx.x < nq && (!idx || __ldg(idx + I * S + q0 + threadIdx.x) >= 0);
+    __syncthreads();
+    bool any = false;
+    for (int q = 0; q < nq; ++q) any |= live[q] != 0;
+    for (int mp = 0; mp < d; mp += (kProjThreads / 32) * kProjM) {
+      const int m0 = mp + warp * kProjM;
+      const int mw = m0 >= d ? 0 : (d - m0 < kProjM ? d - m0 : kProjM);
+      float acc[kProjM];
+#pragma unroll
+      for (int i = 0; i < kProjM; ++i) acc[i] = 0.f;
+      if (any) {
+        for (int k0 = 0; k0 < rep; k0 += kProjK) {
+          const int kc = rep - k0 < kProjK ? rep - k0 : kProjK;
+          __syncthreads();
+          for (int item = threadIdx.x; item < nq * kc * 3; item += kProjThreads) {
+            const int ql = item / (kc * 3), rem = item - ql * (kc * 3);
+            const int k = rem / 3, c = rem - 3 * k;
+            tile[k][ql * 3 + c] = live[ql] ? __ldcs(gin + ((I * S + q0 + ql) * rep + k0) * 3 + rem) : 0.f;
+          }
+          if (threadIdx.x < kc * 2) tile[threadIdx.x >> 1][30 + (threadIdx.x & 1)] = 0.f;
+          __syncthreads();
+          if (mw == kProjM) proj_accumulate(acc, tile, kc, lane, Ue + (size_t)k0 * d + m0, d);
+          else if (mw > 0) {
+            for (int k = 0; k < kc; ++k) {
+              const float av = tile[k][lane];
+              for (int i = 0; i < mw; ++i) acc[i] = fmaf(__ldg(Ue + (size_t)(k0 + k) * d + m0 + i), av, acc[i]);
+            }
+          }
+        }
+      }
+      // transpose through shared memory: slot ql gets [mw][3] contiguous floats at ((I S + q) d + m0) * 3
+#pragma unroll
+      for (int i = 0; i < kProjM; ++i) otile[warp][i][lane] = acc[i];
+      __syncwarp();
+      for (int ql = 0; ql < nq; ++ql) {
+        float* dst = gout + ((I * S + q0 + ql) * (size_t)d + m0) * 3;
+        for (int t = lane; t < mw * 3; t += 32) dst[t] = otile[warp][t / 3][ql * 3 + t % 3];
+      }
+      __syncwarp();
+    }
+  }
+}
+
+int project_neighbor_launch(const float* gin, const int32_t* idx, const int32_t* elem, int64_t n_atoms, int32_t S,
+                            int32_t rep, int32_t d, const float* U, float* gout, cudaStream_t st) {
+  if (n_atoms == 0 || S == 0) return QMLL_OK;
+  project_nbr_kernel<<<(unsigned)n_atoms, kProjThreads, 0, st>>>(gin, idx, elem, S, rep, d, U, gout);
+  QMLL_LAUNCH_CHECK("project_nbr_kernel");
+  return QMLL_OK;
+}
+
 int project_launch(const float* rho, const int32_t* elem, const int32_t* mol_off, int64_t n_atoms, int32_t n_mol,
                    int32_t rep, int32_t d, int32_t n_elem, const float* U, float* x, const float* gin,
                    const int64_t* in_off, float* gout, const int64_t* out_off, cudaStream_t st) {

@@ -253,6 +253,42 @@ int qmll_project(const float* rho, const int32_t* elem, const int32_t* mol_off, 
                         grad_out_off, static_cast<cudaStream_t>(cuda_stream));
 }
 
+int qmll_project_neighbor(const float* grad_in, const int32_t* idx, const int32_t* elem, int64_t n_atoms, int32_t S,
+                          int32_t rep, int32_t d, int32_t n_elem, const float* U, float* grad_out,
+                          void* cuda_stream) {
+  if (n_atoms < 0 || S < 0 || rep <= 0 || d <= 0 || d % 4 != 0 || n_elem < 1 || !U) return QMLL_ERR_INVALID_ARG;
+  if (n_atoms > 0 && S > 0 && (!grad_in || !grad_out || !elem)) return QMLL_ERR_INVALID_ARG;
+  if (n_atoms * (int64_t)S > 0x7fffff00LL) return QMLL_ERR_INVALID_ARG;
+  int rc = check_device();
+  if (rc) return rc;
+  return project_neighbor_launch(grad_in, idx, elem, n_atoms, S, rep, d, U, grad_out,
+                                 static_cast<cudaStream_t>(cuda_stream));
+}
+
+static int check_fchl(const qmll_fchl19_params* fp) {
+  if (!fp) return QMLL_ERR_INVALID_ARG;
+  if (fp->n_elem < 1 || fp->n2 < 1 || fp->n3 < 1) return QMLL_ERR_INVALID_ARG;
+  if (!(fp->eta2 > 0.f) || !(fp->eta3 > 0.f) || !(fp->r_cut > 0.f)) return QMLL_ERR_INVALID_ARG;
+  if (fp->n_elem > 16 || fp->n2 > 32 || fp->n3 > 32) return QMLL_ERR_UNSUPPORTED;
+  return QMLL_OK;
+}
+
+int32_t qmll_fchl19_rep_size(const qmll_fchl19_params* fp) { return check_fchl(fp) ? -1 : fchl19_rep_size(fp); }
+
+int qmll_fchl19(const qmll_fchl19_params* fp, const float* r, const int32_t* elem, int64_t n_atoms,
+                const int32_t* nbr_idx, const float* nbr_shift, int32_t K, float* rho, int32_t* jac_idx,
+                float* jac_val, int32_t* info, void* cuda_stream) {
+  int rc = check_fchl(fp);
+  if (rc) return rc;
+  if (n_atoms < 0 || n_atoms > 0x7fffff00LL || K < 0 || K > 4096 || !info) return QMLL_ERR_INVALID_ARG;
+  if (n_atoms > 0 && ((jac_idx == nullptr) != (jac_val == nullptr) || (!rho && !jac_val))) return QMLL_ERR_INVALID_ARG;
+  if (n_atoms > 0 && (!r || !elem || (K > 0 && !nbr_idx))) return QMLL_ERR_INVALID_ARG;
+  rc = check_device();
+  if (rc) return rc;
+  return fchl19_launch(fp, r, elem, n_atoms, nbr_idx, nbr_shift, K, rho, jac_idx, jac_val, info,
+                       static_cast<cudaStream_t>(cuda_stream));
+}
+
 int qmll_pack_lower(const float* ZtZ, int32_t D, float* packed, void* cuda_stream) {
   if (!ZtZ || !packed || D <= 0 || D > 65535) return QMLL_ERR_INVALID_ARG;
   int rc = check_device();

@@ -113,6 +113,15 @@ int project_launch(const float* rho, const int32_t* elem, const int32_t* mol_off
                    int32_t rep, int32_t d, int32_t n_elem, const float* U, float* x, const float* gin,
                    const int64_t* in_off, float* gout, const int64_t* out_off, cudaStream_t st);
 
+int project_neighbor_launch(const float* gin, const int32_t* idx, const int32_t* elem, int64_t n_atoms, int32_t S,
+                            int32_t rep, int32_t d, const float* U, float* gout, cudaStream_t st);
+
+// ---- FCHL19 representation and Jacobian (fchl19_kernels.cu) --------------------------------------------------
+int fchl19_rep_size(const qmll_fchl19_params* fp);
+int fchl19_launch(const qmll_fchl19_params* fp, const float* r, const int32_t* elem, int64_t n_atoms,
+                  const int32_t* nbr_idx, const float* nbr_shift, int32_t K, float* rho, int32_t* jac_idx,
+                  float* jac_val, int32_t* info, cudaStream_t st);
+
 void syrk_set_timing(bool on);
 int syrk_collect_timing(double* total_ms, int* launches);
 

@@ -292,3 +292,44 @@ def test_project_neighbor_gradient_is_the_per_element_matrix_product():
     for a in range(n_atoms):
         ref = np.einsum("skc,km->smc", gin[a].astype(np.float64), U[elem[a]].astype(np.float64))
         np.testing.assert_allclose(out[a], ref, rtol=1e-12, atol=1e-14)
+
+
+def test_chain_forces_match_finite_differences_of_the_energy():
+    """Whole chain in the oracle: r -> rho (FCHL19) -> x = rho^T U_e -> E = sum_I alpha . z(x_I); the force assembled
+    from the Jacobian (slot 0 = the atom, slot 1 + q = neighbour q), the projected gradient and the SORF backward
+    pass must be -dE/dr.  Coordinates lie on a 2^-10 grid and the step is 2^-6, so every displaced geometry is exact
+    in the fp32 arrays the oracle's interfaces take; the fp32 hand-over of rho limits the agreement to ~1e-5."""
+    from workloads import make_model
+    fp = replace(FP, n_elem=2, n2=6, n3=4, r_cut=4.0)
+    g = molecules_geometry(51, [5], n_elem=2)
+    r0 = (np.round(g.r.astype(np.float64) * 1024) / 1024).astype(np.float32)
+    d, D, T, sigma = 16, 256, 3, 2.5
+    model = make_model(52, d=d, D=D, T=T, sigma=sigma, n_elem=2)
+    rng = np.random.default_rng(53)
+    U = rng.normal(size=(2, fp.rep, d)).astype(np.float32) * 0.5
+    alpha = rng.normal(size=D).astype(np.float32)
+
+    def energy(r):
+        rho = oracle.fchl19(fp, r, g.elem, g.nbr_idx)
+        x = oracle.project(rho.astype(np.float32), g.elem, U)
+        Z = oracle.forward(x.astype(np.float32), g.elem, g.mol_off, d, D, T, sigma, model.signs, model.bias)
+        return float(oracle.energy(Z, alpha)[0])
+
+    rho = oracle.fchl19(fp, r0, g.elem, g.nbr_idx)
+    J = oracle.fchl19_jacobian(fp, r0, g.elem, g.nbr_idx)
+    x = oracle.project(rho.astype(np.float32), g.elem, U).astype(np.float32)
+    dx = oracle.project_neighbor_gradient(J.astype(np.float32), g.elem, U)
+    idx = np.concatenate([np.arange(5, dtype=np.int32)[:, None], g.nbr_idx], axis=1)
+    gx = oracle.backward_g(x, g.elem, d, D, T, sigma, model.signs, model.bias, alpha)
+    F = oracle.forces_neighbor(gx, d, idx, dx.astype(np.float32))
+    h = 2.0 ** -6
+    F_fd = np.zeros_like(F)
+    for a in range(5):
+        for c in range(3):
+            def e(step):
+                r = r0.copy()
+                r[a, c] += np.float32(step)
+                return energy(r)
+            F_fd[a, c] = -(8 * (e(h) - e(-h)) - (e(2 * h) - e(-2 * h))) / (12 * h)
+    assert np.linalg.norm(F) > 0
+    assert np.linalg.norm(F - F_fd) <= 1e-4 * np.linalg.norm(F_fd)

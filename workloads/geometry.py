@@ -58,39 +58,38 @@ def _lattice(seed: int, n_side: int, spacing: float, jitter: float) -> np.ndarra
 
 
 def _neighbours(pos: np.ndarray, groups: np.ndarray, r_list: float, K: Optional[int], box: Optional[float]):
-    """All pairs closer than r_list (same group only when box is None); brute force in blocks.  Returns idx, shift."""
+    """All pairs closer than r_list: same group only (isolated molecules, brute force per group) when box is None, else
+    every periodic image (one per pair since box > 2 r_list; k-d tree with periodic boundaries).  Neighbours of an atom
+    are listed by increasing index j.  Returns idx [n, K] (-1 = padding) and the image shifts [n, K, 3] (or None)."""
     n = pos.shape[0]
     rows = [[] for _ in range(n)]
-    shifts = [[] for _ in range(n)]
-    images = [np.zeros(3)] if box is None else [np.array(v, dtype=np.float64) * box
-                                                 for v in np.ndindex(3, 3, 3)]
-    if box is not None:
-        images = [im - box for im in images]          # offsets -box, 0, +box per axis
-    blk = 1024
-    for lo in range(0, n, blk):
-        p = pos[lo:lo + blk]
-        for im in images:
-            d2 = ((p[:, None, :] - (pos[None, :, :] + im)) ** 2).sum(-1)
-            ii, jj = np.nonzero(d2 < r_list * r_list)
-            for a, b in zip(ii, jj):
-                a_g = lo + a
-                if a_g == b and not im.any():
-                    continue
-                if box is None and groups[a_g] != groups[b]:
-                    continue
-                rows[a_g].append(b)
-                shifts[a_g].append(im)
+    if box is None:
+        for gid in np.unique(groups):
+            members = np.nonzero(groups == gid)[0]
+            p = pos[members]
+            d2 = ((p[:, None, :] - p[None, :, :]) ** 2).sum(-1)
+            for a, row in zip(members, d2):
+                rows[a] = [int(members[b]) for b in np.nonzero(row < r_list * r_list)[0] if members[b] != a]
+    else:
+        from scipy.spatial import cKDTree
+        wrapped = np.mod(pos, box)
+        tree = cKDTree(wrapped, boxsize=box)
+        for a, lst in enumerate(tree.query_ball_point(wrapped, r_list)):
+            rows[a] = sorted(int(b) for b in lst if b != a)
     kmax = max((len(x) for x in rows), default=0)
     K = kmax if K is None else K
     if kmax > K:
         raise ValueError(f"an atom has {kmax} neighbours inside the list radius, more than K = {K}")
     idx = np.full((n, K), -1, dtype=np.int32)
-    sh = np.zeros((n, K, 3), dtype=np.float32)
     for a in range(n):
         idx[a, :len(rows[a])] = rows[a]
-        if rows[a]:
-            sh[a, :len(rows[a])] = np.asarray(shifts[a], dtype=np.float32)
-    return idx, (sh if box is not None else None)
+    if box is None:
+        return idx, None
+    sh = np.zeros((n, K, 3), dtype=np.float32)
+    valid = idx >= 0
+    delta = pos[np.where(valid, idx, 0)] - pos[:, None, :]            # r_j - r_i without images
+    sh[valid] = (-np.round(delta / box) * box)[valid].astype(np.float32)
+    return idx, sh
 
 
 def molecules_geometry(seed: int, counts, n_elem: int = 5, spacing: float = 1.45, jitter: float = 0.25,
