@@ -501,7 +501,59 @@ def other_configs(pk, reps, rows_mode=0):
         del dp, w
         pkg.release_workspaces()
         torch.cuda.empty_cache()
+    out["fchl19_cell"] = fchl19_config(pk, tm)
     return out
+
+
+def fchl19_config(pk, tm):
+    """NEXT row f3: coordinates -> FCHL19 (+ Jacobian) -> per-element projection -> energy + forces on a periodic
+    water-like cell shaped like config 5 (Table V): 25^3 atoms, r_cut 4.8 A (44 neighbours on
+    average, K = 64 slots), Table I parameters (rep = 720), d = 256, D = 32768."""
+    import numpy as np
+    import torch
+    import paper_2206_01580_b200 as pkg
+    from paper_2206_01580_b200 import workload_io
+    from workloads import cell_geometry, make_model, projection_inputs
+    g = cell_geometry(2, 25, r_list=4.8, K=64)
+    fp = pkg.Fchl19Params(r_cut=4.8)
+    t = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
+    r, e, idx, sh, mol_off = t(g.r), t(g.elem), t(g.nbr_idx), t(g.nbr_shift), t(g.mol_off)
+    na, K = g.nbr_idx.shape
+    d, D = 256, 32768
+    model = make_model(20220605, d=d, D=D, T=3, sigma=8.0)
+    params = workload_io.device_params(model, "cuda:0")
+    U = t(projection_inputs(seed=78, counts=[1], rep=fp.rep, d=d).U)
+    alpha = t((np.random.default_rng(5).standard_normal(D) / np.sqrt(D)).astype(np.float32))
+    o = {"n_atoms": na, "K": K, "mean_neighbours": float((g.nbr_idx >= 0).sum(1).mean()), "rep": fp.rep, "d": d, "D": D}
+    o["fchl19_rho_ms"] = tm(lambda: pkg.qmll_fchl19(fp, r, e, idx, sh))
+    rho, jidx, jval, info = pkg.qmll_fchl19(fp, r, e, idx, sh, jacobian=True)
+    assert int(info.item()) == 0
+    holder = {}
+
+    def with_jac():
+        holder["out"] = None
+        holder["out"] = pkg.qmll_fchl19(fp, r, e, idx, sh, jacobian=True)
+    del rho, jidx, jval
+    ms = tm(with_jac)
+    rho, jidx, jval, _ = holder.pop("out")
+    jb = jval.numel() * 4
+    o.update({"fchl19_rho_jacobian_ms": ms, "jacobian_bytes": jb,
+              "jacobian_write_frac_of_hbm": jb / (ms * 1e-3) / 1e9 / pk["hbm_gbs"]})
+    x = torch.empty((na, d), dtype=torch.float32, device="cuda")
+    dx = torch.empty((na, K + 1, d, 3), dtype=torch.float32, device="cuda")
+    o["project_x_ms"] = tm(lambda: pkg.qmll_project(rho, e, U))
+    x, _ = pkg.qmll_project(rho, e, U)
+    o["project_neighbor_ms"] = tm(lambda: pkg.qmll_project_neighbor(jval, e, U, idx=jidx, grad_out=dx))
+    grad = pkg.Grad.make_neighbor(jidx, dx)
+    E = torch.empty((1,), dtype=torch.float32, device="cuda")
+    F = torch.empty((na, 3), dtype=torch.float32, device="cuda")
+    o["predict_ms"] = tm(lambda: pkg.qmll_predict(params, x, e, mol_off, alpha, grad, energies=E, forces=F))
+    tot = o["fchl19_rho_jacobian_ms"] + o["project_x_ms"] + o["project_neighbor_ms"] + o["predict_ms"]
+    o.update({"coordinates_to_forces_ms": tot, "us_per_atom": tot * 1e3 / na})
+    del jval, dx
+    pkg.release_workspaces()
+    torch.cuda.empty_cache()
+    return o
 
 
 def spawn_ranks(args):

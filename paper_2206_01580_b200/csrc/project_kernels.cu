@@ -70,7 +70,9 @@ project_x_kernel(const float* __restrict__ rho, const int32_t* __restrict__ elem
         else if (mw > 0) {
           for (int k = 0; k < kc; ++k) {
             const float av = tile[k][lane];
-            for (int i = 0; i < mw; ++i) acc[i] = fmaf(__ldg(Ue + (size_t)(k0 + k) * d + m0 + i), av, acc[i]);
+#pragma unroll
+            for (int i = 0; i < kProjM; ++i)      // static indices: acc stays in registers
+              if (i < mw) acc[i] = fmaf(__ldg(Ue + (size_t)(k0 + k) * d + m0 + i), av, acc[i]);
           }
         }
       }
@@ -114,7 +116,9 @@ project_grad_kernel(const float* __restrict__ gin, const int64_t* __restrict__ i
         else if (mw > 0) {
           for (int k = 0; k < kc; ++k) {
             const float av = tile[k][lane];
-            for (int i = 0; i < mw; ++i) acc[i] = fmaf(__ldg(Ue + (size_t)(k0 + k) * d + m0 + i), av, acc[i]);
+#pragma unroll
+            for (int i = 0; i < kProjM; ++i)      // static indices: acc stays in registers
+              if (i < mw) acc[i] = fmaf(__ldg(Ue + (size_t)(k0 + k) * d + m0 + i), av, acc[i]);
           }
         }
       }
@@ -131,47 +135,132 @@ project_grad_kernel(const float* __restrict__ gin, const int64_t* __restrict__ i
 // slots (30 columns, lane = (slot, c)) at a time.  Input chunks are staged with coalesced reads (a slot's [64 k][3] piece
 // is 192 contiguous floats), outputs go through a per-warp shared-memory tile so that every slot's [32 m][3] piece is
 // written as 96 contiguous floats.  Slots whose idx is negative are skipped (zero blocks).
+// A Jacobian of FCHL19 is structurally sparse along k: the block of a neighbour of element Z_j is zero outside the
+// two-body bin of Z_j and the pair bins that contain Z_j (n2 + 2 E n3 of E n2 + E (E + 1) n3 rows).  The slots are
+// therefore taken in the order of their neighbour's element (so that the ten slots of a pass share their zero rows) and
+// rows k whose 30 staged values are all zero are skipped with one warp vote (exact: they would add zeros).
 constexpr int kNbrSlots = 10;
+constexpr int kNbrMaxS = 1024;     // slots that are reordered; beyond that the original order is kept
+
+// Rows k of the staged chunk whose 30 values are all zero are skipped: every lane tests rows `lane` and `lane + 32`
+// (conflict-free: row stride 33), two ballots give the 64-bit mask of non-zero rows (the same in every warp), and the
+// non-zero rows are taken two at a time so that the U loads of both are in flight before the first FMA.
+__device__ __forceinline__ void proj_row_fma(float (&acc)[kProjM], const float4 (&u)[kProjM / 4], float a) {
+#pragma unroll
+  for (int q = 0; q < kProjM / 4; ++q) {
+    acc[4 * q + 0] = fmaf(u[q].x, a, acc[4 * q + 0]); acc[4 * q + 1] = fmaf(u[q].y, a, acc[4 * q + 1]);
+    acc[4 * q + 2] = fmaf(u[q].z, a, acc[4 * q + 2]); acc[4 * q + 3] = fmaf(u[q].w, a, acc[4 * q + 3]);
+  }
+}
+__device__ __forceinline__ void proj_accumulate_sparse(float (&acc)[kProjM], const float (*tile)[33], int kc, int lane,
+                                                       const float* __restrict__ Uk, int d) {
+  bool nz0 = false, nz1 = false;
+  if (lane < kc) {
+#pragma unroll 8
+    for (int c = 0; c < 32; ++c) nz0 |= tile[lane][c] != 0.f;
+  }
+  if (lane + 32 < kc) {
+#pragma unroll 8
+    for (int c = 0; c < 32; ++c) nz1 |= tile[lane + 32][c] != 0.f;
+  }
+  unsigned long long mask = (unsigned long long)__ballot_sync(0xffffffffu, nz0) |
+                            ((unsigned long long)__ballot_sync(0xffffffffu, nz1) << 32);
+  while (mask) {
+    const int ka = __ffsll((long long)mask) - 1;
+    mask &= mask - 1;
+    const int kb = mask ? __ffsll((long long)mask) - 1 : -1;
+    if (kb >= 0) mask &= mask - 1;
+    float4 ua[kProjM / 4], ub[kProjM / 4];
+    const float4* pa = reinterpret_cast<const float4*>(Uk + (size_t)ka * d);
+    const float4* pb = reinterpret_cast<const float4*>(Uk + (size_t)(kb >= 0 ? kb : ka) * d);
+#pragma unroll
+    for (int q = 0; q < kProjM / 4; ++q) ua[q] = __ldg(pa + q);
+#pragma unroll
+    for (int q = 0; q < kProjM / 4; ++q) ub[q] = __ldg(pb + q);
+    proj_row_fma(acc, ua, tile[ka][lane]);
+    proj_row_fma(acc, ub, kb >= 0 ? tile[kb][lane] : 0.f);
+  }
+}
+
 __global__ void __launch_bounds__(kProjThreads)
 project_nbr_kernel(const float* __restrict__ gin, const int32_t* __restrict__ idx, const int32_t* __restrict__ elem,
-                   int S, int rep, int d, const float* __restrict__ U, float* __restrict__ gout) {
+                   int S, int rep, int d, int n_elem, const float* __restrict__ U, float* __restrict__ gout) {
   __shared__ float tile[kProjK][33];
   __shared__ float otile[kProjThreads / 32][kProjM][33];
-  __shared__ int live[kNbrSlots];
+  __shared__ short order[kNbrMaxS];      // live slots, grouped by the element of the slot's atom
+  __shared__ int n_live_s;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const size_t I = blockIdx.x;
   const float* Ue = U + (size_t)__ldg(elem + I) * rep * d;
-  for (int q0 = 0; q0 < S; q0 += kNbrSlots) {
-    const int nq = S - q0 < kNbrSlots ? S - q0 : kNbrSlots;
-    __syncthreads();
-    if (threadIdx.x < kNbrSlots)
-      live[threadIdx.x] = threadIdx.x < nq && (!idx || __ldg(idx + I * S + q0 + threadIdx.x) >= 0);
-    __syncthreads();
-    bool any = false;
-    for (int q = 0; q < nq; ++q) any |= live[q] != 0;
+  // dead slots: zero blocks.  live slots: ordered by element (stable), by thread 0 of warp 0 with ballots per element
+  if (warp == 0) {
+    int n_live = 0;
+    const int Sr = S < kNbrMaxS ? S : kNbrMaxS;
+    for (int e = (idx ? 0 : n_elem - 1); e < n_elem; ++e)
+      for (int base = 0; base < Sr; base += 32) {
+        const int q = base + lane;
+        bool take = false;
+        if (q < Sr) {
+          if (!idx) take = true;
+          else {
+            const int j = __ldg(idx + I * S + q);
+            if (j >= 0) {
+              int ej = __ldg(elem + j);
+              ej = ej < 0 ? 0 : (ej >= n_elem ? n_elem - 1 : ej);
+              take = ej == e;
+            }
+          }
+        }
+        const unsigned mask = __ballot_sync(0xffffffffu, take);
+        if (take) order[n_live + __popc(mask & ((1u << lane) - 1u))] = (short)q;
+        n_live += __popc(mask);
+      }
+    if (lane == 0) n_live_s = n_live;
+  }
+  __syncthreads();
+  int n_live = n_live_s;
+  if (idx) {
+    for (int q = warp; q < S; q += kProjThreads / 32) {
+      if (q < kNbrMaxS && __ldg(idx + I * S + q) >= 0) continue;
+      if (q >= kNbrMaxS) continue;
+      float* dst = gout + (I * S + q) * (size_t)d * 3;
+      for (int t = lane; t < d * 3; t += 32) dst[t] = 0.f;
+    }
+  }
+  const int n_total = n_live + (S > kNbrMaxS ? S - kNbrMaxS : 0);       // slots beyond the reorder window: as they are
+  for (int q0 = 0; q0 < n_total; q0 += kNbrSlots) {
+    const int nq = n_total - q0 < kNbrSlots ? n_total - q0 : kNbrSlots;
+    auto slot_of = [&](int ql) { const int t = q0 + ql; return t < n_live ? (int)order[t] : kNbrMaxS + (t - n_live); };
     for (int mp = 0; mp < d; mp += (kProjThreads / 32) * kProjM) {
       const int m0 = mp + warp * kProjM;
       const int mw = m0 >= d ? 0 : (d - m0 < kProjM ? d - m0 : kProjM);
       float acc[kProjM];
 #pragma unroll
       for (int i = 0; i < kProjM; ++i) acc[i] = 0.f;
-      if (any) {
-        for (int k0 = 0; k0 < rep; k0 += kProjK) {
-          const int kc = rep - k0 < kProjK ? rep - k0 : kProjK;
-          __syncthreads();
-          for (int item = threadIdx.x; item < nq * kc * 3; item += kProjThreads) {
-            const int ql = item / (kc * 3), rem = item - ql * (kc * 3);
-            const int k = rem / 3, c = rem - 3 * k;
-            tile[k][ql * 3 + c] = live[ql] ? __ldcs(gin + ((I * S + q0 + ql) * rep + k0) * 3 + rem) : 0.f;
-          }
-          if (threadIdx.x < kc * 2) tile[threadIdx.x >> 1][30 + (threadIdx.x & 1)] = 0.f;
-          __syncthreads();
-          if (mw == kProjM) proj_accumulate(acc, tile, kc, lane, Ue + (size_t)k0 * d + m0, d);
-          else if (mw > 0) {
-            for (int k = 0; k < kc; ++k) {
-              const float av = tile[k][lane];
-              for (int i = 0; i < mw; ++i) acc[i] = fmaf(__ldg(Ue + (size_t)(k0 + k) * d + m0 + i), av, acc[i]);
+      for (int k0 = 0; k0 < rep; k0 += kProjK) {
+        const int kc = rep - k0 < kProjK ? rep - k0 : kProjK;
+        __syncthreads();
+        for (int ql = warp; ql < kNbrSlots + 1; ql += kProjThreads / 32) {   // warp = slot: no runtime division
+          if (ql < nq) {
+            const float* src = gin + ((I * S + slot_of(ql)) * rep + k0) * 3;
+            for (int rem = lane; rem < kc * 3; rem += 32) {
+              const int k = rem / 3;
+              tile[k][ql * 3 + (rem - 3 * k)] = __ldcs(src + rem);
             }
+          } else {                                                            // unused columns read as zeros
+            const int c0 = ql < kNbrSlots ? ql * 3 : 30, c1 = ql < kNbrSlots ? c0 + 3 : 32;
+            for (int k = lane; k < kc; k += 32)
+              for (int c = c0; c < c1; ++c) tile[k][c] = 0.f;
+          }
+        }
+        __syncthreads();
+        if (mw == kProjM) proj_accumulate_sparse(acc, tile, kc, lane, Ue + (size_t)k0 * d + m0, d);
+        else if (mw > 0) {
+          for (int k = 0; k < kc; ++k) {
+            const float av = tile[k][lane];
+#pragma unroll
+            for (int i = 0; i < kProjM; ++i)      // static indices: acc stays in registers
+              if (i < mw) acc[i] = fmaf(__ldg(Ue + (size_t)(k0 + k) * d + m0 + i), av, acc[i]);
           }
         }
       }
@@ -180,7 +269,7 @@ project_nbr_kernel(const float* __restrict__ gin, const int32_t* __restrict__ id
       for (int i = 0; i < kProjM; ++i) otile[warp][i][lane] = acc[i];
       __syncwarp();
       for (int ql = 0; ql < nq; ++ql) {
-        float* dst = gout + ((I * S + q0 + ql) * (size_t)d + m0) * 3;
+        float* dst = gout + ((I * S + slot_of(ql)) * (size_t)d + m0) * 3;
         for (int t = lane; t < mw * 3; t += 32) dst[t] = otile[warp][t / 3][ql * 3 + t % 3];
       }
       __syncwarp();
@@ -189,9 +278,9 @@ project_nbr_kernel(const float* __restrict__ gin, const int32_t* __restrict__ id
 }
 
 int project_neighbor_launch(const float* gin, const int32_t* idx, const int32_t* elem, int64_t n_atoms, int32_t S,
-                            int32_t rep, int32_t d, const float* U, float* gout, cudaStream_t st) {
+                            int32_t rep, int32_t d, int32_t n_elem, const float* U, float* gout, cudaStream_t st) {
   if (n_atoms == 0 || S == 0) return QMLL_OK;
-  project_nbr_kernel<<<(unsigned)n_atoms, kProjThreads, 0, st>>>(gin, idx, elem, S, rep, d, U, gout);
+  project_nbr_kernel<<<(unsigned)n_atoms, kProjThreads, 0, st>>>(gin, idx, elem, S, rep, d, n_elem, U, gout);
   QMLL_LAUNCH_CHECK("project_nbr_kernel");
   return QMLL_OK;
 }

@@ -261,7 +261,7 @@ int qmll_project_neighbor(const float* grad_in, const int32_t* idx, const int32_
   if (n_atoms * (int64_t)S > 0x7fffff00LL) return QMLL_ERR_INVALID_ARG;
   int rc = check_device();
   if (rc) return rc;
-  return project_neighbor_launch(grad_in, idx, elem, n_atoms, S, rep, d, U, grad_out,
+  return project_neighbor_launch(grad_in, idx, elem, n_atoms, S, rep, d, n_elem, U, grad_out,
                                  static_cast<cudaStream_t>(cuda_stream));
 }
 

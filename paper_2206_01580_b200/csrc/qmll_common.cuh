@@ -114,7 +114,7 @@ int project_launch(const float* rho, const int32_t* elem, const int32_t* mol_off
                    const int64_t* in_off, float* gout, const int64_t* out_off, cudaStream_t st);
 
 int project_neighbor_launch(const float* gin, const int32_t* idx, const int32_t* elem, int64_t n_atoms, int32_t S,
-                            int32_t rep, int32_t d, const float* U, float* gout, cudaStream_t st);
+                            int32_t rep, int32_t d, int32_t n_elem, const float* U, float* gout, cudaStream_t st);
 
 // ---- FCHL19 representation and Jacobian (fchl19_kernels.cu) --------------------------------------------------
 int fchl19_rep_size(const qmll_fchl19_params* fp);

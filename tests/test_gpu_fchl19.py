@@ -182,3 +182,34 @@ def test_chain_coordinates_to_forces(q):
     assert rel(x.cpu().numpy(), x_o) <= TOL
     assert rel(E.cpu().numpy(), E_o) <= TOL
     assert rel(F.cpu().numpy(), F_o) <= TOL_J
+
+
+def test_fchl19_fullsize_periodic_cell_15625_atoms(q):
+    """The launch configuration bench.py times (configs.fchl19_cell): 25^3-atom water-like periodic cell, r_cut 4.8,
+    K = 64, Table I parameters.  Sampled atoms against the oracle; properties that hold at any size on all atoms:
+    translation sum rule of the Jacobian, zero blocks exactly where jac_idx is negative, jac_idx itself."""
+    pkg, torch = q
+    fp = replace(FchlParams(), r_cut=4.8)
+    g = cell_geometry(2, 25, r_list=4.8, K=64)
+    rho, jac_idx, jac_val, info = run_gpu(q, fp, g)
+    assert int(info.item()) == 0 and rho.shape == (15625, 720) and jac_val.shape == (15625, 65, 720, 3)
+    rng = np.random.default_rng(17)
+    atoms = np.sort(rng.choice(15625, size=48, replace=False))
+    sub_idx = g.nbr_idx[atoms]
+    # oracle on the sampled atoms only: a reduced problem with the same images (positions of all atoms are needed)
+    ro = np.stack([oracle.fchl19_atom(fp, g.r[i].astype(np.float64),
+                                      g.r[sub_idx[t][sub_idx[t] >= 0]].astype(np.float64) + g.nbr_shift[i][sub_idx[t] >= 0],
+                                      g.elem[sub_idx[t][sub_idx[t] >= 0]]) for t, i in enumerate(atoms)])
+    assert rel(rho[torch_index(q, atoms)].cpu().numpy(), ro) <= TOL
+    J_o = oracle.fchl19_jacobian(fp, g.r, g.elem, g.nbr_idx, g.nbr_shift, atoms=atoms[:12])
+    assert rel(jac_val[torch_index(q, atoms[:12])].cpu().numpy(), J_o) <= TOL_J
+    idx_o, edge = expected_jac_idx(fp, g)
+    got = jac_idx.cpu().numpy()
+    assert np.array_equal(got[~edge], idx_o[~edge])
+    # whole-output properties (device-side reductions; no oracle needed)
+    tot = jac_val.sum(dim=1)                                         # [n, rep, 3]: translation invariance
+    scale = jac_val.abs().amax(dim=(1, 2, 3))                        # per atom
+    assert float((tot.abs().amax(dim=(1, 2)) / scale).max()) < 2e-5
+    dead = jac_idx < 0
+    assert float(jac_val[dead].abs().max()) == 0.0
+    assert bool(torch.isfinite(rho).all()) and bool(torch.isfinite(jac_val).all())
