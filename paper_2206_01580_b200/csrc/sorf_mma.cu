@@ -292,10 +292,15 @@ sorf_rows_mma_kernel(const int32_t* __restrict__ elem, const int32_t* __restrict
       }
     }
   } else if (warp == 1) {
-    // ===================== MMA issuer (one thread) =====================
-    // The MMAs are short (N <= 64: 32 clocks each), so the issue loop is kept lean: all descriptors are formed once
-    // (the W tiles and the ring stages never move), the tile loop is unrolled.
-    if (lane == 0) {
+    // ===================== MMA issuer =====================
+    // The MMAs are short (N <= 96: 48 clocks each), so the issue loop must cost less than that per MMA.  The WHOLE
+    // warp runs the loop in lock-step and one elected lane issues: every operand of tcgen05.mma / commit then lives in
+    // uniform registers (values read from memory are made provably uniform with a shuffle from lane 0).  Under
+    // `if (lane == 0)` the compiler cannot know that and wraps every MMA in a vote / elect / R2UR loop of ~18
+    // instructions, which capped the issue rate at one MMA per ~90 clocks.
+    {
+      const bool leader = elect_one_sync();
+      const uint32_t tmem_base_u = __shfl_sync(0xffffffffu, tmem_base, 0);
       uint64_t a_desc[C::kMT][C::kKB], b_desc[C::kStages];
 #pragma unroll
       for (int t = 0; t < C::kMT; ++t)
@@ -311,24 +316,25 @@ sorf_rows_mma_kernel(const int32_t* __restrict__ elem, const int32_t* __restrict
         task_decode(task, n_mol, n_grp, &M, &grp);
         const int s0 = grp * C::kSPT;
         const int n_tiles = (n_s - s0 < C::kSPT ? n_s - s0 : C::kSPT) * C::kTPS;
-        const int a0 = __ldg(mol_off + M), n = __ldg(mol_off + M + 1) - a0;
+        const int a0 = __shfl_sync(0xffffffffu, __ldg(mol_off + M), 0);
+        const int n = __shfl_sync(0xffffffffu, __ldg(mol_off + M + 1), 0) - a0;
         const int ncol = 3 * n, npad = (ncol + 15) / 16 * 16;
         for (int c0 = 0; c0 < npad; c0 += C::kNMax) {
           const int nc = npad - c0 < C::kNMax ? npad - c0 : C::kNMax;
           // D fp32, A/B fp16, both K-major, N = nc, M = 128
           const uint32_t idesc = (1u << 4) | ((uint32_t)(nc >> 3) << 17) | ((uint32_t)(kTile >> 4) << 24);
           int e_prev = -1;
-          int e_next = __ldg(elem + a0);
+          int e_next = __shfl_sync(0xffffffffu, __ldg(elem + a0), 0);
           for (int I = 0; I < n; ++I, ++n_t) {
             const int e = e_next;
-            e_next = (I + 1 < n) ? __ldg(elem + a0 + I + 1) : -1;
+            e_next = (I + 1 < n) ? __shfl_sync(0xffffffffu, __ldg(elem + a0 + I + 1), 0) : -1;
             const bool first_of_run = e != e_prev;
             if (first_of_run) { ++n_a; e_prev = e; }
             const bool last_of_run = e_next != e;
             const uint32_t tb = n_t % C::kTBuf, tuse = n_t / C::kTBuf;
             if (tuse > 0) mbar_wait(&t_empty[tb], (tuse - 1) & 1);
             tcgen05_fence_after();
-            const uint32_t tmem_atom = tmem_base + tb * (C::kMT * C::kNMax);
+            const uint32_t tmem_atom = tmem_base_u + tb * (C::kMT * C::kNMax);
 #pragma unroll
             for (int kb = 0; kb < C::kKB; ++kb, ++n_b) {
               const uint32_t st = n_b % C::kStages;
@@ -338,25 +344,29 @@ sorf_rows_mma_kernel(const int32_t* __restrict__ elem, const int32_t* __restrict
               uint64_t b_hi = b_desc[0];
 #pragma unroll
               for (int q = 1; q < C::kStages; ++q) b_hi = (st == (uint32_t)q) ? b_desc[q] : b_hi;
-              // Consecutive MMAs go to DIFFERENT accumulators: an MMA that accumulates into the tile its predecessor
-              // wrote waits for it (~96 clocks measured, three times the 32 clocks an N = 64 MMA takes).
+              if (leader) {
+                // Consecutive MMAs go to DIFFERENT accumulators (an MMA that accumulates into the tile its
+                // predecessor wrote waits for it).
 #pragma unroll
-              for (int kk = 0; kk < kKBlk / 16; ++kk) {
-                const uint64_t adv = (uint64_t)((kk * 32) >> 4);
+                for (int kk = 0; kk < kKBlk / 16; ++kk) {
+                  const uint64_t adv = (uint64_t)((kk * 32) >> 4);
 #pragma unroll
-                for (int t = 0; t < C::kMT; ++t)
-                  if (t < n_tiles)
-                    umma<true>(tmem_atom + t * C::kNMax, a_desc[t][kb] + adv, b_hi + kLoOff + adv, idesc,
-                               (kb > 0 || kk > 0) ? 1u : 0u);   // small term first
+                  for (int t = 0; t < C::kMT; ++t)
+                    if (t < n_tiles)
+                      umma<true>(tmem_atom + t * C::kNMax, a_desc[t][kb] + adv, b_hi + kLoOff + adv, idesc,
+                                 (kb > 0 || kk > 0) ? 1u : 0u);   // small term first
 #pragma unroll
-                for (int t = 0; t < C::kMT; ++t)
-                  if (t < n_tiles) umma<true>(tmem_atom + t * C::kNMax, a_desc[t][kb] + adv, b_hi + adv, idesc, 1u);
+                  for (int t = 0; t < C::kMT; ++t)
+                    if (t < n_tiles) umma<true>(tmem_atom + t * C::kNMax, a_desc[t][kb] + adv, b_hi + adv, idesc, 1u);
+                }
+                tcgen05_commit(&b_empty[st]);
+                // the W tiles of this k-block may be replaced once the run's last MMAs on them have completed
+                if (last_of_run) tcgen05_commit(&a_empty[kb]);
               }
-              tcgen05_commit(&b_empty[st]);
-              // the W tiles of this k-block may be replaced once the run's last MMAs on them have completed
-              if (last_of_run) tcgen05_commit(&a_empty[kb]);
+              __syncwarp();
             }
-            tcgen05_commit(&t_full[tb]);
+            if (leader) tcgen05_commit(&t_full[tb]);
+            __syncwarp();
           }
         }
       }

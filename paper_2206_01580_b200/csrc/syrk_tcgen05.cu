@@ -292,15 +292,20 @@ syrk_tcgen05_kernel(const __grid_constant__ CUtensorMap map_hi, const __grid_con
       }
     }
   } else if (warp == 1) {
-    // ===================== MMA issuer (one thread) =====================
-    if (lane == 0) {
+    // ===================== MMA issuer =====================
+    // The whole warp runs the loop in lock-step and one elected lane issues, so that every operand of tcgen05.mma /
+    // commit lives in uniform registers (under `if (lane == 0)` the compiler wraps each MMA in a vote / elect / R2UR
+    // loop because it cannot prove uniformity).
+    {
+      const bool leader = elect_one_sync();
+      const uint32_t tmem_base_u = __shfl_sync(0xffffffffu, tmem_base, 0);
       uint32_t kbc = 0, item = 0;
       for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
         for (int ch = 0; ch < n_chunks; ++ch, ++item) {
           const uint32_t buf = item & 1, tph = (item >> 1) & 1;
           mbar_wait(&tempty_bar[buf], tph ^ 1);  // epilogue has drained this accumulator
           tcgen05_fence_after();
-          const uint32_t tmem_d = tmem_base + buf * kBN;
+          const uint32_t tmem_d = tmem_base_u + buf * kBN;
           const int kb_end = (ch + 1) * kb_per_chunk < n_kb ? (ch + 1) * kb_per_chunk : n_kb;
           for (int kb = ch * kb_per_chunk; kb < kb_end; ++kb, ++kbc) {
             const uint32_t s = kbc % kStages, ph = (kbc / kStages) & 1;
@@ -311,17 +316,21 @@ syrk_tcgen05_kernel(const __grid_constant__ CUtensorMap map_hi, const __grid_con
             const uint64_t a_lo = make_kmajor_sw128_desc(base + kTileABytes);
             const uint64_t b_hi = make_kmajor_sw128_desc(base + 2 * kTileABytes);
             const uint64_t b_lo = make_kmajor_sw128_desc(base + 2 * kTileABytes + kTileBBytes);
+            if (leader) {
 #pragma unroll
-            for (int kk = 0; kk < M::kBK / M::kUmmaK; ++kk) {
-              const uint64_t adv = (uint64_t)((kk * 32) >> 4);  // +32 bytes per K step, in 16 B units
-              const uint32_t acc0 = (kb > ch * kb_per_chunk || kk > 0) ? 1u : 0u;
-              umma<F16>(tmem_d, a_lo + adv, b_hi + adv, M::kIdesc, acc0);   // small terms first
-              umma<F16>(tmem_d, a_hi + adv, b_lo + adv, M::kIdesc, 1u);
-              umma<F16>(tmem_d, a_hi + adv, b_hi + adv, M::kIdesc, 1u);
+              for (int kk = 0; kk < M::kBK / M::kUmmaK; ++kk) {
+                const uint64_t adv = (uint64_t)((kk * 32) >> 4);  // +32 bytes per K step, in 16 B units
+                const uint32_t acc0 = (kb > ch * kb_per_chunk || kk > 0) ? 1u : 0u;
+                umma<F16>(tmem_d, a_lo + adv, b_hi + adv, M::kIdesc, acc0);   // small terms first
+                umma<F16>(tmem_d, a_hi + adv, b_lo + adv, M::kIdesc, 1u);
+                umma<F16>(tmem_d, a_hi + adv, b_hi + adv, M::kIdesc, 1u);
+              }
+              tcgen05_commit(&empty_bar[s]);  // smem stage reusable once these MMAs have read it
             }
-            tcgen05_commit(&empty_bar[s]);  // smem stage reusable once these MMAs have read it
+            __syncwarp();
           }
-          tcgen05_commit(&tfull_bar[buf]);  // accumulator complete
+          if (leader) tcgen05_commit(&tfull_bar[buf]);  // accumulator complete
+          __syncwarp();
         }
       }
     }
