@@ -196,6 +196,28 @@ int qmll_project_neighbor(const float* grad_in, const int32_t* idx, const int32_
                           int32_t rep, int32_t d, int32_t n_elem, const float* U, float* grad_out,
                           void* cuda_stream);
 
+/* NEXT row f4 (variants): the feature map of steps a1-a3 on the TENSOR CORES.
+ *
+ * qmll_sorf_forward_mma: the same Z as qmll_sorf_forward(grad = NULL).  The chain of every (element, stack) is expanded
+ *   once into its d x d integer matrix (exact in fp16 for d <= 256), atoms are sorted by element, x is split into fp16
+ *   hi + lo, and U = W X runs on tcgen05 with the cos and the per-molecule sum in the epilogue (fp32 reductions into Z:
+ *   the summation order over the atoms of a molecule is not fixed, results agree to fp32 rounding).  d = 128 or 256 and
+ *   n_elem <= 16, else QMLL_ERR_UNSUPPORTED.  Workspace: qmll_featmap_workspace_bytes(d, D, n_elem, n_atoms, 0).
+ *
+ * qmll_rff_forward: the random Fourier feature map with a DENSE matrix (eq. 12-14, 18 L99-121, L150-152; the paper's
+ *   RFF-versus-SORF comparison, Fig. 1):
+ *     Z[M, l] = sum_{I in M} sqrt(2/D) cos( sum_k W[e_I, l, k] x_I[k] + b[e_I, l] )
+ *   W [n_elem, D, d] fp32 (row l = w_l, the 1/sigma of eq. 18 already applied), bias [n_elem, D] fp32; W and x are split
+ *   into fp16 hi + lo (hi*hi + hi*lo + lo*hi, fp32 accumulate: fp32-level accuracy).  d = 128 or 256, D a multiple of
+ *   4, n_elem <= 16.  Workspace: qmll_featmap_workspace_bytes(d, D, n_elem, n_atoms, 1). */
+int qmll_sorf_forward_mma(const qmll_sorf_params* p, const float* x, const int32_t* elem, const int32_t* mol_off,
+                          int64_t n_atoms, int32_t n_mol, float* Z, void* workspace, size_t workspace_bytes,
+                          void* cuda_stream);
+int qmll_rff_forward(const float* W, const float* bias, int32_t d, int32_t D, int32_t n_elem, const float* x,
+                     const int32_t* elem, const int32_t* mol_off, int64_t n_atoms, int32_t n_mol, float* Z,
+                     void* workspace, size_t workspace_bytes, void* cuda_stream);
+size_t qmll_featmap_workspace_bytes(int32_t d, int32_t D, int32_t n_elem, int64_t n_atoms, int32_t rff);
+
 /* Exchange step of data-parallel training: the normal equations are sums over rows, so
  * ranks that own different molecules add their ZtZ / Zty.  ZtZ is symmetric: pack its lower triangle row by row
  * (row i holds i + 1 entries at offset i (i + 1) / 2; D (D + 1) / 2 floats), all-reduce the packed buffer, unpack

@@ -94,6 +94,16 @@ def forward(x, elem, mol_off, d, D, T, sigma, signs, bias) -> np.ndarray:
     return Z
 
 
+def rff_forward(W, bias, x, elem, mol_off) -> np.ndarray:
+    """Z[n_mol, D] of the dense-matrix random Fourier feature map (eq. 12-14, 18): W [n_elem, D, d], bias [n_elem, D]."""
+    W, bias, x, elem, mol_off = _f32(W), _f32(bias), _f32(x), _i32(elem), _i32(mol_off)
+    n_elem, D, d = W.shape
+    n_mol = mol_off.shape[0] - 1
+    Z = np.empty((n_mol, D), dtype=np.float64)
+    _load().qo_rff_forward(_p(W), _p(bias), _I(d), _I(D), _p(x), _p(elem), _p(mol_off), _I(n_mol), _p(Z))
+    return Z
+
+
 def energy(Z, alpha) -> np.ndarray:
     Z = np.ascontiguousarray(Z, dtype=np.float64)
     alpha = _f32(alpha)

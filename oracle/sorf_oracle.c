@@ -417,3 +417,28 @@ void qo_project_gradient(const float* gin, const int64_t* in_off, const int32_t*
     }
   }
 }
+
+/* Random Fourier features with a DENSE matrix (eq. 12-14, eq. 18; the RFF arm of Fig. 1
+ * L274-278), summed over the atoms of a molecule (eq. 15):
+ *   Z[M, l] = sum_{I in M} sqrt(2/D) cos( sum_k W[e_I, l, k] x_I[k] + b[e_I, l] )
+ * W [n_elem, D, d]: row l is w_l with the 1/sigma of eq. 18 already applied; per-element W and b as for SORF (A6).
+ * Pins: the SORF oracle when W is the explicit dense SORF matrix (two code paths), numpy brute force, Monte-Carlo
+ * convergence of z(x).z(y) to exp(-|x-y|^2 / 2 sigma^2) for Gaussian W (eq. 12-13). */
+void qo_rff_forward(const float* W, const float* bias, int d, int D, const float* x, const int32_t* elem,
+                    const int32_t* mol_off, int n_mol, double* Z /* [n_mol, D] */) {
+  const double nrm = sqrt(2.0 / (double)D);
+#pragma omp parallel for schedule(dynamic, 1)
+  for (int M = 0; M < n_mol; ++M) {
+    double* z = Z + (size_t)M * D;
+    for (int l = 0; l < D; ++l) z[l] = 0.0;
+    for (int64_t a = mol_off[M]; a < mol_off[M + 1]; ++a) {
+      const int e = elem[a];
+      for (int l = 0; l < D; ++l) {
+        const float* w = W + ((size_t)e * D + l) * d;
+        double u = 0.0;
+        for (int k = 0; k < d; ++k) u += (double)w[k] * (double)x[a * d + k];
+        z[l] += nrm * cos(u + (double)bias[(size_t)e * D + l]);
+      }
+    }
+  }
+}

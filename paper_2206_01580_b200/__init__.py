@@ -31,7 +31,8 @@ EXPORTS = ("qmll_solve", "qmll_sorf_forward", "qmll_sorf_forward_mode", "qmll_so
            "qmll_normal_equations_workspace", "qmll_normal_equations_min_workspace_mode", "qmll_status_string",
            "qmll_launch_count", "qmll_reset_launch_count", "qmll_time_normal_equations_kernel",
            "qmll_collect_normal_equations_kernel_ms", "qmll_microbench", "qmll_pack_lower", "qmll_unpack_lower", "qmll_project",
-           "qmll_project_neighbor", "qmll_fchl19", "qmll_fchl19_rep_size")
+           "qmll_project_neighbor", "qmll_fchl19", "qmll_fchl19_rep_size", "qmll_sorf_forward_mma", "qmll_rff_forward",
+           "qmll_featmap_workspace_bytes")
 
 
 class _CParams(ctypes.Structure):
@@ -92,6 +93,12 @@ def load_library() -> ctypes.CDLL:
     lib.qmll_fchl19.restype = ctypes.c_int
     lib.qmll_fchl19_rep_size.argtypes = [ctypes.POINTER(_CFchl)]
     lib.qmll_fchl19_rep_size.restype = i32
+    lib.qmll_sorf_forward_mma.argtypes = [pp, vp, vp, vp, i64, i32, vp, vp, sz, vp]
+    lib.qmll_sorf_forward_mma.restype = ctypes.c_int
+    lib.qmll_rff_forward.argtypes = [vp, vp, i32, i32, i32, vp, vp, vp, i64, i32, vp, vp, sz, vp]
+    lib.qmll_rff_forward.restype = ctypes.c_int
+    lib.qmll_featmap_workspace_bytes.argtypes = [i32, i32, i32, i64, i32]
+    lib.qmll_featmap_workspace_bytes.restype = sz
     lib.qmll_pack_lower.argtypes = [vp, i32, vp, vp]
     lib.qmll_pack_lower.restype = ctypes.c_int
     lib.qmll_unpack_lower.argtypes = [vp, i32, vp, vp]
@@ -309,6 +316,35 @@ def qmll_project(rho, elem, U, mol_off=None, grad_in=None, grad_in_off=None, gra
                                        _dev(gout, torch.float32, "grad_out"), _dev(grad_out_off, torch.int64, "grad_out_off"),
                                        _stream()))
     return x, gout
+
+
+def qmll_sorf_forward_mma(p: SorfParams, x, elem, mol_off, Z=None):
+    """Z [n_mol, D] of steps a1-a3 on the tensor cores (expanded W, d = 128 / 256): include/qmll.h."""
+    lib = load_library()
+    xp, ep, mp, n_atoms, n_mol = _problem(x, elem, mol_off)
+    if Z is None:
+        Z = torch.empty((n_mol, p.D), dtype=torch.float32, device=x.device)
+    nbytes = int(lib.qmll_featmap_workspace_bytes(p.d, p.D, p.n_elem, n_atoms, 0))
+    ws = workspace(nbytes, x.device)
+    cp = p.c()
+    _check(lib.qmll_sorf_forward_mma(ctypes.byref(cp), xp, ep, mp, n_atoms, n_mol, _dev(Z, torch.float32, "Z"),
+                                     ctypes.c_void_p(ws.data_ptr()), ws.numel(), _stream()))
+    return Z
+
+
+def qmll_rff_forward(W, bias, x, elem, mol_off, Z=None):
+    """Z [n_mol, D] of the dense-matrix random Fourier feature map (eq. 12-14, 18): W [n_elem, D, d], bias [n_elem, D]."""
+    lib = load_library()
+    n_elem, D, d = (int(v) for v in W.shape)
+    xp, ep, mp, n_atoms, n_mol = _problem(x, elem, mol_off)
+    if Z is None:
+        Z = torch.empty((n_mol, D), dtype=torch.float32, device=x.device)
+    nbytes = int(lib.qmll_featmap_workspace_bytes(d, D, n_elem, n_atoms, 1))
+    ws = workspace(nbytes, x.device)
+    _check(lib.qmll_rff_forward(_dev(W, torch.float32, "W"), _dev(bias, torch.float32, "bias"), d, D, n_elem, xp, ep, mp,
+                                n_atoms, n_mol, _dev(Z, torch.float32, "Z"), ctypes.c_void_p(ws.data_ptr()), ws.numel(),
+                                _stream()))
+    return Z
 
 
 @dataclass

@@ -204,6 +204,55 @@ int qmll_sorf_forward(const qmll_sorf_params* p, const float* x, const int32_t* 
                                 QMLL_ROWS_AUTO, cuda_stream);
 }
 
+size_t qmll_featmap_workspace_bytes(int32_t d, int32_t D, int32_t n_elem, int64_t n_atoms, int32_t rff) {
+  if (d <= 0 || D <= 0 || n_elem <= 0 || n_atoms < 0) return 0;
+  qmll_sorf_params q{d, D, 3, n_elem, 1.f, nullptr, nullptr};
+  return featmap_mma_scratch_bytes(d, n_elem, n_atoms) + featmap_mma_w_bytes(d, D, n_elem, rff != 0) +
+         (rff ? 0 : sorf_tables_bytes(&q, false)) + 1024;
+}
+
+int qmll_sorf_forward_mma(const qmll_sorf_params* p, const float* x, const int32_t* elem, const int32_t* mol_off,
+                          int64_t n_atoms, int32_t n_mol, float* Z, void* workspace, size_t workspace_bytes,
+                          void* cuda_stream) {
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  int rc = check_params(p);
+  if (rc) return rc;
+  rc = check_problem(x, elem, mol_off, n_atoms, n_mol);
+  if (rc) return rc;
+  if (!Z) return QMLL_ERR_INVALID_ARG;
+  if (!featmap_mma_supported(p->d, p->n_elem)) return QMLL_ERR_UNSUPPORTED;
+  rc = check_device();
+  if (rc) return rc;
+  rc = check_ws(workspace, workspace_bytes, qmll_featmap_workspace_bytes(p->d, p->D, p->n_elem, n_atoms, 0));
+  if (rc) return rc;
+  Carver ws(workspace, workspace_bytes);
+  SorfTables t;
+  rc = sorf_prepare_tables(p, nullptr, ws, &t, st);
+  if (rc) return rc;
+  void* W16 = ws.take<uint8_t>(sorf_mma_w_bytes(p));
+  if (!ws.fits()) return QMLL_ERR_WORKSPACE;
+  rc = sorf_mma_build_w(p, t, W16, st);
+  if (rc) return rc;
+  SorfProblem pr{p, x, elem, mol_off, n_atoms, n_mol};
+  return featmap_sorf_forward_mma(pr, W16, Z, ws, st);
+}
+
+int qmll_rff_forward(const float* W, const float* bias, int32_t d, int32_t D, int32_t n_elem, const float* x,
+                     const int32_t* elem, const int32_t* mol_off, int64_t n_atoms, int32_t n_mol, float* Z,
+                     void* workspace, size_t workspace_bytes, void* cuda_stream) {
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  if (!W || !bias || !Z || d <= 0 || D <= 0 || D % 4 != 0 || n_elem < 1) return QMLL_ERR_INVALID_ARG;
+  int rc = check_problem(x, elem, mol_off, n_atoms, n_mol);
+  if (rc) return rc;
+  if (!featmap_mma_supported(d, n_elem)) return QMLL_ERR_UNSUPPORTED;
+  rc = check_device();
+  if (rc) return rc;
+  rc = check_ws(workspace, workspace_bytes, qmll_featmap_workspace_bytes(d, D, n_elem, n_atoms, 1));
+  if (rc) return rc;
+  Carver ws(workspace, workspace_bytes);
+  return featmap_rff_forward(W, bias, d, D, n_elem, x, elem, mol_off, n_atoms, n_mol, Z, ws, st);
+}
+
 int qmll_sorf_backward_forces(const qmll_sorf_params* p, const float* x, const int32_t* elem,
                               const int32_t* mol_off, int64_t n_atoms, int32_t n_mol, const float* alpha,
                               const qmll_grad* grad, float* forces, void* workspace, size_t workspace_bytes,

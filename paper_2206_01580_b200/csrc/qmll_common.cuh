@@ -86,6 +86,16 @@ size_t sorf_mma_x_bytes(const qmll_sorf_params* p, int64_t n_atoms, int64_t dens
 int sorf_force_rows_dense_mma(const SorfProblem& pr, const SorfTables& t, const float* zs, const qmll_grad* grad,
                               void* W16, void* Xh, void* Xl, long long* xoff, float* inv_scale, float* G,
                               cudaStream_t st);
+int sorf_mma_build_w(const qmll_sorf_params* p, const SorfTables& t, void* W16, cudaStream_t st);
+
+// ---- feature map on the tensor cores (featmap_mma.cu): SORF with expanded W, dense-W RFF ----------------------------
+bool featmap_mma_supported(int d, int n_elem);
+size_t featmap_mma_scratch_bytes(int d, int n_elem, int64_t n_atoms);
+size_t featmap_mma_w_bytes(int d, int D, int n_elem, bool rff);
+int featmap_sorf_forward_mma(const SorfProblem& pr, const void* W16, float* Z, Carver& ws, cudaStream_t st);
+int featmap_rff_forward(const float* W, const float* bias, int d, int D, int n_elem, const float* x, const int32_t* elem,
+                        const int32_t* mol_off, int64_t n_atoms, int32_t n_mol, float* Z, Carver& ws, cudaStream_t st);
+
 int sorf_launch_force_rows_neighbor(const SorfProblem& pr, const SorfTables& t, const float* zs,
                                     const int32_t* nbr_idx, const float* nbr_val, int K, float* G,
                                     cudaStream_t st);

@@ -24,16 +24,6 @@
 
 namespace qmll {
 
-constexpr int kTile = 128;         // MMA M: output features per tile (TMEM lanes)
-constexpr int kKBlk = 64;          // fp16 elements per 128-byte swizzle span (one k-block)
-constexpr uint32_t kTileBytes = kTile * 128;   // one A tile (128 outputs x 64 inputs): 16 KB
-
-// 16-byte chunk `ch` of row `row` inside a [rows][64 halves] k-block tile, SWIZZLE_128B pattern (what TMA would
-// write and what the K-major UMMA descriptor expects): chunk index XOR (row mod 8).
-__host__ __device__ inline size_t swz_half_index(size_t row, int jj) {
-  const int ch = jj >> 3;
-  return row * 64 + (size_t)(((ch ^ (int)(row & 7)) << 3) | (jj & 7));
-}
 
 // ---------------------------------------------------------------------------------------------------
 // 1. W table.  Warp = (element e, stack group sg, input index j); lanes = stacks (as everywhere).  The unit vector
@@ -472,6 +462,27 @@ sorf_rows_mma_kernel(const int32_t* __restrict__ elem, const int32_t* __restrict
 // ---------------------------------------------------------------------------------------------------
 // Host side
 // ---------------------------------------------------------------------------------------------------
+int sorf_mma_build_w(const qmll_sorf_params* p, const SorfTables& t, void* W16, cudaStream_t st) {
+  const int n_s = p->D / p->d;
+  if (p->d == 128) {
+    using S = Shape<shape_E(128), shape_P(128)>;
+    const int n_sg = (n_s + S::SPW - 1) / S::SPW;
+    const long long w_tasks = (long long)p->n_elem * n_sg * p->d;
+    build_w_kernel<S><<<(unsigned)((w_tasks + 3) / 4), kFwdThreads, 0, st>>>(t.sign_bits, p->n_elem, n_s, n_sg,
+                                                                            p->n_transform, (__half*)W16);
+  } else if (p->d == 256) {
+    using S = Shape<shape_E(256), shape_P(256)>;
+    const int n_sg = (n_s + S::SPW - 1) / S::SPW;
+    const long long w_tasks = (long long)p->n_elem * n_sg * p->d;
+    build_w_kernel<S><<<(unsigned)((w_tasks + 3) / 4), kFwdThreads, 0, st>>>(t.sign_bits, p->n_elem, n_s, n_sg,
+                                                                            p->n_transform, (__half*)W16);
+  } else {
+    return QMLL_ERR_UNSUPPORTED;
+  }
+  QMLL_LAUNCH_CHECK("build_w_kernel");
+  return QMLL_OK;
+}
+
 bool sorf_mma_supported(const qmll_sorf_params* p) {
   return (p->d == 128 || p->d == 256) && p->n_transform >= 1 && p->n_transform <= 3;
 }

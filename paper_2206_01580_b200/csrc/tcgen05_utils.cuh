@@ -9,6 +9,19 @@
 
 namespace qmll {
 
+// Operand tiles of the fp16 tcgen05 kernels (force rows, feature map): [128 rows][64 halves] = one 128-byte swizzle span
+// per row, K-major.
+constexpr int kTile = 128;         // MMA M: output features per tile (TMEM lanes)
+constexpr int kKBlk = 64;          // fp16 elements per 128-byte swizzle span (one k-block)
+constexpr uint32_t kTileBytes = kTile * 128;   // one A tile (128 outputs x 64 inputs): 16 KB
+
+// 16-byte chunk `ch` of row `row` inside a [rows][64 halves] k-block tile, SWIZZLE_128B pattern (what TMA would
+// write and what the K-major UMMA descriptor expects): chunk index XOR (row mod 8).
+__host__ __device__ inline size_t swz_half_index(size_t row, int jj) {
+  const int ch = jj >> 3;
+  return row * 64 + (size_t)(((ch ^ (int)(row & 7)) << 3) | (jj & 7));
+}
+
 __device__ __forceinline__ void tcgen05_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
 __device__ __forceinline__ void tcgen05_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
 __device__ __forceinline__ void tcgen05_commit(uint64_t* bar) {

@@ -413,3 +413,40 @@ def test_project_gradient_is_the_jacobian_of_the_projected_descriptor():
     ref = np.einsum("ikjc,ikm->imjc", drho.astype(np.float32).astype(np.float64),
                     pi.U[pi.elem].astype(np.float64))
     assert np.allclose(gout, ref, atol=1e-10)
+
+
+# ----------------------------------------------------------------------------- dense-matrix RFF (variant f4)
+def test_rff_forward_equals_sorf_forward_for_the_dense_sorf_matrix():
+    """The SORF map IS a random-feature map with a particular W (eq. 20 vs eq. 14/18): feeding the explicit D x d
+    matrix of every element to the RFF oracle must reproduce the SORF oracle (two code paths, independent W)."""
+    w = tiny_workload(seed=5, d=16, D=64, T=3, sigma=1.5, counts=[3, 1, 4, 2], n_elem=3, grad=None)
+    m = w.model
+    W = np.stack([dense_W(m, e) for e in range(m.n_elem)]).astype(np.float32)      # entries c * integer: exact in fp32?
+    Zs = oracle.forward_w(w)
+    Zr = oracle.rff_forward(W, m.bias, w.x, w.elem, w.mol_off)
+    assert np.allclose(Zr, Zs, rtol=0, atol=2e-6)      # fp32 rounding of c * integer entries of W
+
+
+def test_rff_forward_brute_force_and_gaussian_kernel():
+    rng = np.random.default_rng(8)
+    n_elem, D, d = 2, 96, 8
+    W = rng.standard_normal((n_elem, D, d)).astype(np.float32)
+    b = rng.uniform(0, 2 * np.pi, size=(n_elem, D)).astype(np.float32)
+    x = rng.standard_normal((7, d)).astype(np.float32)
+    elem = np.array([0, 1, 1, 0, 0, 1, 0], dtype=np.int32)
+    mol_off = np.array([0, 3, 3, 7], dtype=np.int32)          # an empty molecule in the middle
+    Z = oracle.rff_forward(W, b, x, elem, mol_off)
+    z = np.sqrt(2.0 / D) * np.cos(np.einsum("alk,ak->al", W[elem].astype(np.float64), x.astype(np.float64)) + b[elem])
+    ref = np.stack([z[0:3].sum(0), np.zeros(D), z[3:7].sum(0)])
+    assert np.allclose(Z, ref, rtol=1e-13, atol=1e-14)
+    # eq. 12-13: E[z(x).z(y)] = exp(-|x - y|^2 / 2 sigma^2) for w ~ N(0, I / sigma^2), b ~ U[0, 2 pi]
+    d, D, sigma = 16, 65536, 1.7
+    Wg = (rng.standard_normal((1, D, d)) / sigma).astype(np.float32)
+    bg = rng.uniform(0, 2 * np.pi, size=(1, D)).astype(np.float32)
+    xa = rng.standard_normal(d)
+    for delta in (0.5, 1.0, 2.0):
+        dirn = rng.standard_normal(d); dirn /= np.linalg.norm(dirn)
+        xy = np.stack([xa, xa + delta * sigma * dirn]).astype(np.float32)
+        Zg = oracle.rff_forward(Wg, bg, xy, [0, 0], [0, 1, 2])
+        k = np.exp(-np.sum((xy[0].astype(np.float64) - xy[1]) ** 2) / (2 * sigma ** 2))
+        assert abs(Zg[0] @ Zg[1] - k) < 0.015
