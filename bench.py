@@ -60,7 +60,8 @@ def peaks():
         with open(path) as f:
             p = json.load(f)
         out.update({"fadd_per_s": p["alu"]["0"]["per_s"], "fadd_source": "measured (profiles/peaks_r2.json, FADD loop on all SMs)",
-                    "tf32_burst": p["tensor"]["tf32_tflops_burst"], "tf32_sustained": p["tensor"]["tf32_tflops_sustained"]})
+                    "tf32_burst": p["tensor"]["tf32_tflops_burst"], "tf32_sustained": p["tensor"]["tf32_tflops_sustained"],
+                    "mufu_per_s": p["alu"]["9"]["per_s"]})
     return out
 
 
@@ -472,6 +473,18 @@ def other_configs(pk, reps, rows_mode=0):
                 t = tm(lambda: pkg.qmll_sorf_forward(p, dp.x, dp.elem, dp.mol_off, Z=A))
             o.update({"forward_ms": t, "forward_molecules_per_s": nm / (t * 1e-3),
                       "forward_alu_frac": (fwd_ops + fr_ops) / (t * 1e-3) / fadd})
+            if not train:
+                # row f4 variants: the same Z on the tensor cores (expanded W) and the dense-matrix RFF map of equal size
+                Zm = torch.empty((nm, D), dtype=torch.float32, device="cuda")
+                t = tm(lambda: pkg.qmll_sorf_forward_mma(p, dp.x, dp.elem, dp.mol_off, Z=Zm))
+                cos_s = na * D / (t * 1e-3)
+                o.update({"forward_mma_ms": t, "forward_mma_molecules_per_s": nm / (t * 1e-3),
+                          "forward_mma_useful_f16_tflops": 2.0 * 2.0 * m.d * D * na / (t * 1e-3) / 1e12,
+                          "forward_mma_cos_frac_of_mufu_peak": cos_s / pk.get("mufu_per_s", 4.3e12)})
+                Wr = torch.randn((m.n_elem, D, m.d), dtype=torch.float32, device="cuda") / m.sigma
+                t = tm(lambda: pkg.qmll_rff_forward(Wr, p.bias, dp.x, dp.elem, dp.mol_off, Z=Zm))
+                o.update({"rff_forward_ms": t, "rff_useful_f16_tflops": 3.0 * 2.0 * m.d * D * na / (t * 1e-3) / 1e12})
+                del Zm, Wr
             ZtZ = torch.empty((D, D), dtype=torch.float32, device="cuda")
             Zty = torch.empty((D,), dtype=torch.float32, device="cuda")
             pkg.time_normal_equations_kernel(True)

@@ -28,12 +28,13 @@ int device_sm_count();   // sorf_dispatch.cu
 
 constexpr int kFmMaxElem = 16;
 constexpr int kFmSortThreads = 1024;
+constexpr int kFmGrpBlks = 8;          // 1024-atom blocks per sort group (8192 atoms: their Z rows stay in L2)
 constexpr int kFmChunkTiles = 16;      // atom tiles per task: the W tiles are loaded once per (task, element run)
 
 __host__ __device__ constexpr int fm_nt(int d) { return d <= 128 ? 64 : 96; }   // atoms per tile (MMA N)
 
 // ---------------------------------------------------------------------------------------------------
-// 1. Sort by element.  blk_cnt / blk_off [n_blk][E]; e_tile0[E + 1] first tile of every element (e_tile0[E] = tiles).
+// 1. Sort by (atom group, element).  blk_cnt / blk_off [n_blk][E]; key_tile0[n_keys + 1] first tile of every key.
 // ---------------------------------------------------------------------------------------------------
 static __global__ void __launch_bounds__(kFmSortThreads)
 fm_block_count_kernel(const int32_t* __restrict__ elem, long long n_atoms, int E, int* __restrict__ blk_cnt) {
@@ -50,32 +51,47 @@ fm_block_count_kernel(const int32_t* __restrict__ elem, long long n_atoms, int E
   if (threadIdx.x < E) blk_cnt[(size_t)blockIdx.x * E + threadIdx.x] = cnt[threadIdx.x];
 }
 
-static __global__ void __launch_bounds__(32)
-fm_scan_kernel(const int* __restrict__ blk_cnt, int n_blk, int E, int nt, int* __restrict__ blk_off,
-               int* __restrict__ e_tile0) {
-  __shared__ int total[kFmMaxElem];
-  const int e = threadIdx.x;
-  if (e < E) {
-    int run = 0;
-    for (int b = 0; b < n_blk; ++b) {
-      const int t = blk_cnt[(size_t)b * E + e];
-      blk_off[(size_t)b * E + e] = run;
-      run += t;
-    }
-    total[e] = run;
+// Sort key = (group of kFmGrpBlks consecutive 1024-atom blocks, element): atoms are sorted by element only INSIDE a
+// group (8192 atoms), so that all the reductions into the Z rows of a group's molecules happen close in time and stay in
+// L2 (a global sort by element turned every reduction into a DRAM read-modify-write: 45 GB of traffic on config 3).
+static __global__ void fm_group_scan_kernel(const int* __restrict__ blk_cnt, int n_blk, int n_grp, int E,
+                                            int* __restrict__ blk_off, int* __restrict__ key_cnt) {
+  const int k = blockIdx.x * blockDim.x + threadIdx.x;       // key = g * E + e
+  if (k >= n_grp * E) return;
+  const int g = k / E, e = k % E;
+  int run = 0;
+  for (int b = g * kFmGrpBlks; b < (g + 1) * kFmGrpBlks && b < n_blk; ++b) {
+    const int t = blk_cnt[(size_t)b * E + e];
+    blk_off[(size_t)b * E + e] = run;
+    run += t;
   }
-  __syncwarp();
-  if (e == 0) {
-    int t0 = 0;
-    for (int q = 0; q < E; ++q) { e_tile0[q] = t0; t0 += (total[q] + nt - 1) / nt; }
-    e_tile0[E] = t0;
-  }
+  key_cnt[k] = run;
 }
 
-// col_atom / col_mol [tiles * nt] (pre-set to -1); tile_elem [tiles_max] (-1 beyond the last tile)
+// key_tile0[n_keys + 1]: first tile of every key (one warp, chunks of 32 keys, shuffle scan)
+static __global__ void __launch_bounds__(32)
+fm_tile_scan_kernel(const int* __restrict__ key_cnt, int n_keys, int nt, int* __restrict__ key_tile0) {
+  const int lane = threadIdx.x;
+  int carry = 0;
+  for (int base = 0; base < n_keys; base += 32) {
+    const int k = base + lane;
+    const int tiles = k < n_keys ? (key_cnt[k] + nt - 1) / nt : 0;
+    int incl = tiles;
+#pragma unroll
+    for (int off = 1; off < 32; off <<= 1) {
+      const int t = __shfl_up_sync(0xffffffffu, incl, off);
+      if (lane >= off) incl += t;
+    }
+    if (k < n_keys) key_tile0[k] = carry + incl - tiles;
+    carry += __shfl_sync(0xffffffffu, incl, 31);
+  }
+  if (lane == 0) key_tile0[n_keys] = carry;
+}
+
+// col_atom / col_mol [tiles * nt] (pre-set to -1)
 static __global__ void __launch_bounds__(kFmSortThreads)
 fm_place_kernel(const int32_t* __restrict__ elem, const int32_t* __restrict__ mol_off, long long n_atoms, int n_mol,
-                int E, int nt, const int* __restrict__ blk_off, const int* __restrict__ e_tile0,
+                int E, int nt, const int* __restrict__ blk_off, const int* __restrict__ key_tile0,
                 int* __restrict__ col_atom, int* __restrict__ col_mol) {
   __shared__ int wcnt[kFmSortThreads / 32][kFmMaxElem];
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -97,32 +113,67 @@ fm_place_kernel(const int32_t* __restrict__ elem, const int32_t* __restrict__ mo
   }
   __syncthreads();
   if (e >= 0) {
-    const size_t pos = (size_t)__ldg(e_tile0 + e) * nt + __ldg(blk_off + (size_t)blockIdx.x * E + e) + wcnt[warp][e] + rank;
+    const int key = (blockIdx.x / kFmGrpBlks) * E + e;
+    const size_t pos = (size_t)__ldg(key_tile0 + key) * nt + __ldg(blk_off + (size_t)blockIdx.x * E + e) + wcnt[warp][e] + rank;
     col_atom[pos] = (int)a;
     col_mol[pos] = owner_molecule(mol_off, n_mol, (int)a);
   }
 }
 
-static __global__ void fm_tile_elem_kernel(const int* __restrict__ e_tile0, int E, int tiles_max, int* __restrict__ tile_elem) {
+// tile_elem [tiles_max]: element of the key that owns the tile (-1 beyond the last tile)
+static __global__ void fm_tile_elem_kernel(const int* __restrict__ key_tile0, int n_keys, int E, int tiles_max,
+                                           int* __restrict__ tile_elem) {
   const int t = blockIdx.x * blockDim.x + threadIdx.x;
   if (t >= tiles_max) return;
   int e = -1;
-  if (t < __ldg(e_tile0 + E))
-    for (int q = 0; q < E; ++q)
-      if (t >= __ldg(e_tile0 + q)) e = q;
+  if (t < __ldg(key_tile0 + n_keys)) {
+    int lo = 0, hi = n_keys;                 // smallest k in [0, n_keys] with key_tile0[k] > t
+    while (lo < hi) {
+      const int mid = (lo + hi) >> 1;
+      if (__ldg(key_tile0 + mid) > t) hi = mid; else lo = mid + 1;
+    }
+    e = (lo - 1) % E;
+  }
   tile_elem[t] = e;
+}
+
+// Runs of columns that belong to the same molecule, per tile: end_mask[tile][4] has bit c set if column c is the last
+// column of its run (the tile's last column always is); run_mol[tile * nt + k] = molecule of the k-th run (-1: padding).
+// The epilogue then needs no per-column comparison: one bit test per column, one load per run.
+static __global__ void __launch_bounds__(128)
+fm_runs_kernel(const int* __restrict__ col_mol, const int* __restrict__ n_tiles_ptr, int nt, int mult,
+               uint32_t* __restrict__ end_mask, int* __restrict__ run_mol) {
+  const int lane = threadIdx.x & 31;
+  const int tile = blockIdx.x * 4 + (threadIdx.x >> 5);
+  if (tile >= __ldg(n_tiles_ptr)) return;
+  const int* cm = col_mol + (size_t)tile * nt;
+  int n_before = 0;
+  for (int w = 0; w < 4; ++w) {
+    const int c = w * 32 + lane;
+    bool end = false;
+    int m = -1;
+    if (c < nt) {
+      m = __ldg(cm + c);
+      end = c == nt - 1 || __ldg(cm + c + 1) != m;
+    }
+    const unsigned mask = __ballot_sync(0xffffffffu, end);
+    // mult = D if every Z offset m * D fits 31 bits (the epilogue then adds it to a 64-bit base), else 1
+    if (end) run_mol[(size_t)tile * nt + n_before + __popc(mask & ((1u << lane) - 1u))] = m < 0 ? -1 : m * mult;
+    if (lane == 0) end_mask[(size_t)tile * 4 + w] = mask;
+    n_before += __popc(mask);
+  }
 }
 
 // ---------------------------------------------------------------------------------------------------
 // 2. X tiles: block = one tile of nt columns.  Xh / Xl [tile][kb][nt][64 halves] swizzled; inv_scale[tile].
 // ---------------------------------------------------------------------------------------------------
 static __global__ void __launch_bounds__(256)
-fm_prep_x_kernel(const float* __restrict__ x, const int* __restrict__ col_atom, const int* __restrict__ e_tile0, int E,
+fm_prep_x_kernel(const float* __restrict__ x, const int* __restrict__ col_atom, const int* __restrict__ n_tiles_ptr,
                  int d, int nt, __half* __restrict__ Xh, __half* __restrict__ Xl, float* __restrict__ inv_scale) {
   __shared__ float red[8];
   __shared__ int atom_s[128];
   const int tile = blockIdx.x;
-  if (tile >= __ldg(e_tile0 + E)) return;
+  if (tile >= __ldg(n_tiles_ptr)) return;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   if (threadIdx.x < nt) atom_s[threadIdx.x] = __ldg(col_atom + (size_t)tile * nt + threadIdx.x);
   __syncthreads();
@@ -239,22 +290,22 @@ struct FmCfg {
   static constexpr int kTBuf = kTBufRaw > 4 ? 4 : kTBufRaw;
   static constexpr uint32_t kABytes = kParts * kG * kKB * kTileBytes;          // 128 KB
   static constexpr uint32_t kStageBytes = 2 * kNT * 128;                       // hi + lo tile of one k-block
-  static constexpr int kEpiWarps = 8;
-  static constexpr int kTPW = kG >= 2 ? kG / 2 : 1;                            // feature tiles per epilogue warp
-  static constexpr int kColSplit = kG >= 2 ? 1 : 2;                            // kG = 1: the two warp groups split the columns
+  static constexpr int kEpiWarps = 16;                                         // 4 groups of 4 TMEM lane quarters
+  static constexpr int kTPW = kG >= 4 ? kG / 4 : 1;                            // feature tiles per epilogue warp
+  static constexpr int kColSplit = kG >= 4 ? 1 : 4 / kG;                       // groups that share a tile split its columns
   static constexpr int kThreads = 64 + 32 * kEpiWarps;
   static constexpr uint32_t kSmem = kABytes + kStages * kStageBytes + 512 + 1024;
   static_assert(kTBuf >= 2, "TMEM double buffering");
-  static_assert((kNT / kColSplit) % 16 == 0, "column pieces of 16");
+  static_assert((kNT / kColSplit) % 8 == 0, "column pieces of 8");
 };
 
 template <int D_, bool kRff>
 __global__ void __launch_bounds__(FmCfg<D_, kRff>::kThreads, 1)
-featmap_mma_kernel(const int* __restrict__ tile_elem, const int* __restrict__ e_tile0, int E,
-                   const int* __restrict__ col_mol, int D, int n_ft, float c, const float* __restrict__ c_elem,
+featmap_mma_kernel(const int* __restrict__ tile_elem, const int* __restrict__ n_tiles_ptr,
+                   const uint32_t* __restrict__ end_mask, const int* __restrict__ run_mol, int D, int n_ft, float c, const float* __restrict__ c_elem,
                    float nrm, const __half* __restrict__ Wh, const __half* __restrict__ Wl,
                    const __half* __restrict__ Xh, const __half* __restrict__ Xl, const float* __restrict__ inv_scale,
-                   const float* __restrict__ bias, int n_chunks, float* __restrict__ Z) {
+                   const float* __restrict__ bias, int n_chunks, int run_stride, float* __restrict__ Z) {
   using C = FmCfg<D_, kRff>;
   extern __shared__ uint8_t smem_raw[];
   uint8_t* smem = reinterpret_cast<uint8_t*>(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
@@ -271,7 +322,7 @@ featmap_mma_kernel(const int* __restrict__ tile_elem, const int* __restrict__ e_
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int n_fg = (n_ft + C::kG - 1) / C::kG;              // feature groups
-  const int n_tiles = __ldg(e_tile0 + E);
+  const int n_tiles = __ldg(n_tiles_ptr);
   const long long n_tasks = (long long)n_chunks * n_fg;
 
   if (threadIdx.x == 0) {
@@ -405,40 +456,37 @@ featmap_mma_kernel(const int* __restrict__ tile_elem, const int* __restrict__ e_
     }
   } else {
     // ===================== epilogue warps: thread = output feature =====================
-    const int quarter = warp & 3;               // TMEM lanes [32 q, 32 q + 32)
-    const int half = (warp - 2) >> 2;
+    // 16 warps = 4 groups x 4 TMEM lane quarters.  A group owns kTPW feature tiles (all columns) or, when there are
+    // fewer tiles than groups, a range of columns of one tile.  Per column: FFMA, cos, FADD and one bit test; per run of
+    // columns of one molecule: one load of the molecule index and one fp32 reduction into Z per owned tile.
+    const int warp_u = __shfl_sync(0xffffffffu, warp, 0);   // provably uniform: the column bit tests become uniform branches
+    const int quarter = warp_u & 3;             // TMEM lanes [32 q, 32 q + 32)
+    const int grp = (warp_u - 2) >> 2;          // 0..3
     const int row = quarter * 32 + lane;
     constexpr int kCols = C::kNT / C::kColSplit;
-    const int col_lo = C::kColSplit == 2 ? half * kCols : 0;
-    const int t_lo = C::kColSplit == 2 ? 0 : half * C::kTPW;
+    const int col_lo = (grp % C::kColSplit) * kCols;
+    const int t_lo = C::kColSplit > 1 ? grp / C::kColSplit : grp * C::kTPW;
     uint32_t n_t = 0;
     for (long long task = blockIdx.x; task < n_tasks; task += gridDim.x) {
       const int fg = (int)(task % n_fg), ch = (int)(task / n_fg);
       const int t_begin = ch * kFmChunkTiles;
       const int t_end = t_begin + kFmChunkTiles < n_tiles ? t_begin + kFmChunkTiles : n_tiles;
-      int feat[C::kTPW];
+      float* zf[C::kTPW];                       // Z + feature (features past D: a column of the last valid feature, never added)
       bool live[C::kTPW];
+      int feat[C::kTPW];
       float acc[C::kTPW], bv[C::kTPW];
 #pragma unroll
       for (int w = 0; w < C::kTPW; ++w) {
         feat[w] = (fg * C::kG + t_lo + w) * kTile + row;
         live[w] = feat[w] < D;
+        zf[w] = Z + (live[w] ? feat[w] : 0);
         acc[w] = 0.f;
         bv[w] = 0.f;
       }
-      int cur_mol = -1, e_prev = -1;
+      int e_prev = -1;
       float ce = c;
-      auto flush = [&]() {
-        if (cur_mol >= 0) {
-#pragma unroll
-          for (int w = 0; w < C::kTPW; ++w)
-            if (live[w]) atomicAdd(Z + (size_t)cur_mol * D + feat[w], nrm * acc[w]);
-        }
-#pragma unroll
-        for (int w = 0; w < C::kTPW; ++w) acc[w] = 0.f;
-      };
       for (int tile = t_begin; tile < t_end; ++tile, ++n_t) {
-        const int e = __ldg(tile_elem + tile);
+        const int e = __shfl_sync(0xffffffffu, __ldg(tile_elem + tile), 0);
         if (e != e_prev) {
 #pragma unroll
           for (int w = 0; w < C::kTPW; ++w) bv[w] = live[w] ? __ldg(bias + (size_t)e * D + feat[w]) : 0.f;
@@ -446,36 +494,63 @@ featmap_mma_kernel(const int* __restrict__ tile_elem, const int* __restrict__ e_
           e_prev = e;
         }
         const float sc = ce * __ldg(inv_scale + tile);
-        const int* cm = col_mol + (size_t)tile * C::kNT + col_lo;
+        // run ends of this tile (uniform: made provably so with a shuffle, so that the bit tests are uniform branches)
+        const uint32_t em0 = __shfl_sync(0xffffffffu, __ldg(end_mask + (size_t)tile * 4 + 0), 0);
+        const uint32_t em1 = __shfl_sync(0xffffffffu, __ldg(end_mask + (size_t)tile * 4 + 1), 0);
+        const uint32_t em2 = __shfl_sync(0xffffffffu, __ldg(end_mask + (size_t)tile * 4 + 2), 0);
+        const unsigned long long em01 = (unsigned long long)em0 | ((unsigned long long)em1 << 32);
+        // index of the run that contains column col_lo = number of run ends before it
+        int run = col_lo >= 64 ? __popcll(em01) + __popc(em2 & ((1u << (col_lo - 64)) - 1u))
+                               : __popcll(em01 & ((1ull << col_lo) - 1ull));
+        const int* rm = run_mol + (size_t)tile * C::kNT;
         const uint32_t tb = n_t % C::kTBuf;
         mbar_wait(&t_full[tb], (n_t / C::kTBuf) & 1);
         tcgen05_fence_after();
+        constexpr int kP = kCols % 16 == 0 ? 16 : 8;     // columns per TMEM load
 #pragma unroll 1
-        for (int r0 = 0; r0 < kCols; r0 += 16) {
-          uint32_t u[C::kTPW][16];
+        for (int r0 = 0; r0 < kCols; r0 += kP) {
+          uint32_t u[C::kTPW][kP];
 #pragma unroll
           for (int w = 0; w < C::kTPW; ++w) {
             const uint32_t taddr = tmem_base + ((uint32_t)(quarter * 32) << 16) + tb * (C::kG * C::kNT) +
                                    (t_lo + w) * C::kNT + col_lo + r0;
-            tmem_ld_32x32b_x16(taddr, u[w]);
+            if constexpr (kP == 16) {
+              tmem_ld_32x32b_x16(taddr, u[w]);
+            } else {
+              tmem_ld_32x32b_x8(taddr, u[w]);
+            }
           }
+          const int c0 = col_lo + r0;
+          const uint32_t true_ends = (c0 >= 64 ? em2 >> (c0 - 64) : (uint32_t)(em01 >> c0)) & ((1u << kP) - 1u);
+          const uint32_t bits = true_ends | (r0 + kP == kCols ? 1u << (kP - 1) : 0u);   // the group's last column closes its run
           tmem_ld_wait();
+          // all cos of the piece first (independent: the MUFU latencies overlap), then the sequential run logic
+          float z[C::kTPW][kP];
 #pragma unroll
-          for (int r = 0; r < 16; ++r) {
-            const int m = __ldg(cm + r0 + r);
-            if (m != cur_mol) { flush(); cur_mol = m; }
-            if (m >= 0) {
+          for (int w = 0; w < C::kTPW; ++w)
 #pragma unroll
-              for (int w = 0; w < C::kTPW; ++w) acc[w] += __cosf(fmaf(sc, __uint_as_float(u[w][r]), bv[w]));
+            for (int r = 0; r < kP; ++r) z[w][r] = __cosf(fmaf(sc, __uint_as_float(u[w][r]), bv[w]));
+#pragma unroll
+          for (int r = 0; r < kP; ++r) {
+#pragma unroll
+            for (int w = 0; w < C::kTPW; ++w) acc[w] += z[w][r];
+            if (bits & (1u << r)) {
+              const int m = __ldg(rm + run);
+              if (m >= 0) {
+#pragma unroll
+                for (int w = 0; w < C::kTPW; ++w)
+                  if (live[w]) atomicAdd(zf[w] + (size_t)(uint32_t)m * (size_t)(uint32_t)run_stride, nrm * acc[w]);
+              }
+#pragma unroll
+              for (int w = 0; w < C::kTPW; ++w) acc[w] = 0.f;
+              run += (true_ends >> r) & 1u;
             }
           }
         }
         tcgen05_fence_before();
         __syncwarp();
         if (lane == 0) mbar_arrive(&t_empty[tb]);
-        if (C::kColSplit == 2) { flush(); cur_mol = -1; }
       }
-      flush();
     }
   }
 
@@ -492,15 +567,21 @@ featmap_mma_kernel(const int* __restrict__ tile_elem, const int* __restrict__ e_
 // ---------------------------------------------------------------------------------------------------
 bool featmap_mma_supported(int d, int n_elem) { return (d == 128 || d == 256) && n_elem >= 1 && n_elem <= kFmMaxElem; }
 
-static size_t fm_tiles_max(int64_t n_atoms, int d, int n_elem) { return (size_t)((n_atoms + fm_nt(d) - 1) / fm_nt(d)) + n_elem; }
+static size_t fm_groups(int64_t n_atoms) {
+  const size_t n_blk = (size_t)((n_atoms + kFmSortThreads - 1) / kFmSortThreads);
+  return (n_blk + kFmGrpBlks - 1) / kFmGrpBlks;
+}
+static size_t fm_tiles_max(int64_t n_atoms, int d, int n_elem) {
+  return (size_t)((n_atoms + fm_nt(d) - 1) / fm_nt(d)) + fm_groups(n_atoms) * n_elem;
+}
 
 // bytes of everything but the W tables
 size_t featmap_mma_scratch_bytes(int d, int n_elem, int64_t n_atoms) {
   const size_t tiles = fm_tiles_max(n_atoms, d, n_elem), cols = tiles * fm_nt(d);
   const size_t n_blk = (size_t)((n_atoms + kFmSortThreads - 1) / kFmSortThreads);
-  return 2 * align_up(cols * (size_t)d * sizeof(__half), 256) + 2 * align_up(cols * sizeof(int), 256) +
-         2 * align_up(tiles * sizeof(int), 256) + 2 * align_up(n_blk * n_elem * sizeof(int) + 4, 256) +
-         align_up((size_t)(n_elem + 1) * sizeof(int), 256) + 16 * 256;
+  return 2 * align_up(cols * (size_t)d * sizeof(__half), 256) + 3 * align_up(cols * sizeof(int), 256) +
+         2 * align_up(tiles * sizeof(int), 256) + align_up(tiles * 16, 256) + 2 * align_up(n_blk * n_elem * sizeof(int) + 4, 256) +
+         2 * align_up((fm_groups(n_atoms) * n_elem + 1) * sizeof(int), 256) + 16 * 256;
 }
 size_t featmap_mma_w_bytes(int d, int D, int n_elem, bool rff) {
   const size_t n_ft = (size_t)(D + kTile - 1) / kTile;
@@ -522,23 +603,33 @@ static int launch_featmap(int n_elem, int D, float c, const float* c_elem, const
   int* col_mol = ws.take<int>(cols);
   int* tile_elem = ws.take<int>(tiles);
   float* inv_scale = ws.take<float>(tiles);
+  uint32_t* end_mask = ws.take<uint32_t>(tiles * 4);
+  int* run_mol = ws.take<int>(cols);
   int* blk_cnt = ws.take<int>((size_t)n_blk * n_elem + 1);
   int* blk_off = ws.take<int>((size_t)n_blk * n_elem + 1);
-  int* e_tile0 = ws.take<int>(n_elem + 1);
+  const int n_grp = (int)fm_groups(n_atoms), n_keys = n_grp * n_elem;
+  int* key_cnt = ws.take<int>((size_t)n_keys + 1);
+  int* key_tile0 = ws.take<int>((size_t)n_keys + 1);
   if (!ws.fits()) return QMLL_ERR_WORKSPACE;
   QMLL_CUDA_TRY(cudaMemsetAsync(Z, 0, (size_t)n_mol * D * sizeof(float), st));
   QMLL_CUDA_TRY(cudaMemsetAsync(col_atom, 0xff, cols * sizeof(int), st));
   QMLL_CUDA_TRY(cudaMemsetAsync(col_mol, 0xff, cols * sizeof(int), st));
   fm_block_count_kernel<<<n_blk, kFmSortThreads, 0, st>>>(elem, n_atoms, n_elem, blk_cnt);
   QMLL_LAUNCH_CHECK("fm_block_count_kernel");
-  fm_scan_kernel<<<1, 32, 0, st>>>(blk_cnt, n_blk, n_elem, nt, blk_off, e_tile0);
-  QMLL_LAUNCH_CHECK("fm_scan_kernel");
-  fm_place_kernel<<<n_blk, kFmSortThreads, 0, st>>>(elem, mol_off, n_atoms, n_mol, n_elem, nt, blk_off, e_tile0, col_atom,
-                                                    col_mol);
+  fm_group_scan_kernel<<<(n_keys + 255) / 256, 256, 0, st>>>(blk_cnt, n_blk, n_grp, n_elem, blk_off, key_cnt);
+  QMLL_LAUNCH_CHECK("fm_group_scan_kernel");
+  fm_tile_scan_kernel<<<1, 32, 0, st>>>(key_cnt, n_keys, nt, key_tile0);
+  QMLL_LAUNCH_CHECK("fm_tile_scan_kernel");
+  fm_place_kernel<<<n_blk, kFmSortThreads, 0, st>>>(elem, mol_off, n_atoms, n_mol, n_elem, nt, blk_off, key_tile0,
+                                                    col_atom, col_mol);
   QMLL_LAUNCH_CHECK("fm_place_kernel");
-  fm_tile_elem_kernel<<<(unsigned)((tiles + 255) / 256), 256, 0, st>>>(e_tile0, n_elem, (int)tiles, tile_elem);
+  fm_tile_elem_kernel<<<(unsigned)((tiles + 255) / 256), 256, 0, st>>>(key_tile0, n_keys, n_elem, (int)tiles, tile_elem);
   QMLL_LAUNCH_CHECK("fm_tile_elem_kernel");
-  fm_prep_x_kernel<<<(unsigned)tiles, 256, 0, st>>>(x, col_atom, e_tile0, n_elem, D_, nt, Xh, Xl, inv_scale);
+  const bool small = (long long)n_mol * D < 0x7fffffffLL;      // every Z offset fits 31 bits: the run table holds m * D
+  fm_runs_kernel<<<(unsigned)((tiles + 3) / 4), 128, 0, st>>>(col_mol, key_tile0 + n_keys, nt, small ? D : 1, end_mask,
+                                                              run_mol);
+  QMLL_LAUNCH_CHECK("fm_runs_kernel");
+  fm_prep_x_kernel<<<(unsigned)tiles, 256, 0, st>>>(x, col_atom, key_tile0 + n_keys, D_, nt, Xh, Xl, inv_scale);
   QMLL_LAUNCH_CHECK("fm_prep_x_kernel");
   auto kern = featmap_mma_kernel<D_, kRff>;
   QMLL_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::kSmem));
@@ -547,8 +638,8 @@ static int launch_featmap(int n_elem, int D, float c, const float* c_elem, const
   const long long n_tasks = (long long)n_chunks * ((n_ft + C::kG - 1) / C::kG);
   const int grid = (int)(n_tasks < device_sm_count() ? n_tasks : device_sm_count());
   const float nrm = (float)sqrt(2.0 / (double)D);
-  kern<<<grid, C::kThreads, C::kSmem, st>>>(tile_elem, e_tile0, n_elem, col_mol, D, n_ft, c, c_elem, nrm, Wh, Wl, Xh, Xl,
-                                            inv_scale, bias, n_chunks, Z);
+  kern<<<grid, C::kThreads, C::kSmem, st>>>(tile_elem, key_tile0 + n_keys, end_mask, run_mol, D, n_ft, c, c_elem, nrm, Wh, Wl, Xh, Xl,
+                                            inv_scale, bias, n_chunks, small ? 1 : D, Z);
   QMLL_LAUNCH_CHECK("featmap_mma_kernel");
   return QMLL_OK;
 }
