@@ -38,6 +38,8 @@ def parse():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-configs", action="store_true", help="skip the per-config block (C2, C3, C5)")
+    ap.add_argument("--only-config", default=None, choices=["c2", "c3", "c5", "fchl19_cell"],
+                    help="run only this entry of the per-config block and print it (used for the ncu captures in profiles/)")
     ap.add_argument("--force-rows", default="auto", choices=["auto", "fwht", "mma"],
                     help="how the force rows are computed (qmll_sorf_forward_mode); the bench line uses auto")
     return ap.parse_args()
@@ -434,7 +436,7 @@ def ours_arm(args):
         dist.destroy_process_group()
 
 
-def other_configs(pk, reps, rows_mode=0):
+def other_configs(pk, reps, rows_mode=0, only=None):
     """Absolute numbers and the binding roofline fraction for the other timed configs (north_star): C2, C3, C5."""
     import torch
     import paper_2206_01580_b200 as pkg
@@ -456,6 +458,8 @@ def other_configs(pk, reps, rows_mode=0):
 
     out = {}
     for name in ("c2", "c3", "c5"):
+        if only is not None and name != only:
+            continue
         w = make_workload(name)
         dp = workload_io.device_problem(w)
         p, m = dp.params, w.model
@@ -514,7 +518,8 @@ def other_configs(pk, reps, rows_mode=0):
         del dp, w
         pkg.release_workspaces()
         torch.cuda.empty_cache()
-    out["fchl19_cell"] = fchl19_config(pk, tm)
+    if only is None or only == "fchl19_cell":
+        out["fchl19_cell"] = fchl19_config(pk, tm)
     return out
 
 
@@ -581,6 +586,8 @@ if __name__ == "__main__":
     a = parse()
     if a.impl == "reference":
         reference_arm(a)
+    elif a.only_config:
+        print(json.dumps({"configs": other_configs(peaks(), max(2, a.steps // 2), only=a.only_config)}))
     elif a.gpus > 1 and "WORLD_SIZE" not in os.environ:
         spawn_ranks(a)
     else:
