@@ -188,6 +188,25 @@ int qmll_fchl19(const qmll_fchl19_params* fp, const float* r, const int32_t* ele
                 const int32_t* nbr_idx, const float* nbr_shift, int32_t K, float* rho, int32_t* jac_idx,
                 float* jac_val, int32_t* info, void* cuda_stream);
 
+/* The backward pass of the same chain WITHOUT a Jacobian (what the paper does for prediction, L268: "for the backwards
+ * pass ... the force components are stored and summed in on-chip memory"):
+ *   coordinates -> qmll_fchl19 -> qmll_project -> qmll_sorf_backward_g -> qmll_project_back -> qmll_fchl19_backward.
+ *
+ * qmll_sorf_backward_g: g[I, m] = dE / dx_I[m] = -c sum_s (W_{e,s}^T (sqrt(2/D) alpha .* sin(u_I + b)))[m]  (step a5 alone,
+ *   [n_atoms, d] fp32 out) and, if energies != NULL, the energies of qmll_predict.  Workspace as QMLL_CALL_PREDICT.
+ * qmll_project_back:    w[I, k] = sum_m U[e_I, k, m] g[I, m] = dE / d rho_I[k]     ([n_atoms, rep] fp32 out).
+ * qmll_fchl19_backward: forces[j, c] = -sum_I sum_k w[I, k] d rho_I[k] / d r_{j,c}  ([n_atoms, 3] fp32, overwritten); the
+ *   sum runs over every atom I and every neighbour image of I (contributions of an image are added to the atom it is an
+ *   image of) plus I itself.  Arguments as qmll_fchl19. */
+int qmll_sorf_backward_g(const qmll_sorf_params* p, const float* x, const int32_t* elem, const int32_t* mol_off,
+                         int64_t n_atoms, int32_t n_mol, const float* alpha, float* energies, float* g,
+                         void* workspace, size_t workspace_bytes, void* cuda_stream);
+int qmll_project_back(const float* g, const int32_t* elem, int64_t n_atoms, int32_t rep, int32_t d, int32_t n_elem,
+                      const float* U, float* w, void* cuda_stream);
+int qmll_fchl19_backward(const qmll_fchl19_params* fp, const float* r, const int32_t* elem, int64_t n_atoms,
+                         const int32_t* nbr_idx, const float* nbr_shift, int32_t K, const float* w, float* forces,
+                         int32_t* info, void* cuda_stream);
+
 /* The per-element projection (qmll_project) of a NEIGHBOR-layout gradient, e.g. the Jacobian of qmll_fchl19:
  *   grad_out[I, q, m, c] = sum_k grad_in[I, q, k, c] U[e_I, k, m]
  *   grad_in [n_atoms, S, rep, 3] fp32, grad_out [n_atoms, S, d, 3] fp32, U [n_elem, rep, d] fp32, d % 4 == 0.

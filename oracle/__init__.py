@@ -263,6 +263,29 @@ def fchl19_atom(fp, centre, img, img_elem, jacobian: bool = False):
     return (rho, jac) if jacobian else rho
 
 
+def project_back(g, elem, U) -> np.ndarray:
+    """w [n_atoms, rep] = U_e g: dE / d rho from g = dE / dx (backward pass of eq. 22)."""
+    g = np.ascontiguousarray(g, dtype=np.float64)
+    elem, U = _i32(elem), _f32(U)
+    n_atoms, d = g.shape
+    rep = U.shape[1]
+    w = np.empty((n_atoms, rep), dtype=np.float64)
+    _load().qo_project_back(_p(g), _p(elem), _L(n_atoms), _I(rep), _I(d), _p(U), _p(w))
+    return w
+
+
+def fchl19_backward(fp, r, elem, nbr_idx, w, nbr_shift=None) -> np.ndarray:
+    """F [n_atoms, 3] = -sum_i w_i . d rho_i / d r: contraction of the oracle's Jacobian with w = dE / d rho."""
+    r, elem, nbr_idx = _f32(r), _i32(elem), _i32(nbr_idx)
+    nbr_shift = None if nbr_shift is None else _f32(nbr_shift)
+    w = np.ascontiguousarray(w, dtype=np.float64)
+    n_atoms, K = nbr_idx.shape
+    F = np.empty((n_atoms, 3), dtype=np.float64)
+    _load().qo_fchl19_backward(_p(r), _p(elem), _L(n_atoms), _p(nbr_idx), _p(nbr_shift), _I(K), _p(w), *_fchl_args(fp),
+                               _p(F))
+    return F
+
+
 def project_neighbor_gradient(gin, elem, U) -> np.ndarray:
     """[n_atoms, S, rep, 3] fp32 -> [n_atoms, S, d, 3] float64 with every atom's own U_e (eq. 21-22)."""
     gin, elem, U = _f32(gin), _i32(elem), _f32(U)

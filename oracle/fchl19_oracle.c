@@ -246,3 +246,37 @@ void qo_fchl19_atom_f64(const double* centre, const double* img /* [nn, 3] */, c
   }
   free(z); free(ze); free(out);
 }
+
+/* Backward pass of the projection x = rho^T U_e (eq. 22): w[at, k] = dE/d rho[at, k] = sum_m U[e_at, k, m] g[at, m]. */
+void qo_project_back(const double* g, const int32_t* elem, int64_t n_atoms, int rep, int d, const float* U, double* w) {
+#pragma omp parallel for schedule(static)
+  for (int64_t at = 0; at < n_atoms; ++at) {
+    const float* Ue = U + (size_t)elem[at] * rep * d;
+    for (int k = 0; k < rep; ++k) {
+      double acc = 0.0;
+      for (int m = 0; m < d; ++m) acc += (double)Ue[(size_t)k * d + m] * g[at * d + m];
+      w[at * rep + k] = acc;
+    }
+  }
+}
+
+/* Backward pass of the representation: F[j, c] = -sum_i sum_k w[i, k] d rho_i[k] / d r_{j,c}, summed over every atom i,
+ * the atom itself (slot 0 of its Jacobian) and its neighbour images (slot 1 + q -> atom nbr_idx[i, q]).  Plain
+ * contraction of the complex-step Jacobian above (the definition), nothing fused. */
+void qo_fchl19_backward(const float* r, const int32_t* elem, int64_t n_atoms, const int32_t* nbr_idx,
+                        const float* nbr_shift, int K, const double* w, int n_elem, int n2, int n3, double eta2,
+                        double eta3, double N2, double N3, double c3, double zeta, double rcut, double* F) {
+  const int rep = qo_fchl19_rep_size(n_elem, n2, n3);
+  for (int64_t t = 0; t < 3 * n_atoms; ++t) F[t] = 0.0;
+  double* jac = malloc(sizeof(double) * (size_t)(K + 1) * rep * 3);
+  for (int64_t i = 0; i < n_atoms; ++i) {
+    qo_fchl19_jacobian(r, elem, nbr_idx, nbr_shift, K, &i, 1, n_elem, n2, n3, eta2, eta3, N2, N3, c3, zeta, rcut, jac);
+    for (int slot = 0; slot <= K; ++slot) {
+      const int64_t j = slot == 0 ? i : nbr_idx[i * K + slot - 1];
+      if (j < 0) continue;
+      for (int k = 0; k < rep; ++k)
+        for (int c = 0; c < 3; ++c) F[3 * j + c] -= w[i * rep + k] * jac[((size_t)slot * rep + k) * 3 + c];
+    }
+  }
+  free(jac);
+}

@@ -32,7 +32,7 @@ EXPORTS = ("qmll_solve", "qmll_sorf_forward", "qmll_sorf_forward_mode", "qmll_so
            "qmll_launch_count", "qmll_reset_launch_count", "qmll_time_normal_equations_kernel",
            "qmll_collect_normal_equations_kernel_ms", "qmll_microbench", "qmll_pack_lower", "qmll_unpack_lower", "qmll_project",
            "qmll_project_neighbor", "qmll_fchl19", "qmll_fchl19_rep_size", "qmll_sorf_forward_mma", "qmll_rff_forward",
-           "qmll_featmap_workspace_bytes")
+           "qmll_featmap_workspace_bytes", "qmll_sorf_backward_g", "qmll_project_back", "qmll_fchl19_backward")
 
 
 class _CParams(ctypes.Structure):
@@ -93,6 +93,12 @@ def load_library() -> ctypes.CDLL:
     lib.qmll_fchl19.restype = ctypes.c_int
     lib.qmll_fchl19_rep_size.argtypes = [ctypes.POINTER(_CFchl)]
     lib.qmll_fchl19_rep_size.restype = i32
+    lib.qmll_sorf_backward_g.argtypes = [pp, vp, vp, vp, i64, i32, vp, vp, vp, vp, sz, vp]
+    lib.qmll_sorf_backward_g.restype = ctypes.c_int
+    lib.qmll_project_back.argtypes = [vp, vp, i64, i32, i32, i32, vp, vp, vp]
+    lib.qmll_project_back.restype = ctypes.c_int
+    lib.qmll_fchl19_backward.argtypes = [ctypes.POINTER(_CFchl), vp, vp, i64, vp, vp, i32, vp, vp, vp, vp]
+    lib.qmll_fchl19_backward.restype = ctypes.c_int
     lib.qmll_sorf_forward_mma.argtypes = [pp, vp, vp, vp, i64, i32, vp, vp, sz, vp]
     lib.qmll_sorf_forward_mma.restype = ctypes.c_int
     lib.qmll_rff_forward.argtypes = [vp, vp, i32, i32, i32, vp, vp, vp, i64, i32, vp, vp, sz, vp]
@@ -390,6 +396,47 @@ def qmll_fchl19(fp: Fchl19Params, r, elem, nbr_idx, nbr_shift=None, jacobian: bo
                                       _dev(jac_idx, torch.int32, "jac_idx"), _dev(jac_val, torch.float32, "jac_val"),
                                       _dev(info, torch.int32, "info"), _stream()))
     return rho, jac_idx, jac_val, info
+
+
+def qmll_sorf_backward_g(p: SorfParams, x, elem, mol_off, alpha, want_energies: bool = True):
+    """(energies [n_mol] | None, g [n_atoms, d] = dE/dx): include/qmll.h qmll_sorf_backward_g (step a5 alone)."""
+    lib = load_library()
+    xp, ep, mp, n_atoms, n_mol = _problem(x, elem, mol_off)
+    g = torch.empty((n_atoms, p.d), dtype=torch.float32, device=x.device)
+    E = torch.empty((n_mol,), dtype=torch.float32, device=x.device) if want_energies else None
+    ws = workspace(workspace_bytes(CALL_PREDICT, p, n_atoms, n_mol), x.device)
+    cp = p.c()
+    _check(lib.qmll_sorf_backward_g(ctypes.byref(cp), xp, ep, mp, n_atoms, n_mol, _dev(alpha, torch.float32, "alpha"),
+                                    _dev(E, torch.float32, "energies"), _dev(g, torch.float32, "g"),
+                                    ctypes.c_void_p(ws.data_ptr()), ws.numel(), _stream()))
+    return E, g
+
+
+def qmll_project_back(g, elem, U):
+    """w [n_atoms, rep] = U_e g (dE / d rho from dE / dx): include/qmll.h qmll_project_back."""
+    n_elem, rep, d = (int(v) for v in U.shape)
+    n_atoms = int(elem.shape[0])
+    w = torch.empty((n_atoms, rep), dtype=torch.float32, device=U.device)
+    _check(load_library().qmll_project_back(_dev(g, torch.float32, "g"), _dev(elem, torch.int32, "elem"), n_atoms, rep, d,
+                                            n_elem, _dev(U, torch.float32, "U"), _dev(w, torch.float32, "w"), _stream()))
+    return w
+
+
+def qmll_fchl19_backward(fp: "Fchl19Params", r, elem, nbr_idx, w, nbr_shift=None, forces=None):
+    """(forces [n_atoms, 3], info): F = -sum_I w_I . d rho_I / d r without a Jacobian: include/qmll.h."""
+    n_atoms, K = int(nbr_idx.shape[0]), int(nbr_idx.shape[1])
+    if fp.rep < 0:
+        raise QmllError(-1, "qmll_fchl19_params invalid or outside the supported range (include/qmll.h)")
+    if forces is None:
+        forces = torch.empty((n_atoms, 3), dtype=torch.float32, device=r.device)
+    info = torch.zeros((1,), dtype=torch.int32, device=r.device)
+    cp = fp.c()
+    _check(load_library().qmll_fchl19_backward(ctypes.byref(cp), _dev(r, torch.float32, "r"), _dev(elem, torch.int32, "elem"),
+                                               n_atoms, _dev(nbr_idx, torch.int32, "nbr_idx"),
+                                               _dev(nbr_shift, torch.float32, "nbr_shift"), K, _dev(w, torch.float32, "w"),
+                                               _dev(forces, torch.float32, "forces"), _dev(info, torch.int32, "info"),
+                                               _stream()))
+    return forces, info
 
 
 def qmll_project_neighbor(grad_in, elem, U, idx=None, grad_out=None):

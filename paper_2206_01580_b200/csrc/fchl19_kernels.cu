@@ -79,20 +79,26 @@ __device__ __forceinline__ void f_cut_pair(float r, const FchlDev& P, float* f, 
   *df = -0.5f * CUDART_PI_F * P.inv_rcut * sn;
 }
 
-template <bool kJac>
+// kMode 0: representation only; 1: + Jacobian blocks; 2: vector-Jacobian product (backward pass, L268: "the force
+// components are stored and summed in on-chip memory"): F[j] -= sum_k w_i[k] d rho_i[k] / d r_j for every neighbour
+// image j, F[i] += the same sum (translation invariance), with w_i = dE / d rho_i given -- no Jacobian is materialised.
+template <int kMode>
 __global__ void __launch_bounds__(kFchlThreads, 2)
 fchl19_kernel(const FchlDev P, const float* __restrict__ r, const int32_t* __restrict__ elem,
               const int32_t* __restrict__ nbr_idx, const float* __restrict__ nbr_shift, long long n_atoms,
               float* __restrict__ rho, int32_t* __restrict__ jac_idx, float* __restrict__ jac_val,
-              int32_t* __restrict__ info) {
+              int32_t* __restrict__ info, const float* __restrict__ w_in, float* __restrict__ forces) {
+  constexpr bool kJac = kMode == 1, kVjp = kMode == 2, kGrad = kMode != 0;
   extern __shared__ __align__(16) float sm_raw[];
-  const FchlSmem S = fchl_carve(sm_raw, P.rep, P.K, kJac);
+  const FchlSmem S = fchl_carve(sm_raw, P.rep, P.K, kGrad);
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const long long i = blockIdx.x;
   const int rep = P.rep, K = P.K, off3 = P.E * P.n2;
   const float rix = __ldg(r + 3 * i), riy = __ldg(r + 3 * i + 1), riz = __ldg(r + 3 * i + 2);
 
   for (int t = threadIdx.x; t < rep * (kJac ? 4 : 1); t += kFchlThreads) S.rho_acc[t] = 0.f;   // rho_acc + self_acc
+  if (kVjp)                                                                                    // w_i in place of self_acc
+    for (int t = threadIdx.x; t < rep; t += kFchlThreads) S.self_acc[t] = __ldg(w_in + (size_t)i * rep + t);
 
   // ---- phase 0a: warp 0 compacts the neighbours inside r_cut (in slot order: deterministic) ----
   if (warp == 0) {
@@ -117,7 +123,7 @@ fchl19_kernel(const FchlDev P, const float* __restrict__ r, const int32_t* __res
       const int pos = cnt + __popc(mask & lt);
       if (valid && pos < kFchlMaxN) {
         S.vx[pos] = dx; S.vy[pos] = dy; S.vz[pos] = dz; S.rr[pos] = sqrtf(d2);
-        S.ne[pos] = __ldg(elem + j); S.nslot[pos] = q;
+        S.ne[pos] = __ldg(elem + j); S.nslot[pos] = kVjp ? j : q;     // backward: the atom that receives the force
       }
       if (q < K && !valid) S.inv_list[n_inv + __popc(imask & lt)] = q;
       if (kJac && q < K) jac_idx[i * (K + 1) + 1 + q] = (valid && pos < kFchlMaxN) ? j : -1;
@@ -171,7 +177,10 @@ fchl19_kernel(const FchlDev P, const float* __restrict__ r, const int32_t* __res
   // ---- phase 1: one warp per neighbour slot ----
   float* pt = S.pair_tab + warp * (kFchlMaxN * kPairF);
   float* stage = S.stage + warp * 192;
+  const float* wv = S.self_acc;                 // kVjp: dE / d rho_i
+  float self_x = 0.f, self_y = 0.f, self_z = 0.f;
   for (int m = warp; m < nn; m += kFchlWarps) {
+    float fx = 0.f, fy = 0.f, fz = 0.f;         // kVjp: sum_k w[k] d rho_i[k] / d r_j, per lane
     const float ax = S.vx[m], ay = S.vy[m], az = S.vz[m], ra = S.rr[m], Fa = S.fc[m], dFa = S.dfc[m];
     const float ira = 1.f / ra, hx = ax * ira, hy = ay * ira, hz = az * ira;     // unit vector i -> j
     const int Zj = S.ne[m];
@@ -193,6 +202,10 @@ fchl19_kernel(const FchlDev P, const float* __restrict__ r, const int32_t* __res
         atomicAdd(&S.rho_acc[Zj * P.n2 + lane], Fa * rpw * L);
         const float dlnL = (-0.5f * dsig2 + t * dmu + 0.5f * t * t * dsig2 / sig2) / sig2;
         dg = rpw * L * (dFa + Fa * (dlnL - P.N2 * ira));
+      }
+      if (kVjp && lane < P.n2) {
+        const float t = wv[Zj * P.n2 + lane] * dg;
+        fx = t * hx; fy = t * hy; fz = t * hz;
       }
       if (kJac) {
         if (lane < P.n2) { stage[3 * lane] = dg * hx; stage[3 * lane + 1] = dg * hy; stage[3 * lane + 2] = dg * hz; }
@@ -230,7 +243,7 @@ fchl19_kernel(const FchlDev P, const float* __restrict__ r, const int32_t* __res
           const float FF = Fa * Fb * Fc;
           const float Pv = P.c3d * Nn * Dn * FF;
           o1.z = Pv * cosi; o1.w = Pv * sini; o2.x = 0.5f * (ra + rb);
-          if (kJac) {
+          if (kGrad) {
             // gradients with respect to the position of j
             const float ci_x = (gx - cosi * hx) * ira, ci_y = (gy - cosi * hy) * ira, ci_z = (gz - cosi * hz) * ira;
             const float cj_x = -((ux + cosj * hx) * ira - (hx + cosj * ux) * irc);
@@ -280,16 +293,22 @@ fchl19_kernel(const FchlDev P, const float* __restrict__ r, const int32_t* __res
             const float4 q0 = q[0], q1 = q[1];
             const float dm = q[2].x - Rs;
             const float R = P.norm3 * __expf(-P.eta3 * dm * dm);          // eq. 29
-            if (kJac) {
+            if (kGrad) {
               const float w = -P.eta3 * dm * R;                            // dR/dm * dm/dr_ij, times h below
               acx = fmaf(R, q0.x, acx); acy = fmaf(R, q0.y, acy); acz = fmaf(R, q0.z, acz); bc = fmaf(w, q1.z, bc);
               asx = fmaf(R, q0.w, asx); asy = fmaf(R, q1.x, asy); asz = fmaf(R, q1.y, asz); bs = fmaf(w, q1.w, bs);
             }
             if (kk > m) { vc = fmaf(R, q1.z, vc); vs = fmaf(R, q1.w, vs); }   // every unordered pair once (B6)
           }
-          if (k1 > k0) {
+          if (k1 > k0 && !kVjp) {
             atomicAdd(&S.rho_acc[off3 + (p * P.n3 + lane) * 2], vc);
             atomicAdd(&S.rho_acc[off3 + (p * P.n3 + lane) * 2 + 1], vs);
+          }
+          if (kVjp && k1 > k0) {
+            const float wc = wv[off3 + (p * P.n3 + lane) * 2], wsn = wv[off3 + (p * P.n3 + lane) * 2 + 1];
+            fx += wc * (acx + bc * hx) + wsn * (asx + bs * hx);
+            fy += wc * (acy + bc * hy) + wsn * (asy + bs * hy);
+            fz += wc * (acz + bc * hz) + wsn * (asz + bs * hz);
           }
         }
         if (kJac) {
@@ -306,12 +325,29 @@ fchl19_kernel(const FchlDev P, const float* __restrict__ r, const int32_t* __res
           __syncwarp();
         }
       }
+    if (kVjp) {
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1) {
+        fx += __shfl_xor_sync(0xffffffffu, fx, o);
+        fy += __shfl_xor_sync(0xffffffffu, fy, o);
+        fz += __shfl_xor_sync(0xffffffffu, fz, o);
+      }
+      if (lane == 0) {
+        float* Fj = forces + 3 * (size_t)S.nslot[m];
+        atomicAdd(Fj, -fx); atomicAdd(Fj + 1, -fy); atomicAdd(Fj + 2, -fz);
+      }
+      self_x += fx; self_y += fy; self_z += fz;
+    }
     __syncwarp();
+  }
+  if (kVjp && lane == 0 && (self_x != 0.f || self_y != 0.f || self_z != 0.f)) {
+    float* Fi = forces + 3 * (size_t)i;
+    atomicAdd(Fi, self_x); atomicAdd(Fi + 1, self_y); atomicAdd(Fi + 2, self_z);
   }
   __syncthreads();
 
   // ---- phase 2: results of the atom ----
-  if (rho)
+  if (rho && !kVjp)
     for (int t = threadIdx.x; t < rep; t += kFchlThreads) rho[(size_t)i * rep + t] = S.rho_acc[t];
   if (kJac) {
     float* jb = jac_val + (size_t)i * (K + 1) * (size_t)rep * 3;
@@ -323,7 +359,7 @@ int fchl19_rep_size(const qmll_fchl19_params* fp) { return fp->n_elem * fp->n2 +
 
 int fchl19_launch(const qmll_fchl19_params* fp, const float* r, const int32_t* elem, int64_t n_atoms,
                   const int32_t* nbr_idx, const float* nbr_shift, int32_t K, float* rho, int32_t* jac_idx,
-                  float* jac_val, int32_t* info, cudaStream_t st) {
+                  float* jac_val, int32_t* info, const float* w_in, float* forces, cudaStream_t st) {
   FchlDev P;
   P.E = fp->n_elem; P.n2 = fp->n2; P.n3 = fp->n3; P.rep = fchl19_rep_size(fp); P.K = K;
   P.eta2 = fp->eta2; P.eta3 = fp->eta3; P.N2 = fp->two_body_decay; P.N3 = fp->three_body_decay;
@@ -332,19 +368,19 @@ int fchl19_launch(const qmll_fchl19_params* fp, const float* r, const int32_t* e
   P.rs2_step = fp->r_cut / (float)fp->n2; P.rs3_step = fp->r_cut / (float)fp->n3;
   P.norm3 = (float)sqrt((double)fp->eta3 / 3.14159265358979323846);
   QMLL_CUDA_TRY(cudaMemsetAsync(info, 0, sizeof(int32_t), st));
+  if (forces) QMLL_CUDA_TRY(cudaMemsetAsync(forces, 0, (size_t)n_atoms * 3 * sizeof(float), st));
   if (n_atoms == 0) return QMLL_OK;
-  const bool jac = jac_val != nullptr;
-  const size_t smem = fchl_smem_floats(P.rep, K, jac) * sizeof(float);
+  const int mode = forces ? 2 : (jac_val ? 1 : 0);
+  const size_t smem = fchl_smem_floats(P.rep, K, mode != 0) * sizeof(float);
   if (smem > 227 * 1024) return QMLL_ERR_UNSUPPORTED;
-  if (jac) {
-    auto kern = fchl19_kernel<true>;
+  auto launch = [&](auto kern) -> int {
     QMLL_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    kern<<<(unsigned)n_atoms, kFchlThreads, smem, st>>>(P, r, elem, nbr_idx, nbr_shift, n_atoms, rho, jac_idx, jac_val, info);
-  } else {
-    auto kern = fchl19_kernel<false>;
-    QMLL_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    kern<<<(unsigned)n_atoms, kFchlThreads, smem, st>>>(P, r, elem, nbr_idx, nbr_shift, n_atoms, rho, jac_idx, jac_val, info);
-  }
+    kern<<<(unsigned)n_atoms, kFchlThreads, smem, st>>>(P, r, elem, nbr_idx, nbr_shift, n_atoms, rho, jac_idx, jac_val, info,
+                                                        w_in, forces);
+    return QMLL_OK;
+  };
+  int rc = mode == 2 ? launch(fchl19_kernel<2>) : (mode == 1 ? launch(fchl19_kernel<1>) : launch(fchl19_kernel<0>));
+  if (rc) return rc;
   QMLL_LAUNCH_CHECK("fchl19_kernel");
   return QMLL_OK;
 }

@@ -277,6 +277,38 @@ project_nbr_kernel(const float* __restrict__ gin, const int32_t* __restrict__ id
   }
 }
 
+// Transposed projection (backward pass of x = rho^T U_e): w[I, k] = sum_m U[e_I, k, m] g[I, m].  Block = one atom, g in
+// shared memory, one warp per row k of U_e (coalesced along m, shuffle reduction).
+__global__ void __launch_bounds__(kProjThreads)
+project_back_kernel(const float* __restrict__ g, const int32_t* __restrict__ elem, int rep, int d,
+                    const float* __restrict__ U, float* __restrict__ w) {
+  extern __shared__ float gs[];
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const size_t I = blockIdx.x;
+  for (int m = threadIdx.x; m < d; m += kProjThreads) gs[m] = __ldg(g + I * d + m);
+  __syncthreads();
+  const float* Ue = U + (size_t)__ldg(elem + I) * rep * d;
+  for (int k = warp; k < rep; k += kProjThreads / 32) {
+    float acc = 0.f;
+    for (int m = 4 * lane; m < d; m += 128) {
+      const float4 u = __ldg(reinterpret_cast<const float4*>(Ue + (size_t)k * d + m));
+      acc = fmaf(u.x, gs[m], acc); acc = fmaf(u.y, gs[m + 1], acc);
+      acc = fmaf(u.z, gs[m + 2], acc); acc = fmaf(u.w, gs[m + 3], acc);
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
+    if (lane == 0) w[I * rep + k] = acc;
+  }
+}
+
+int project_back_launch(const float* g, const int32_t* elem, int64_t n_atoms, int32_t rep, int32_t d, const float* U,
+                        float* w, cudaStream_t st) {
+  if (n_atoms == 0) return QMLL_OK;
+  project_back_kernel<<<(unsigned)n_atoms, kProjThreads, d * sizeof(float), st>>>(g, elem, rep, d, U, w);
+  QMLL_LAUNCH_CHECK("project_back_kernel");
+  return QMLL_OK;
+}
+
 int project_neighbor_launch(const float* gin, const int32_t* idx, const int32_t* elem, int64_t n_atoms, int32_t S,
                             int32_t rep, int32_t d, int32_t n_elem, const float* U, float* gout, cudaStream_t st) {
   if (n_atoms == 0 || S == 0) return QMLL_OK;

@@ -79,7 +79,8 @@ static size_t e_bytes(int32_t n_mol) { return align_up((size_t)n_mol * sizeof(do
 // shared body of qmll_sorf_backward_forces and qmll_predict
 static int backward_impl(const qmll_sorf_params* p, const float* x, const int32_t* elem, const int32_t* mol_off,
                          int64_t n_atoms, int32_t n_mol, const float* alpha, const qmll_grad* grad, float* energies,
-                         float* forces, void* workspace, size_t workspace_bytes, cudaStream_t st, int which) {
+                         float* forces, void* workspace, size_t workspace_bytes, cudaStream_t st, int which,
+                         float* g_out = nullptr) {
   int rc = check_params(p);
   if (rc) return rc;
   rc = check_problem(x, elem, mol_off, n_atoms, n_mol);
@@ -87,7 +88,8 @@ static int backward_impl(const qmll_sorf_params* p, const float* x, const int32_
   if (!alpha) return QMLL_ERR_INVALID_ARG;
   if (forces) { rc = check_grad(grad); if (rc) return rc; }
   else if (grad) return QMLL_ERR_INVALID_ARG;
-  if (!forces && !energies) return QMLL_ERR_INVALID_ARG;
+  if (!forces && !energies && !g_out) return QMLL_ERR_INVALID_ARG;
+  if (g_out && forces) return QMLL_ERR_INVALID_ARG;
   rc = check_device();
   if (rc) return rc;
   rc = check_ws(workspace, workspace_bytes, qmll_workspace_bytes(which, p, n_atoms, n_mol, 0));
@@ -102,7 +104,8 @@ static int backward_impl(const qmll_sorf_params* p, const float* x, const int32_
   if (eacc && n_mol > 0) QMLL_CUDA_TRY(cudaMemsetAsync(eacc, 0, (size_t)n_mol * sizeof(double), st));
   if (forces && n_atoms > 0) QMLL_CUDA_TRY(cudaMemsetAsync(forces, 0, (size_t)n_atoms * 3 * sizeof(float), st));
   SorfProblem pr{p, x, elem, mol_off, n_atoms, n_mol};
-  rc = sorf_launch_predict(pr, t, forces ? grad : nullptr, forces, eacc, st);
+  rc = g_out ? sorf_launch_predict(pr, t, nullptr, g_out, eacc, st, true)
+             : sorf_launch_predict(pr, t, forces ? grad : nullptr, forces, eacc, st);
   if (rc) return rc;
   if (energies) { rc = sorf_finish_energies(eacc, energies, n_mol, st); if (rc) return rc; }
   return QMLL_OK;
@@ -262,6 +265,41 @@ int qmll_sorf_backward_forces(const qmll_sorf_params* p, const float* x, const i
                        workspace_bytes, static_cast<cudaStream_t>(cuda_stream), QMLL_CALL_BACKWARD_FORCES);
 }
 
+static int check_fchl(const qmll_fchl19_params* fp);
+
+int qmll_sorf_backward_g(const qmll_sorf_params* p, const float* x, const int32_t* elem, const int32_t* mol_off,
+                         int64_t n_atoms, int32_t n_mol, const float* alpha, float* energies, float* g,
+                         void* workspace, size_t workspace_bytes, void* cuda_stream) {
+  if (!g) return QMLL_ERR_INVALID_ARG;
+  return backward_impl(p, x, elem, mol_off, n_atoms, n_mol, alpha, nullptr, energies, nullptr, workspace,
+                       workspace_bytes, static_cast<cudaStream_t>(cuda_stream), QMLL_CALL_PREDICT, g);
+}
+
+int qmll_project_back(const float* g, const int32_t* elem, int64_t n_atoms, int32_t rep, int32_t d, int32_t n_elem,
+                      const float* U, float* w, void* cuda_stream) {
+  if (n_atoms < 0 || rep <= 0 || d <= 0 || d % 4 != 0 || n_elem < 1 || !U) return QMLL_ERR_INVALID_ARG;
+  if (n_atoms > 0 && (!g || !elem || !w)) return QMLL_ERR_INVALID_ARG;
+  if (n_atoms > 0x7fffff00LL || d > 8192) return QMLL_ERR_INVALID_ARG;
+  int rc = check_device();
+  if (rc) return rc;
+  return project_back_launch(g, elem, n_atoms, rep, d, U, w, static_cast<cudaStream_t>(cuda_stream));
+}
+
+int qmll_fchl19_backward(const qmll_fchl19_params* fp, const float* r, const int32_t* elem, int64_t n_atoms,
+                         const int32_t* nbr_idx, const float* nbr_shift, int32_t K, const float* w, float* forces,
+                         int32_t* info, void* cuda_stream) {
+  int rc = check_fchl(fp);
+  if (rc) return rc;
+  if (n_atoms < 0 || n_atoms > 0x7fffff00LL || K < 0 || K > 4096 || !info) return QMLL_ERR_INVALID_ARG;
+  if (n_atoms > 0 && (!r || !elem || !w || !forces || (K > 0 && !nbr_idx))) return QMLL_ERR_INVALID_ARG;
+  rc = check_device();
+  if (rc) return rc;
+  if (n_atoms == 0) return fchl19_launch(fp, r, elem, 0, nbr_idx, nbr_shift, K, nullptr, nullptr, nullptr, info, nullptr,
+                                         nullptr, static_cast<cudaStream_t>(cuda_stream));
+  return fchl19_launch(fp, r, elem, n_atoms, nbr_idx, nbr_shift, K, nullptr, nullptr, nullptr, info, w, forces,
+                       static_cast<cudaStream_t>(cuda_stream));
+}
+
 int qmll_predict(const qmll_sorf_params* p, const float* x, const int32_t* elem, const int32_t* mol_off,
                  int64_t n_atoms, int32_t n_mol, const float* alpha, const qmll_grad* grad, float* energies,
                  float* forces, void* workspace, size_t workspace_bytes, void* cuda_stream) {
@@ -334,7 +372,7 @@ int qmll_fchl19(const qmll_fchl19_params* fp, const float* r, const int32_t* ele
   if (n_atoms > 0 && (!r || !elem || (K > 0 && !nbr_idx))) return QMLL_ERR_INVALID_ARG;
   rc = check_device();
   if (rc) return rc;
-  return fchl19_launch(fp, r, elem, n_atoms, nbr_idx, nbr_shift, K, rho, jac_idx, jac_val, info,
+  return fchl19_launch(fp, r, elem, n_atoms, nbr_idx, nbr_shift, K, rho, jac_idx, jac_val, info, nullptr, nullptr,
                        static_cast<cudaStream_t>(cuda_stream));
 }
 

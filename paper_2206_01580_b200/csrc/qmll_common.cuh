@@ -74,7 +74,7 @@ int sorf_prepare_tables(const qmll_sorf_params* p, const float* alpha, Carver& w
                         cudaStream_t st);
 int sorf_launch_forward(const SorfProblem& pr, const SorfTables& t, float* Z, float* zs_out, cudaStream_t st);
 int sorf_launch_predict(const SorfProblem& pr, const SorfTables& t, const qmll_grad* grad, float* forces,
-                        double* energy_acc, cudaStream_t st);
+                        double* energy_acc, cudaStream_t st, bool g_out = false);
 int sorf_launch_force_rows_dense(const SorfProblem& pr, const SorfTables& t, const float* zs,
                                  const float* dense_t, const int64_t* dense_off, float* G, cudaStream_t st);
 size_t sorf_zs_floats(const qmll_sorf_params* p, int64_t n_atoms);
@@ -123,6 +123,8 @@ int project_launch(const float* rho, const int32_t* elem, const int32_t* mol_off
                    int32_t rep, int32_t d, int32_t n_elem, const float* U, float* x, const float* gin,
                    const int64_t* in_off, float* gout, const int64_t* out_off, cudaStream_t st);
 
+int project_back_launch(const float* g, const int32_t* elem, int64_t n_atoms, int32_t rep, int32_t d, const float* U,
+                        float* w, cudaStream_t st);
 int project_neighbor_launch(const float* gin, const int32_t* idx, const int32_t* elem, int64_t n_atoms, int32_t S,
                             int32_t rep, int32_t d, int32_t n_elem, const float* U, float* gout, cudaStream_t st);
 
@@ -130,7 +132,7 @@ int project_neighbor_launch(const float* gin, const int32_t* idx, const int32_t*
 int fchl19_rep_size(const qmll_fchl19_params* fp);
 int fchl19_launch(const qmll_fchl19_params* fp, const float* r, const int32_t* elem, int64_t n_atoms,
                   const int32_t* nbr_idx, const float* nbr_shift, int32_t K, float* rho, int32_t* jac_idx,
-                  float* jac_val, int32_t* info, cudaStream_t st);
+                  float* jac_val, int32_t* info, const float* w_in, float* forces, cudaStream_t st);
 
 void syrk_set_timing(bool on);
 int syrk_collect_timing(double* total_ms, int* launches);

@@ -173,10 +173,12 @@ int sorf_launch_forward(const SorfProblem& pr, const SorfTables& t, float* Z, fl
   QMLL_SWITCH_D(pr.p->d, CALL)
 #undef CALL
 }
+// forces: [n_atoms, 3] with grad, or (grad == NULL, g_out = true) g [n_atoms, d] = dE/dx
 int sorf_launch_predict(const SorfProblem& pr, const SorfTables& t, const qmll_grad* grad, float* forces,
-                        double* energy_acc, cudaStream_t st) {
+                        double* energy_acc, cudaStream_t st, bool g_out) {
   GradView gv{QMLL_GRAD_NONE, nullptr, nullptr, nullptr, nullptr, 0};
   if (grad) gv = GradView{grad->layout, grad->dense, grad->dense_off, grad->nbr_idx, grad->nbr_val, grad->K};
+  if (g_out) gv.layout = kGradGOut;
 #define CALL(TAG) sorf_predict_##TAG(pr, t, gv, forces, energy_acc, st)
   QMLL_SWITCH_D(pr.p->d, CALL)
 #undef CALL

@@ -129,6 +129,7 @@ __device__ __forceinline__ float warp_sum(float v) {
   return v;
 }
 
+constexpr int kGradGOut = 3;   // internal layout value: write g = dE/dx instead of contracting (qmll_sorf_backward_g)
 struct GradView {          // qmll_grad flattened for the device
   int layout;              // QMLL_GRAD_NONE / DENSE / NEIGHBOR
   const float* dense;
@@ -366,9 +367,11 @@ sorf_predict_kernel(const float* __restrict__ x, const int32_t* __restrict__ ele
       if (grad.layout == QMLL_GRAD_DENSE) {
         const float* blk = grad.dense + __ldg(grad.dense_off + M) + (size_t)(a - m_lo) * S::d * 3 * n;
         contract_dense_atom<S>(gbuf, blk, 3 * n, forces + (size_t)m_lo * 3, lane);
-      } else {
+      } else if (grad.layout == QMLL_GRAD_NEIGHBOR) {
         contract_neighbor_atom<S>(gbuf, grad.nbr_idx + (size_t)a * grad.K,
                                   grad.nbr_val + (size_t)a * grad.K * S::d * 3, grad.K, forces, lane);
+      } else {   // kGradGOut: no contraction, `forces` is g [n_atoms, d] = dE/dx (gbuf holds -dE/dx)
+        for (int m = lane; m < S::d; m += kWarp) forces[(size_t)a * S::d + m] = -gbuf[m];
       }
       __syncwarp();
     }

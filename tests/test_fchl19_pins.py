@@ -333,3 +333,35 @@ def test_chain_forces_match_finite_differences_of_the_energy():
             F_fd[a, c] = -(8 * (e(h) - e(-h)) - (e(2 * h) - e(-2 * h))) / (12 * h)
     assert np.linalg.norm(F) > 0
     assert np.linalg.norm(F - F_fd) <= 1e-4 * np.linalg.norm(F_fd)
+
+
+def test_backward_chain_equals_jacobian_chain_and_finite_differences():
+    """The Jacobian-free backward pass in the oracle (dE/dx -> dE/d rho -> forces) is the same contraction in another
+    order: it must equal the force assembled through the projected Jacobian (pinned above by finite differences of
+    E(r)), to rounding; project_back is the plain transposed matrix product."""
+    from workloads import make_model
+    fp = replace(FP, n_elem=3, n2=7, n3=5, r_cut=4.5)
+    g = molecules_geometry(61, [6, 4], n_elem=3)
+    d, D, T, sigma = 16, 128, 3, 2.0
+    model = make_model(62, d=d, D=D, T=T, sigma=sigma, n_elem=3)
+    rng = np.random.default_rng(63)
+    U = rng.normal(size=(3, fp.rep, d)).astype(np.float32) * 0.4
+    alpha = rng.normal(size=D).astype(np.float32)
+    rho = oracle.fchl19(fp, g.r, g.elem, g.nbr_idx)
+    J = oracle.fchl19_jacobian(fp, g.r, g.elem, g.nbr_idx)
+    x = oracle.project(rho.astype(np.float32), g.elem, U).astype(np.float32)
+    gx = oracle.backward_g(x, g.elem, d, D, T, sigma, model.signs, model.bias, alpha)
+    w = oracle.project_back(gx, g.elem, U)
+    for a in range(10):
+        np.testing.assert_allclose(w[a], U[g.elem[a]].astype(np.float64) @ gx[a], rtol=1e-12, atol=1e-14)
+    F_back = oracle.fchl19_backward(fp, g.r, g.elem, g.nbr_idx, w)
+    # the same force through the (exact, FP64) projected Jacobian: einsum written out in the test
+    idx = np.concatenate([np.arange(10, dtype=np.int32)[:, None], g.nbr_idx], axis=1)
+    F_jac = np.zeros((10, 3))
+    for a in range(10):
+        dx = np.einsum("skc,km->smc", J[a], U[g.elem[a]].astype(np.float64))
+        for s, j in enumerate(idx[a]):
+            if j >= 0:
+                F_jac[j] -= gx[a] @ dx[s]
+    np.testing.assert_allclose(F_back, F_jac, rtol=1e-10, atol=1e-12 * np.abs(F_jac).max())
+    assert np.abs(F_back.sum(0)).max() < 1e-10 * np.abs(F_back).max()       # no net force (translation invariance)

@@ -213,3 +213,111 @@ def test_fchl19_fullsize_periodic_cell_15625_atoms(q):
     dead = jac_idx < 0
     assert float(jac_val[dead].abs().max()) == 0.0
     assert bool(torch.isfinite(rho).all()) and bool(torch.isfinite(jac_val).all())
+
+
+def _backward_chain_gpu(q, fp, g, model, U, alpha):
+    """coordinates -> forces without a Jacobian: fchl19 -> project -> backward_g -> project_back -> fchl19_backward."""
+    pkg, torch = q
+    t = lambda a: None if a is None else torch.from_numpy(np.ascontiguousarray(a)).cuda()
+    dfp = dev_params(pkg, fp)
+    r, e, idx, sh = t(g.r), t(g.elem), t(g.nbr_idx), t(g.nbr_shift)
+    rho, _, _, info = pkg.qmll_fchl19(dfp, r, e, idx, sh)
+    x, _ = pkg.qmll_project(rho, e, t(U))
+    params = pkg.SorfParams(d=model.d, D=model.D, n_transform=model.T, n_elem=model.n_elem, sigma=model.sigma,
+                            signs=t(model.signs), bias=t(model.bias))
+    E, gx = pkg.qmll_sorf_backward_g(params, x, e, t(g.mol_off), t(alpha))
+    w = pkg.qmll_project_back(gx, e, t(U))
+    F, info2 = pkg.qmll_fchl19_backward(dfp, r, e, idx, w, nbr_shift=sh)
+    torch.cuda.synchronize()
+    assert int(info.item()) == 0 and int(info2.item()) == 0
+    return x, E, gx, w, F
+
+
+def _backward_chain_oracle(fp, g, model, U, alpha):
+    rho = oracle.fchl19(fp, g.r, g.elem, g.nbr_idx, g.nbr_shift)
+    x = oracle.project(rho.astype(np.float32), g.elem, U)
+    x32 = x.astype(np.float32)
+    Z = oracle.forward(x32, g.elem, g.mol_off, model.d, model.D, model.T, model.sigma, model.signs, model.bias)
+    E = oracle.energy(Z, alpha)
+    gx = oracle.backward_g(x32, g.elem, model.d, model.D, model.T, model.sigma, model.signs, model.bias, alpha)
+    w = oracle.project_back(gx, g.elem, U)
+    F = oracle.fchl19_backward(fp, g.r, g.elem, g.nbr_idx, w, g.nbr_shift)
+    return x, E, gx, w, F
+
+
+@pytest.mark.parametrize("kind", ["molecules", "cell"])
+def test_backward_chain_without_jacobian(q, kind):
+    """qmll_sorf_backward_g, qmll_project_back and qmll_fchl19_backward against the oracle, step by step and as a chain;
+    and the same forces as the Jacobian route (qmll_fchl19 + qmll_project_neighbor + qmll_predict)."""
+    pkg, torch = q
+    if kind == "molecules":
+        fp = FchlParams()
+        g = molecules_geometry(23, [9, 21, 27, 2, 1], probs=[0.5, 0.3, 0.06, 0.12, 0.02])
+    else:
+        fp = replace(FchlParams(), r_cut=3.6)
+        g = cell_geometry(14, 6, spacing=2.0, jitter=0.35, r_list=3.9)
+    d, D = 128, 1024
+    model = make_model(81, d=d, D=D, T=3, sigma=3.0)
+    U = projection_inputs(seed=82, counts=[1], rep=fp.rep, d=d).U
+    alpha = (np.random.default_rng(83).normal(size=D) / np.sqrt(D)).astype(np.float32)
+    x, E, gx, w, F = _backward_chain_gpu(q, fp, g, model, U, alpha)
+    xo, Eo, gxo, wo, Fo = _backward_chain_oracle(fp, g, model, U, alpha)
+    assert rel(x.cpu().numpy(), xo) <= TOL
+    assert rel(E.cpu().numpy(), Eo) <= TOL
+    assert rel(gx.cpu().numpy(), gxo) <= TOL_J
+    assert rel(w.cpu().numpy(), wo) <= TOL_J
+    assert rel(F.cpu().numpy(), Fo) <= TOL_J
+    # each backward kernel alone on the oracle's own inputs
+    t = lambda a: None if a is None else torch.from_numpy(np.ascontiguousarray(a)).cuda()
+    w1 = pkg.qmll_project_back(t(gxo.astype(np.float32)), t(g.elem), t(U))
+    assert rel(w1.cpu().numpy(), oracle.project_back(gxo.astype(np.float32), g.elem, U)) <= TOL
+    F1, _ = pkg.qmll_fchl19_backward(dev_params(pkg, fp), t(g.r), t(g.elem), t(g.nbr_idx), t(wo.astype(np.float32)),
+                                     nbr_shift=t(g.nbr_shift))
+    assert rel(F1.cpu().numpy(), oracle.fchl19_backward(fp, g.r, g.elem, g.nbr_idx, wo.astype(np.float32), g.nbr_shift)) <= TOL_J
+    # the Jacobian route gives the same forces
+    dfp = dev_params(pkg, fp)
+    rho, jidx, jval, _ = pkg.qmll_fchl19(dfp, t(g.r), t(g.elem), t(g.nbr_idx), t(g.nbr_shift), jacobian=True)
+    dx = pkg.qmll_project_neighbor(jval, t(g.elem), t(U), idx=jidx)
+    params = pkg.SorfParams(d=d, D=D, n_transform=3, n_elem=5, sigma=3.0, signs=t(model.signs), bias=t(model.bias))
+    E2, F2 = pkg.qmll_predict(params, x, t(g.elem), t(g.mol_off), t(alpha), pkg.Grad.make_neighbor(jidx, dx))
+    assert rel(F2.cpu().numpy(), Fo) <= TOL_J
+    assert rel(F.cpu().numpy(), F2.cpu().numpy()) <= TOL_J
+
+
+def test_backward_chain_fullsize_cell_properties(q):
+    """15 625-atom cell (the configuration bench.py times): forces of the Jacobian-free chain equal those of the
+    Jacobian route on ALL atoms, sum to zero, and match the oracle's contraction on sampled source atoms."""
+    pkg, torch = q
+    fp = replace(FchlParams(), r_cut=4.8)
+    g = cell_geometry(2, 25, r_list=4.8, K=64)
+    d, D = 256, 4096
+    model = make_model(91, d=d, D=D, T=3, sigma=8.0)
+    U = projection_inputs(seed=78, counts=[1], rep=fp.rep, d=d).U
+    alpha = (np.random.default_rng(93).normal(size=D) / np.sqrt(D)).astype(np.float32)
+    x, E, gx, w, F = _backward_chain_gpu(q, fp, g, model, U, alpha)
+    t = lambda a: None if a is None else torch.from_numpy(np.ascontiguousarray(a)).cuda()
+    dfp = dev_params(pkg, fp)
+    rho, jidx, jval, _ = pkg.qmll_fchl19(dfp, t(g.r), t(g.elem), t(g.nbr_idx), t(g.nbr_shift), jacobian=True)
+    dx = pkg.qmll_project_neighbor(jval, t(g.elem), t(U), idx=jidx)
+    del jval
+    params = pkg.SorfParams(d=d, D=D, n_transform=3, n_elem=5, sigma=8.0, signs=t(model.signs), bias=t(model.bias))
+    E2, F2 = pkg.qmll_predict(params, x, t(g.elem), t(g.mol_off), t(alpha), pkg.Grad.make_neighbor(jidx, dx))
+    torch.cuda.synchronize()
+    Fn, F2n = F.cpu().numpy().astype(np.float64), F2.cpu().numpy().astype(np.float64)
+    assert rel(Fn, F2n) <= TOL_J
+    assert rel(E.cpu().numpy(), E2.cpu().numpy()) <= TOL
+    assert np.abs(Fn.sum(0)).max() <= 1e-4 * np.abs(Fn).sum(0).max()
+    # oracle on sampled source atoms: contributions of atom i alone (w zero elsewhere) scattered to its neighbours
+    rng = np.random.default_rng(5)
+    wn = w.cpu().numpy()
+    for i in rng.choice(g.r.shape[0], size=6, replace=False):
+        w1 = np.zeros_like(wn)
+        w1[i] = wn[i]
+        Fg, _ = pkg.qmll_fchl19_backward(dfp, t(g.r), t(g.elem), t(g.nbr_idx), t(w1), nbr_shift=t(g.nbr_shift))
+        J = oracle.fchl19_jacobian(fp, g.r, g.elem, g.nbr_idx, g.nbr_shift, atoms=np.array([i]))[0]
+        Fo = np.zeros((g.r.shape[0], 3))
+        slots = np.concatenate([[i], g.nbr_idx[i]])
+        for s, j in enumerate(slots):
+            if j >= 0:
+                Fo[j] -= wn[i].astype(np.float64) @ J[s]
+        assert rel(Fg.cpu().numpy(), Fo) <= TOL_J
