@@ -567,8 +567,17 @@ def fchl19_config(pk, tm):
     F = torch.empty((na, 3), dtype=torch.float32, device="cuda")
     o["predict_ms"] = tm(lambda: pkg.qmll_predict(params, x, e, mol_off, alpha, grad, energies=E, forces=F))
     tot = o["fchl19_rho_jacobian_ms"] + o["project_x_ms"] + o["project_neighbor_ms"] + o["predict_ms"]
+    o.update({"coordinates_to_forces_jacobian_route_ms": tot, "jacobian_route_us_per_atom": tot * 1e3 / na})
+    del jval, dx, grad
+    torch.cuda.empty_cache()
+    # the Jacobian-free backward pass (L268): rho -> x -> (E, dE/dx) -> dE/drho -> forces
+    o["backward_g_ms"] = tm(lambda: pkg.qmll_sorf_backward_g(params, x, e, mol_off, alpha))
+    _, gx = pkg.qmll_sorf_backward_g(params, x, e, mol_off, alpha)
+    o["project_back_ms"] = tm(lambda: pkg.qmll_project_back(gx, e, U))
+    wv = pkg.qmll_project_back(gx, e, U)
+    o["fchl19_backward_ms"] = tm(lambda: pkg.qmll_fchl19_backward(fp, r, e, idx, wv, nbr_shift=sh, forces=F))
+    tot = o["fchl19_rho_ms"] + o["project_x_ms"] + o["backward_g_ms"] + o["project_back_ms"] + o["fchl19_backward_ms"]
     o.update({"coordinates_to_forces_ms": tot, "us_per_atom": tot * 1e3 / na})
-    del jval, dx
     pkg.release_workspaces()
     torch.cuda.empty_cache()
     return o
