@@ -417,6 +417,19 @@ def ours_arm(args):
             "roofline": roofline, "sorf_rooflines": sorf_rooflines, "e2e": e2e, "gpu_launches": int(launches),
             "clocks": clocks}
 
+    if not args.no_configs and world == 1:
+        # NEXT row f1 beside the line: alpha = (ZtZ + lambda I)^-1 Zty of the step's own normal equations (FP64 Cholesky)
+        lam = 1e-6 * float(torch.diagonal(ZtZ).mean())
+        pkg.qmll_solve(ZtZ, Zty, lam)
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        _, info = pkg.qmll_solve(ZtZ, Zty, lam)
+        e1.record()
+        torch.cuda.synchronize()
+        sms = e0.elapsed_time(e1)
+        line["solve"] = {"D": D, "lambda": lam, "ms": sms, "info": int(info.item()),
+                         "fp64_tflops": (D ** 3 / 3.0) / (sms * 1e-3) / 1e12}
     del A, ZtZ, dt_, di_
     pkg.release_workspaces()
     torch.cuda.empty_cache()
