@@ -72,6 +72,32 @@ def test_host_side_argument_checks_need_no_gpu(lib):
     assert l.qmll_sorf_backward_forces(None, None, None, None, 0, 0, None, None, None, None, 0, None) == -1
 
 
+def test_next_row_entry_points_check_arguments_on_the_host(lib):
+    """FCHL19, projections, tensor-core feature map: parameter checks and size arithmetic need no GPU."""
+    pkg, l = lib
+    fp = pkg.Fchl19Params().c()
+    assert l.qmll_fchl19_rep_size(ctypes.byref(fp)) == 5 * 24 + 5 * 6 * 20 == 720          # Table I (E + F), 5 elements
+    e = pkg.Fchl19Params(n2=23, n3=22).c()
+    assert l.qmll_fchl19_rep_size(ctypes.byref(e)) == 5 * 23 + 30 * 22
+    assert l.qmll_fchl19_rep_size(ctypes.byref(pkg.Fchl19Params(n3=40).c())) == -1          # beyond 32 grid points
+    assert l.qmll_fchl19_rep_size(ctypes.byref(pkg.Fchl19Params(r_cut=0.0).c())) == -1
+    assert l.qmll_fchl19(None, None, None, 0, None, None, 0, None, None, None, None, None) == -1
+    bad = pkg.Fchl19Params(n_elem=17).c()
+    assert l.qmll_fchl19(ctypes.byref(bad), None, None, 0, None, None, 0, None, None, None, None, None) == -2
+    assert l.qmll_fchl19(ctypes.byref(fp), None, None, 5, None, None, 4, None, None, None, None, None) == -1   # no info
+    assert l.qmll_fchl19_backward(ctypes.byref(fp), None, None, 5, None, None, 4, None, None, None, None) == -1
+    assert l.qmll_project_neighbor(None, None, None, 3, 2, 0, 16, 2, None, None, None) == -1
+    assert l.qmll_project_back(None, None, 3, 10, 18, 2, None, None, None) == -1              # d % 4 != 0
+    assert l.qmll_rff_forward(None, None, 128, 512, 2, None, None, None, 0, 0, None, None, 0, None) == -1
+    assert l.qmll_sorf_forward_mma(None, None, None, None, 0, 0, None, None, 0, None) == -1
+    assert l.qmll_sorf_backward_g(None, None, None, None, 0, 0, None, None, None, None, 0, None) == -1
+    ws_s = l.qmll_featmap_workspace_bytes(128, 16384, 5, 1_600_000, 0)
+    ws_r = l.qmll_featmap_workspace_bytes(128, 16384, 5, 1_600_000, 1)
+    assert ws_s >= 5 * 16384 * 128 * 2 + 2 * 1_600_000 * 128 * 2        # fp16 W table + hi / lo copies of x
+    assert ws_r - ws_s >= 5 * 16384 * 128 * 2 - (1 << 22)               # RFF: W as hi + lo
+    assert l.qmll_featmap_workspace_bytes(0, 16384, 5, 10, 0) == 0
+
+
 def test_launch_counter(lib):
     pkg, l = lib
     pkg.reset_launch_count()
@@ -84,6 +110,7 @@ def test_product_never_imports_oracle():
         for f in files:
             if f.endswith((".py", ".cu", ".cuh", ".h")):
                 text = open(os.path.join(dirpath, f)).read()
-                assert "import oracle" not in text and "from oracle" not in text and "sorf_oracle" not in text, f
-    otext = open(os.path.join(ROOT, "oracle", "__init__.py")).read() + open(os.path.join(ROOT, "oracle", "sorf_oracle.c")).read()
+                assert "import oracle" not in text and "from oracle" not in text and "sorf_oracle" not in text \
+                    and "fchl19_oracle" not in text, f
+    otext = "".join(open(os.path.join(ROOT, "oracle", f)).read() for f in ("__init__.py", "sorf_oracle.c", "fchl19_oracle.c"))
     assert "import paper_2206_01580_b200" not in otext and "qmll.h" not in otext
