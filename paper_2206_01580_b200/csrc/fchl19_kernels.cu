@@ -18,8 +18,11 @@
 //   * the [rep, 3] Jacobian block of the slot is written exactly once, coalesced, zeros included (no memset pass, no
 //     global atomics); the block of the central atom is minus the sum of the others (translation invariance) and is
 //     accumulated in shared memory.
-// The Jacobian is the output that matters: (K + 1) rep 3 floats per atom (config-5-like cell: 6.9 GB), so the kernel
-// is bound by HBM WRITES; the arithmetic (~70 k warp instructions per atom) hides under them.
+// The Jacobian is the big output: (K + 1) rep 3 floats per atom (15 625-atom cell, K = 64: 8.8 GB).  Measured
+// (profiles/r2_fchl19_featmap.md): 3.9 ms = 2.25 TB/s of writes (0.35 of the HBM copy peak) with 58 % of the issue
+// slots busy at 16 warps / SM -- issue-bound (~170 k warp instructions per atom), not yet write-bound.
+// Mode 2 (qmll_fchl19_backward) is the Jacobian-free backward pass: the same loops, but every lane multiplies what it
+// would have written by dE/d rho and the warp reduces to one force vector per neighbour (2.0 ms, nothing materialised).
 #include <math_constants.h>
 
 #include "qmll_common.cuh"

@@ -7,13 +7,16 @@
 //
 // Why it pays on B200: per feature the FWHT chain costs T log2(d) adds + T sign flips on the fp32 pipe (~1 ps at the
 // measured 25 T adds/s); the explicit product costs 2 d MACs per pass on tcgen05, 2 passes for SORF (x split hi/lo, W
-// exact) = 0.37 ps at d = 128, and then the cos (MUFU, 16 per clock and SM) is what bounds the kernel.
+// exact) = 0.37 ps at d = 128.  Measured (config 3, profiles/r2_fchl19_featmap.md): 22-23 ms against 30.5 ms; the tensor
+// pipe and MUFU are each ~28 % busy, the instruction issue of the epilogue (14.5 warp instructions per 32 features x 1
+// atom) is what bounds the kernel.
 //
 // Dataflow: W tiles are the stationary operand (128 KB of shared memory: 4 stacks at d = 128, 1 stack at d = 256), so
-// the atoms are first SORTED BY ELEMENT (stable, so the atoms of a molecule that share an element stay adjacent) into
-// tiles of kNT columns that never mix elements; x rows are gathered, scaled by one power of two per tile and split into
+// the atoms are first SORTED BY ELEMENT inside groups of 8192 atoms (stable, so the atoms of a molecule that share an
+// element stay adjacent; group-local, so that the reductions into a molecule's row of Z stay in L2) into tiles of kNT
+// columns that never mix elements; x rows are gathered, scaled by one power of two per tile and split into
 // fp16 hi + lo in the swizzled K-major layout (one contiguous bulk copy per k-block).  Task = (chunk of atom tiles,
-// group of feature tiles): producer warp (bulk copies) / MMA warp (one elected lane issues) / 8 epilogue warps.  Epilogue
+// group of feature tiles): producer warp (bulk copies) / MMA warp (one elected lane issues) / 16 epilogue warps.  Epilogue
 // thread = output feature: cos(c u + b) of every atom column, summed in a register over the run of columns that belong
 // to the same molecule, one fp32 reduction (RED.ADD) into Z per (run, feature).  Z is zeroed first.
 #include <cuda_fp16.h>
