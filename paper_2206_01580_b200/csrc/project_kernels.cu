@@ -138,22 +138,13 @@ project_grad_kernel(const float* __restrict__ gin, const int64_t* __restrict__ i
 // A Jacobian of FCHL19 is structurally sparse along k: the block of a neighbour of element Z_j is zero outside the
 // two-body bin of Z_j and the pair bins that contain Z_j (n2 + 2 E n3 of E n2 + E (E + 1) n3 rows).  The slots are
 // therefore taken in the order of their neighbour's element (so that the ten slots of a pass share their zero rows) and
-// rows k whose 30 staged values are all zero are skipped with one warp vote (exact: they would add zeros).
+// rows k whose 30 staged values are all zero are skipped (exact: they would add zeros): every lane tests two rows of the
+// staged chunk, two ballots give the 64-bit mask of non-zero rows.
 constexpr int kNbrSlots = 10;
 constexpr int kNbrMaxS = 1024;     // slots that are reordered; beyond that the original order is kept
 
-// Rows k of the staged chunk whose 30 values are all zero are skipped: every lane tests rows `lane` and `lane + 32`
-// (conflict-free: row stride 33), two ballots give the 64-bit mask of non-zero rows (the same in every warp), and the
-// non-zero rows are taken two at a time so that the U loads of both are in flight before the first FMA.
-__device__ __forceinline__ void proj_row_fma(float (&acc)[kProjM], const float4 (&u)[kProjM / 4], float a) {
-#pragma unroll
-  for (int q = 0; q < kProjM / 4; ++q) {
-    acc[4 * q + 0] = fmaf(u[q].x, a, acc[4 * q + 0]); acc[4 * q + 1] = fmaf(u[q].y, a, acc[4 * q + 1]);
-    acc[4 * q + 2] = fmaf(u[q].z, a, acc[4 * q + 2]); acc[4 * q + 3] = fmaf(u[q].w, a, acc[4 * q + 3]);
-  }
-}
-__device__ __forceinline__ void proj_accumulate_sparse(float (&acc)[kProjM], const float (*tile)[33], int kc, int lane,
-                                                       const float* __restrict__ Uk, int d) {
+// 64-bit mask of the rows k of the staged chunk that hold a non-zero value (identical in every warp)
+__device__ __forceinline__ unsigned long long proj_chunk_mask(const float (*tile)[33], int kc, int lane) {
   bool nz0 = false, nz1 = false;
   if (lane < kc) {
 #pragma unroll 8
@@ -163,30 +154,22 @@ __device__ __forceinline__ void proj_accumulate_sparse(float (&acc)[kProjM], con
 #pragma unroll 8
     for (int c = 0; c < 32; ++c) nz1 |= tile[lane + 32][c] != 0.f;
   }
-  unsigned long long mask = (unsigned long long)__ballot_sync(0xffffffffu, nz0) |
-                            ((unsigned long long)__ballot_sync(0xffffffffu, nz1) << 32);
-  while (mask) {
-    const int ka = __ffsll((long long)mask) - 1;
-    mask &= mask - 1;
-    const int kb = mask ? __ffsll((long long)mask) - 1 : -1;
-    if (kb >= 0) mask &= mask - 1;
-    float4 ua[kProjM / 4], ub[kProjM / 4];
-    const float4* pa = reinterpret_cast<const float4*>(Uk + (size_t)ka * d);
-    const float4* pb = reinterpret_cast<const float4*>(Uk + (size_t)(kb >= 0 ? kb : ka) * d);
-#pragma unroll
-    for (int q = 0; q < kProjM / 4; ++q) ua[q] = __ldg(pa + q);
-#pragma unroll
-    for (int q = 0; q < kProjM / 4; ++q) ub[q] = __ldg(pb + q);
-    proj_row_fma(acc, ua, tile[ka][lane]);
-    proj_row_fma(acc, ub, kb >= 0 ? tile[kb][lane] : 0.f);
-  }
+  return (unsigned long long)__ballot_sync(0xffffffffu, nz0) | ((unsigned long long)__ballot_sync(0xffffffffu, nz1) << 32);
 }
+__device__ __forceinline__ int nth_set_bit(unsigned long long m, int j) {
+  const unsigned lo = (unsigned)m, hi = (unsigned)(m >> 32);
+  const int c = __popc(lo);
+  return j < c ? (int)__fns(lo, 0, j + 1) : 32 + (int)__fns(hi, 0, j - c + 1);
+}
+constexpr int kURow = (kProjThreads / 32) * kProjM;   // 256 columns of U per pass
+constexpr int kUR = 32;                                // U rows staged at once (32 KB, shared with the output tiles)
 
 __global__ void __launch_bounds__(kProjThreads)
 project_nbr_kernel(const float* __restrict__ gin, const int32_t* __restrict__ idx, const int32_t* __restrict__ elem,
                    int S, int rep, int d, int n_elem, const float* __restrict__ U, float* __restrict__ gout) {
   __shared__ float tile[kProjK][33];
-  __shared__ float otile[kProjThreads / 32][kProjM][33];
+  __shared__ __align__(16) float otile[kProjThreads / 32][kProjM][33];
+  float4* us4 = reinterpret_cast<float4*>(&otile[0][0][0]);       // [kUR][kURow] staged rows of U_e (kUR * kURow <= 8448)
   __shared__ short order[kNbrMaxS];      // live slots, grouped by the element of the slot's atom
   __shared__ int n_live_s;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -254,16 +237,43 @@ project_nbr_kernel(const float* __restrict__ gin, const int32_t* __restrict__ id
           }
         }
         __syncthreads();
-        if (mw == kProjM) proj_accumulate_sparse(acc, tile, kc, lane, Ue + (size_t)k0 * d + m0, d);
-        else if (mw > 0) {
-          for (int k = 0; k < kc; ++k) {
-            const float av = tile[k][lane];
+        // Non-zero rows of the chunk (the same mask in every warp).  Their U rows are staged in shared memory by the
+        // whole block -- every load of a group of up to kUR rows is in flight at once -- and then read as broadcasts
+        // (loading them row by row behind the zero test left the warps waiting on L2: 47 % long-scoreboard stalls).
+        const unsigned long long mask = proj_chunk_mask(tile, kc, lane);
+        const int nz = __popcll(mask);
+        const int mlen = d - mp < kURow ? d - mp : kURow, m4 = mlen >> 2;     // columns of this pass (multiple of 4)
+        unsigned long long rest = mask;
+        for (int g0 = 0; g0 < nz; g0 += kUR) {
+          const int ng = nz - g0 < kUR ? nz - g0 : kUR;
+          if (g0 > 0) __syncthreads();                                        // the previous group has been consumed
+          for (int item = threadIdx.x; item < ng * m4; item += kProjThreads) {
+            const int jj = item / m4, c4 = item - jj * m4;
+            const int k = nth_set_bit(mask, g0 + jj);
+            us4[jj * (kURow / 4) + c4] = __ldg(reinterpret_cast<const float4*>(Ue + (size_t)(k0 + k) * d + mp) + c4);
+          }
+          __syncthreads();
+          for (int jj = 0; jj < ng; ++jj) {
+            const int k = __ffsll((long long)rest) - 1;
+            rest &= rest - 1;
+            if (mw > 0) {
+              const float a = tile[k][lane];
+              const float4* u4 = us4 + jj * (kURow / 4) + warp * (kProjM / 4);
 #pragma unroll
-            for (int i = 0; i < kProjM; ++i)      // static indices: acc stays in registers
-              if (i < mw) acc[i] = fmaf(__ldg(Ue + (size_t)(k0 + k) * d + m0 + i), av, acc[i]);
+              for (int q = 0; q < kProjM / 4; ++q) {
+                if (4 * q < mw) {
+                  const float4 u = u4[q];
+                  acc[4 * q + 0] = fmaf(u.x, a, acc[4 * q + 0]);
+                  if (4 * q + 1 < mw) acc[4 * q + 1] = fmaf(u.y, a, acc[4 * q + 1]);
+                  if (4 * q + 2 < mw) acc[4 * q + 2] = fmaf(u.z, a, acc[4 * q + 2]);
+                  if (4 * q + 3 < mw) acc[4 * q + 3] = fmaf(u.w, a, acc[4 * q + 3]);
+                }
+              }
+            }
           }
         }
       }
+      __syncthreads();      // the staged U rows share their storage with the output tiles
       // transpose through shared memory: slot ql gets [mw][3] contiguous floats at ((I S + q) d + m0) * 3
 #pragma unroll
       for (int i = 0; i < kProjM; ++i) otile[warp][i][lane] = acc[i];
