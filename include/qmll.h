@@ -90,8 +90,10 @@ int qmll_sorf_forward(const qmll_sorf_params* p, const float* x, const int32_t* 
  *   QMLL_ROWS_MMA   the chain of each (element, stack) is expanded once into its d x d integer matrix (exact in
  *                   fp16 for d <= 256) and applied to the columns on the tensor cores (tcgen05, columns split into
  *                   fp16 hi + lo); d = 128 or 256 only, else QMLL_ERR_UNSUPPORTED.
+ *   QMLL_ROWS_MMA2  the same product on CTA pairs (tcgen05 cta_group::2: an MMA spans two SMs, each holds its own stacks'
+ *                   W and half of the gradient columns); same support as QMLL_ROWS_MMA.
  *   QMLL_ROWS_AUTO  MMA where supported, else FWHT (what qmll_sorf_forward does). */
-enum { QMLL_ROWS_AUTO = 0, QMLL_ROWS_FWHT = 1, QMLL_ROWS_MMA = 2 };
+enum { QMLL_ROWS_AUTO = 0, QMLL_ROWS_FWHT = 1, QMLL_ROWS_MMA = 2, QMLL_ROWS_MMA2 = 3 };
 int qmll_sorf_forward_mode(const qmll_sorf_params* p, const float* x, const int32_t* elem, const int32_t* mol_off,
                            int64_t n_atoms, int32_t n_mol, const qmll_grad* grad, float* Z, float* G,
                            void* workspace, size_t workspace_bytes, int32_t force_rows_mode, void* cuda_stream);

@@ -158,9 +158,9 @@ int qmll_sorf_forward_mode(const qmll_sorf_params* p, const float* x, const int3
   if (rc) return rc;
   if ((G != nullptr) != (grad != nullptr)) return QMLL_ERR_INVALID_ARG;
   if (!Z && !G) return QMLL_ERR_INVALID_ARG;
-  if (force_rows_mode < QMLL_ROWS_AUTO || force_rows_mode > QMLL_ROWS_MMA) return QMLL_ERR_INVALID_ARG;
+  if (force_rows_mode < QMLL_ROWS_AUTO || force_rows_mode > QMLL_ROWS_MMA2) return QMLL_ERR_INVALID_ARG;
   if (grad) { rc = check_grad(grad); if (rc) return rc; }
-  if (force_rows_mode == QMLL_ROWS_MMA && !(grad && grad->layout == QMLL_GRAD_DENSE && sorf_mma_supported(p)))
+  if ((force_rows_mode == QMLL_ROWS_MMA || force_rows_mode == QMLL_ROWS_MMA2) && !(grad && grad->layout == QMLL_GRAD_DENSE && sorf_mma_supported(p)))
     return QMLL_ERR_UNSUPPORTED;
   rc = check_device();
   if (rc) return rc;
@@ -186,7 +186,8 @@ int qmll_sorf_forward_mode(const qmll_sorf_params* p, const float* x, const int3
       long long* xoff = ws.take<long long>((size_t)n_mol + 1);
       float* inv_scale = ws.take<float>((size_t)n_atoms);
       if (!ws.fits()) return QMLL_ERR_WORKSPACE;
-      rc = sorf_force_rows_dense_mma(pr, t, zs, grad, W16, Xh, Xl, xoff, inv_scale, G, st);
+      rc = sorf_force_rows_dense_mma(pr, t, zs, grad, W16, Xh, Xl, xoff, inv_scale, G, st,
+                                     force_rows_mode == QMLL_ROWS_MMA2);
     } else if (grad->layout == QMLL_GRAD_DENSE) {
       float* gt = ws.take<float>((size_t)grad->dense_floats);
       if (!ws.fits()) return QMLL_ERR_WORKSPACE;

@@ -85,7 +85,7 @@ size_t sorf_mma_w_bytes(const qmll_sorf_params* p);
 size_t sorf_mma_x_bytes(const qmll_sorf_params* p, int64_t n_atoms, int64_t dense_floats);
 int sorf_force_rows_dense_mma(const SorfProblem& pr, const SorfTables& t, const float* zs, const qmll_grad* grad,
                               void* W16, void* Xh, void* Xl, long long* xoff, float* inv_scale, float* G,
-                              cudaStream_t st);
+                              cudaStream_t st, bool pairs = false);
 int sorf_mma_build_w(const qmll_sorf_params* p, const SorfTables& t, void* W16, cudaStream_t st);
 
 // ---- feature map on the tensor cores (featmap_mma.cu): SORF with expanded W, dense-W RFF ----------------------------

@@ -460,6 +460,311 @@ sorf_rows_mma_kernel(const int32_t* __restrict__ elem, const int32_t* __restrict
 }
 
 // ---------------------------------------------------------------------------------------------------
+// 3b. The same kernel on CTA PAIRS (cta_group::2).  Measured with a stand-alone loop of MMAs (M 128, both operands in
+//     shared memory): one MMA takes max(N / 2, 32 + N / 4) clocks -- 4 KB of A and 32 N bytes of B cross the 128 B / clock
+//     shared-memory port -- whatever the number of accumulators in rotation: N = 96 costs 56 clocks for 48 clocks of
+//     work, N = 64 costs 48 for 32.  In a pair every CTA reads its own 128 rows of A and only HALF of the columns of B
+//     (32 + N / 8 clocks: below N / 2), and only half of every column tile has to come from L2 into each SM.
+//     Mapping: the pair takes two consecutive stack groups of one molecule; CTA r keeps the W tiles of group 2 g + r
+//     and runs the epilogue of its own stacks exactly as in the single-CTA kernel; the MMA of tile t has M = 256 =
+//     tile t of CTA 0 on top of tile t of CTA 1.  Producers of both CTAs load their W tiles and their half of the
+//     columns; the peer's MMA warp forwards its "full" barriers to the leader, the leader issues and commits to both.
+// ---------------------------------------------------------------------------------------------------
+template <int D_>
+struct Mma2Cfg : MmaCfg<D_> {
+  using B = MmaCfg<D_>;
+  static constexpr int kStages2 = 2 * B::kStages;                       // half-size stages: twice as many
+  static constexpr uint32_t kStageBytes2 = B::kStageBytes / 2;         // hi + lo of kNMax / 2 columns
+  static constexpr uint32_t kSmem2 = B::kABytes + kStages2 * kStageBytes2 + 1024 + 1024;
+};
+
+template <int D_>
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(MmaCfg<D_>::kThreads, 1)
+sorf_rows_mma2_kernel(const int32_t* __restrict__ elem, const int32_t* __restrict__ mol_off, int n_mol, int n_s,
+                      int n_sg, float c, const __half* __restrict__ W16, const __half* __restrict__ Xh,
+                      const __half* __restrict__ Xl, const long long* __restrict__ xoff,
+                      const float* __restrict__ inv_scale, const float* __restrict__ zs, float* __restrict__ G) {
+  using C = Mma2Cfg<D_>;
+  extern __shared__ uint8_t smem_raw[];
+  uint8_t* smem = reinterpret_cast<uint8_t*>(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
+  uint8_t* a_smem = smem;                        // [kMT][kKB] tiles of 16 KB (this CTA's stacks)
+  uint8_t* b_smem = smem + C::kABytes;           // [kStages2] x (hi, lo) of this CTA's half of the columns
+  uint64_t* bars = reinterpret_cast<uint64_t*>(b_smem + C::kStages2 * C::kStageBytes2);
+  uint64_t* a_full = bars;                       // [kKB]
+  uint64_t* a_empty = a_full + C::kKB;           // [kKB]       (multicast commit)
+  uint64_t* pa_full = a_empty + C::kKB;          // [kKB]       leader: the peer's W k-block has landed
+  uint64_t* b_full = pa_full + C::kKB;           // [kStages2]
+  uint64_t* b_empty = b_full + C::kStages2;      // [kStages2]  (multicast commit)
+  uint64_t* pb_full = b_empty + C::kStages2;     // [kStages2]  leader: the peer's half stage has landed
+  uint64_t* t_full = pb_full + C::kStages2;      // [kTBuf]     (multicast commit)
+  uint64_t* t_empty = t_full + C::kTBuf;         // [kTBuf]     leader: epilogue warps of BOTH CTAs
+  uint32_t* tmem_ptr_smem = reinterpret_cast<uint32_t*>(t_empty + C::kTBuf);
+
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const uint32_t rank = cluster_ctarank();
+  const int n_pairs = gridDim.x >> 1, pair = blockIdx.x >> 1;
+  const int n_grp = (n_s + C::kSPT - 1) / C::kSPT;          // stack groups per molecule
+  const int n_gp = (n_grp + 1) / 2;                         // pairs of groups
+  const long long n_tasks = (long long)n_mol * n_gp;
+
+  if (threadIdx.x == 0) {
+    for (int i = 0; i < C::kKB; ++i) { mbar_init(&a_full[i], 1); mbar_init(&a_empty[i], 1); mbar_init(&pa_full[i], 1); }
+    for (int i = 0; i < C::kStages2; ++i) { mbar_init(&b_full[i], 1); mbar_init(&b_empty[i], 1); mbar_init(&pb_full[i], 1); }
+    for (int i = 0; i < C::kTBuf; ++i) { mbar_init(&t_full[i], 1); mbar_init(&t_empty[i], 2 * C::kEpiWarps); }
+    fence_mbarrier_init();
+  }
+  if (warp == 2) {
+    asm volatile("tcgen05.alloc.cta_group::2.sync.aligned.shared::cta.b32 [%0], 512;" ::"r"(smem_u32(tmem_ptr_smem))
+                 : "memory");
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::2.sync.aligned;" ::: "memory");
+  }
+  tcgen05_fence_before();
+  __syncthreads();
+  cluster_sync_all();                              // the peer's barriers exist before anything arrives on them
+  tcgen05_fence_after();
+  const uint32_t tmem_base = *tmem_ptr_smem;
+
+  // this CTA's stack group of a task (the last pair of an odd number of groups: the peer repeats the last group and
+  // writes nothing)
+  auto my_group = [&](int gp, bool* live_grp) {
+    int g = 2 * gp + (int)rank;
+    *live_grp = g < n_grp;
+    return g < n_grp ? g : n_grp - 1;
+  };
+
+  if (warp == 0) {
+    // ===================== producer (both CTAs): own W tiles, own half of the columns =====================
+    if (lane == 0) {
+      uint32_t n_a = 0, n_b = 0;
+      for (long long task = pair; task < n_tasks; task += n_pairs) {
+        int M, gp;
+        task_decode(task, n_mol, n_gp, &M, &gp);
+        bool live_grp;
+        const int s0 = my_group(gp, &live_grp) * C::kSPT;
+        const int n_st = n_s - s0 < C::kSPT ? n_s - s0 : C::kSPT;
+        const int a0 = __ldg(mol_off + M), n = __ldg(mol_off + M + 1) - a0;
+        const int ncol = 3 * n, npad = (ncol + 15) / 16 * 16;
+        const size_t row_m = (size_t)__ldg(xoff + M);
+        for (int c0 = 0; c0 < npad; c0 += C::kNMax) {
+          const int nc = npad - c0 < C::kNMax ? npad - c0 : C::kNMax;
+          const int nh = nc >> 1;                                        // this CTA's columns: [c0 + rank nh, + nh)
+          int e_prev = -1;
+          for (int I = 0; I < n; ++I) {
+            const int e = __ldg(elem + a0 + I);
+            if (e != e_prev) {
+              const __half* w = W16 + ((size_t)e * n_s + s0) * (size_t)(C::kTPS * C::kKB) * (kTile * kKBlk);
+#pragma unroll 1
+              for (int kb = 0; kb < C::kKB; ++kb) {
+                if (n_a > 0) mbar_wait(&a_empty[kb], (n_a - 1) & 1);
+                mbar_expect_tx(&a_full[kb], (uint32_t)(n_st * C::kTPS) * kTileBytes);
+                for (int t = 0; t < n_st * C::kTPS; ++t)
+                  bulk_copy_g2s(a_smem + (t * C::kKB + kb) * kTileBytes,
+                                w + (size_t)(t * C::kKB + kb) * (kTile * kKBlk), kTileBytes, &a_full[kb]);
+              }
+              ++n_a;
+              e_prev = e;
+            }
+            for (int kb = 0; kb < C::kKB; ++kb, ++n_b) {
+              const uint32_t st = n_b % C::kStages2, use = n_b / C::kStages2;
+              if (use > 0) mbar_wait(&b_empty[st], (use - 1) & 1);
+              const uint32_t bytes = (uint32_t)nh * 128;
+              mbar_expect_tx(&b_full[st], 2 * bytes);
+              const size_t row = row_m + ((size_t)I * C::kKB + kb) * npad + c0 + (size_t)rank * nh;
+              uint8_t* dst = b_smem + st * C::kStageBytes2;
+              bulk_copy_g2s(dst, Xh + row * 64, bytes, &b_full[st]);
+              bulk_copy_g2s(dst + (C::kNMax / 2) * 128, Xl + row * 64, bytes, &b_full[st]);
+            }
+          }
+        }
+      }
+    }
+  } else if (warp == 1) {
+    // ===================== MMA warp: the leader issues for the pair, the peer forwards its "full" barriers ==========
+    const bool leader_lane = elect_one_sync();
+    const uint32_t tmem_base_u = __shfl_sync(0xffffffffu, tmem_base, 0);
+    const uint32_t rank_u = __shfl_sync(0xffffffffu, rank, 0);
+    uint64_t a_desc[C::kMT][C::kKB], b_desc[C::kStages2];
+#pragma unroll
+    for (int t = 0; t < C::kMT; ++t)
+#pragma unroll
+      for (int kb = 0; kb < C::kKB; ++kb)
+        a_desc[t][kb] = make_kmajor_sw128_desc(smem_u32(a_smem + (t * C::kKB + kb) * kTileBytes));
+#pragma unroll
+    for (int st = 0; st < C::kStages2; ++st) b_desc[st] = make_kmajor_sw128_desc(smem_u32(b_smem + st * C::kStageBytes2));
+    constexpr uint64_t kLoOff = (uint64_t)(((C::kNMax / 2) * 128) >> 4);
+    uint32_t n_a = 0, n_b = 0, n_t = 0;
+    for (long long task = pair; task < n_tasks; task += n_pairs) {
+      int M, gp;
+      task_decode(task, n_mol, n_gp, &M, &gp);
+      // tiles of the LEADER's group (2 gp): it always has at least as many stacks as the peer's
+      const int s0l = 2 * gp * C::kSPT;
+      const int n_tiles = (n_s - s0l < C::kSPT ? n_s - s0l : C::kSPT) * C::kTPS;
+      const int a0 = __shfl_sync(0xffffffffu, __ldg(mol_off + M), 0);
+      const int n = __shfl_sync(0xffffffffu, __ldg(mol_off + M + 1), 0) - a0;
+      const int ncol = 3 * n, npad = (ncol + 15) / 16 * 16;
+      for (int c0 = 0; c0 < npad; c0 += C::kNMax) {
+        const int nc = npad - c0 < C::kNMax ? npad - c0 : C::kNMax;
+        // D fp32, A/B fp16, both K-major, N = nc (both halves), M = 256 (both CTAs)
+        const uint32_t idesc = (1u << 4) | ((uint32_t)(nc >> 3) << 17) | ((uint32_t)((2 * kTile) >> 4) << 24);
+        int e_prev = -1;
+        int e_next = __shfl_sync(0xffffffffu, __ldg(elem + a0), 0);
+        for (int I = 0; I < n; ++I, ++n_t) {
+          const int e = e_next;
+          e_next = (I + 1 < n) ? __shfl_sync(0xffffffffu, __ldg(elem + a0 + I + 1), 0) : -1;
+          const bool first_of_run = e != e_prev;
+          if (first_of_run) { ++n_a; e_prev = e; }
+          const bool last_of_run = e_next != e;
+          const uint32_t tb = n_t % C::kTBuf, tuse = n_t / C::kTBuf;
+          if (rank_u == 0) {
+            if (tuse > 0) mbar_wait(&t_empty[tb], (tuse - 1) & 1);
+            tcgen05_fence_after();
+          }
+          const uint32_t tmem_atom = tmem_base_u + tb * (C::kMT * C::kNMax);
+#pragma unroll
+          for (int kb = 0; kb < C::kKB; ++kb, ++n_b) {
+            const uint32_t st = n_b % C::kStages2;
+            if (first_of_run) mbar_wait(&a_full[kb], (n_a - 1) & 1);
+            mbar_wait(&b_full[st], (n_b / C::kStages2) & 1);
+            if (rank_u != 0) {
+              // peer: this k-block of W and this half stage are in my shared memory -- tell the leader
+              if (leader_lane) {
+                if (first_of_run) mbar_arrive_remote(&pa_full[kb], 0);
+                mbar_arrive_remote(&pb_full[st], 0);
+              }
+              __syncwarp();
+              continue;
+            }
+            if (first_of_run) mbar_wait(&pa_full[kb], (n_a - 1) & 1);
+            mbar_wait(&pb_full[st], (n_b / C::kStages2) & 1);
+            tcgen05_fence_after();
+            uint64_t b_hi = b_desc[0];
+#pragma unroll
+            for (int q = 1; q < C::kStages2; ++q) b_hi = (st == (uint32_t)q) ? b_desc[q] : b_hi;
+            if (leader_lane) {
+#pragma unroll
+              for (int kk = 0; kk < kKBlk / 16; ++kk) {
+                const uint64_t adv = (uint64_t)((kk * 32) >> 4);
+#pragma unroll
+                for (int t = 0; t < C::kMT; ++t)
+                  if (t < n_tiles)
+                    umma2<true>(tmem_atom + t * C::kNMax, a_desc[t][kb] + adv, b_hi + kLoOff + adv, idesc,
+                                (kb > 0 || kk > 0) ? 1u : 0u);   // small term first
+#pragma unroll
+                for (int t = 0; t < C::kMT; ++t)
+                  if (t < n_tiles) umma2<true>(tmem_atom + t * C::kNMax, a_desc[t][kb] + adv, b_hi + adv, idesc, 1u);
+              }
+              tcgen05_commit2(&b_empty[st]);                      // both producers may refill this stage
+              if (last_of_run) tcgen05_commit2(&a_empty[kb]);     // both producers may replace this k-block of W
+            }
+            __syncwarp();
+          }
+          if (rank_u == 0 && leader_lane) tcgen05_commit2(&t_full[tb]);   // accumulators of both CTAs complete
+          __syncwarp();
+        }
+      }
+    }
+  } else {
+    // ===================== epilogue warps (both CTAs): thread = output feature of this CTA's stacks =====================
+    const int quarter = warp & 3;
+    const int half = (warp - 2) >> 2;
+    const int row = quarter * 32 + lane;
+    using ZS = Shape<(D_ < kMaxE ? D_ : kMaxE), (D_ < kMaxE ? 1 : D_ / kMaxE)>;
+    constexpr int E = ZS::E, P = ZS::P, SPW = ZS::SPW, E4 = ZS::E4;
+    const size_t zs_atom = (size_t)n_sg * E * kWarp;
+    uint32_t n_t = 0;
+    for (long long task = pair; task < n_tasks; task += n_pairs) {
+      int M, gp;
+      task_decode(task, n_mol, n_gp, &M, &gp);
+      bool live_grp;
+      const int s0 = my_group(gp, &live_grp) * C::kSPT;
+      const int a0 = __ldg(mol_off + M), n = __ldg(mol_off + M + 1) - a0;
+      const int ncol = 3 * n, npad = (ncol + 15) / 16 * 16;
+      size_t zs_idx[C::kTPW];
+      bool live[C::kTPW];
+      int feat[C::kTPW];
+#pragma unroll
+      for (int w = 0; w < C::kTPW; ++w) {
+        const int t = half * C::kTPW + w;
+        const int s = s0 + t / C::kTPS, m = (t % C::kTPS) * kTile + row;
+        live[w] = live_grp && s < n_s;
+        const int sc = s < n_s ? s : n_s - 1;
+        const int zp = m / E, zj = m % E;
+        zs_idx[w] = ((((size_t)(sc / SPW)) * E4 + zj / 4) * kWarp + (sc % SPW) * P + zp) * 4 + (zj & 3);
+        feat[w] = sc * C::d + m;
+      }
+      for (int c0 = 0; c0 < npad; c0 += C::kNMax) {
+        const int nc = npad - c0 < C::kNMax ? npad - c0 : C::kNMax;
+        float acc[C::kTPW][C::kNMax];
+#pragma unroll
+        for (int w = 0; w < C::kTPW; ++w)
+#pragma unroll
+          for (int r = 0; r < C::kNMax; ++r) acc[w][r] = 0.f;
+        float f_next[C::kTPW];
+#pragma unroll
+        for (int w = 0; w < C::kTPW; ++w)
+          f_next[w] = c * __ldg(inv_scale + a0) * __ldg(zs + (size_t)a0 * zs_atom + zs_idx[w]);
+        for (int I = 0; I < n; ++I, ++n_t) {
+          float f[C::kTPW];
+#pragma unroll
+          for (int w = 0; w < C::kTPW; ++w) {
+            f[w] = f_next[w];
+            if (I + 1 < n)
+              f_next[w] = c * __ldg(inv_scale + a0 + I + 1) * __ldg(zs + (size_t)(a0 + I + 1) * zs_atom + zs_idx[w]);
+          }
+          const uint32_t tb = n_t % C::kTBuf;
+          mbar_wait(&t_full[tb], (n_t / C::kTBuf) & 1);
+          tcgen05_fence_after();
+#pragma unroll
+          for (int w = 0; w < C::kTPW; ++w) {
+            const uint32_t taddr = tmem_base + ((uint32_t)(quarter * 32) << 16) + tb * (C::kMT * C::kNMax) +
+                                   (half * C::kTPW + w) * C::kNMax;
+            if (live[w]) {
+#pragma unroll
+              for (int r0 = 0; r0 < C::kNMax; r0 += 32) {
+                if (r0 + 32 <= nc) {
+                  uint32_t u[32];
+                  tmem_ld_32x32b_x32(taddr + r0, u);
+                  tmem_ld_wait();
+#pragma unroll
+                  for (int r = 0; r < 32; ++r) acc[w][r0 + r] = fmaf(f[w], __uint_as_float(u[r]), acc[w][r0 + r]);
+                } else if (r0 < nc) {
+                  uint32_t u[16];
+                  tmem_ld_32x32b_x16(taddr + r0, u);
+                  tmem_ld_wait();
+#pragma unroll
+                  for (int r = 0; r < 16; ++r) acc[w][r0 + r] = fmaf(f[w], __uint_as_float(u[r]), acc[w][r0 + r]);
+                }
+              }
+            }
+          }
+          tcgen05_fence_before();
+          __syncwarp();
+          if (lane == 0) {                       // the leader's MMA warp waits for the epilogues of both CTAs
+            if (rank == 0) mbar_arrive(&t_empty[tb]); else mbar_arrive_remote(&t_empty[tb], 0);
+          }
+        }
+#pragma unroll
+        for (int w = 0; w < C::kTPW; ++w) {
+          if (!live[w]) continue;
+          float* dst = G + ((size_t)3 * a0 + c0) * (size_t)(n_s * C::d) + feat[w];
+#pragma unroll
+          for (int r = 0; r < C::kNMax; ++r)
+            if (r < nc && c0 + r < ncol) dst[(size_t)r * (n_s * C::d)] = acc[w][r];
+        }
+      }
+    }
+  }
+
+  tcgen05_fence_before();
+  __syncthreads();
+  cluster_sync_all();                              // nobody leaves while the peer may still touch its memory
+  if (warp == 2) {
+    tcgen05_fence_after();
+    asm volatile("tcgen05.dealloc.cta_group::2.sync.aligned.b32 %0, 512;" ::"r"(tmem_base) : "memory");
+  }
+}
+
+// ---------------------------------------------------------------------------------------------------
 // Host side
 // ---------------------------------------------------------------------------------------------------
 int sorf_mma_build_w(const qmll_sorf_params* p, const SorfTables& t, void* W16, cudaStream_t st) {
@@ -497,7 +802,7 @@ size_t sorf_mma_x_bytes(const qmll_sorf_params* p, int64_t n_atoms, int64_t dens
 template <int D_>
 static int launch_rows_mma(const SorfProblem& pr, const SorfTables& t, const float* zs, const qmll_grad* grad,
                            __half* W16, __half* Xh, __half* Xl, long long* xoff, float* inv_scale, float* G,
-                           cudaStream_t st) {
+                           cudaStream_t st, bool pairs) {
   using S = Shape<shape_E(D_), shape_P(D_)>;
   using C = MmaCfg<D_>;
   const qmll_sorf_params* p = pr.p;
@@ -511,11 +816,24 @@ static int launch_rows_mma(const SorfProblem& pr, const SorfTables& t, const flo
   prep_columns_kernel<<<(unsigned)pr.n_atoms, 256, 0, st>>>(grad->dense, grad->dense_off, pr.mol_off, pr.n_mol, p->d,
                                                            xoff, Xh, Xl, inv_scale);
   QMLL_LAUNCH_CHECK("prep_columns_kernel");
+  const float c = (float)(sqrt((double)p->d) / (double)p->sigma * pow((double)p->d, -0.5 * p->n_transform));
+  const int n_grp = (n_s + C::kSPT - 1) / C::kSPT;
+  if (pairs) {
+    using C2 = Mma2Cfg<D_>;
+    auto kern = sorf_rows_mma2_kernel<D_>;
+    QMLL_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C2::kSmem2));
+    const long long n_tasks = (long long)pr.n_mol * ((n_grp + 1) / 2);
+    const int max_pairs = device_sm_count() / 2;
+    const int n_pairs = (int)(n_tasks < max_pairs ? n_tasks : max_pairs);
+    kern<<<2 * n_pairs, C::kThreads, C2::kSmem2, st>>>(pr.elem, pr.mol_off, pr.n_mol, n_s, n_sg, c, W16, Xh, Xl, xoff,
+                                                       inv_scale, zs, G);
+    QMLL_LAUNCH_CHECK("sorf_rows_mma2_kernel");
+    return QMLL_OK;
+  }
   auto kern = sorf_rows_mma_kernel<D_>;
   QMLL_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::kSmem));
-  const long long n_tasks = (long long)pr.n_mol * ((n_s + C::kSPT - 1) / C::kSPT);
+  const long long n_tasks = (long long)pr.n_mol * n_grp;
   const int grid = (int)(n_tasks < device_sm_count() ? n_tasks : device_sm_count());
-  const float c = (float)(sqrt((double)p->d) / (double)p->sigma * pow((double)p->d, -0.5 * p->n_transform));
   kern<<<grid, C::kThreads, C::kSmem, st>>>(pr.elem, pr.mol_off, pr.n_mol, n_s, n_sg, c, W16, Xh, Xl, xoff,
                                             inv_scale, zs, G);
   QMLL_LAUNCH_CHECK("sorf_rows_mma_kernel");
@@ -524,12 +842,12 @@ static int launch_rows_mma(const SorfProblem& pr, const SorfTables& t, const flo
 
 int sorf_force_rows_dense_mma(const SorfProblem& pr, const SorfTables& t, const float* zs, const qmll_grad* grad,
                               void* W16, void* Xh, void* Xl, long long* xoff, float* inv_scale, float* G,
-                              cudaStream_t st) {
+                              cudaStream_t st, bool pairs) {
   if (pr.n_atoms == 0 || pr.n_mol == 0) return QMLL_OK;
   if (pr.p->d == 128)
-    return launch_rows_mma<128>(pr, t, zs, grad, (__half*)W16, (__half*)Xh, (__half*)Xl, xoff, inv_scale, G, st);
+    return launch_rows_mma<128>(pr, t, zs, grad, (__half*)W16, (__half*)Xh, (__half*)Xl, xoff, inv_scale, G, st, pairs);
   if (pr.p->d == 256)
-    return launch_rows_mma<256>(pr, t, zs, grad, (__half*)W16, (__half*)Xh, (__half*)Xl, xoff, inv_scale, G, st);
+    return launch_rows_mma<256>(pr, t, zs, grad, (__half*)W16, (__half*)Xh, (__half*)Xl, xoff, inv_scale, G, st, pairs);
   return QMLL_ERR_UNSUPPORTED;
 }
 
