@@ -40,7 +40,7 @@ def parse():
     ap.add_argument("--no-configs", action="store_true", help="skip the per-config block (C2, C3, C5)")
     ap.add_argument("--only-config", default=None, choices=["c2", "c3", "c5", "fchl19_cell"],
                     help="run only this entry of the per-config block and print it (used for the ncu captures in profiles/)")
-    ap.add_argument("--force-rows", default="auto", choices=["auto", "fwht", "mma"],
+    ap.add_argument("--force-rows", default="auto", choices=["auto", "fwht", "mma", "mma2"],
                     help="how the force rows are computed (qmll_sorf_forward_mode); the bench line uses auto")
     return ap.parse_args()
 
@@ -250,7 +250,7 @@ def ours_arm(args):
     F = torch.empty((wi.n_atoms, 3), dtype=torch.float32, device=dev)
     reducer = qdist.NormalEquationsReducer(D, dev) if world > 1 else None
 
-    rows_mode = {"auto": pkg.ROWS_AUTO, "fwht": pkg.ROWS_FWHT, "mma": pkg.ROWS_MMA}[args.force_rows]
+    rows_mode = {"auto": pkg.ROWS_AUTO, "fwht": pkg.ROWS_FWHT, "mma": pkg.ROWS_MMA, "mma2": pkg.ROWS_MMA2}[args.force_rows]
 
     def step(tr, inf, ZtZ_, Zty_, E_, F_):
         pkg.qmll_sorf_forward(p, tr.x, tr.elem, tr.mol_off, tr.grad, Z=Z, G=G, force_rows_mode=rows_mode)

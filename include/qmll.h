@@ -92,7 +92,7 @@ int qmll_sorf_forward(const qmll_sorf_params* p, const float* x, const int32_t* 
  *                   fp16 hi + lo); d = 128 or 256 only, else QMLL_ERR_UNSUPPORTED.
  *   QMLL_ROWS_MMA2  the same product on CTA pairs (tcgen05 cta_group::2: an MMA spans two SMs, each holds its own stacks'
  *                   W and half of the gradient columns); same support as QMLL_ROWS_MMA.
- *   QMLL_ROWS_AUTO  MMA where supported, else FWHT (what qmll_sorf_forward does). */
+ *   QMLL_ROWS_AUTO  MMA2 where supported, else FWHT (what qmll_sorf_forward does). */
 enum { QMLL_ROWS_AUTO = 0, QMLL_ROWS_FWHT = 1, QMLL_ROWS_MMA = 2, QMLL_ROWS_MMA2 = 3 };
 int qmll_sorf_forward_mode(const qmll_sorf_params* p, const float* x, const int32_t* elem, const int32_t* mol_off,
                            int64_t n_atoms, int32_t n_mol, const qmll_grad* grad, float* Z, float* G,

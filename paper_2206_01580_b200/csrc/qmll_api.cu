@@ -187,7 +187,7 @@ int qmll_sorf_forward_mode(const qmll_sorf_params* p, const float* x, const int3
       float* inv_scale = ws.take<float>((size_t)n_atoms);
       if (!ws.fits()) return QMLL_ERR_WORKSPACE;
       rc = sorf_force_rows_dense_mma(pr, t, zs, grad, W16, Xh, Xl, xoff, inv_scale, G, st,
-                                     force_rows_mode == QMLL_ROWS_MMA2);
+                                     force_rows_mode != QMLL_ROWS_MMA);   // AUTO: CTA pairs
     } else if (grad->layout == QMLL_GRAD_DENSE) {
       float* gt = ws.take<float>((size_t)grad->dense_floats);
       if (!ws.fits()) return QMLL_ERR_WORKSPACE;

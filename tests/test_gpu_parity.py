@@ -49,7 +49,7 @@ def run_all(q, w, check_ne=True):
     Go = oracle.force_rows_w(w)
     modes = [pkg.ROWS_FWHT]
     if w.grad.layout == "dense" and w.model.d in (128, 256):
-        modes.append(pkg.ROWS_MMA)
+        modes += [pkg.ROWS_MMA, pkg.ROWS_MMA2]
     for mode in modes + [pkg.ROWS_AUTO]:
         Z2, G = pkg.qmll_sorf_forward(dp.params, dp.x, dp.elem, dp.mol_off, dp.grad, force_rows_mode=mode)
         assert rel(Z2.cpu().numpy(), Zo) <= TOL
@@ -100,6 +100,17 @@ def test_tiny_neighbor(q, d, D):
     run_all(q, w, check_ne=False)
 
 
+def test_force_rows_cta_pairs_one_stack_and_many_molecules(q):
+    """QMLL_ROWS_MMA2 edge cases: a single stack group (the peer CTA of every pair has nothing of its own), an odd
+    number of groups, more tasks than CTA pairs (persistent loop), a one-atom molecule."""
+    pkg, wio, torch = q
+    for d, D, counts in ((256, 256, [3, 1]), (128, 128 * 9, [6] * 40), (256, 256 * 5, [9] * 100 + [1])):
+        w = tiny_workload(seed=500 + D, d=d, D=D, T=3, sigma=np.sqrt(d) / 2, counts=counts, n_elem=3, grad="dense")
+        dp = wio.device_problem(w)
+        _, G = pkg.qmll_sorf_forward(dp.params, dp.x, dp.elem, dp.mol_off, dp.grad, force_rows_mode=pkg.ROWS_MMA2)
+        assert rel(G.cpu().numpy(), oracle.force_rows_w(w)) <= TOL, (d, D)
+
+
 def test_force_rows_mma_long_molecule_and_odd_stacks(q):
     """Tensor-core force rows: a molecule whose 3n columns need several column chunks (n = 50 > 42), mixed with small
     and empty ones, unsorted elements (a W reload per atom), stack counts that are not a multiple of the warp's."""
@@ -109,9 +120,12 @@ def test_force_rows_mma_long_molecule_and_odd_stacks(q):
                           grad="dense")
         dp = wio.device_problem(w)
         Go = oracle.force_rows_w(w)
-        for mode in (pkg.ROWS_MMA, pkg.ROWS_FWHT):
+        Gs = {}
+        for mode in (pkg.ROWS_MMA, pkg.ROWS_MMA2, pkg.ROWS_FWHT):
             _, G = pkg.qmll_sorf_forward(dp.params, dp.x, dp.elem, dp.mol_off, dp.grad, force_rows_mode=mode)
             assert rel(G.cpu().numpy(), Go) <= TOL, (d, mode)
+            Gs[mode] = G
+        assert torch.equal(Gs[pkg.ROWS_MMA], Gs[pkg.ROWS_MMA2])     # CTA pairs: the same MMAs in the same order
     w = tiny_workload(seed=9, d=64, D=128, T=3, sigma=2.0, counts=[2], grad="dense")
     dp = wio.device_problem(w)
     with pytest.raises(pkg.QmllError) as ei:                      # d = 64 has no tensor-core path
@@ -124,8 +138,9 @@ def test_force_rows_mma_fewer_transforms(q, T):
     pkg, wio, torch = q
     w = tiny_workload(seed=40 + T, d=128, D=1024, T=T, sigma=4.0, counts=[5, 9], n_elem=3, grad="dense")
     dp = wio.device_problem(w)
-    _, G = pkg.qmll_sorf_forward(dp.params, dp.x, dp.elem, dp.mol_off, dp.grad, force_rows_mode=pkg.ROWS_MMA)
-    assert rel(G.cpu().numpy(), oracle.force_rows_w(w)) <= TOL
+    for mode in (pkg.ROWS_MMA, pkg.ROWS_MMA2):
+        _, G = pkg.qmll_sorf_forward(dp.params, dp.x, dp.elem, dp.mol_off, dp.grad, force_rows_mode=mode)
+        assert rel(G.cpu().numpy(), oracle.force_rows_w(w)) <= TOL
 
 
 @pytest.mark.parametrize("rep,d,counts,n_elem", [(37, 16, [4, 0, 7, 1], 3), (384, 128, [21] * 6, 3), (431, 256, [27, 3, 40], 5),
