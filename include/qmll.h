@@ -121,8 +121,12 @@ int qmll_sorf_backward_forces(const qmll_sorf_params* p, const float* x, const i
  *                       exponent range and is undone exactly.  Entries smaller than 2^-38 of the largest entry of
  *                       their 128 x 128 block lose their low bits (irrelevant for the Frobenius-norm accuracy of
  *                       a Gram matrix; use QMLL_NE_SPLIT_TF32 if single tiny entries matter).
- *   QMLL_NE_SPLIT_TF32  hi/lo in TF32 (the 3xTF32 scheme): full fp32 exponent range, half the speed. */
-enum { QMLL_NE_SPLIT_F16 = 0, QMLL_NE_SPLIT_TF32 = 1 };
+ *   QMLL_NE_SPLIT_TF32  hi/lo in TF32 (the 3xTF32 scheme): full fp32 exponent range, half the speed.
+ *   QMLL_NE_SPLIT_F16_PAIRS  the arithmetic of QMLL_NE_SPLIT_F16, bit for bit, on CTA pairs (tcgen05 cta_group::2: a
+ *                       256 x 256 block of ZtZ per pair of SMs, each SM loads its own 128 rows of one operand and half
+ *                       of the other).  Same workspace.  Measured: 3 % faster at D = 8192, 9 % slower at D = 16384 (the
+ *                       kernel runs under the power cap either way), so it is not the default. */
+enum { QMLL_NE_SPLIT_F16 = 0, QMLL_NE_SPLIT_TF32 = 1, QMLL_NE_SPLIT_F16_PAIRS = 2 };
 int qmll_normal_equations(const float* A, const float* y, int64_t rows, int32_t D, int32_t accumulate,
                           float* ZtZ, float* Zty, void* workspace, size_t workspace_bytes, void* cuda_stream);
 int qmll_normal_equations_mode(const float* A, const float* y, int64_t rows, int32_t D, int32_t accumulate,

@@ -23,7 +23,7 @@ LIB_PATH = os.path.join(_HERE, "libqmll.so")
 QMLL_GRAD_DENSE, QMLL_GRAD_NEIGHBOR = 1, 2
 CALL_FORWARD, CALL_FORWARD_GRAD, CALL_BACKWARD_FORCES, CALL_NORMAL_EQUATIONS, CALL_PREDICT, CALL_SOLVE = range(6)
 
-NE_SPLIT_F16, NE_SPLIT_TF32 = 0, 1
+NE_SPLIT_F16, NE_SPLIT_TF32, NE_SPLIT_F16_PAIRS = 0, 1, 2
 ROWS_AUTO, ROWS_FWHT, ROWS_MMA, ROWS_MMA2 = 0, 1, 2, 3
 
 EXPORTS = ("qmll_solve", "qmll_sorf_forward", "qmll_sorf_forward_mode", "qmll_sorf_backward_forces", "qmll_normal_equations",

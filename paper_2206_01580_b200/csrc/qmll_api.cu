@@ -117,7 +117,9 @@ using namespace qmll;
 
 extern "C" {
 
-static bool valid_mode(int32_t mode) { return mode == QMLL_NE_SPLIT_F16 || mode == QMLL_NE_SPLIT_TF32; }
+static bool valid_mode(int32_t mode) {
+  return mode == QMLL_NE_SPLIT_F16 || mode == QMLL_NE_SPLIT_TF32 || mode == QMLL_NE_SPLIT_F16_PAIRS;
+}
 size_t qmll_normal_equations_min_workspace(int32_t D) { return D > 0 ? syrk_min_workspace(D, QMLL_NE_SPLIT_F16) : 0; }
 size_t qmll_normal_equations_min_workspace_mode(int32_t D, int32_t mode) {
   return (D > 0 && valid_mode(mode)) ? syrk_min_workspace(D, mode) : 0;

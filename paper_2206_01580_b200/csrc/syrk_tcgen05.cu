@@ -47,6 +47,11 @@ constexpr uint32_t kTileABytes = kBM * 128;                 // 128 features x 12
 constexpr uint32_t kTileBBytes = kBN * 128;                 // 32 KB
 constexpr uint32_t kStageBytes = 2 * kTileABytes + 2 * kTileBBytes;  // hi + lo of both operands: 96 KB
 constexpr uint32_t kSmemBytes = kStages * kStageBytes + 256 + 1024;  // + barriers + alignment slack
+// CTA pairs (cta_group::2): the pair computes a 256 x 256 block of C; each CTA holds its own 128 rows of the I operand
+// and HALF of the J operand (128 of the 256 columns), so a stage is 64 KB per CTA and three of them fit.
+constexpr int kStagesP = 3;
+constexpr uint32_t kStageBytesP = 4 * kTileABytes;
+constexpr uint32_t kSmemBytesP = kStagesP * kStageBytesP + 512 + 1024;
 
 template <bool F16>
 struct SplitMode {
@@ -228,39 +233,86 @@ __host__ __device__ inline void tile_decode(int tile, int n_ti, int n_tj, int* t
   *tj_out = r1 - 1; *ti_out = 0;  // not reached for tile < n_tiles
 }
 
-template <bool F16>
+// Pair tiles: (tj, tip) covers C rows [256 tj, +256) x cols [256 tip, +256), needed iff tip <= tj; same band order.
+__host__ __device__ inline int ptiles_in_row(int tj, int n_tip) { return tj + 1 < n_tip ? tj + 1 : n_tip; }
+__host__ __device__ inline void tile_decode2(int tile, int n_tip, int n_tj, int* tj_out, int* tip_out) {
+  int r0 = 0, r1 = 0;
+  for (r0 = 0; r0 < n_tj; r0 += kBandRows) {
+    r1 = r0 + kBandRows < n_tj ? r0 + kBandRows : n_tj;
+    int cnt = 0;
+    for (int tj = r0; tj < r1; ++tj) cnt += ptiles_in_row(tj, n_tip);
+    if (tile < cnt) break;
+    tile -= cnt;
+  }
+  for (int tip = 0; tip < n_tip; ++tip) {
+    const int lo = tip > r0 ? tip : r0;      // first tile row of the band that needs column pair tip
+    const int cnt = r1 - lo;
+    if (cnt <= 0) continue;
+    if (tile < cnt) { *tj_out = lo + tile; *tip_out = tip; return; }
+    tile -= cnt;
+  }
+  *tj_out = r1 - 1; *tip_out = 0;
+}
+
+// tile of this CTA: rows [256 tj, +256) x cols [128 ti, +128); pairs: ti = 2 tip + rank (ti >= n_ti: nothing stored)
+template <bool kPair>
+__device__ __forceinline__ void decode_my_tile(int tile, int n_ti, int n_tj, int rank, int* tj, int* ti) {
+  if constexpr (kPair) {
+    int tip;
+    tile_decode2(tile, (n_ti + 1) / 2, n_tj, tj, &tip);
+    *ti = 2 * tip + rank;
+  } else {
+    tile_decode(tile, n_ti, n_tj, tj, ti);
+  }
+}
+
+template <bool F16, bool kPair>
 __global__ void __launch_bounds__(kSyrkThreads, 1)
 syrk_tcgen05_kernel(const __grid_constant__ CUtensorMap map_hi, const __grid_constant__ CUtensorMap map_lo,
                     float* __restrict__ C, int D, int n_kb /* BK-row blocks in the panel */, int n_tiles,
                     int first_store, const float* __restrict__ inv_scale /* [n_chunks][n_cb], F16 only */, int n_cb) {
   using M = SplitMode<F16>;
+  static_assert(!kPair || F16, "CTA pairs: fp16 container only");
   constexpr int kb_per_chunk = kChunkRows / M::kBK;
+  constexpr int kSt = kPair ? kStagesP : kStages;
+  constexpr uint32_t kSB = kPair ? kStageBytesP : kStageBytes;
   extern __shared__ uint8_t smem_raw[];
   uint8_t* smem = reinterpret_cast<uint8_t*>(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
-  uint64_t* bars = reinterpret_cast<uint64_t*>(smem + kStages * kStageBytes);
-  uint64_t* full_bar = bars;                 // [kStages]  TMA -> MMA
-  uint64_t* empty_bar = bars + kStages;      // [kStages]  MMA -> TMA
-  uint64_t* tfull_bar = bars + 2 * kStages;  // [2]        MMA -> epilogue
-  uint64_t* tempty_bar = bars + 2 * kStages + 2;  // [2]   epilogue -> MMA
-  uint32_t* tmem_ptr_smem = reinterpret_cast<uint32_t*>(bars + 2 * kStages + 4);
+  uint64_t* bars = reinterpret_cast<uint64_t*>(smem + kSt * kSB);
+  uint64_t* full_bar = bars;                 // [kSt]  TMA -> MMA
+  uint64_t* empty_bar = bars + kSt;          // [kSt]  MMA -> TMA (pairs: multicast commit)
+  uint64_t* tfull_bar = bars + 2 * kSt;      // [2]    MMA -> epilogue (pairs: multicast commit)
+  uint64_t* tempty_bar = bars + 2 * kSt + 2; // [2]    epilogue -> MMA (pairs: the epilogues of both CTAs -> leader)
+  uint64_t* pfull_bar = bars + 2 * kSt + 4;  // [kSt]  pairs, leader: the peer's stage has landed
+  uint32_t* tmem_ptr_smem = reinterpret_cast<uint32_t*>(bars + 3 * kSt + 4);
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int n_ti = (D + kBM - 1) / kBM, n_tj = (D + kBN - 1) / kBN;
   const int n_chunks = (n_kb + kb_per_chunk - 1) / kb_per_chunk;
-
+  // work unit = CTA (single) or CTA pair; `rank` = position in the pair
+  const int rank = kPair ? (int)cluster_ctarank() : 0;
+  const int unit = kPair ? (int)(blockIdx.x >> 1) : (int)blockIdx.x;
+  const int n_units = kPair ? (int)(gridDim.x >> 1) : (int)gridDim.x;
   if (threadIdx.x == 0) {
-    for (int s = 0; s < kStages; ++s) { mbar_init(&full_bar[s], 1); mbar_init(&empty_bar[s], 1); }
-    for (int b = 0; b < 2; ++b) { mbar_init(&tfull_bar[b], 1); mbar_init(&tempty_bar[b], 8); }
+    for (int s = 0; s < kSt; ++s) { mbar_init(&full_bar[s], 1); mbar_init(&empty_bar[s], 1); mbar_init(&pfull_bar[s], 1); }
+    for (int b = 0; b < 2; ++b) { mbar_init(&tfull_bar[b], 1); mbar_init(&tempty_bar[b], kPair ? 16 : 8); }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
   }
   if (warp == 2) {  // TMEM: all 512 columns = two 128 x 256 fp32 accumulators
-    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], 512;" ::"r"(smem_u32(tmem_ptr_smem))
-                 : "memory");
-    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+    if constexpr (kPair) {
+      asm volatile("tcgen05.alloc.cta_group::2.sync.aligned.shared::cta.b32 [%0], 512;" ::"r"(smem_u32(tmem_ptr_smem))
+                   : "memory");
+      asm volatile("tcgen05.relinquish_alloc_permit.cta_group::2.sync.aligned;" ::: "memory");
+    } else {
+      asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], 512;" ::"r"(smem_u32(tmem_ptr_smem))
+                   : "memory");
+      asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+    }
   }
   tcgen05_fence_before();
   __syncthreads();
+  if constexpr (kPair) cluster_sync_all();   // the peer's barriers exist before anything arrives on them
   tcgen05_fence_after();
   const uint32_t tmem_base = *tmem_ptr_smem;
 
@@ -270,24 +322,29 @@ syrk_tcgen05_kernel(const __grid_constant__ CUtensorMap map_hi, const __grid_con
       asm volatile("prefetch.tensormap [%0];" ::"l"(&map_hi) : "memory");
       asm volatile("prefetch.tensormap [%0];" ::"l"(&map_lo) : "memory");
       uint32_t kbc = 0;  // running k-block counter -> stage / phase
-      for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
+      for (int tile = unit; tile < n_tiles; tile += n_units) {
         int tj, rem;
-        tile_decode(tile, n_ti, n_tj, &tj, &rem);
+        decode_my_tile<kPair>(tile, n_ti, n_tj, rank, &tj, &rem);
         const int I0 = rem * kBM, J0 = tj * kBN;
         for (int kb = 0; kb < n_kb; ++kb, ++kbc) {
-          const uint32_t s = kbc % kStages, ph = (kbc / kStages) & 1;
+          const uint32_t s = kbc % kSt, ph = (kbc / kSt) & 1;
           mbar_wait(&empty_bar[s], ph ^ 1);
-          uint8_t* st = smem + s * kStageBytes;
-          mbar_expect_tx(&full_bar[s], kStageBytes);
+          uint8_t* st = smem + s * kSB;
+          mbar_expect_tx(&full_bar[s], kSB);
           // tensor = [n_kb * D][BK]: box row index = kb * D + feature.  Features past D alias the next k-block
           // (finite values; those accumulator rows / columns are masked at the store), past the end TMA fills zeros.
           const int base = kb * D;
           tma_load_2d(st, &map_hi, &full_bar[s], 0, base + I0);
           tma_load_2d(st + kTileABytes, &map_lo, &full_bar[s], 0, base + I0);
-          tma_load_2d(st + 2 * kTileABytes, &map_hi, &full_bar[s], 0, base + J0);
-          tma_load_2d(st + 2 * kTileABytes + kTileABytes, &map_hi, &full_bar[s], 0, base + J0 + 128);
-          tma_load_2d(st + 2 * kTileABytes + kTileBBytes, &map_lo, &full_bar[s], 0, base + J0);
-          tma_load_2d(st + 2 * kTileABytes + kTileBBytes + kTileABytes, &map_lo, &full_bar[s], 0, base + J0 + 128);
+          if constexpr (kPair) {     // this CTA's half of the J operand
+            tma_load_2d(st + 2 * kTileABytes, &map_hi, &full_bar[s], 0, base + J0 + 128 * rank);
+            tma_load_2d(st + 3 * kTileABytes, &map_lo, &full_bar[s], 0, base + J0 + 128 * rank);
+          } else {
+            tma_load_2d(st + 2 * kTileABytes, &map_hi, &full_bar[s], 0, base + J0);
+            tma_load_2d(st + 2 * kTileABytes + kTileABytes, &map_hi, &full_bar[s], 0, base + J0 + 128);
+            tma_load_2d(st + 2 * kTileABytes + kTileBBytes, &map_lo, &full_bar[s], 0, base + J0);
+            tma_load_2d(st + 2 * kTileABytes + kTileBBytes + kTileABytes, &map_lo, &full_bar[s], 0, base + J0 + 128);
+          }
         }
       }
     }
@@ -299,37 +356,60 @@ syrk_tcgen05_kernel(const __grid_constant__ CUtensorMap map_hi, const __grid_con
     {
       const bool leader = elect_one_sync();
       const uint32_t tmem_base_u = __shfl_sync(0xffffffffu, tmem_base, 0);
+      const int rank_u = __shfl_sync(0xffffffffu, rank, 0);
+      // pairs: one MMA has M = 256 (the I tiles of both CTAs) and N = 256 (both halves of the J operand)
+      constexpr uint32_t kIdescP = (1u << 4) | (M::kFmt << 7) | (M::kFmt << 10) | ((uint32_t)(256 >> 3) << 17) |
+                                   ((uint32_t)(256 >> 4) << 24);
       uint32_t kbc = 0, item = 0;
-      for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
+      for (int tile = unit; tile < n_tiles; tile += n_units) {
         for (int ch = 0; ch < n_chunks; ++ch, ++item) {
           const uint32_t buf = item & 1, tph = (item >> 1) & 1;
-          mbar_wait(&tempty_bar[buf], tph ^ 1);  // epilogue has drained this accumulator
-          tcgen05_fence_after();
+          if (rank_u == 0) {
+            mbar_wait(&tempty_bar[buf], tph ^ 1);  // the epilogue(s) have drained this accumulator
+            tcgen05_fence_after();
+          }
           const uint32_t tmem_d = tmem_base_u + buf * kBN;
           const int kb_end = (ch + 1) * kb_per_chunk < n_kb ? (ch + 1) * kb_per_chunk : n_kb;
           for (int kb = ch * kb_per_chunk; kb < kb_end; ++kb, ++kbc) {
-            const uint32_t s = kbc % kStages, ph = (kbc / kStages) & 1;
+            const uint32_t s = kbc % kSt, ph = (kbc / kSt) & 1;
             mbar_wait(&full_bar[s], ph);
+            if constexpr (kPair) {
+              if (rank_u != 0) {           // peer: my half of the stage is in my shared memory -- tell the leader
+                if (leader) mbar_arrive_remote(&pfull_bar[s], 0);
+                __syncwarp();
+                continue;
+              }
+              mbar_wait(&pfull_bar[s], ph);
+            }
             tcgen05_fence_after();
-            const uint32_t base = smem_u32(smem + s * kStageBytes);
+            const uint32_t base = smem_u32(smem + s * kSB);
             const uint64_t a_hi = make_kmajor_sw128_desc(base);
             const uint64_t a_lo = make_kmajor_sw128_desc(base + kTileABytes);
             const uint64_t b_hi = make_kmajor_sw128_desc(base + 2 * kTileABytes);
-            const uint64_t b_lo = make_kmajor_sw128_desc(base + 2 * kTileABytes + kTileBBytes);
+            const uint64_t b_lo = make_kmajor_sw128_desc(base + 2 * kTileABytes + (kPair ? kTileABytes : kTileBBytes));
             if (leader) {
 #pragma unroll
               for (int kk = 0; kk < M::kBK / M::kUmmaK; ++kk) {
                 const uint64_t adv = (uint64_t)((kk * 32) >> 4);  // +32 bytes per K step, in 16 B units
                 const uint32_t acc0 = (kb > ch * kb_per_chunk || kk > 0) ? 1u : 0u;
-                umma<F16>(tmem_d, a_lo + adv, b_hi + adv, M::kIdesc, acc0);   // small terms first
-                umma<F16>(tmem_d, a_hi + adv, b_lo + adv, M::kIdesc, 1u);
-                umma<F16>(tmem_d, a_hi + adv, b_hi + adv, M::kIdesc, 1u);
+                if constexpr (kPair) {
+                  umma2<true>(tmem_d, a_lo + adv, b_hi + adv, kIdescP, acc0);   // small terms first
+                  umma2<true>(tmem_d, a_hi + adv, b_lo + adv, kIdescP, 1u);
+                  umma2<true>(tmem_d, a_hi + adv, b_hi + adv, kIdescP, 1u);
+                } else {
+                  umma<F16>(tmem_d, a_lo + adv, b_hi + adv, M::kIdesc, acc0);   // small terms first
+                  umma<F16>(tmem_d, a_hi + adv, b_lo + adv, M::kIdesc, 1u);
+                  umma<F16>(tmem_d, a_hi + adv, b_hi + adv, M::kIdesc, 1u);
+                }
               }
-              tcgen05_commit(&empty_bar[s]);  // smem stage reusable once these MMAs have read it
+              // smem stage reusable once these MMAs have read it (pairs: in both CTAs)
+              if constexpr (kPair) tcgen05_commit2(&empty_bar[s]); else tcgen05_commit(&empty_bar[s]);
             }
             __syncwarp();
           }
-          if (leader) tcgen05_commit(&tfull_bar[buf]);  // accumulator complete
+          if (leader && rank_u == 0) {   // accumulator(s) complete
+            if constexpr (kPair) tcgen05_commit2(&tfull_bar[buf]); else tcgen05_commit(&tfull_bar[buf]);
+          }
           __syncwarp();
         }
       }
@@ -343,9 +423,9 @@ syrk_tcgen05_kernel(const __grid_constant__ CUtensorMap map_hi, const __grid_con
     const int chalf = (warp - 2) >> 2;  // 0: columns [0,128), 1: columns [128,256)
     const int i_loc = quarter * 32 + lane;
     uint32_t item = 0;
-    for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
+    for (int tile = unit; tile < n_tiles; tile += n_units) {
       int tj, rem;
-      tile_decode(tile, n_ti, n_tj, &tj, &rem);
+      decode_my_tile<kPair>(tile, n_ti, n_tj, rank, &tj, &rem);
       const int I0 = rem * kBM, J0 = tj * kBN + chalf * 128;
       const int col = I0 + i_loc;  // column of C this thread writes (transposed store)
       const int cbI = rem, cbJ = 2 * tj + chalf;  // 128-column blocks of the two operands
@@ -355,7 +435,8 @@ syrk_tcgen05_kernel(const __grid_constant__ CUtensorMap map_hi, const __grid_con
       for (int ch = 0; ch < n_chunks; ++ch, ++item) {
         float f = 1.f;
         if constexpr (F16)
-          f = __ldg(inv_scale + (size_t)ch * n_cb + cbI) * (cbJ < n_cb ? __ldg(inv_scale + (size_t)ch * n_cb + cbJ) : 1.f);
+          f = (cbI < n_cb ? __ldg(inv_scale + (size_t)ch * n_cb + cbI) : 1.f) *
+              (cbJ < n_cb ? __ldg(inv_scale + (size_t)ch * n_cb + cbJ) : 1.f);
         const uint32_t buf = item & 1, tph = (item >> 1) & 1;
         mbar_wait(&tfull_bar[buf], tph);
         tcgen05_fence_after();
@@ -373,7 +454,9 @@ syrk_tcgen05_kernel(const __grid_constant__ CUtensorMap map_hi, const __grid_con
         }
         tcgen05_fence_before();  // all TMEM reads of this warp are done: hand the accumulator back
         __syncwarp();
-        if (lane == 0) mbar_arrive(&tempty_bar[buf]);
+        if (lane == 0) {
+          if (kPair && rank != 0) mbar_arrive_remote(&tempty_bar[buf], 0); else mbar_arrive(&tempty_bar[buf]);
+        }
       }
       if (col < D) {
         float* dst = C + (size_t)J0 * D + col;
@@ -391,9 +474,13 @@ syrk_tcgen05_kernel(const __grid_constant__ CUtensorMap map_hi, const __grid_con
 
   tcgen05_fence_before();
   __syncthreads();
+  if constexpr (kPair) cluster_sync_all();   // nobody leaves while the peer may still touch its memory
   if (warp == 2) {
     tcgen05_fence_after();
-    asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, 512;" ::"r"(tmem_base) : "memory");
+    if constexpr (kPair)
+      asm volatile("tcgen05.dealloc.cta_group::2.sync.aligned.b32 %0, 512;" ::"r"(tmem_base) : "memory");
+    else
+      asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, 512;" ::"r"(tmem_base) : "memory");
   }
 }
 
@@ -537,10 +624,10 @@ struct PanelLayout {
   size_t op_bytes, scale_bytes, part_bytes;
   size_t total() const { return 2 * op_bytes + scale_bytes + part_bytes + 4 * 256; }
 };
-static long long tile_rows(int mode) { return mode == QMLL_NE_SPLIT_F16 ? 128 : 64; }
+static long long tile_rows(int mode) { return mode != QMLL_NE_SPLIT_TF32 ? 128 : 64; }
 static long long pad_rows(long long r, int mode) { return (r + tile_rows(mode) - 1) / tile_rows(mode) * tile_rows(mode); }
 static PanelLayout panel_layout(long long rp, int D, int mode) {
-  const int eb = mode == QMLL_NE_SPLIT_F16 ? 2 : 4;
+  const int eb = mode != QMLL_NE_SPLIT_TF32 ? 2 : 4;
   const int n_cb = (D + kColBlock - 1) / kColBlock;
   PanelLayout l;
   l.op_bytes = align_up((size_t)D * rp * eb, 256);
@@ -556,7 +643,7 @@ size_t syrk_full_workspace(int64_t rows, int32_t D, int mode) {
   return panel_layout(rp, D, mode).total();
 }
 
-template <bool F16>
+template <bool F16, bool kPair>
 static int syrk_impl(const float* A, const float* y, int64_t rows, int32_t D, int accumulate, float* ZtZ, float* Zty,
                      void* ws, size_t ws_bytes, cudaStream_t st) {
   using M = SplitMode<F16>;
@@ -589,10 +676,12 @@ static int syrk_impl(const float* A, const float* y, int64_t rows, int32_t D, in
 
   const int n_ti = (D + kBM - 1) / kBM, n_tj = (D + kBN - 1) / kBN;
   int n_tiles = 0;
-  for (int tj = 0; tj < n_tj; ++tj) n_tiles += tiles_in_row(tj, n_ti);
-  const int grid = n_tiles < device_sm_count() ? n_tiles : device_sm_count();
-  QMLL_CUDA_TRY(cudaFuncSetAttribute(syrk_tcgen05_kernel<F16>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                     (int)kSmemBytes));
+  for (int tj = 0; tj < n_tj; ++tj) n_tiles += kPair ? ptiles_in_row(tj, (n_ti + 1) / 2) : tiles_in_row(tj, n_ti);
+  const int max_units = kPair ? device_sm_count() / 2 : device_sm_count();
+  const int grid = (n_tiles < max_units ? n_tiles : max_units) * (kPair ? 2 : 1);
+  constexpr uint32_t smem_bytes = kPair ? kSmemBytesP : kSmemBytes;
+  auto kern = syrk_tcgen05_kernel<F16, kPair>;
+  QMLL_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes));
   QMLL_CUDA_TRY(cudaFuncSetAttribute(split_kernel<F16>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSplitSmem));
   int first_store = accumulate ? 0 : 1;
   int zty_acc = accumulate ? 1 : 0;
@@ -625,8 +714,23 @@ static int syrk_impl(const float* A, const float* y, int64_t rows, int32_t D, in
         QMLL_CUDA_TRY(cudaEventRecord(g_timed[g_n_timed].a, st));
       }
     }
-    syrk_tcgen05_kernel<F16><<<grid, kSyrkThreads, kSmemBytes, st>>>(map_hi, map_lo, ZtZ, D, (int)n_kb, n_tiles,
-                                                                     first_store, inv_scale, n_cb);
+    {
+      cudaLaunchConfig_t cfg = {};
+      cfg.gridDim = dim3((unsigned)grid);
+      cfg.blockDim = dim3(kSyrkThreads);
+      cfg.dynamicSmemBytes = smem_bytes;
+      cfg.stream = st;
+      cudaLaunchAttribute attr[1];
+      attr[0].id = cudaLaunchAttributeClusterDimension;
+      attr[0].val.clusterDim.x = kPair ? 2 : 1;
+      attr[0].val.clusterDim.y = 1;
+      attr[0].val.clusterDim.z = 1;
+      cfg.attrs = attr;
+      cfg.numAttrs = 1;
+      const int n_kb_i = (int)n_kb;
+      const float* inv_c = inv_scale;
+      QMLL_CUDA_TRY(cudaLaunchKernelEx(&cfg, kern, map_hi, map_lo, ZtZ, (int)D, n_kb_i, n_tiles, first_store, inv_c, n_cb));
+    }
     QMLL_LAUNCH_CHECK("syrk_tcgen05_kernel");
     if (timed) {
       std::lock_guard<std::mutex> lock(g_timing_mutex);
@@ -649,8 +753,9 @@ int syrk_normal_equations(const float* A, const float* y, int64_t rows, int32_t 
   }
   if (rows == 0) return QMLL_OK;
   if (ws == nullptr || ((uintptr_t)ws & 255) != 0) return QMLL_ERR_WORKSPACE;
-  if (mode == QMLL_NE_SPLIT_F16) return syrk_impl<true>(A, y, rows, D, accumulate, ZtZ, Zty, ws, ws_bytes, st);
-  return syrk_impl<false>(A, y, rows, D, accumulate, ZtZ, Zty, ws, ws_bytes, st);
+  if (mode == QMLL_NE_SPLIT_F16) return syrk_impl<true, false>(A, y, rows, D, accumulate, ZtZ, Zty, ws, ws_bytes, st);
+  if (mode == QMLL_NE_SPLIT_F16_PAIRS) return syrk_impl<true, true>(A, y, rows, D, accumulate, ZtZ, Zty, ws, ws_bytes, st);
+  return syrk_impl<false, false>(A, y, rows, D, accumulate, ZtZ, Zty, ws, ws_bytes, st);
 }
 
 }  // namespace qmll

@@ -206,7 +206,7 @@ def test_empty_inputs(q):
     assert float(E.abs().max()) == 0.0
 
 
-@pytest.mark.parametrize("mode", [0, 1])      # QMLL_NE_SPLIT_F16, QMLL_NE_SPLIT_TF32
+@pytest.mark.parametrize("mode", [0, 1, 2])   # QMLL_NE_SPLIT_F16, QMLL_NE_SPLIT_TF32, QMLL_NE_SPLIT_F16_PAIRS
 @pytest.mark.parametrize("rows,D", [(1, 256), (777, 384), (1500, 128), (2500, 520), (4096, 1024), (300, 451), (130, 7)])
 def test_normal_equations_shapes(q, rows, D, mode):
     pkg, wio, torch = q
@@ -229,6 +229,19 @@ def test_normal_equations_shapes(q, rows, D, mode):
     assert rel(Zn, ZtZo + ZtZo2) <= TOL
     assert rel(Zty.cpu().numpy(), Ztyo + Ztyo2) <= TOL
     assert np.array_equal(Zn, Zn.T)
+
+
+def test_normal_equations_cta_pairs_are_bit_identical(q):
+    """QMLL_NE_SPLIT_F16_PAIRS issues the same MMAs in the same order on cta_group::2: identical bits, also across
+    several row panels and an odd number of 128-column tiles (the last pair has a CTA without a tile)."""
+    pkg, wio, torch = q
+    torch.manual_seed(4)
+    for rows, D in ((3000, 384), (70000, 640), (900, 2176)):
+        A = (0.3 + torch.randn((rows, D), device="cuda")).contiguous()
+        y = torch.randn((rows,), device="cuda")
+        Z1, t1 = pkg.qmll_normal_equations(A, y, mode=pkg.NE_SPLIT_F16)
+        Z2, t2 = pkg.qmll_normal_equations(A, y, mode=pkg.NE_SPLIT_F16_PAIRS)
+        assert torch.equal(Z1, Z2) and torch.equal(t1, t2), (rows, D)
 
 
 def test_normal_equations_wide_dynamic_range(q):
