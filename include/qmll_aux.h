@@ -30,6 +30,12 @@ int qmll_collect_normal_equations_kernel_ms(double* total_ms, int* launches);
 int qmll_microbench(int kind, int iters, int blocks_per_sm, void* workspace, size_t workspace_bytes,
                     double* ops_per_launch, int* n_blocks, void* cuda_stream);
 
+/* Timing of tcgen05.mma itself: M = 128, kind::f16, both operands in shared memory, one CTA per SM; `iters` x 4 x
+ * `accumulators` MMAs of width n (64, 96, 128 or 256) rotating over `accumulators` (1, 2 or 4; 1 or 2 for n = 256) TMEM
+ * accumulators, issued back to back by one elected lane.  workspace (device, >= 8 bytes): int64 clock64 ticks of block 0
+ * from the first issue to completion.  Behind the "max(n/2, 32 + n/4) clocks per MMA" law of DESIGN.md section 5.2. */
+int qmll_microbench_mma(int n, int accumulators, int iters, void* workspace, size_t workspace_bytes, void* cuda_stream);
+
 #ifdef __cplusplus
 }
 #endif

@@ -30,7 +30,7 @@ EXPORTS = ("qmll_solve", "qmll_sorf_forward", "qmll_sorf_forward_mode", "qmll_so
            "qmll_normal_equations_mode", "qmll_predict", "qmll_workspace_bytes", "qmll_normal_equations_min_workspace",
            "qmll_normal_equations_workspace", "qmll_normal_equations_min_workspace_mode", "qmll_status_string",
            "qmll_launch_count", "qmll_reset_launch_count", "qmll_time_normal_equations_kernel",
-           "qmll_collect_normal_equations_kernel_ms", "qmll_microbench", "qmll_pack_lower", "qmll_unpack_lower", "qmll_project",
+           "qmll_collect_normal_equations_kernel_ms", "qmll_microbench", "qmll_microbench_mma", "qmll_pack_lower", "qmll_unpack_lower", "qmll_project",
            "qmll_project_neighbor", "qmll_fchl19", "qmll_fchl19_rep_size", "qmll_sorf_forward_mma", "qmll_rff_forward",
            "qmll_featmap_workspace_bytes", "qmll_sorf_backward_g", "qmll_project_back", "qmll_fchl19_backward")
 

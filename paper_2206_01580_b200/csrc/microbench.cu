@@ -7,6 +7,7 @@
 #include <stdint.h>
 
 #include "qmll_common.cuh"
+#include "tcgen05_utils.cuh"
 
 namespace qmll {
 
@@ -168,9 +169,78 @@ static int mb_launch(float* out, int iters, unsigned long long* cyc, int blocks,
 
 int device_sm_count();
 
+// ---- tcgen05.mma issue / operand timing: M = 128, kind::f16, both operands in shared memory, one CTA per SM; an elected
+// lane issues `iters` x 4 x R MMAs of width N rotating over R accumulators, then commits and waits.  out[0] = clock64
+// ticks of block 0 from the first issue to completion.
+template <int N, int R>
+__global__ void __launch_bounds__(128, 1) mma_clock_kernel(long long* out, int iters) {
+  extern __shared__ uint8_t mb_smem_raw[];
+  uint8_t* sm = reinterpret_cast<uint8_t*>(((uintptr_t)mb_smem_raw + 1023) & ~(uintptr_t)1023);
+  __shared__ uint64_t bar;
+  __shared__ uint32_t tptr;
+  for (int i = threadIdx.x; i < (64 * 1024) / 4; i += 128) reinterpret_cast<uint32_t*>(sm)[i] = 0;
+  if (threadIdx.x == 0) { mbar_init(&bar, 1); fence_mbarrier_init(); }
+  if (threadIdx.x < 32) {
+    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], 512;" ::"r"(smem_u32(&tptr)) : "memory");
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+  }
+  asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+  tcgen05_fence_before();
+  __syncthreads();
+  tcgen05_fence_after();
+  const uint32_t tb = tptr;
+  if (threadIdx.x < 32) {
+    const bool leader = elect_one_sync();
+    const uint32_t tbu = __shfl_sync(0xffffffffu, tb, 0);
+    const uint64_t a = make_kmajor_sw128_desc(smem_u32(sm)), b = make_kmajor_sw128_desc(smem_u32(sm + 16384));
+    constexpr uint32_t idesc = (1u << 4) | ((uint32_t)(N >> 3) << 17) | ((uint32_t)(128 >> 4) << 24);
+    const long long t0 = clock64();
+    if (leader) {
+      for (int it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int kk = 0; kk < 4; ++kk)
+#pragma unroll
+          for (int r = 0; r < R; ++r) umma<true>(tbu + r * N, a + 2 * kk, b + 2 * kk, idesc, 1u);
+      }
+      tcgen05_commit(&bar);
+    }
+    __syncwarp();
+    mbar_wait(&bar, 0);
+    const long long t1 = clock64();
+    if (threadIdx.x == 0 && blockIdx.x == 0) out[0] = t1 - t0;
+  }
+  tcgen05_fence_before();
+  __syncthreads();
+  if (threadIdx.x < 32) {
+    tcgen05_fence_after();
+    asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, 512;" ::"r"(tb) : "memory");
+  }
+}
+
+template <int N, int R>
+static int mma_clock_launch(long long* out, int iters, cudaStream_t st) {
+  auto kern = mma_clock_kernel<N, R>;
+  QMLL_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 70 * 1024));
+  kern<<<device_sm_count(), 128, 70 * 1024, st>>>(out, iters);
+  QMLL_LAUNCH_CHECK("mma_clock_kernel");
+  return QMLL_OK;
+}
+
 }  // namespace qmll
 
 using namespace qmll;
+
+extern "C" int qmll_microbench_mma(int n, int accumulators, int iters, void* workspace, size_t workspace_bytes,
+                                   void* cuda_stream) {
+  if (iters < 1 || !workspace || workspace_bytes < 8) return QMLL_ERR_INVALID_ARG;
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  long long* out = static_cast<long long*>(workspace);
+#define QMLL_MB(N_, R_) if (n == N_ && accumulators == R_) return mma_clock_launch<N_, R_>(out, iters, st);
+  QMLL_MB(64, 1) QMLL_MB(64, 2) QMLL_MB(64, 4) QMLL_MB(96, 1) QMLL_MB(96, 2) QMLL_MB(96, 4)
+  QMLL_MB(128, 1) QMLL_MB(128, 2) QMLL_MB(128, 4) QMLL_MB(256, 1) QMLL_MB(256, 2)
+#undef QMLL_MB
+  return QMLL_ERR_UNSUPPORTED;
+}
 
 extern "C" int qmll_microbench(int kind, int iters, int blocks_per_sm, void* workspace, size_t workspace_bytes,
                                double* ops_per_launch, int* n_blocks, void* cuda_stream) {

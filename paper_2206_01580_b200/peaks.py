@@ -96,6 +96,27 @@ def tf32_gemm(n: int = 8192, sustained_s: float = 4.0) -> dict:
             "how": f"torch.matmul fp32 with allow_tf32, {n}^3: best of 10 (burst) and back to back for {sustained_s} s"}
 
 
+def mma_clocks(iters: int = 512) -> dict:
+    """Clocks per tcgen05.mma (M 128, kind::f16, operands in shared memory) for several widths and accumulator counts."""
+    lib = load_library()
+    lib.qmll_microbench_mma.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_void_p, ctypes.c_size_t,
+                                        ctypes.c_void_p]
+    lib.qmll_microbench_mma.restype = ctypes.c_int
+    ws = torch.zeros(1, dtype=torch.int64, device="cuda")
+    stream = ctypes.c_void_p(torch.cuda.current_stream().cuda_stream)
+    out = {}
+    for n, accs in ((64, (1, 2, 4)), (96, (1, 2, 4)), (128, (1, 2, 4)), (256, (1, 2))):
+        for r in accs:
+            for _ in range(2):
+                rc = lib.qmll_microbench_mma(n, r, iters, ctypes.c_void_p(ws.data_ptr()), 8, stream)
+                if rc != 0:
+                    raise RuntimeError(f"qmll_microbench_mma({n}, {r}) -> {rc}")
+                torch.cuda.synchronize()
+            out[f"N{n}_acc{r}"] = {"clocks_per_mma": ws.item() / (iters * 4.0 * r), "work_clocks": n / 2}
+    out["how"] = "clock64 ticks of one CTA per SM issuing back to back; work_clocks = 128 * N / 256 (tensor-core floor)"
+    return out
+
+
 def main() -> None:
     props = torch.cuda.get_device_properties(0)
     out = {"gpu_name": props.name, "sm_count": props.multi_processor_count, "torch": torch.__version__,
@@ -104,6 +125,7 @@ def main() -> None:
     for k in sorted(KINDS):
         out["alu"][str(k)] = microbench(k)
     out["tensor"] = tf32_gemm()
+    out["mma_clocks"] = mma_clocks()
     json.dump(out, sys.stdout, indent=1)
     print()
 
