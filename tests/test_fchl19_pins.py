@@ -365,3 +365,44 @@ def test_backward_chain_equals_jacobian_chain_and_finite_differences():
                 F_jac[j] -= gx[a] @ dx[s]
     np.testing.assert_allclose(F_back, F_jac, rtol=1e-10, atol=1e-12 * np.abs(F_jac).max())
     assert np.abs(F_back.sum(0)).max() < 1e-10 * np.abs(F_back).max()       # no net force (translation invariance)
+
+
+def test_table_1_parameters_are_the_papers():
+    """tests/golden/fchl19_table1.json holds Table I as the paper prints it (L248-260); the generator's defaults, its
+    energy-only set and the binding's defaults must be those numbers."""
+    import json
+    import os
+    with open(os.path.join(os.path.dirname(__file__), "golden", "fchl19_table1.json")) as f:
+        tab = json.load(f)
+    from workloads import FCHL_E
+    ef, e = FchlParams(), replace(FchlParams(), **FCHL_E)
+    for got, want in ((ef, tab["E+F"]), (e, tab["E"])):
+        for k, v in want.items():
+            assert getattr(got, k) == pytest.approx(v, rel=0, abs=1e-15), k
+    import paper_2206_01580_b200 as pkg
+    b = pkg.Fchl19Params()
+    w = tab["E+F"]
+    assert (b.n2, b.n3, b.eta2, b.eta3, b.two_body_decay, b.three_body_decay, b.three_body_weight, b.r_cut) == \
+        (w["n2"], w["n3"], w["eta2"], w["eta3"], w["N2"], w["N3"], w["c3"], w["r_cut"])
+    assert b.zeta == pytest.approx(np.pi)
+
+
+def test_fchl19_golden_regression():
+    """tests/golden/fchl19_oracle.json was written by tests/golden/make_golden.py (oracle only): a guard against
+    accidental changes of the oracle's arithmetic, not a pin."""
+    import json
+    import os
+    with open(os.path.join(os.path.dirname(__file__), "golden", "fchl19_oracle.json")) as f:
+        gold = json.load(f)
+    g = molecules_geometry(99, [7])
+    assert g.elem.tolist() == gold["elements"]
+    rho = oracle.fchl19(FP, g.r, g.elem, g.nbr_idx)
+    J = oracle.fchl19_jacobian(FP, g.r, g.elem, g.nbr_idx, atoms=np.array([0]))
+    i0 = gold["rho_atom0_first_nonzero_index"]
+    nz = np.nonzero(rho[0])[0]
+    assert rho.shape[1] == gold["rep"] and nz[0] == i0
+    np.testing.assert_allclose(np.linalg.norm(rho), gold["rho_fro"], rtol=1e-12)
+    np.testing.assert_allclose(rho[0, nz[:8]], gold["rho_atom0_first8_nonzero"], rtol=1e-11)
+    np.testing.assert_allclose(rho.sum(1), gold["rho_row_sums"], rtol=1e-11)
+    np.testing.assert_allclose(np.linalg.norm(J), gold["jac_atom0_fro"], rtol=1e-11)
+    np.testing.assert_allclose(J[0, 0, i0], gold["jac_atom0_self_first_nonzero_row"], rtol=1e-9, atol=1e-14)
