@@ -127,3 +127,24 @@ def test_sorf_forward_mma_fullsize_c3(q):
     num = float((Z - Z2).double().norm())
     den = float(Z2.double().norm())
     assert num / den <= TOL
+
+
+def test_sorf_forward_mma_offsets_beyond_31_bits(q):
+    """n_mol * D > 2^31: the per-run table then holds molecule indices instead of Z offsets (64-bit addressing in the
+    epilogue).  131 073 one- and two-atom molecules, D = 16384; all of Z against the FWHT path, samples against the oracle."""
+    pkg, wio, torch = q
+    n_mol = 131073
+    counts = [1 + (i % 2) for i in range(n_mol)]
+    w = tiny_workload(seed=77, d=128, D=16384, T=3, sigma=5.0, counts=counts, n_elem=3, grad=None)
+    assert n_mol * 16384 > 2 ** 31
+    dp = wio.device_problem(w)
+    Z = pkg.qmll_sorf_forward_mma(dp.params, dp.x, dp.elem, dp.mol_off)
+    Z2 = pkg.qmll_sorf_forward(dp.params, dp.x, dp.elem, dp.mol_off)
+    torch.cuda.synchronize()
+    assert float((Z - Z2).double().norm() / Z2.double().norm()) <= TOL
+    m = w.model
+    for M in (0, 1, 65536, 131071, 131072):
+        a0, a1 = int(w.mol_off[M]), int(w.mol_off[M + 1])
+        Zo = oracle.forward(w.x[a0:a1], w.elem[a0:a1], np.array([0, a1 - a0], dtype=np.int32), m.d, m.D, m.T, m.sigma,
+                            m.signs, m.bias)
+        assert rel(Z[M].cpu().numpy(), Zo[0]) <= TOL
