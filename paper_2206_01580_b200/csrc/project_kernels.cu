@@ -85,6 +85,83 @@ project_x_kernel(const float* __restrict__ rho, const int32_t* __restrict__ elem
   }
 }
 
+// x, tiled: block = 64 consecutive atoms x 128 outputs, k in chunks of 16 through shared memory (rho transposed, U as is);
+// thread = 4 atoms x 8 outputs (32 accumulators, 3 LDS.128 per 32 FMAs).  Atoms of different elements use different
+// matrices: the block runs once per element present in its 64 atoms and keeps the rows of that element.  Used when
+// d % 128 == 0 (the configs' d = 128 / 256); measured 15 625 atoms, rep 720, d 256: see DESIGN.md 5.5.
+constexpr int kPxAtoms = 64, kPxOut = 128, kPxK = 16;
+__global__ void __launch_bounds__(256)
+project_x_tiled_kernel(const float* __restrict__ rho, const int32_t* __restrict__ elem, long long n_atoms, int rep, int d,
+                       int n_elem, const float* __restrict__ U, float* __restrict__ x) {
+  __shared__ __align__(16) float rt[kPxK][kPxAtoms + 4];     // rho^T chunk
+  __shared__ __align__(16) float ut[kPxK][kPxOut];           // U chunk
+  __shared__ int el[kPxAtoms];
+  __shared__ int present[64];
+  const int tid = threadIdx.x;
+  const int ta = tid >> 4, tm = tid & 15;                    // 16 x 16 threads: atoms 4 ta .. +3, outputs 8 tm .. +7
+  const long long a0 = (long long)blockIdx.x * kPxAtoms;
+  const int m0 = blockIdx.y * kPxOut;
+  if (tid < 64) present[tid] = 0;
+  __syncthreads();
+  if (tid < kPxAtoms) {
+    const int e = a0 + tid < n_atoms ? __ldg(elem + a0 + tid) : -1;
+    el[tid] = e;
+    if (e >= 0) present[e & 63] = 1;
+  }
+  __syncthreads();
+  for (int e = 0; e < n_elem; ++e) {
+    if (n_elem <= 64 && !present[e]) continue;
+    const float* Ue = U + (size_t)e * rep * d + m0;
+    float acc[4][8];
+#pragma unroll
+    for (int i = 0; i < 4; ++i)
+#pragma unroll
+      for (int j = 0; j < 8; ++j) acc[i][j] = 0.f;
+    for (int k0 = 0; k0 < rep; k0 += kPxK) {
+      const int kc = rep - k0 < kPxK ? rep - k0 : kPxK;
+      __syncthreads();
+      // rho: 64 atoms x 16 k, thread = (atom tid / 4, 4 consecutive k); U: 16 k x 128 m, thread = (k tid / 16, 8 m)
+      {
+        const int at = tid >> 2, kq = (tid & 3) * 4;
+        const bool ok = a0 + at < n_atoms && el[at] == e;
+#pragma unroll
+        for (int u = 0; u < 4; ++u)
+          rt[kq + u][at] = (ok && kq + u < kc) ? __ldg(rho + (size_t)(a0 + at) * rep + k0 + kq + u) : 0.f;
+        const int kk = tid >> 4, mq = (tid & 15) * 8;
+        float4 u0 = make_float4(0.f, 0.f, 0.f, 0.f), u1 = u0;
+        if (kk < kc) {
+          u0 = __ldg(reinterpret_cast<const float4*>(Ue + (size_t)(k0 + kk) * d + mq));
+          u1 = __ldg(reinterpret_cast<const float4*>(Ue + (size_t)(k0 + kk) * d + mq) + 1);
+        }
+        *reinterpret_cast<float4*>(&ut[kk][mq]) = u0;
+        *reinterpret_cast<float4*>(&ut[kk][mq + 4]) = u1;
+      }
+      __syncthreads();
+#pragma unroll
+      for (int k = 0; k < kPxK; ++k) {
+        const float4 r4 = *reinterpret_cast<const float4*>(&rt[k][4 * ta]);
+        const float4 ua = *reinterpret_cast<const float4*>(&ut[k][8 * tm]);
+        const float4 ub = *reinterpret_cast<const float4*>(&ut[k][8 * tm + 4]);
+        const float rr[4] = {r4.x, r4.y, r4.z, r4.w};
+        const float uu[8] = {ua.x, ua.y, ua.z, ua.w, ub.x, ub.y, ub.z, ub.w};
+#pragma unroll
+        for (int i = 0; i < 4; ++i)
+#pragma unroll
+          for (int j = 0; j < 8; ++j) acc[i][j] = fmaf(rr[i], uu[j], acc[i][j]);
+      }
+    }
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+      const int at = 4 * ta + i;
+      if (a0 + at < n_atoms && el[at] == e) {
+        float* dst = x + (size_t)(a0 + at) * d + m0 + 8 * tm;
+        *reinterpret_cast<float4*>(dst) = make_float4(acc[i][0], acc[i][1], acc[i][2], acc[i][3]);
+        *reinterpret_cast<float4*>(dst + 4) = make_float4(acc[i][4], acc[i][5], acc[i][6], acc[i][7]);
+      }
+    }
+  }
+}
+
 // gradient: block = one atom I; its [rep][3n] block is projected to [d][3n], 32 columns at a time (lane = column).
 __global__ void __launch_bounds__(kProjThreads)
 project_grad_kernel(const float* __restrict__ gin, const int64_t* __restrict__ in_off, const int32_t* __restrict__ elem,
@@ -332,8 +409,14 @@ int project_launch(const float* rho, const int32_t* elem, const int32_t* mol_off
                    const int64_t* in_off, float* gout, const int64_t* out_off, cudaStream_t st) {
   if (n_atoms == 0) return QMLL_OK;
   if (x) {
-    project_x_kernel<<<(unsigned)((n_atoms + 31) / 32), kProjThreads, 0, st>>>(rho, elem, n_atoms, rep, d, n_elem, U, x);
-    QMLL_LAUNCH_CHECK("project_x_kernel");
+    if (d % kPxOut == 0) {
+      dim3 grid((unsigned)((n_atoms + kPxAtoms - 1) / kPxAtoms), (unsigned)(d / kPxOut));
+      project_x_tiled_kernel<<<grid, 256, 0, st>>>(rho, elem, n_atoms, rep, d, n_elem, U, x);
+      QMLL_LAUNCH_CHECK("project_x_tiled_kernel");
+    } else {
+      project_x_kernel<<<(unsigned)((n_atoms + 31) / 32), kProjThreads, 0, st>>>(rho, elem, n_atoms, rep, d, n_elem, U, x);
+      QMLL_LAUNCH_CHECK("project_x_kernel");
+    }
   }
   if (gout) {
     project_grad_kernel<<<(unsigned)n_atoms, kProjThreads, 0, st>>>(gin, in_off, elem, mol_off, n_mol, rep, d, U,
