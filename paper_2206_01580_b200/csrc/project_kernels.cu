@@ -388,9 +388,87 @@ project_back_kernel(const float* __restrict__ g, const int32_t* __restrict__ ele
   }
 }
 
-int project_back_launch(const float* g, const int32_t* elem, int64_t n_atoms, int32_t rep, int32_t d, const float* U,
-                        float* w, cudaStream_t st) {
+// The same product tiled like project_x_tiled_kernel: block = 64 atoms x 128 rows k of U_e, the contraction index m in
+// chunks of 16 (g transposed and U^T in shared memory), thread = 4 atoms x 8 rows; once per element present in the block.
+__global__ void __launch_bounds__(256)
+project_back_tiled_kernel(const float* __restrict__ g, const int32_t* __restrict__ elem, long long n_atoms, int rep, int d,
+                          int n_elem, const float* __restrict__ U, float* __restrict__ w) {
+  __shared__ __align__(16) float gt[kPxK][kPxAtoms + 4];     // g^T chunk
+  __shared__ __align__(16) float ut[kPxK][kPxOut + 4];       // U^T chunk: [m][row k]
+  __shared__ int el[kPxAtoms];
+  __shared__ int present[64];
+  const int tid = threadIdx.x;
+  const int ta = tid >> 4, tm = tid & 15;
+  const long long a0 = (long long)blockIdx.x * kPxAtoms;
+  const int r0 = blockIdx.y * kPxOut;
+  if (tid < 64) present[tid] = 0;
+  __syncthreads();
+  if (tid < kPxAtoms) {
+    const int e = a0 + tid < n_atoms ? __ldg(elem + a0 + tid) : -1;
+    el[tid] = e;
+    if (e >= 0) present[e & 63] = 1;
+  }
+  __syncthreads();
+  for (int e = 0; e < n_elem; ++e) {
+    if (n_elem <= 64 && !present[e]) continue;
+    const float* Ue = U + (size_t)e * rep * d;
+    float acc[4][8];
+#pragma unroll
+    for (int i = 0; i < 4; ++i)
+#pragma unroll
+      for (int j = 0; j < 8; ++j) acc[i][j] = 0.f;
+    for (int m0 = 0; m0 < d; m0 += kPxK) {          // d is a multiple of 16 here
+      __syncthreads();
+      {
+        const int at = tid >> 2, mq = (tid & 3) * 4;
+        const bool ok = a0 + at < n_atoms && el[at] == e;
+        float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
+        if (ok) v = __ldg(reinterpret_cast<const float4*>(g + (size_t)(a0 + at) * d + m0 + mq));
+        gt[mq][at] = v.x; gt[mq + 1][at] = v.y; gt[mq + 2][at] = v.z; gt[mq + 3][at] = v.w;
+        const int rr = tid >> 1, mh = (tid & 1) * 8;      // row r0 + rr of U_e, 8 consecutive m
+        float4 u0 = make_float4(0.f, 0.f, 0.f, 0.f), u1 = u0;
+        if (r0 + rr < rep) {
+          const float4* src = reinterpret_cast<const float4*>(Ue + (size_t)(r0 + rr) * d + m0 + mh);
+          u0 = __ldg(src); u1 = __ldg(src + 1);
+        }
+        ut[mh][rr] = u0.x; ut[mh + 1][rr] = u0.y; ut[mh + 2][rr] = u0.z; ut[mh + 3][rr] = u0.w;
+        ut[mh + 4][rr] = u1.x; ut[mh + 5][rr] = u1.y; ut[mh + 6][rr] = u1.z; ut[mh + 7][rr] = u1.w;
+      }
+      __syncthreads();
+#pragma unroll
+      for (int k = 0; k < kPxK; ++k) {
+        const float4 r4 = *reinterpret_cast<const float4*>(&gt[k][4 * ta]);
+        const float4 ua = *reinterpret_cast<const float4*>(&ut[k][8 * tm]);
+        const float4 ub = *reinterpret_cast<const float4*>(&ut[k][8 * tm + 4]);
+        const float rr[4] = {r4.x, r4.y, r4.z, r4.w};
+        const float uu[8] = {ua.x, ua.y, ua.z, ua.w, ub.x, ub.y, ub.z, ub.w};
+#pragma unroll
+        for (int i = 0; i < 4; ++i)
+#pragma unroll
+          for (int j = 0; j < 8; ++j) acc[i][j] = fmaf(rr[i], uu[j], acc[i][j]);
+      }
+    }
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+      const int at = 4 * ta + i;
+      if (a0 + at < n_atoms && el[at] == e) {
+#pragma unroll
+        for (int j = 0; j < 8; ++j)
+          if (r0 + 8 * tm + j < rep) w[(size_t)(a0 + at) * rep + r0 + 8 * tm + j] = acc[i][j];
+      }
+    }
+  }
+}
+
+int project_back_launch(const float* g, const int32_t* elem, int64_t n_atoms, int32_t rep, int32_t d, int32_t n_elem,
+                        const float* U, float* w, cudaStream_t st) {
   if (n_atoms == 0) return QMLL_OK;
+  if (d % kPxK == 0) {
+    dim3 grid((unsigned)((n_atoms + kPxAtoms - 1) / kPxAtoms), (unsigned)((rep + kPxOut - 1) / kPxOut));
+    project_back_tiled_kernel<<<grid, 256, 0, st>>>(g, elem, n_atoms, rep, d, n_elem, U, w);
+    QMLL_LAUNCH_CHECK("project_back_tiled_kernel");
+    return QMLL_OK;
+  }
   project_back_kernel<<<(unsigned)n_atoms, kProjThreads, d * sizeof(float), st>>>(g, elem, rep, d, U, w);
   QMLL_LAUNCH_CHECK("project_back_kernel");
   return QMLL_OK;

@@ -285,7 +285,7 @@ int qmll_project_back(const float* g, const int32_t* elem, int64_t n_atoms, int3
   if (n_atoms > 0x7fffff00LL || d > 8192) return QMLL_ERR_INVALID_ARG;
   int rc = check_device();
   if (rc) return rc;
-  return project_back_launch(g, elem, n_atoms, rep, d, U, w, static_cast<cudaStream_t>(cuda_stream));
+  return project_back_launch(g, elem, n_atoms, rep, d, n_elem, U, w, static_cast<cudaStream_t>(cuda_stream));
 }
 
 int qmll_fchl19_backward(const qmll_fchl19_params* fp, const float* r, const int32_t* elem, int64_t n_atoms,

@@ -123,8 +123,8 @@ int project_launch(const float* rho, const int32_t* elem, const int32_t* mol_off
                    int32_t rep, int32_t d, int32_t n_elem, const float* U, float* x, const float* gin,
                    const int64_t* in_off, float* gout, const int64_t* out_off, cudaStream_t st);
 
-int project_back_launch(const float* g, const int32_t* elem, int64_t n_atoms, int32_t rep, int32_t d, const float* U,
-                        float* w, cudaStream_t st);
+int project_back_launch(const float* g, const int32_t* elem, int64_t n_atoms, int32_t rep, int32_t d, int32_t n_elem,
+                        const float* U, float* w, cudaStream_t st);
 int project_neighbor_launch(const float* gin, const int32_t* idx, const int32_t* elem, int64_t n_atoms, int32_t S,
                             int32_t rep, int32_t d, int32_t n_elem, const float* U, float* gout, cudaStream_t st);
 
