@@ -498,6 +498,11 @@ def other_configs(pk, reps, rows_mode=0, only=None):
                 o.update({"forward_mma_ms": t, "forward_mma_molecules_per_s": nm / (t * 1e-3),
                           "forward_mma_useful_f16_tflops": 2.0 * 2.0 * m.d * D * na / (t * 1e-3) / 1e12,
                           "forward_mma_cos_frac_of_mufu_peak": cos_s / pk.get("mufu_per_s", 4.3e12)})
+                # the paper's own N_transform = 2 (L268, L278): the FWHT chain is a third shorter, the expanded-W map is not
+                p2 = pkg.SorfParams(d=m.d, D=D, n_transform=2, n_elem=m.n_elem, sigma=m.sigma,
+                                    signs=p.signs[:, :, :2, :].contiguous(), bias=p.bias)
+                o["forward_T2_ms"] = tm(lambda: pkg.qmll_sorf_forward(p2, dp.x, dp.elem, dp.mol_off, Z=Zm))
+                o["forward_mma_T2_ms"] = tm(lambda: pkg.qmll_sorf_forward_mma(p2, dp.x, dp.elem, dp.mol_off, Z=Zm))
                 Wr = torch.randn((m.n_elem, D, m.d), dtype=torch.float32, device="cuda") / m.sigma
                 t = tm(lambda: pkg.qmll_rff_forward(Wr, p.bias, dp.x, dp.elem, dp.mol_off, Z=Zm))
                 o.update({"rff_forward_ms": t, "rff_useful_f16_tflops": 3.0 * 2.0 * m.d * D * na / (t * 1e-3) / 1e12})
