@@ -17,7 +17,8 @@ constexpr int kMbUnroll = 16;   // independent chains per thread
 enum MbKind {
   kMbFadd = 0, kMbFfma = 1, kMbFadd2 = 2, kMbFfma2 = 3, kMbLop3 = 4, kMbShf = 5, kMbFadd2Lop3 = 6,
   kMbFaddSign = 7, kMbFadd2Sign = 8, kMbMufuCos = 9, kMbLds128 = 10, kMbShfl = 11, kMbFadd2Lop3Shf = 12,
-  kMbCount = 13
+  kMbDfma = 13, kMbDmma = 14,   // FP64: scalar DFMA, mma.sync.m8n8k4.f64 (the solve's trailing update)
+  kMbCount = 15
 };
 
 __device__ __forceinline__ uint64_t pack2(float a, float b) {
@@ -50,6 +51,10 @@ microbench_kernel(float* __restrict__ out, int iters, unsigned long long* __rest
   sm[tid + kMbThreads] = make_float4(f[4], f[5], f[6], f[7]);
   const float k1 = 1.0000001f, k2 = 1e-7f;
   const uint64_t kk = pack2(k2, -k2), km = pack2(k1, k1);
+  double g[kMbUnroll];
+#pragma unroll
+  for (int i = 0; i < kMbUnroll; ++i) g[i] = (double)f[i];
+  const double gk1 = 1.0 + 1e-9 * (double)(tid & 3), gk2 = 1e-9;
   __syncthreads();
   const unsigned long long t0 = clock64();
 #pragma unroll 1
@@ -135,12 +140,25 @@ microbench_kernel(float* __restrict__ out, int iters, unsigned long long* __rest
     } else if constexpr (KIND == kMbShfl) {
 #pragma unroll
       for (int i = 0; i < kMbUnroll; ++i) f[i] = __shfl_xor_sync(0xffffffffu, f[i], 1 + (i & 15));
+    } else if constexpr (KIND == kMbDfma) {
+#pragma unroll
+      for (int r = 0; r < 4; ++r)
+#pragma unroll
+        for (int i = 0; i < kMbUnroll; ++i)
+          asm volatile("fma.rn.f64 %0, %0, %1, %2;" : "+d"(g[i]) : "d"(gk1), "d"(gk2));
+    } else if constexpr (KIND == kMbDmma) {          // 8 independent 8x8 accumulators (2 doubles per thread each)
+#pragma unroll
+      for (int r = 0; r < 4; ++r)
+#pragma unroll
+        for (int i = 0; i < kMbUnroll; i += 2)
+          asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0, %1}, {%2}, {%3}, {%0, %1};"
+                       : "+d"(g[i]), "+d"(g[i + 1]) : "d"(gk1), "d"(gk2));
     }
   }
   const unsigned long long t1 = clock64();
   float acc = 0.f;
 #pragma unroll
-  for (int i = 0; i < kMbUnroll; ++i) acc += f[i] + lo_of(d[i]) + __uint_as_float(u[i] & 0x3fffffffu);
+  for (int i = 0; i < kMbUnroll; ++i) acc += f[i] + lo_of(d[i]) + __uint_as_float(u[i] & 0x3fffffffu) + (float)g[i];
   out[(size_t)blockIdx.x * kMbThreads + tid] = acc;
   if (tid == 0) cycles[blockIdx.x] = t1 - t0;
 }
@@ -156,6 +174,8 @@ static double mb_ops_per_iter(int kind) {
     case kMbFadd2Lop3Shf: return 4.0 * kMbUnroll;
     case kMbMufuCos: case kMbShfl: return 1.0 * kMbUnroll;
     case kMbLds128: return 16.0 * kMbUnroll;              // bytes
+    case kMbDfma: return 4.0 * kMbUnroll;                 // FP64 FMAs
+    case kMbDmma: return 4.0 * (kMbUnroll / 2) * 8.0;     // FP64 FMAs: 8 x 8 x 4 = 256 per warp instruction, 8 per lane
     default: return 0.0;
   }
 }
@@ -269,6 +289,8 @@ extern "C" int qmll_microbench(int kind, int iters, int blocks_per_sm, void* wor
     case 10: return mb_launch<10>(out, iters, cyc, blocks, st);
     case 11: return mb_launch<11>(out, iters, cyc, blocks, st);
     case 12: return mb_launch<12>(out, iters, cyc, blocks, st);
+    case 13: return mb_launch<13>(out, iters, cyc, blocks, st);
+    case 14: return mb_launch<14>(out, iters, cyc, blocks, st);
     default: return QMLL_ERR_INVALID_ARG;
   }
 }

@@ -2,210 +2,324 @@
 // "solved by LU decomposition", L137 -- the matrix is symmetric positive definite, so Cholesky).  FP64 throughout: the
 // Gram matrix of random features is ill-conditioned (the paper's FP32 round-off remark, L351), and the O(D^3/3) solve
 // is small beside the O(rows D^2) accumulation.  Two-level blocked right-looking Cholesky:
-//   potrf_diag_kernel (one CTA, 64 x 64 diagonal block in shared memory)  ->  trsm_panel_kernel (thread per row)
-//   ->  syrk_update_kernel on the 256-wide panel's own columns; after the panel one rank-256 syrk_update_kernel of
-//   the trailing matrix (128 x 128 tiles, 8 x 8 DFMA register tiles),
-// then forward / backward substitution by blocks.  `info` (device int) follows LAPACK: 0 = success, k > 0 = the
-// leading minor of order k is not positive definite (the factorisation then carries NaNs).
+//   potrf_diag_kernel (64 x 64 diagonal block, one row per thread in registers)  ->  trsm_panel_kernel (thread per
+//   row, column-oriented substitution)  ->  syrk_update_kernel on the 256-wide panel's own columns; after the panel
+//   one rank-256 syrk_update_kernel of the trailing matrix,
+// then forward / backward substitution, one launch per 64-wide block (trsv_step_kernel).
+// syrk_update_kernel is the O(D^3) part: 128 x 64 tiles on the FP64 tensor-core path (mma.sync.m8n8k4.f64, DMMA: the
+// measured peak, profiles/peaks_r2.json kinds 13 / 14, is 18.5 T FMA/s against 17.0 for scalar DFMA, with 1/8 of the
+// instructions and 1/5 of the shared-memory loads), operands through a 3-stage cp.async ring, two CTAs per SM so that
+// the read-modify-write epilogue of one overlaps the main loop of the other.
+// `info` (device int) follows LAPACK: 0 = success, k > 0 = the leading minor of order k is not positive definite (the
+// factorisation then carries NaNs).  The working matrix has leading dimension ld = D rounded up to 8 (16-byte copies).
 #include "qmll_common.cuh"
 
 namespace qmll {
 
-constexpr int kNB = 64;     // inner step: diagonal block factorised in shared memory
+constexpr int kNB = 64;     // inner step: diagonal block factorised in registers
 constexpr int kNB2 = 256;   // outer panel: one trailing update per 256 columns
 
-__global__ void solve_prepare_kernel(const float* __restrict__ ZtZ, const float* __restrict__ Zty, int D, double lambda,
-                                     double* __restrict__ M, double* __restrict__ rhs, int* __restrict__ info) {
+static inline int solve_ld(int D) { return (D + 7) & ~7; }
+
+// The 64 x 64 diagonal block goes to shared memory by 8-byte cp.async: all of a thread's copies are in flight at once
+// (a load -> store loop serialised one L2 round trip per unrolled group and was half of every panel kernel's time).
+__device__ __forceinline__ void cp_async8(void* smem_dst, const void* src) {
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"((uint32_t)__cvta_generic_to_shared(smem_dst)), "l"(src) : "memory");
+}
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
+
+__global__ void solve_prepare_kernel(const float* __restrict__ ZtZ, const float* __restrict__ Zty, int D, int ld,
+                                     double lambda, double* __restrict__ M, double* __restrict__ rhs,
+                                     int* __restrict__ info) {
   const long long n = (long long)D * D;
   for (long long idx = blockIdx.x * (long long)blockDim.x + threadIdx.x; idx < n;
        idx += (long long)gridDim.x * blockDim.x) {
     const int i = (int)(idx / D), j = (int)(idx % D);
-    M[idx] = (double)ZtZ[idx] + (i == j ? lambda : 0.0);
+    M[(size_t)i * ld + j] = (double)ZtZ[idx] + (i == j ? lambda : 0.0);
     if (j == 0) rhs[i] = (double)Zty[i];
   }
   if (blockIdx.x == 0 && threadIdx.x == 0) *info = 0;
 }
 
-// Cholesky of the nb x nb diagonal block at (k0, k0): A = L L^T, L overwrites the lower triangle.
-__global__ void __launch_bounds__(256) potrf_diag_kernel(double* __restrict__ M, int D, int k0, int nb, int* info) {
-  __shared__ double a[kNB][kNB + 1];
-  const int t = threadIdx.x;
-  for (int idx = t; idx < nb * nb; idx += 256) a[idx / nb][idx % nb] = M[(size_t)(k0 + idx / nb) * D + k0 + idx % nb];
-  __syncthreads();
-  for (int j = 0; j < nb; ++j) {
-    const double piv = a[j][j];
-    __syncthreads();
-    if (t == 0) {
-      if (!(piv > 0.0) && *info == 0) *info = k0 + j + 1;
-      a[j][j] = sqrt(piv);
-    }
-    __syncthreads();
-    const double dinv = 1.0 / a[j][j];
-    for (int i = j + 1 + t; i < nb; i += 256) a[i][j] *= dinv;
-    __syncthreads();
-    // trailing update of the lower triangle: a[i][c] -= a[i][j] * a[c][j],  j < c <= i < nb
-    const int m = nb - j - 1;
-    for (int idx = t; idx < m * m; idx += 256) {
-      const int i = j + 1 + idx / m, c = j + 1 + idx % m;
-      if (c <= i) a[i][c] -= a[i][j] * a[c][j];
-    }
-    __syncthreads();
+// Cholesky of the nb x nb diagonal block at (k0, k0): A = L L^T, L overwrites the lower triangle.  Thread i holds row
+// i in registers (right-looking): per column ONE barrier -- every thread publishes its entry of column j, reads the
+// pivot and the column back, and updates its own row with independent FMAs.  Rows / columns >= nb are an identity pad.
+__global__ void __launch_bounds__(kNB) potrf_diag_kernel(double* __restrict__ M, int ld, int k0, int nb, int* info) {
+  __shared__ double tile[kNB][kNB + 1];
+  __shared__ double col[2][kNB];
+  const int i = threadIdx.x;
+  for (int idx = i; idx < kNB * kNB; idx += kNB) {
+    const int r = idx / kNB, c = idx % kNB;
+    if (r < nb && c <= r) cp_async8(&tile[r][c], M + (size_t)(k0 + r) * ld + k0 + c);
+    else tile[r][c] = r == c ? 1.0 : 0.0;
   }
-  for (int idx = t; idx < nb * nb; idx += 256) {
-    const int i = idx / nb, c = idx % nb;
-    if (c <= i) M[(size_t)(k0 + i) * D + k0 + c] = a[i][c];
+  cp_async_wait_all();
+  __syncthreads();
+  double a[kNB];
+#pragma unroll
+  for (int c = 0; c < kNB; ++c) a[c] = tile[i][c];
+#pragma unroll
+  for (int j = 0; j < kNB; ++j) {
+    col[j & 1][i] = a[j];
+    __syncthreads();
+    const double piv = col[j & 1][j];
+    if (i == j && j < nb && !(piv > 0.0) && *info == 0) *info = k0 + j + 1;
+    const double dinv = rsqrt(piv);
+    a[j] *= dinv;                       // row j: sqrt(piv); rows below: l_ij
+    const double s = a[j] * dinv;       // l_ij / sqrt(piv); col[c] * (1 / sqrt(piv)) = l_cj
+#pragma unroll
+    for (int c = j + 1; c < kNB; ++c) a[c] = fma(-s, col[j & 1][c], a[c]);   // rows above j hold a[j] = 0
+  }
+#pragma unroll
+  for (int c = 0; c < kNB; ++c) tile[i][c] = a[c];
+  __syncthreads();
+  for (int idx = i; idx < nb * nb; idx += kNB) {
+    const int r = idx / nb, c = idx % nb;
+    if (c <= r) M[(size_t)(k0 + r) * ld + k0 + c] = tile[r][c];
   }
 }
 
-// Rows below the diagonal block: X = A21 L11^-T, one thread per row (forward substitution along the row).
-__global__ void __launch_bounds__(128) trsm_panel_kernel(double* __restrict__ M, int D, int k0, int nb) {
-  __shared__ double l[kNB][kNB + 1];
-  for (int idx = threadIdx.x; idx < nb * nb; idx += 128) l[idx / nb][idx % nb] = M[(size_t)(k0 + idx / nb) * D + k0 + idx % nb];
+// Rows below a full 64 x 64 diagonal block: X = A21 L11^-T, one thread per row, column-oriented forward substitution
+// (x_c final -> every later x_k gets its term: independent FMAs); L11 transposed in shared memory so that one
+// broadcast LDS.128 serves two FMAs.
+constexpr int kLtLd = kNB + 2;
+__global__ void __launch_bounds__(128) trsm_panel_kernel(double* __restrict__ M, int D, int ld, int k0) {
+  __shared__ __align__(16) double lt[kNB][kLtLd];   // lt[c][k] = L11[k][c]
+  __shared__ double dinv[kNB];
+  for (int idx = threadIdx.x; idx < kNB * kNB; idx += 128) {
+    const int r = idx / kNB, c = idx % kNB;
+    cp_async8(&lt[c][r], M + (size_t)(k0 + r) * ld + k0 + c);
+  }
+  cp_async_wait_all();
   __syncthreads();
-  const int i = k0 + nb + blockIdx.x * 128 + threadIdx.x;
+  if (threadIdx.x < kNB) dinv[threadIdx.x] = 1.0 / lt[threadIdx.x][threadIdx.x];
+  __syncthreads();
+  const int i = k0 + kNB + blockIdx.x * 128 + threadIdx.x;
   if (i >= D) return;
-  double* row = M + (size_t)i * D + k0;
+  double2* row = reinterpret_cast<double2*>(M + (size_t)i * ld + k0);
   double x[kNB];
 #pragma unroll
-  for (int c = 0; c < kNB; ++c) x[c] = c < nb ? row[c] : 0.0;
+  for (int c = 0; c < kNB; c += 2) { const double2 v = row[c / 2]; x[c] = v.x; x[c + 1] = v.y; }
 #pragma unroll
   for (int c = 0; c < kNB; ++c) {
-    if (c < nb) {
-      double s = x[c];
+    x[c] *= dinv[c];
+    const double xc = x[c];
+    int k = c + 1;
+    if (k & 1) { if (k < kNB) x[k] = fma(-xc, lt[c][k], x[k]); ++k; }
 #pragma unroll
-      for (int m = 0; m < c; ++m) s = fma(-x[m], l[c][m], s);
-      x[c] = s / l[c][c];
+    for (; k < kNB; k += 2) {
+      const double2 l2 = *reinterpret_cast<const double2*>(&lt[c][k]);
+      x[k] = fma(-xc, l2.x, x[k]);
+      x[k + 1] = fma(-xc, l2.y, x[k + 1]);
     }
   }
 #pragma unroll
-  for (int c = 0; c < kNB; ++c)
-    if (c < nb) row[c] = x[c];
+  for (int c = 0; c < kNB; c += 2) row[c / 2] = make_double2(x[c], x[c + 1]);
 }
 
 // Symmetric rank-kn update on the lower triangle:  C[i][j] -= sum_{m < kn} M[i][k0 + m] * M[j][k0 + m]  for rows
-// i >= r0, columns c0 <= j < c1, j <= i.  CTA = 128 x 128 tile (blockIdx.x: row tile from r0, blockIdx.y: column tile
-// from c0), thread = 8 x 8 outputs (rows ty + 16 u, columns tx + 16 v: shared-memory reads are broadcasts or
-// conflict-free, the write-back is coalesced), k in chunks of 16 through shared memory.  64 DFMA per 16 LDS.64: the
-// FP64 pipe, not shared memory, bounds it.
-constexpr int kUT = 128;   // tile
-constexpr int kUK = 16;    // k chunk
-__global__ void __launch_bounds__(256) syrk_update_kernel(double* __restrict__ M, int D, int r0, int c0, int c1, int k0,
-                                                          int kn) {
-  const int i0 = r0 + blockIdx.x * kUT, j0 = c0 + blockIdx.y * kUT;
-  if (j0 >= c1 || j0 > i0 + kUT - 1) return;          // tile entirely above the diagonal or outside the column range
-  __shared__ double li[kUK][kUT + 2], lj[kUK][kUT + 2];
-  const int t = threadIdx.x, tx = t & 15, ty = t >> 4;
-  double acc[8][8];
+// i >= r0, columns c0 <= j < c1, j <= i (c0 even).  CTA = 128 x 64 tile (blockIdx.x: row tile from r0, blockIdx.y:
+// column tile from c0), 4 warps as 2 x 2, warp tile 64 x 32 = 8 x 4 DMMA tiles (128 accumulator registers).  Both
+// operands are row-major slices of M with k contiguous, which is exactly the m8n8k4 fragment order (A: row lane / 4,
+// k lane % 4; B the same with the row as n), so the stages are plain copies: [rows][16 k] with a row pitch of 20
+// doubles (conflict-free LDS.64 for the 8 rows x 4 k a fragment touches), filled by 16-byte cp.async (zero-filled
+// beyond kn and beyond row D).
+constexpr int kUM = 128, kUN = 64, kUK = 16, kUPitch = 20, kUStages = 3;
+constexpr int kUStageDoubles = (kUM + kUN) * kUPitch;
+constexpr int kUSmemBytes = kUStages * kUStageDoubles * 8;
+
+__device__ __forceinline__ void cp_async16_zfill(uint32_t dst, const void* src, int src_bytes) {
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(dst), "l"(src), "r"(src_bytes) : "memory");
+}
+__device__ __forceinline__ void dmma_m8n8k4(double& c0, double& c1, double a, double b) {
+  asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0, %1}, {%2}, {%3}, {%0, %1};" : "+d"(c0), "+d"(c1) : "d"(a), "d"(b));
+}
+
+__global__ void __launch_bounds__(128, 2) syrk_update_kernel(double* __restrict__ M, int D, int ld, int r0, int c0,
+                                                             int c1, int k0, int kn) {
+  const int i0 = r0 + blockIdx.x * kUM, j0 = c0 + blockIdx.y * kUN;
+  if (j0 >= c1 || j0 > i0 + kUM - 1) return;          // tile entirely above the diagonal or outside the column range
+  extern __shared__ __align__(16) double usm[];
+  const int t = threadIdx.x, lane = t & 31, warp = t >> 5;
+  const int wr = warp >> 1, wc = warp & 1, g = lane >> 2, tg = lane & 3;
+  const uint32_t usm_addr = (uint32_t)__cvta_generic_to_shared(usm);
+
+  // loader: a stage is 192 rows x 8 pieces of 16 bytes; thread t copies piece t % 8 of rows t / 8 + 16 q, q < 12
+  const int lrow = t >> 3, lch = t & 7;
+  auto load_stage = [&](int chunk, int slot) {
+    const int kk = chunk * kUK + lch * 2;
+    int bytes = (kn - kk) * 8;
+    bytes = bytes < 0 ? 0 : (bytes > 16 ? 16 : bytes);
+    const double* col = M + k0 + (bytes ? kk : 0);
+    const uint32_t dst = usm_addr + (uint32_t)((slot * kUStageDoubles + lrow * kUPitch + lch * 2) * 8);
+#pragma unroll
+    for (int q = 0; q < 12; ++q) {
+      const int gr = q < 8 ? i0 + lrow + 16 * q : j0 + lrow + 16 * (q - 8);
+      const bool ok = gr < D;
+      cp_async16_zfill(dst + (uint32_t)(16 * q * kUPitch * 8), col + (size_t)(ok ? gr : 0) * ld, ok ? bytes : 0);
+    }
+  };
+
+  double acc[8][4][2];
 #pragma unroll
   for (int u = 0; u < 8; ++u)
 #pragma unroll
-    for (int v = 0; v < 8; ++v) acc[u][v] = 0.0;
-  // 128 rows x 16 k doubles per operand and chunk: thread t owns row t / 2, k half t % 2 (8 doubles = 64 contiguous
-  // bytes).  The next chunk is fetched into registers while the current one is multiplied (software pipeline).
-  const int lr = t >> 1, lkh = (t & 1) * 8;
-  const bool oki = i0 + lr < D, okj = j0 + lr < D;
-  const double* pi = M + (size_t)(oki ? i0 + lr : 0) * D + k0 + lkh;
-  const double* pj = M + (size_t)(okj ? j0 + lr : 0) * D + k0 + lkh;
-  double ni[8], nj[8];
-  auto fetch = [&](int m0) {
+    for (int v = 0; v < 4; ++v) acc[u][v][0] = acc[u][v][1] = 0.0;
+
+  const int n_chunks = (kn + kUK - 1) / kUK;
 #pragma unroll
-    for (int q = 0; q < 8; ++q) {
-      const bool okm = m0 + lkh + q < kn;
-      ni[q] = (oki && okm) ? pi[m0 + q] : 0.0;
-      nj[q] = (okj && okm) ? pj[m0 + q] : 0.0;
-    }
-  };
-  fetch(0);
-  for (int m0 = 0; m0 < kn; m0 += kUK) {
-    __syncthreads();
+  for (int s = 0; s < kUStages - 1; ++s) {
+    if (s < n_chunks) load_stage(s, s);
+    asm volatile("cp.async.commit_group;" ::: "memory");
+  }
+  for (int ch = 0; ch < n_chunks; ++ch) {
+    asm volatile("cp.async.wait_group %0;" ::"n"(kUStages - 2) : "memory");
+    __syncthreads();                    // stage ch has landed for every thread; slot (ch - 1) % stages is free again
+    if (ch + kUStages - 1 < n_chunks) load_stage(ch + kUStages - 1, (ch + kUStages - 1) % kUStages);
+    asm volatile("cp.async.commit_group;" ::: "memory");
+    const double* A = usm + (ch % kUStages) * kUStageDoubles + (wr * 64 + g) * kUPitch + tg;
+    const double* B = usm + (ch % kUStages) * kUStageDoubles + (kUM + wc * 32 + g) * kUPitch + tg;
 #pragma unroll
-    for (int q = 0; q < 8; ++q) { li[lkh + q][lr] = ni[q]; lj[lkh + q][lr] = nj[q]; }
-    __syncthreads();
-    if (m0 + kUK < kn) fetch(m0 + kUK);
+    for (int k4 = 0; k4 < kUK / 4; ++k4) {
+      double a[8], b[4];
 #pragma unroll
-    for (int m = 0; m < kUK; ++m) {
-      double a[8], b[8];
+      for (int u = 0; u < 8; ++u) a[u] = A[u * 8 * kUPitch + k4 * 4];
 #pragma unroll
-      for (int u = 0; u < 8; ++u) { a[u] = li[m][ty + 16 * u]; b[u] = lj[m][tx + 16 * u]; }
+      for (int v = 0; v < 4; ++v) b[v] = B[v * 8 * kUPitch + k4 * 4];
 #pragma unroll
       for (int u = 0; u < 8; ++u)
 #pragma unroll
-        for (int v = 0; v < 8; ++v) acc[u][v] = fma(a[u], b[v], acc[u][v]);
+        for (int v = 0; v < 4; ++v) dmma_m8n8k4(acc[u][v][0], acc[u][v][1], a[u], b[v]);
     }
   }
+  // epilogue: the thread holds C[row g][columns 2 tg, 2 tg + 1] of every 8 x 8 tile: 16-byte read-modify-write
 #pragma unroll
-  for (int u = 0; u < 8; ++u)
+  for (int u = 0; u < 8; ++u) {
+    const int i = i0 + wr * 64 + 8 * u + g;
+    if (i >= D) continue;
 #pragma unroll
-    for (int v = 0; v < 8; ++v) {
-      const int i = i0 + ty + 16 * u, j = j0 + tx + 16 * v;
-      if (i < D && j < c1 && j <= i) M[(size_t)i * D + j] -= acc[u][v];
+    for (int v = 0; v < 4; ++v) {
+      const int j = j0 + wc * 32 + 8 * v + 2 * tg;
+      double* p = M + (size_t)i * ld + j;
+      if (j + 1 <= i && j + 1 < c1) {
+        double2 c = *reinterpret_cast<double2*>(p);
+        c.x -= acc[u][v][0]; c.y -= acc[u][v][1];
+        *reinterpret_cast<double2*>(p) = c;
+      } else if (j <= i && j < c1) {
+        *p -= acc[u][v][0];
+      }
     }
+  }
 }
 
-// Substitution, diagonal block: transposed = 0 solves L11 y = b (forward), 1 solves L11^T a = y (backward).
-__global__ void __launch_bounds__(64) trsv_diag_kernel(const double* __restrict__ M, int D, int k0, int nb, int transposed,
-                                                       double* __restrict__ rhs) {
+// One block step of a substitution.  transposed = 0 (forward, L y = b): solves the nb x nb diagonal block for
+// sol[k0 .. k0 + nb) from run[k0 ..) and subtracts L[i][k0 ..] . sol from run[i] for every row i >= k0 + nb.
+// transposed = 1 (backward, L^T a = y): the same with L11^T, and run[j] -= sum_m L[k0 + m][j] sol[k0 + m] for j < k0.
+// Every CTA repeats the small diagonal solve (warp 0: two rows per lane, the solved entry travels by shuffle), so a
+// step is ONE launch; CTA 0 writes `sol`.  `run` entries of the block itself are only read.
+__global__ void __launch_bounds__(128) trsv_step_kernel(const double* __restrict__ M, int D, int ld, int k0, int nb,
+                                                        int transposed, double* __restrict__ run,
+                                                        double* __restrict__ sol) {
   __shared__ double l[kNB][kNB + 1];
-  __shared__ double b[kNB];
-  const int t = threadIdx.x;
-  for (int idx = t; idx < nb * nb; idx += 64) l[idx / nb][idx % nb] = M[(size_t)(k0 + idx / nb) * D + k0 + idx % nb];
-  if (t < nb) b[t] = rhs[k0 + t];
+  __shared__ double dinv[kNB];
+  __shared__ __align__(16) double y[kNB];
+  const int t = threadIdx.x, lane = t & 31;
+  for (int idx = t; idx < kNB * kNB; idx += 128) {
+    const int r = idx / kNB, c = idx % kNB;
+    if (r < nb && c <= r) cp_async8(&l[r][c], M + (size_t)(k0 + r) * ld + k0 + c);
+    else l[r][c] = r == c ? 1.0 : 0.0;
+  }
+  cp_async_wait_all();
   __syncthreads();
-  if (!transposed) {
-    for (int c = 0; c < nb; ++c) {
-      if (t == c) b[c] /= l[c][c];
-      __syncthreads();
-      if (t > c && t < nb) b[t] -= l[t][c] * b[c];
-      __syncthreads();
+  if (t < kNB) dinv[t] = 1.0 / l[t][t];
+  __syncthreads();
+  if (t < 32) {
+    double b0 = lane < nb ? run[k0 + lane] : 0.0, b1 = lane + 32 < nb ? run[k0 + 32 + lane] : 0.0;
+    if (!transposed) {
+      for (int c = 0; c < kNB; ++c) {
+        const double bc = __shfl_sync(0xffffffffu, c < 32 ? b0 : b1, c & 31) * dinv[c];
+        if (lane == (c & 31)) { if (c < 32) b0 = bc; else b1 = bc; }
+        if (lane > c) b0 = fma(-l[lane][c], bc, b0);
+        if (lane + 32 > c) b1 = fma(-l[lane + 32][c], bc, b1);
+      }
+    } else {
+      for (int c = kNB - 1; c >= 0; --c) {
+        const double bc = __shfl_sync(0xffffffffu, c < 32 ? b0 : b1, c & 31) * dinv[c];
+        if (lane == (c & 31)) { if (c < 32) b0 = bc; else b1 = bc; }
+        if (lane < c) b0 = fma(-l[c][lane], bc, b0);
+        if (lane + 32 < c) b1 = fma(-l[c][lane + 32], bc, b1);
+      }
     }
-  } else {
-    for (int c = nb - 1; c >= 0; --c) {
-      if (t == c) b[c] /= l[c][c];
-      __syncthreads();
-      if (t < c) b[t] -= l[c][t] * b[c];
-      __syncthreads();
+    y[lane] = b0; y[lane + 32] = b1;
+    if (blockIdx.x == 0) {
+      if (lane < nb) sol[k0 + lane] = b0;
+      if (lane + 32 < nb) sol[k0 + 32 + lane] = b1;
     }
   }
-  if (t < nb) rhs[k0 + t] = b[t];
-}
-
-// Forward: rhs[i] -= sum_m L[i][k0+m] y[k0+m] for i >= k0+nb.  Backward: rhs[j] -= sum_m L[k0+m][j] a[k0+m] for j < k0.
-__global__ void __launch_bounds__(128) trsv_update_kernel(const double* __restrict__ M, int D, int k0, int nb,
-                                                          int transposed, double* __restrict__ rhs) {
-  __shared__ double y[kNB];
-  if (threadIdx.x < nb) y[threadIdx.x] = rhs[k0 + threadIdx.x];
   __syncthreads();
-  const int idx = blockIdx.x * 128 + threadIdx.x;
   if (!transposed) {
-    const int i = k0 + nb + idx;
-    if (i >= D) return;
-    const double* row = M + (size_t)i * D + k0;
-    double s = 0.0;
-    for (int m = 0; m < nb; ++m) s = fma(row[m], y[m], s);
-    rhs[i] -= s;
+    // rows below the block: 8 lanes per row (16-byte loads, 128 contiguous bytes per row and load), 16 rows per pass
+    const int sub = t & 7, rloc = t >> 3;
+    const int base = k0 + nb + blockIdx.x * 128;
+    if (base >= D) return;
+    double s[8];
+#pragma unroll
+    for (int p = 0; p < 8; ++p) {
+      const int row = base + p * 16 + rloc;
+      s[p] = 0.0;
+      if (row < D) {
+        const double2* src = reinterpret_cast<const double2*>(M + (size_t)row * ld + k0);
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+          const double2 v = src[sub + 8 * q];
+          const double2 w = *reinterpret_cast<const double2*>(&y[2 * sub + 16 * q]);
+          s[p] = fma(v.x, w.x, s[p]);
+          s[p] = fma(v.y, w.y, s[p]);
+        }
+      }
+    }
+#pragma unroll
+    for (int p = 0; p < 8; ++p) {
+      s[p] += __shfl_xor_sync(0xffffffffu, s[p], 1);
+      s[p] += __shfl_xor_sync(0xffffffffu, s[p], 2);
+      s[p] += __shfl_xor_sync(0xffffffffu, s[p], 4);
+      const int row = base + p * 16 + rloc;
+      if (sub == 0 && row < D) run[row] -= s[p];
+    }
   } else {
-    const int j = idx;
+    const int j = blockIdx.x * 128 + t;
     if (j >= k0) return;
     double s = 0.0;
-    for (int m = 0; m < nb; ++m) s = fma(M[(size_t)(k0 + m) * D + j], y[m], s);
-    rhs[j] -= s;
+#pragma unroll 8
+    for (int m = 0; m < nb; ++m) s = fma(M[(size_t)(k0 + m) * ld + j], y[m], s);
+    run[j] -= s;
   }
 }
 
-__global__ void solve_finish_kernel(const double* __restrict__ rhs, float* __restrict__ alpha, int D) {
+__global__ void solve_finish_kernel(const double* __restrict__ sol, float* __restrict__ alpha, int D) {
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
-  if (i < D) alpha[i] = (float)rhs[i];
+  if (i < D) alpha[i] = (float)sol[i];
 }
 
-size_t solve_workspace_bytes(int32_t D) { return align_up((size_t)D * D * 8, 256) + align_up((size_t)D * 8, 256) + 512; }
+size_t solve_workspace_bytes(int32_t D) {
+  return align_up((size_t)D * solve_ld(D) * 8, 256) + 2 * align_up((size_t)D * 8, 256) + 512;
+}
 
 int solve_normal_equations(const float* ZtZ, const float* Zty, int32_t D, double lambda, float* alpha, int32_t* info,
                            void* ws_ptr, size_t ws_bytes, cudaStream_t st) {
+  const int ld = solve_ld(D);
   Carver ws(ws_ptr, ws_bytes);
-  double* M = ws.take<double>((size_t)D * D);
-  double* rhs = ws.take<double>((size_t)D);
+  double* M = ws.take<double>((size_t)D * ld);
+  double* buf0 = ws.take<double>((size_t)D);
+  double* buf1 = ws.take<double>((size_t)D);
   if (!ws_ptr || ((uintptr_t)ws_ptr & 255) != 0 || !ws.fits()) return QMLL_ERR_WORKSPACE;
-  solve_prepare_kernel<<<1184, 256, 0, st>>>(ZtZ, Zty, D, lambda, M, rhs, info);
+  static bool attr_set = false;   // idempotent
+  if (!attr_set) {
+    if (cudaFuncSetAttribute(syrk_update_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kUSmemBytes) != cudaSuccess)
+      return QMLL_ERR_CUDA;
+    attr_set = true;
+  }
+  solve_prepare_kernel<<<1184, 256, 0, st>>>(ZtZ, Zty, D, ld, lambda, M, buf0, info);
   QMLL_LAUNCH_CHECK("solve_prepare_kernel");
   // Two levels: 64-wide steps factor a 256-wide panel (their updates touch the panel's own columns only), then ONE
   // rank-256 update of the trailing matrix: the trailing matrix is read and written D / 256 times instead of D / 64.
@@ -213,47 +327,39 @@ int solve_normal_equations(const float* ZtZ, const float* Zty, int32_t D, double
     const int nb2 = D - K0 < kNB2 ? D - K0 : kNB2;
     for (int k0 = K0; k0 < K0 + nb2; k0 += kNB) {
       const int nb = K0 + nb2 - k0 < kNB ? K0 + nb2 - k0 : kNB;
-      potrf_diag_kernel<<<1, 256, 0, st>>>(M, D, k0, nb, info);
+      potrf_diag_kernel<<<1, kNB, 0, st>>>(M, ld, k0, nb, info);
       QMLL_LAUNCH_CHECK("potrf_diag_kernel");
       const int rest = D - k0 - nb;
-      if (rest > 0) {
-        trsm_panel_kernel<<<(rest + 127) / 128, 128, 0, st>>>(M, D, k0, nb);
+      if (rest > 0) {                                      // then nb == kNB
+        trsm_panel_kernel<<<(rest + 127) / 128, 128, 0, st>>>(M, D, ld, k0);
         QMLL_LAUNCH_CHECK("trsm_panel_kernel");
         const int c0 = k0 + nb, c1 = K0 + nb2;             // the panel's remaining columns
         if (c1 > c0) {
-          dim3 g((unsigned)((D - c0 + kUT - 1) / kUT), (unsigned)((c1 - c0 + kUT - 1) / kUT));
-          syrk_update_kernel<<<g, 256, 0, st>>>(M, D, c0, c0, c1, k0, nb);
+          dim3 g((unsigned)((D - c0 + kUM - 1) / kUM), (unsigned)((c1 - c0 + kUN - 1) / kUN));
+          syrk_update_kernel<<<g, 128, kUSmemBytes, st>>>(M, D, ld, c0, c0, c1, k0, nb);
           QMLL_LAUNCH_CHECK("syrk_update_kernel(panel)");
         }
       }
     }
     const int t0 = K0 + nb2;                                // trailing matrix
     if (t0 < D) {
-      const unsigned nt = (unsigned)((D - t0 + kUT - 1) / kUT);
-      syrk_update_kernel<<<dim3(nt, nt), 256, 0, st>>>(M, D, t0, t0, D, K0, nb2);
+      dim3 g((unsigned)((D - t0 + kUM - 1) / kUM), (unsigned)((D - t0 + kUN - 1) / kUN));
+      syrk_update_kernel<<<g, 128, kUSmemBytes, st>>>(M, D, ld, t0, t0, D, K0, nb2);
       QMLL_LAUNCH_CHECK("syrk_update_kernel(trailing)");
     }
   }
-  for (int k0 = 0; k0 < D; k0 += kNB) {  // L y = b
+  for (int k0 = 0; k0 < D; k0 += kNB) {  // L y = b: running right-hand side in buf0, y into buf1
     const int nb = D - k0 < kNB ? D - k0 : kNB;
-    trsv_diag_kernel<<<1, 64, 0, st>>>(M, D, k0, nb, 0, rhs);
-    QMLL_LAUNCH_CHECK("trsv_diag_kernel");
     const int rest = D - k0 - nb;
-    if (rest > 0) {
-      trsv_update_kernel<<<(rest + 127) / 128, 128, 0, st>>>(M, D, k0, nb, 0, rhs);
-      QMLL_LAUNCH_CHECK("trsv_update_kernel");
-    }
+    trsv_step_kernel<<<rest > 0 ? (rest + 127) / 128 : 1, 128, 0, st>>>(M, D, ld, k0, nb, 0, buf0, buf1);
+    QMLL_LAUNCH_CHECK("trsv_step_kernel");
   }
-  for (int k0 = (D - 1) / kNB * kNB; k0 >= 0; k0 -= kNB) {  // L^T alpha = y
+  for (int k0 = (D - 1) / kNB * kNB; k0 >= 0; k0 -= kNB) {  // L^T alpha = y: running y in buf1, alpha into buf0
     const int nb = D - k0 < kNB ? D - k0 : kNB;
-    trsv_diag_kernel<<<1, 64, 0, st>>>(M, D, k0, nb, 1, rhs);
-    QMLL_LAUNCH_CHECK("trsv_diag_kernel");
-    if (k0 > 0) {
-      trsv_update_kernel<<<(k0 + 127) / 128, 128, 0, st>>>(M, D, k0, nb, 1, rhs);
-      QMLL_LAUNCH_CHECK("trsv_update_kernel");
-    }
+    trsv_step_kernel<<<k0 > 0 ? (k0 + 127) / 128 : 1, 128, 0, st>>>(M, D, ld, k0, nb, 1, buf1, buf0);
+    QMLL_LAUNCH_CHECK("trsv_step_kernel");
   }
-  solve_finish_kernel<<<(D + 255) / 256, 256, 0, st>>>(rhs, alpha, D);
+  solve_finish_kernel<<<(D + 255) / 256, 256, 0, st>>>(buf0, alpha, D);
   QMLL_LAUNCH_CHECK("solve_finish_kernel");
   return QMLL_OK;
 }

@@ -24,7 +24,8 @@ from . import load_library
 
 KINDS = {0: "fadd", 1: "ffma", 2: "fadd2", 3: "ffma2", 4: "lop3", 5: "shf", 6: "fadd2+lop3 (1:1), fp32 adds",
          7: "7 fadd + shf + lop3 (round-1 chain), fp32 adds", 8: "3 fadd2 + fadd + shf + lop3 (packed chain), fp32 adds",
-         9: "mufu.cos", 10: "lds.128 bytes", 11: "shfl", 12: "2 fadd2 + shf + lop3, fp32 adds"}
+         9: "mufu.cos", 10: "lds.128 bytes", 11: "shfl", 12: "2 fadd2 + shf + lop3, fp32 adds",
+         13: "dfma (FP64 FMAs)", 14: "dmma m8n8k4 (FP64 FMAs)"}
 
 
 def microbench(kind: int, iters: int = 4096, blocks_per_sm: int = 4, reps: int = 5) -> dict:
