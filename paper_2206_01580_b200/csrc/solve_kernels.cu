@@ -5,7 +5,8 @@
 //   potrf_diag_kernel (64 x 64 diagonal block, one row per thread in registers)  ->  trsm_panel_kernel (thread per
 //   row, column-oriented substitution)  ->  syrk_update_kernel on the 256-wide panel's own columns; after the panel
 //   one rank-256 syrk_update_kernel of the trailing matrix,
-// then forward / backward substitution, one launch per 64-wide block (trsv_step_kernel).
+// the right-hand side rides along as row D of the working matrix (so L y = b costs nothing extra), then the backward
+// substitution, one launch per 64-wide block (trsv_back_kernel).
 // syrk_update_kernel is the O(D^3) part: 128 x 64 tiles on the FP64 tensor-core path (mma.sync.m8n8k4.f64, DMMA: the
 // measured peak, profiles/peaks_r2.json kinds 13 / 14, is 18.5 T FMA/s against 17.0 for scalar DFMA, with 1/8 of the
 // instructions and 1/5 of the shared-memory loads), operands through a 3-stage cp.async ring, two CTAs per SM so that
@@ -43,35 +44,64 @@ __global__ void solve_prepare_kernel(const float* __restrict__ ZtZ, const float*
 
 // Cholesky of the nb x nb diagonal block at (k0, k0): A = L L^T, L overwrites the lower triangle.  Thread i holds row
 // i in registers (right-looking): per column ONE barrier -- every thread publishes its entry of column j, reads the
-// pivot and the column back, and updates its own row with independent FMAs.  Rows / columns >= nb are an identity pad.
+// pivot and the column back, and updates its own row with independent FMAs.  The row SHIFTS by one register per
+// column (a[p - 1] = fma(.., a[p])), so that register p always holds column j + p and the loop over j stays rolled:
+// fully unrolled it is 93 KB of straight-line code that runs once, at instruction-fetch speed (43 % "no instruction"
+// stalls, 32 us per block against 12 us now).  Rows / columns >= nb are an identity pad.
+template <int kPar>
+__device__ __forceinline__ void potrf_column(double (&a)[kNB], const double* __restrict__ colp, double* tile_row, int i,
+                                             int j, int nb, int k0, int* info) {
+  // colp = &col[kPar][j], j % 2 == kPar: colp + p is 16-byte aligned for p % 2 == kPar
+  const double piv = colp[0];
+  if (i == j && j < nb && !(piv > 0.0) && *info == 0) *info = k0 + j + 1;
+  const double dinv = rsqrt(piv);
+  const double l = a[0] * dinv;         // row j: sqrt(piv); rows below: l_ij; rows above: 0
+  if (i >= j) tile_row[j] = l;
+  const double s = l * dinv;            // l_ij / sqrt(piv); colp[p] * (1 / sqrt(piv)) = l_{j+p, j}
+  if (kPar == 0) {
+    a[0] = fma(-s, colp[1], a[1]);
+#pragma unroll
+    for (int p = 2; p < kNB; p += 2) {
+      const double2 c = *reinterpret_cast<const double2*>(colp + p);
+      a[p - 1] = fma(-s, c.x, a[p]);
+      a[p] = fma(-s, c.y, a[p + 1 < kNB ? p + 1 : p]);
+    }
+  } else {
+#pragma unroll
+    for (int p = 1; p < kNB - 1; p += 2) {
+      const double2 c = *reinterpret_cast<const double2*>(colp + p);
+      a[p - 1] = fma(-s, c.x, a[p]);
+      a[p] = fma(-s, c.y, a[p + 1]);
+    }
+    a[kNB - 2] = fma(-s, colp[kNB - 1], a[kNB - 1]);
+  }
+  a[kNB - 1] = 0.0;
+}
+
 __global__ void __launch_bounds__(kNB) potrf_diag_kernel(double* __restrict__ M, int ld, int k0, int nb, int* info) {
   __shared__ double tile[kNB][kNB + 1];
-  __shared__ double col[2][kNB];
+  __shared__ __align__(16) double col[2][2 * kNB];      // column j of every row; the upper half stays zero
   const int i = threadIdx.x;
   for (int idx = i; idx < kNB * kNB; idx += kNB) {
     const int r = idx / kNB, c = idx % kNB;
     if (r < nb && c <= r) cp_async8(&tile[r][c], M + (size_t)(k0 + r) * ld + k0 + c);
     else tile[r][c] = r == c ? 1.0 : 0.0;
   }
+  col[0][kNB + i] = col[1][kNB + i] = 0.0;
   cp_async_wait_all();
   __syncthreads();
   double a[kNB];
 #pragma unroll
   for (int c = 0; c < kNB; ++c) a[c] = tile[i][c];
-#pragma unroll
-  for (int j = 0; j < kNB; ++j) {
-    col[j & 1][i] = a[j];
+#pragma unroll 1
+  for (int j = 0; j < kNB; j += 2) {
+    col[0][i] = a[0];
     __syncthreads();
-    const double piv = col[j & 1][j];
-    if (i == j && j < nb && !(piv > 0.0) && *info == 0) *info = k0 + j + 1;
-    const double dinv = rsqrt(piv);
-    a[j] *= dinv;                       // row j: sqrt(piv); rows below: l_ij
-    const double s = a[j] * dinv;       // l_ij / sqrt(piv); col[c] * (1 / sqrt(piv)) = l_cj
-#pragma unroll
-    for (int c = j + 1; c < kNB; ++c) a[c] = fma(-s, col[j & 1][c], a[c]);   // rows above j hold a[j] = 0
+    potrf_column<0>(a, &col[0][j], tile[i], i, j, nb, k0, info);
+    col[1][i] = a[0];
+    __syncthreads();
+    potrf_column<1>(a, &col[1][j + 1], tile[i], i, j + 1, nb, k0, info);
   }
-#pragma unroll
-  for (int c = 0; c < kNB; ++c) tile[i][c] = a[c];
   __syncthreads();
   for (int idx = i; idx < nb * nb; idx += kNB) {
     const int r = idx / nb, c = idx % nb;
@@ -79,27 +109,33 @@ __global__ void __launch_bounds__(kNB) potrf_diag_kernel(double* __restrict__ M,
   }
 }
 
-// Rows below a full 64 x 64 diagonal block: X = A21 L11^-T, one thread per row, column-oriented forward substitution
-// (x_c final -> every later x_k gets its term: independent FMAs); L11 transposed in shared memory so that one
-// broadcast LDS.128 serves two FMAs.
+// Rows below the nb x nb diagonal block (rows k0 + nb .. n_rows - 1): X = A21 L11^-T, one thread per row,
+// column-oriented forward substitution (x_c final -> every later x_k gets its term: independent FMAs); L11 transposed
+// in shared memory so that one broadcast LDS.128 serves two FMAs.  Columns >= nb are an identity pad.
 constexpr int kLtLd = kNB + 2;
-__global__ void __launch_bounds__(128) trsm_panel_kernel(double* __restrict__ M, int D, int ld, int k0) {
+__global__ void __launch_bounds__(128) trsm_panel_kernel(double* __restrict__ M, int n_rows, int ld, int k0, int nb) {
   __shared__ __align__(16) double lt[kNB][kLtLd];   // lt[c][k] = L11[k][c]
   __shared__ double dinv[kNB];
   for (int idx = threadIdx.x; idx < kNB * kNB; idx += 128) {
     const int r = idx / kNB, c = idx % kNB;
-    cp_async8(&lt[c][r], M + (size_t)(k0 + r) * ld + k0 + c);
+    if (r < nb && c < nb) cp_async8(&lt[c][r], M + (size_t)(k0 + r) * ld + k0 + c);
+    else lt[c][r] = r == c ? 1.0 : 0.0;
   }
   cp_async_wait_all();
   __syncthreads();
   if (threadIdx.x < kNB) dinv[threadIdx.x] = 1.0 / lt[threadIdx.x][threadIdx.x];
   __syncthreads();
-  const int i = k0 + kNB + blockIdx.x * 128 + threadIdx.x;
-  if (i >= D) return;
+  const int i = k0 + nb + blockIdx.x * 128 + threadIdx.x;
+  if (i >= n_rows) return;
   double2* row = reinterpret_cast<double2*>(M + (size_t)i * ld + k0);
   double x[kNB];
+  if (nb == kNB) {
 #pragma unroll
-  for (int c = 0; c < kNB; c += 2) { const double2 v = row[c / 2]; x[c] = v.x; x[c + 1] = v.y; }
+    for (int c = 0; c < kNB; c += 2) { const double2 v = row[c / 2]; x[c] = v.x; x[c + 1] = v.y; }
+  } else {
+#pragma unroll
+    for (int c = 0; c < kNB; ++c) x[c] = c < nb ? M[(size_t)i * ld + k0 + c] : 0.0;
+  }
 #pragma unroll
   for (int c = 0; c < kNB; ++c) {
     x[c] *= dinv[c];
@@ -113,8 +149,14 @@ __global__ void __launch_bounds__(128) trsm_panel_kernel(double* __restrict__ M,
       x[k + 1] = fma(-xc, l2.y, x[k + 1]);
     }
   }
+  if (nb == kNB) {
 #pragma unroll
-  for (int c = 0; c < kNB; c += 2) row[c / 2] = make_double2(x[c], x[c + 1]);
+    for (int c = 0; c < kNB; c += 2) row[c / 2] = make_double2(x[c], x[c + 1]);
+  } else {
+#pragma unroll
+    for (int c = 0; c < kNB; ++c)
+      if (c < nb) M[(size_t)i * ld + k0 + c] = x[c];
+  }
 }
 
 // Symmetric rank-kn update on the lower triangle:  C[i][j] -= sum_{m < kn} M[i][k0 + m] * M[j][k0 + m]  for rows
@@ -123,7 +165,7 @@ __global__ void __launch_bounds__(128) trsm_panel_kernel(double* __restrict__ M,
 // operands are row-major slices of M with k contiguous, which is exactly the m8n8k4 fragment order (A: row lane / 4,
 // k lane % 4; B the same with the row as n), so the stages are plain copies: [rows][16 k] with a row pitch of 20
 // doubles (conflict-free LDS.64 for the 8 rows x 4 k a fragment touches), filled by 16-byte cp.async (zero-filled
-// beyond kn and beyond row D).
+// beyond kn and beyond the last row).  n_rows = D + 1: the extra row carries the right-hand side.
 constexpr int kUM = 128, kUN = 64, kUK = 16, kUPitch = 20, kUStages = 3;
 constexpr int kUStageDoubles = (kUM + kUN) * kUPitch;
 constexpr int kUSmemBytes = kUStages * kUStageDoubles * 8;
@@ -135,7 +177,7 @@ __device__ __forceinline__ void dmma_m8n8k4(double& c0, double& c1, double a, do
   asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0, %1}, {%2}, {%3}, {%0, %1};" : "+d"(c0), "+d"(c1) : "d"(a), "d"(b));
 }
 
-__global__ void __launch_bounds__(128, 2) syrk_update_kernel(double* __restrict__ M, int D, int ld, int r0, int c0,
+__global__ void __launch_bounds__(128, 2) syrk_update_kernel(double* __restrict__ M, int n_rows, int ld, int r0, int c0,
                                                              int c1, int k0, int kn) {
   const int i0 = r0 + blockIdx.x * kUM, j0 = c0 + blockIdx.y * kUN;
   if (j0 >= c1 || j0 > i0 + kUM - 1) return;          // tile entirely above the diagonal or outside the column range
@@ -155,7 +197,7 @@ __global__ void __launch_bounds__(128, 2) syrk_update_kernel(double* __restrict_
 #pragma unroll
     for (int q = 0; q < 12; ++q) {
       const int gr = q < 8 ? i0 + lrow + 16 * q : j0 + lrow + 16 * (q - 8);
-      const bool ok = gr < D;
+      const bool ok = gr < n_rows;
       cp_async16_zfill(dst + (uint32_t)(16 * q * kUPitch * 8), col + (size_t)(ok ? gr : 0) * ld, ok ? bytes : 0);
     }
   };
@@ -192,37 +234,35 @@ __global__ void __launch_bounds__(128, 2) syrk_update_kernel(double* __restrict_
         for (int v = 0; v < 4; ++v) dmma_m8n8k4(acc[u][v][0], acc[u][v][1], a[u], b[v]);
     }
   }
-  // epilogue: the thread holds C[row g][columns 2 tg, 2 tg + 1] of every 8 x 8 tile: 16-byte read-modify-write
+  // epilogue: the thread holds C[row g][columns 2 tg, 2 tg + 1] of every 8 x 8 tile
 #pragma unroll
   for (int u = 0; u < 8; ++u) {
     const int i = i0 + wr * 64 + 8 * u + g;
-    if (i >= D) continue;
+    if (i >= n_rows) continue;
 #pragma unroll
     for (int v = 0; v < 4; ++v) {
       const int j = j0 + wc * 32 + 8 * v + 2 * tg;
       double* p = M + (size_t)i * ld + j;
-      if (j + 1 <= i && j + 1 < c1) {
-        double2 c = *reinterpret_cast<double2*>(p);
-        c.x -= acc[u][v][0]; c.y -= acc[u][v][1];
-        *reinterpret_cast<double2*>(p) = c;
-      } else if (j <= i && j < c1) {
-        *p -= acc[u][v][0];
-      }
+      // fire-and-forget reductions (RED.ADD.F64): every element belongs to exactly one thread of one CTA, so the
+      // result is deterministic, and no load latency is exposed at the end of the tile (a read-modify-write epilogue
+      // cost 30 % of the warp stalls)
+      if (j <= i && j < c1) atomicAdd(p, -acc[u][v][0]);
+      if (j + 1 <= i && j + 1 < c1) atomicAdd(p + 1, -acc[u][v][1]);
     }
   }
 }
 
-// One block step of a substitution.  transposed = 0 (forward, L y = b): solves the nb x nb diagonal block for
-// sol[k0 .. k0 + nb) from run[k0 ..) and subtracts L[i][k0 ..] . sol from run[i] for every row i >= k0 + nb.
-// transposed = 1 (backward, L^T a = y): the same with L11^T, and run[j] -= sum_m L[k0 + m][j] sol[k0 + m] for j < k0.
-// Every CTA repeats the small diagonal solve (warp 0: two rows per lane, the solved entry travels by shuffle), so a
-// step is ONE launch; CTA 0 writes `sol`.  `run` entries of the block itself are only read.
-__global__ void __launch_bounds__(128) trsv_step_kernel(const double* __restrict__ M, int D, int ld, int k0, int nb,
-                                                        int transposed, double* __restrict__ run,
-                                                        double* __restrict__ sol) {
+// One block step of the backward substitution L^T a = y (the forward substitution L y = b needs no kernel: the
+// right-hand side rides through the factorisation as row D of the working matrix, so that trsm_panel_kernel solves it
+// and syrk_update_kernel updates it like any other row).  Solves the nb x nb diagonal block for sol[k0 .. k0 + nb) from
+// run[k0 ..) with L11^T, then run[j] -= sum_m L[k0 + m][j] sol[k0 + m] for j < k0.  Every CTA repeats the small
+// diagonal solve (warp 0: two rows per lane, the solved entry travels by shuffle), so a step is ONE launch; CTA 0
+// writes `sol`.  `run` entries of the block itself are only read.
+__global__ void __launch_bounds__(128) trsv_back_kernel(const double* __restrict__ M, int ld, int k0, int nb,
+                                                        double* __restrict__ run, double* __restrict__ sol) {
   __shared__ double l[kNB][kNB + 1];
   __shared__ double dinv[kNB];
-  __shared__ __align__(16) double y[kNB];
+  __shared__ double y[kNB];
   const int t = threadIdx.x, lane = t & 31;
   for (int idx = t; idx < kNB * kNB; idx += 128) {
     const int r = idx / kNB, c = idx % kNB;
@@ -235,20 +275,11 @@ __global__ void __launch_bounds__(128) trsv_step_kernel(const double* __restrict
   __syncthreads();
   if (t < 32) {
     double b0 = lane < nb ? run[k0 + lane] : 0.0, b1 = lane + 32 < nb ? run[k0 + 32 + lane] : 0.0;
-    if (!transposed) {
-      for (int c = 0; c < kNB; ++c) {
-        const double bc = __shfl_sync(0xffffffffu, c < 32 ? b0 : b1, c & 31) * dinv[c];
-        if (lane == (c & 31)) { if (c < 32) b0 = bc; else b1 = bc; }
-        if (lane > c) b0 = fma(-l[lane][c], bc, b0);
-        if (lane + 32 > c) b1 = fma(-l[lane + 32][c], bc, b1);
-      }
-    } else {
-      for (int c = kNB - 1; c >= 0; --c) {
-        const double bc = __shfl_sync(0xffffffffu, c < 32 ? b0 : b1, c & 31) * dinv[c];
-        if (lane == (c & 31)) { if (c < 32) b0 = bc; else b1 = bc; }
-        if (lane < c) b0 = fma(-l[c][lane], bc, b0);
-        if (lane + 32 < c) b1 = fma(-l[c][lane + 32], bc, b1);
-      }
+    for (int c = kNB - 1; c >= 0; --c) {
+      const double bc = __shfl_sync(0xffffffffu, c < 32 ? b0 : b1, c & 31) * dinv[c];
+      if (lane == (c & 31)) { if (c < 32) b0 = bc; else b1 = bc; }
+      if (lane < c) b0 = fma(-l[c][lane], bc, b0);
+      if (lane + 32 < c) b1 = fma(-l[c][lane + 32], bc, b1);
     }
     y[lane] = b0; y[lane + 32] = b1;
     if (blockIdx.x == 0) {
@@ -257,43 +288,18 @@ __global__ void __launch_bounds__(128) trsv_step_kernel(const double* __restrict
     }
   }
   __syncthreads();
-  if (!transposed) {
-    // rows below the block: 8 lanes per row (16-byte loads, 128 contiguous bytes per row and load), 16 rows per pass
-    const int sub = t & 7, rloc = t >> 3;
-    const int base = k0 + nb + blockIdx.x * 128;
-    if (base >= D) return;
-    double s[8];
-#pragma unroll
-    for (int p = 0; p < 8; ++p) {
-      const int row = base + p * 16 + rloc;
-      s[p] = 0.0;
-      if (row < D) {
-        const double2* src = reinterpret_cast<const double2*>(M + (size_t)row * ld + k0);
-#pragma unroll
-        for (int q = 0; q < 4; ++q) {
-          const double2 v = src[sub + 8 * q];
-          const double2 w = *reinterpret_cast<const double2*>(&y[2 * sub + 16 * q]);
-          s[p] = fma(v.x, w.x, s[p]);
-          s[p] = fma(v.y, w.y, s[p]);
-        }
-      }
-    }
-#pragma unroll
-    for (int p = 0; p < 8; ++p) {
-      s[p] += __shfl_xor_sync(0xffffffffu, s[p], 1);
-      s[p] += __shfl_xor_sync(0xffffffffu, s[p], 2);
-      s[p] += __shfl_xor_sync(0xffffffffu, s[p], 4);
-      const int row = base + p * 16 + rloc;
-      if (sub == 0 && row < D) run[row] -= s[p];
-    }
-  } else {
-    const int j = blockIdx.x * 128 + t;
-    if (j >= k0) return;
-    double s = 0.0;
-#pragma unroll 8
-    for (int m = 0; m < nb; ++m) s = fma(M[(size_t)(k0 + m) * ld + j], y[m], s);
-    run[j] -= s;
+  const int j = blockIdx.x * 128 + t;
+  if (j >= k0) return;
+  double s0 = 0.0, s1 = 0.0, s2 = 0.0, s3 = 0.0;      // four chains: 16 loads in flight per thread
+  const double* colp = M + (size_t)k0 * ld + j;
+#pragma unroll 4
+  for (int m = 0; m < kNB; m += 4) {
+    if (m + 0 < nb) s0 = fma(colp[(size_t)(m + 0) * ld], y[m + 0], s0);
+    if (m + 1 < nb) s1 = fma(colp[(size_t)(m + 1) * ld], y[m + 1], s1);
+    if (m + 2 < nb) s2 = fma(colp[(size_t)(m + 2) * ld], y[m + 2], s2);
+    if (m + 3 < nb) s3 = fma(colp[(size_t)(m + 3) * ld], y[m + 3], s3);
   }
+  run[j] -= (s0 + s1) + (s2 + s3);
 }
 
 __global__ void solve_finish_kernel(const double* __restrict__ sol, float* __restrict__ alpha, int D) {
@@ -301,17 +307,17 @@ __global__ void solve_finish_kernel(const double* __restrict__ sol, float* __res
   if (i < D) alpha[i] = (float)sol[i];
 }
 
+// working matrix: D + 1 rows (row D = right-hand side) plus one row of slack for 16-byte accesses at the end
 size_t solve_workspace_bytes(int32_t D) {
-  return align_up((size_t)D * solve_ld(D) * 8, 256) + 2 * align_up((size_t)D * 8, 256) + 512;
+  return align_up((size_t)(D + 2) * solve_ld(D) * 8, 256) + align_up((size_t)D * 8, 256) + 512;
 }
 
 int solve_normal_equations(const float* ZtZ, const float* Zty, int32_t D, double lambda, float* alpha, int32_t* info,
                            void* ws_ptr, size_t ws_bytes, cudaStream_t st) {
-  const int ld = solve_ld(D);
+  const int ld = solve_ld(D), n_rows = D + 1;
   Carver ws(ws_ptr, ws_bytes);
-  double* M = ws.take<double>((size_t)D * ld);
-  double* buf0 = ws.take<double>((size_t)D);
-  double* buf1 = ws.take<double>((size_t)D);
+  double* M = ws.take<double>((size_t)(D + 2) * ld);
+  double* sol = ws.take<double>((size_t)D);
   if (!ws_ptr || ((uintptr_t)ws_ptr & 255) != 0 || !ws.fits()) return QMLL_ERR_WORKSPACE;
   static bool attr_set = false;   // idempotent
   if (!attr_set) {
@@ -319,7 +325,8 @@ int solve_normal_equations(const float* ZtZ, const float* Zty, int32_t D, double
       return QMLL_ERR_CUDA;
     attr_set = true;
   }
-  solve_prepare_kernel<<<1184, 256, 0, st>>>(ZtZ, Zty, D, ld, lambda, M, buf0, info);
+  double* y = M + (size_t)D * ld;                           // row D: b on entry, y = L^-1 b after the factorisation
+  solve_prepare_kernel<<<1184, 256, 0, st>>>(ZtZ, Zty, D, ld, lambda, M, y, info);
   QMLL_LAUNCH_CHECK("solve_prepare_kernel");
   // Two levels: 64-wide steps factor a 256-wide panel (their updates touch the panel's own columns only), then ONE
   // rank-256 update of the trailing matrix: the trailing matrix is read and written D / 256 times instead of D / 64.
@@ -329,37 +336,29 @@ int solve_normal_equations(const float* ZtZ, const float* Zty, int32_t D, double
       const int nb = K0 + nb2 - k0 < kNB ? K0 + nb2 - k0 : kNB;
       potrf_diag_kernel<<<1, kNB, 0, st>>>(M, ld, k0, nb, info);
       QMLL_LAUNCH_CHECK("potrf_diag_kernel");
-      const int rest = D - k0 - nb;
-      if (rest > 0) {                                      // then nb == kNB
-        trsm_panel_kernel<<<(rest + 127) / 128, 128, 0, st>>>(M, D, ld, k0);
-        QMLL_LAUNCH_CHECK("trsm_panel_kernel");
-        const int c0 = k0 + nb, c1 = K0 + nb2;             // the panel's remaining columns
-        if (c1 > c0) {
-          dim3 g((unsigned)((D - c0 + kUM - 1) / kUM), (unsigned)((c1 - c0 + kUN - 1) / kUN));
-          syrk_update_kernel<<<g, 128, kUSmemBytes, st>>>(M, D, ld, c0, c0, c1, k0, nb);
-          QMLL_LAUNCH_CHECK("syrk_update_kernel(panel)");
-        }
+      const int rest = n_rows - k0 - nb;                    // >= 1: the right-hand side row
+      trsm_panel_kernel<<<(rest + 127) / 128, 128, 0, st>>>(M, n_rows, ld, k0, nb);
+      QMLL_LAUNCH_CHECK("trsm_panel_kernel");
+      const int c0 = k0 + nb, c1 = K0 + nb2;               // the panel's remaining columns
+      if (c1 > c0) {
+        dim3 g((unsigned)((n_rows - c0 + kUM - 1) / kUM), (unsigned)((c1 - c0 + kUN - 1) / kUN));
+        syrk_update_kernel<<<g, 128, kUSmemBytes, st>>>(M, n_rows, ld, c0, c0, c1, k0, nb);
+        QMLL_LAUNCH_CHECK("syrk_update_kernel(panel)");
       }
     }
     const int t0 = K0 + nb2;                                // trailing matrix
     if (t0 < D) {
-      dim3 g((unsigned)((D - t0 + kUM - 1) / kUM), (unsigned)((D - t0 + kUN - 1) / kUN));
-      syrk_update_kernel<<<g, 128, kUSmemBytes, st>>>(M, D, ld, t0, t0, D, K0, nb2);
+      dim3 g((unsigned)((n_rows - t0 + kUM - 1) / kUM), (unsigned)((D - t0 + kUN - 1) / kUN));
+      syrk_update_kernel<<<g, 128, kUSmemBytes, st>>>(M, n_rows, ld, t0, t0, D, K0, nb2);
       QMLL_LAUNCH_CHECK("syrk_update_kernel(trailing)");
     }
   }
-  for (int k0 = 0; k0 < D; k0 += kNB) {  // L y = b: running right-hand side in buf0, y into buf1
+  for (int k0 = (D - 1) / kNB * kNB; k0 >= 0; k0 -= kNB) {  // L^T alpha = y: running y in row D, alpha into sol
     const int nb = D - k0 < kNB ? D - k0 : kNB;
-    const int rest = D - k0 - nb;
-    trsv_step_kernel<<<rest > 0 ? (rest + 127) / 128 : 1, 128, 0, st>>>(M, D, ld, k0, nb, 0, buf0, buf1);
-    QMLL_LAUNCH_CHECK("trsv_step_kernel");
+    trsv_back_kernel<<<k0 > 0 ? (k0 + 127) / 128 : 1, 128, 0, st>>>(M, ld, k0, nb, y, sol);
+    QMLL_LAUNCH_CHECK("trsv_back_kernel");
   }
-  for (int k0 = (D - 1) / kNB * kNB; k0 >= 0; k0 -= kNB) {  // L^T alpha = y: running y in buf1, alpha into buf0
-    const int nb = D - k0 < kNB ? D - k0 : kNB;
-    trsv_step_kernel<<<k0 > 0 ? (k0 + 127) / 128 : 1, 128, 0, st>>>(M, D, ld, k0, nb, 1, buf1, buf0);
-    QMLL_LAUNCH_CHECK("trsv_step_kernel");
-  }
-  solve_finish_kernel<<<(D + 255) / 256, 256, 0, st>>>(buf0, alpha, D);
+  solve_finish_kernel<<<(D + 255) / 256, 256, 0, st>>>(sol, alpha, D);
   QMLL_LAUNCH_CHECK("solve_finish_kernel");
   return QMLL_OK;
 }
