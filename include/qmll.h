@@ -261,7 +261,11 @@ int qmll_predict(const qmll_sorf_params* p, const float* x, const int32_t* elem,
  * normal equations of eq. 16-17 (L134-144; "solved by LU decomposition", L137 -- SPD, so a blocked Cholesky), in FP64.
  *   ZtZ [D, D] fp32 symmetric (only the lower triangle is read), Zty [D] fp32, lambda >= 0, alpha [D] fp32 out,
  *   info: device int32, LAPACK convention: 0 = success, k > 0 = leading minor of order k not positive definite
- *   (alpha is then NaN-contaminated).  The inputs are not modified. */
+ *   (alpha is then NaN-contaminated).  The inputs are not modified.  D <= 65534 (else QMLL_ERR_UNSUPPORTED).
+ *   Stream behaviour: panel factorisations run on an internal high-priority stream, forked from and joined back into
+ *   `cuda_stream` with events (look-ahead, overlapping the trailing update); every effect of the call is ordered on
+ *   `cuda_stream` as usual, and the pattern is stream-capturable.  The internal stream and its events are created
+ *   once per device on first use and live for the process; concurrent calls are serialised at enqueue by a mutex. */
 int qmll_solve(const float* ZtZ, const float* Zty, int32_t D, double lambda, float* alpha, int32_t* info,
                void* workspace, size_t workspace_bytes, void* cuda_stream);
 

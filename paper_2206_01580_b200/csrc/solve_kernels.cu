@@ -13,6 +13,8 @@
 // the read-modify-write epilogue of one overlaps the main loop of the other.
 // `info` (device int) follows LAPACK: 0 = success, k > 0 = the leading minor of order k is not positive definite (the
 // factorisation then carries NaNs).  The working matrix has leading dimension ld = D rounded up to 8 (16-byte copies).
+#include <mutex>
+
 #include "qmll_common.cuh"
 
 namespace qmll {
@@ -29,17 +31,25 @@ __device__ __forceinline__ void cp_async8(void* smem_dst, const void* src) {
 }
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
 
-__global__ void solve_prepare_kernel(const float* __restrict__ ZtZ, const float* __restrict__ Zty, int D, int ld,
-                                     double lambda, double* __restrict__ M, double* __restrict__ rhs,
-                                     int* __restrict__ info) {
-  const long long n = (long long)D * D;
-  for (long long idx = blockIdx.x * (long long)blockDim.x + threadIdx.x; idx < n;
-       idx += (long long)gridDim.x * blockDim.x) {
-    const int i = (int)(idx / D), j = (int)(idx % D);
-    M[(size_t)i * ld + j] = (double)ZtZ[idx] + (i == j ? lambda : 0.0);
-    if (j == 0) rhs[i] = (double)Zty[i];
+// M = lower triangle of ZtZ + lambda I in FP64 (row i, columns 0 .. i; the upper triangle is never read), row D = Zty
+__global__ void __launch_bounds__(256) solve_prepare_kernel(const float* __restrict__ ZtZ, const float* __restrict__ Zty,
+                                                            int D, int ld, double lambda, double* __restrict__ M,
+                                                            double* __restrict__ rhs, int* __restrict__ info) {
+  const int i = blockIdx.y;
+  const int j = blockIdx.x * 1024 + threadIdx.x * 4;
+  if (blockIdx.x == 0 && i == 0 && threadIdx.x == 0) *info = 0;
+  if (i == D) {
+#pragma unroll
+    for (int q = 0; q < 4; ++q)
+      if (j + q < D) rhs[j + q] = (double)Zty[j + q];
+    return;
   }
-  if (blockIdx.x == 0 && threadIdx.x == 0) *info = 0;
+  if (j > i) return;
+  const float* src = ZtZ + (size_t)i * D + j;
+  double* dst = M + (size_t)i * ld + j;
+#pragma unroll
+  for (int q = 0; q < 4; ++q)
+    if (j + q <= i) dst[q] = (double)src[q] + (j + q == i ? lambda : 0.0);
 }
 
 // Cholesky of the nb x nb diagonal block at (k0, k0): A = L L^T, L overwrites the lower triangle.  Thread i holds row
@@ -312,47 +322,101 @@ size_t solve_workspace_bytes(int32_t D) {
   return align_up((size_t)(D + 2) * solve_ld(D) * 8, 256) + align_up((size_t)D * 8, 256) + 512;
 }
 
+// Look-ahead (the classic one): the panel steps are short, serial kernels that leave the GPU mostly idle, so panel
+// P + 1 is factorised on an internal high-priority stream WHILE the caller's stream runs the rank-256 update of the
+// rest of the trailing matrix with panel P.  Per panel: [hi] factor P, update only the columns of panel P + 1 ->
+// [caller] update the columns beyond P + 1 || [hi] factor P + 1 -> ...  Fork / join by events (capturable).  The
+// stream and events are created once per device and live for the process; a mutex serialises the enqueue.
+struct SolveSide {
+  cudaStream_t hi = nullptr;
+  cudaEvent_t ev_main = nullptr, ev_hi = nullptr;
+  bool ready = false;
+};
+static std::mutex g_solve_mutex;
+static SolveSide g_solve_side[64];
+
+static int solve_side(SolveSide** out) {
+  int dev = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) return QMLL_ERR_CUDA;
+  SolveSide& s = g_solve_side[dev];
+  if (!s.ready) {
+    int lo = 0, hi = 0;
+    if (cudaDeviceGetStreamPriorityRange(&lo, &hi) != cudaSuccess) return QMLL_ERR_CUDA;
+    if (cudaStreamCreateWithPriority(&s.hi, cudaStreamNonBlocking, hi) != cudaSuccess) return QMLL_ERR_CUDA;
+    if (cudaEventCreateWithFlags(&s.ev_main, cudaEventDisableTiming) != cudaSuccess) return QMLL_ERR_CUDA;
+    if (cudaEventCreateWithFlags(&s.ev_hi, cudaEventDisableTiming) != cudaSuccess) return QMLL_ERR_CUDA;
+    if (cudaFuncSetAttribute(syrk_update_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kUSmemBytes) != cudaSuccess)
+      return QMLL_ERR_CUDA;
+    s.ready = true;
+  }
+  *out = &s;
+  return QMLL_OK;
+}
+
+#define QMLL_SOLVE_CUDA(call) do { if ((call) != cudaSuccess) return QMLL_ERR_CUDA; } while (0)
+
+// 64-wide steps over the 256-wide panel at K0; their updates touch the panel's own columns only
+static int solve_factor_panel(double* M, int D, int ld, int K0, int32_t* info, cudaStream_t st) {
+  const int n_rows = D + 1;
+  const int nb2 = D - K0 < kNB2 ? D - K0 : kNB2;
+  for (int k0 = K0; k0 < K0 + nb2; k0 += kNB) {
+    const int nb = K0 + nb2 - k0 < kNB ? K0 + nb2 - k0 : kNB;
+    potrf_diag_kernel<<<1, kNB, 0, st>>>(M, ld, k0, nb, info);
+    QMLL_LAUNCH_CHECK("potrf_diag_kernel");
+    const int rest = n_rows - k0 - nb;                    // >= 1: the right-hand side row
+    trsm_panel_kernel<<<(rest + 127) / 128, 128, 0, st>>>(M, n_rows, ld, k0, nb);
+    QMLL_LAUNCH_CHECK("trsm_panel_kernel");
+    const int c0 = k0 + nb, c1 = K0 + nb2;               // the panel's remaining columns
+    if (c1 > c0) {
+      dim3 g((unsigned)((n_rows - c0 + kUM - 1) / kUM), (unsigned)((c1 - c0 + kUN - 1) / kUN));
+      syrk_update_kernel<<<g, 128, kUSmemBytes, st>>>(M, n_rows, ld, c0, c0, c1, k0, nb);
+      QMLL_LAUNCH_CHECK("syrk_update_kernel(panel)");
+    }
+  }
+  return QMLL_OK;
+}
+
 int solve_normal_equations(const float* ZtZ, const float* Zty, int32_t D, double lambda, float* alpha, int32_t* info,
                            void* ws_ptr, size_t ws_bytes, cudaStream_t st) {
+  if (D > 65534) return QMLL_ERR_UNSUPPORTED;             // grid.y of the prepare pass; 34 GB of FP64 beyond that
   const int ld = solve_ld(D), n_rows = D + 1;
   Carver ws(ws_ptr, ws_bytes);
   double* M = ws.take<double>((size_t)(D + 2) * ld);
   double* sol = ws.take<double>((size_t)D);
   if (!ws_ptr || ((uintptr_t)ws_ptr & 255) != 0 || !ws.fits()) return QMLL_ERR_WORKSPACE;
-  static bool attr_set = false;   // idempotent
-  if (!attr_set) {
-    if (cudaFuncSetAttribute(syrk_update_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kUSmemBytes) != cudaSuccess)
-      return QMLL_ERR_CUDA;
-    attr_set = true;
-  }
+  std::lock_guard<std::mutex> lock(g_solve_mutex);
+  SolveSide* side = nullptr;
+  if (int rc = solve_side(&side)) return rc;
+  cudaStream_t hi = side->hi;
   double* y = M + (size_t)D * ld;                           // row D: b on entry, y = L^-1 b after the factorisation
-  solve_prepare_kernel<<<1184, 256, 0, st>>>(ZtZ, Zty, D, ld, lambda, M, y, info);
+  solve_prepare_kernel<<<dim3((unsigned)((D + 1023) / 1024), (unsigned)(D + 1)), 256, 0, st>>>(ZtZ, Zty, D, ld, lambda, M, y, info);
   QMLL_LAUNCH_CHECK("solve_prepare_kernel");
-  // Two levels: 64-wide steps factor a 256-wide panel (their updates touch the panel's own columns only), then ONE
-  // rank-256 update of the trailing matrix: the trailing matrix is read and written D / 256 times instead of D / 64.
+  QMLL_SOLVE_CUDA(cudaEventRecord(side->ev_main, st));
+  QMLL_SOLVE_CUDA(cudaStreamWaitEvent(hi, side->ev_main, 0));
+  if (int rc = solve_factor_panel(M, D, ld, 0, info, hi)) return rc;
   for (int K0 = 0; K0 < D; K0 += kNB2) {
     const int nb2 = D - K0 < kNB2 ? D - K0 : kNB2;
-    for (int k0 = K0; k0 < K0 + nb2; k0 += kNB) {
-      const int nb = K0 + nb2 - k0 < kNB ? K0 + nb2 - k0 : kNB;
-      potrf_diag_kernel<<<1, kNB, 0, st>>>(M, ld, k0, nb, info);
-      QMLL_LAUNCH_CHECK("potrf_diag_kernel");
-      const int rest = n_rows - k0 - nb;                    // >= 1: the right-hand side row
-      trsm_panel_kernel<<<(rest + 127) / 128, 128, 0, st>>>(M, n_rows, ld, k0, nb);
-      QMLL_LAUNCH_CHECK("trsm_panel_kernel");
-      const int c0 = k0 + nb, c1 = K0 + nb2;               // the panel's remaining columns
-      if (c1 > c0) {
-        dim3 g((unsigned)((n_rows - c0 + kUM - 1) / kUM), (unsigned)((c1 - c0 + kUN - 1) / kUN));
-        syrk_update_kernel<<<g, 128, kUSmemBytes, st>>>(M, n_rows, ld, c0, c0, c1, k0, nb);
-        QMLL_LAUNCH_CHECK("syrk_update_kernel(panel)");
-      }
+    const int t0 = K0 + nb2;                                // trailing matrix starts here
+    if (t0 >= D) break;
+    const int t1 = D - t0 < kNB2 ? D : t0 + kNB2;           // end of the next panel's columns
+    {                                                       // [hi] columns of the next panel only
+      dim3 g((unsigned)((n_rows - t0 + kUM - 1) / kUM), (unsigned)((t1 - t0 + kUN - 1) / kUN));
+      syrk_update_kernel<<<g, 128, kUSmemBytes, hi>>>(M, n_rows, ld, t0, t0, t1, K0, nb2);
+      QMLL_LAUNCH_CHECK("syrk_update_kernel(look-ahead)");
     }
-    const int t0 = K0 + nb2;                                // trailing matrix
-    if (t0 < D) {
-      dim3 g((unsigned)((n_rows - t0 + kUM - 1) / kUM), (unsigned)((D - t0 + kUN - 1) / kUN));
-      syrk_update_kernel<<<g, 128, kUSmemBytes, st>>>(M, n_rows, ld, t0, t0, D, K0, nb2);
+    QMLL_SOLVE_CUDA(cudaEventRecord(side->ev_hi, hi));
+    QMLL_SOLVE_CUDA(cudaStreamWaitEvent(st, side->ev_hi, 0));
+    if (t1 < D) {                                           // [caller] the rest of the trailing matrix
+      dim3 g((unsigned)((n_rows - t1 + kUM - 1) / kUM), (unsigned)((D - t1 + kUN - 1) / kUN));
+      syrk_update_kernel<<<g, 128, kUSmemBytes, st>>>(M, n_rows, ld, t1, t1, D, K0, nb2);
       QMLL_LAUNCH_CHECK("syrk_update_kernel(trailing)");
     }
+    QMLL_SOLVE_CUDA(cudaEventRecord(side->ev_main, st));
+    if (int rc = solve_factor_panel(M, D, ld, t0, info, hi)) return rc;   // [hi] overlaps the trailing update
+    QMLL_SOLVE_CUDA(cudaStreamWaitEvent(hi, side->ev_main, 0));           // before hi touches columns >= t1
   }
+  QMLL_SOLVE_CUDA(cudaEventRecord(side->ev_hi, hi));
+  QMLL_SOLVE_CUDA(cudaStreamWaitEvent(st, side->ev_hi, 0));
   for (int k0 = (D - 1) / kNB * kNB; k0 >= 0; k0 -= kNB) {  // L^T alpha = y: running y in row D, alpha into sol
     const int nb = D - k0 < kNB ? D - k0 : kNB;
     trsv_back_kernel<<<k0 > 0 ? (k0 + 127) / 128 : 1, 128, 0, st>>>(M, ld, k0, nb, y, sol);

@@ -305,7 +305,8 @@ def test_error_codes(q):
         pkg.qmll_sorf_forward(bad2, dp.x, dp.elem, dp.mol_off)
 
 
-@pytest.mark.parametrize("D,rows", [(1, 4), (50, 300), (256, 448), (1000, 3000), (4096, 6000)])
+@pytest.mark.parametrize("D,rows", [(1, 4), (37, 100), (50, 300), (256, 448), (321, 700), (577, 900), (1000, 3000),
+                                    (4096, 6000)])
 def test_solve_matches_oracle(q, D, rows):
     """qmll_solve (blocked FP64 Cholesky) against the oracle's unblocked one on the same fp32 ZtZ / Zty."""
     pkg, wio, torch = q
@@ -326,6 +327,42 @@ def test_solve_reports_non_positive_definite(q):
     bad = torch.tensor([[1.0, 2.0], [2.0, 1.0]], device="cuda")
     _, info = pkg.qmll_solve(bad, torch.ones(2, device="cuda"), 0.0)
     assert int(info.item()) == 2
+    # the first bad pivot lies in a later panel (order 334 = second 256-wide panel, second 64-wide step)
+    diag = torch.ones(600, device="cuda")
+    diag[333] = -1.0
+    diag[500] = -1.0
+    _, info = pkg.qmll_solve(torch.diag(diag), torch.ones(600, device="cuda"), 0.0)
+    assert int(info.item()) == 334
+
+
+def test_solve_on_a_side_stream_and_under_graph_capture(q):
+    """qmll_solve forks panel work onto an internal stream (look-ahead): the result must not depend on the caller's
+    stream, and the fork / join must be capturable."""
+    pkg, wio, torch = q
+    rng = np.random.default_rng(5)
+    D = 700
+    A = rng.standard_normal((1500, D)).astype(np.float32)
+    ZtZ = torch.from_numpy((A.T @ A).astype(np.float32)).cuda()
+    Zty = torch.from_numpy((A.T @ rng.standard_normal(1500).astype(np.float32))).cuda()
+    ref, info = pkg.qmll_solve(ZtZ, Zty, 1e-2)
+    assert int(info.item()) == 0
+    torch.cuda.synchronize()
+    s = torch.cuda.Stream()
+    with torch.cuda.stream(s):
+        for _ in range(3):
+            a2, _ = pkg.qmll_solve(ZtZ, Zty, 1e-2)
+    s.synchronize()
+    assert torch.equal(a2, ref)
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.stream(s):
+        a3, _ = pkg.qmll_solve(ZtZ, Zty, 1e-2)          # warm-up on the capture stream (workspace allocation)
+    s.synchronize()
+    with torch.cuda.graph(g, stream=s):
+        a3, info3 = pkg.qmll_solve(ZtZ, Zty, 1e-2)
+    a3.zero_()
+    g.replay()
+    torch.cuda.synchronize()
+    assert torch.equal(a3, ref) and int(info3.item()) == 0
 
 
 def test_train_then_predict_recovers_targets(q):
