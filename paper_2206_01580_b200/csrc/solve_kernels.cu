@@ -6,7 +6,7 @@
 //   row, column-oriented substitution)  ->  syrk_update_kernel on the 256-wide panel's own columns; after the panel
 //   one rank-256 syrk_update_kernel of the trailing matrix,
 // the right-hand side rides along as row D of the working matrix (so L y = b costs nothing extra), then the backward
-// substitution, one launch per 64-wide block (trsv_back_kernel).
+// substitution in one kernel whose CTAs hand the solved blocks to one another through flags (trsv_back_kernel).
 // syrk_update_kernel is the O(D^3) part: 128 x 64 tiles on the FP64 tensor-core path (mma.sync.m8n8k4.f64, DMMA: the
 // measured peak, profiles/peaks_r2.json kinds 13 / 14, is 18.5 T FMA/s against 17.0 for scalar DFMA, with 1/8 of the
 // instructions and 1/5 of the shared-memory loads), operands through a 3-stage cp.async ring, two CTAs per SM so that
@@ -34,10 +34,14 @@ __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wai
 // M = lower triangle of ZtZ + lambda I in FP64 (row i, columns 0 .. i; the upper triangle is never read), row D = Zty
 __global__ void __launch_bounds__(256) solve_prepare_kernel(const float* __restrict__ ZtZ, const float* __restrict__ Zty,
                                                             int D, int ld, double lambda, double* __restrict__ M,
-                                                            double* __restrict__ rhs, int* __restrict__ info) {
+                                                            double* __restrict__ rhs, int* __restrict__ info,
+                                                            int* __restrict__ flags, int n_flags) {
   const int i = blockIdx.y;
   const int j = blockIdx.x * 1024 + threadIdx.x * 4;
-  if (blockIdx.x == 0 && i == 0 && threadIdx.x == 0) *info = 0;
+  if (blockIdx.x == 0 && i == 0) {
+    if (threadIdx.x == 0) *info = 0;
+    for (int k = threadIdx.x; k < n_flags; k += 256) flags[k] = 0;
+  }
   if (i == D) {
 #pragma unroll
     for (int q = 0; q < 4; ++q)
@@ -262,54 +266,90 @@ __global__ void __launch_bounds__(128, 2) syrk_update_kernel(double* __restrict_
   }
 }
 
-// One block step of the backward substitution L^T a = y (the forward substitution L y = b needs no kernel: the
-// right-hand side rides through the factorisation as row D of the working matrix, so that trsm_panel_kernel solves it
-// and syrk_update_kernel updates it like any other row).  Solves the nb x nb diagonal block for sol[k0 .. k0 + nb) from
-// run[k0 ..) with L11^T, then run[j] -= sum_m L[k0 + m][j] sol[k0 + m] for j < k0.  Every CTA repeats the small
-// diagonal solve (warp 0: two rows per lane, the solved entry travels by shuffle), so a step is ONE launch; CTA 0
-// writes `sol`.  `run` entries of the block itself are only read.
-__global__ void __launch_bounds__(128) trsv_back_kernel(const double* __restrict__ M, int ld, int k0, int nb,
-                                                        double* __restrict__ run, double* __restrict__ sol) {
+// Backward substitution L^T a = y in ONE kernel (the forward substitution L y = b needs none: the right-hand side
+// rides through the factorisation as row D of the working matrix, so that trsm_panel_kernel solves it and
+// syrk_update_kernel updates it like any other row).  CTA b owns the 128 entries j in [128 b, 128 b + 128) -- thread =
+// entry, the running value lives in a register -- and walks the 64-wide blocks kb from the last one down to its own:
+//   * the owner of block kb (b = kb / 2) solves the diagonal block with L11^T (warp 0: two rows per lane, the solved
+//     entry travels by shuffle), writes sol[k0 .. k0 + nb) and raises flag[kb] (release);
+//   * every CTA below waits for the flag (acquire), then subtracts sum_m L[k0 + m][j] sol[k0 + m] from its entries;
+//     its 64 values of L are loaded BEFORE the wait.
+// A CTA depends only on CTAs with larger b; b is handed out by an atomic ticket in reverse, so whatever a CTA waits
+// for belongs to a CTA that has already started: no co-residency requirement, no deadlock.  256 launches of 16 us
+// (4.2 ms at D = 16384) became one kernel.
+__device__ __forceinline__ int ld_acquire_gpu(const int* p) {
+  int v;
+  asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+  return v;
+}
+__device__ __forceinline__ void st_release_gpu(int* p, int v) {
+  asm volatile("st.release.gpu.global.s32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
+}
+
+__global__ void __launch_bounds__(128) trsv_back_kernel(const double* __restrict__ M, int D, int ld,
+                                                        const double* __restrict__ y, double* __restrict__ sol,
+                                                        int* __restrict__ flags, int* __restrict__ ticket) {
   __shared__ double l[kNB][kNB + 1];
   __shared__ double dinv[kNB];
-  __shared__ double y[kNB];
+  __shared__ double s_sol[kNB];
+  __shared__ double s_run[2 * kNB];
+  __shared__ int s_b;
   const int t = threadIdx.x, lane = t & 31;
-  for (int idx = t; idx < kNB * kNB; idx += 128) {
-    const int r = idx / kNB, c = idx % kNB;
-    if (r < nb && c <= r) cp_async8(&l[r][c], M + (size_t)(k0 + r) * ld + k0 + c);
-    else l[r][c] = r == c ? 1.0 : 0.0;
-  }
-  cp_async_wait_all();
+  if (t == 0) s_b = (int)gridDim.x - 1 - atomicAdd(ticket, 1);
   __syncthreads();
-  if (t < kNB) dinv[t] = 1.0 / l[t][t];
-  __syncthreads();
-  if (t < 32) {
-    double b0 = lane < nb ? run[k0 + lane] : 0.0, b1 = lane + 32 < nb ? run[k0 + 32 + lane] : 0.0;
-    for (int c = kNB - 1; c >= 0; --c) {
-      const double bc = __shfl_sync(0xffffffffu, c < 32 ? b0 : b1, c & 31) * dinv[c];
-      if (lane == (c & 31)) { if (c < 32) b0 = bc; else b1 = bc; }
-      if (lane < c) b0 = fma(-l[c][lane], bc, b0);
-      if (lane + 32 < c) b1 = fma(-l[c][lane + 32], bc, b1);
+  const int b = s_b;
+  const int j = b * 128 + t;
+  double r = j < D ? y[j] : 0.0;
+  const int n_blk = (D + kNB - 1) / kNB;
+  for (int kb = n_blk - 1; kb >= 2 * b; --kb) {
+    const int k0 = kb * kNB, nb = D - k0 < kNB ? D - k0 : kNB;
+    const bool upd = j < k0;                              // this entry receives block kb's term
+    double lc[kNB];                                       // L[k0 + m][j]: issued before the wait
+#pragma unroll
+    for (int m = 0; m < kNB; ++m) lc[m] = (upd && m < nb) ? M[(size_t)(k0 + m) * ld + j] : 0.0;
+    if ((kb >> 1) == b) {                                 // owner: diagonal solve
+      for (int idx = t; idx < kNB * kNB; idx += 128) {
+        const int rr = idx / kNB, c = idx % kNB;
+        if (rr < nb && c <= rr) cp_async8(&l[rr][c], M + (size_t)(k0 + rr) * ld + k0 + c);
+        else l[rr][c] = rr == c ? 1.0 : 0.0;
+      }
+      s_run[t] = r;
+      cp_async_wait_all();
+      __syncthreads();
+      if (t < kNB) dinv[t] = 1.0 / l[t][t];
+      __syncthreads();
+      if (t < 32) {
+        const int o = (kb & 1) * kNB;                     // the block's entries sit in threads o .. o + 63
+        double b0 = lane < nb ? s_run[o + lane] : 0.0, b1 = lane + 32 < nb ? s_run[o + 32 + lane] : 0.0;
+        for (int c = kNB - 1; c >= 0; --c) {
+          const double bc = __shfl_sync(0xffffffffu, c < 32 ? b0 : b1, c & 31) * dinv[c];
+          if (lane == (c & 31)) { if (c < 32) b0 = bc; else b1 = bc; }
+          if (lane < c) b0 = fma(-l[c][lane], bc, b0);
+          if (lane + 32 < c) b1 = fma(-l[c][lane + 32], bc, b1);
+        }
+        s_sol[lane] = b0; s_sol[lane + 32] = b1;
+        if (lane < nb) sol[k0 + lane] = b0;
+        if (lane + 32 < nb) sol[k0 + 32 + lane] = b1;
+      }
+      __syncthreads();
+      if (t == 0) { __threadfence(); st_release_gpu(flags + kb, 1); }
+    } else {
+      if (t == 0) while (ld_acquire_gpu(flags + kb) == 0) {}
+      __syncthreads();
+      if (t < kNB) s_sol[t] = t < nb ? __ldcg(sol + k0 + t) : 0.0;
+      __syncthreads();
     }
-    y[lane] = b0; y[lane + 32] = b1;
-    if (blockIdx.x == 0) {
-      if (lane < nb) sol[k0 + lane] = b0;
-      if (lane + 32 < nb) sol[k0 + 32 + lane] = b1;
+    double s0 = 0.0, s1 = 0.0, s2 = 0.0, s3 = 0.0;
+#pragma unroll
+    for (int m = 0; m < kNB; m += 4) {
+      s0 = fma(lc[m], s_sol[m], s0);
+      s1 = fma(lc[m + 1], s_sol[m + 1], s1);
+      s2 = fma(lc[m + 2], s_sol[m + 2], s2);
+      s3 = fma(lc[m + 3], s_sol[m + 3], s3);
     }
+    r -= (s0 + s1) + (s2 + s3);
+    __syncthreads();                                      // s_sol / s_run are rewritten in the next round
   }
-  __syncthreads();
-  const int j = blockIdx.x * 128 + t;
-  if (j >= k0) return;
-  double s0 = 0.0, s1 = 0.0, s2 = 0.0, s3 = 0.0;      // four chains: 16 loads in flight per thread
-  const double* colp = M + (size_t)k0 * ld + j;
-#pragma unroll 4
-  for (int m = 0; m < kNB; m += 4) {
-    if (m + 0 < nb) s0 = fma(colp[(size_t)(m + 0) * ld], y[m + 0], s0);
-    if (m + 1 < nb) s1 = fma(colp[(size_t)(m + 1) * ld], y[m + 1], s1);
-    if (m + 2 < nb) s2 = fma(colp[(size_t)(m + 2) * ld], y[m + 2], s2);
-    if (m + 3 < nb) s3 = fma(colp[(size_t)(m + 3) * ld], y[m + 3], s3);
-  }
-  run[j] -= (s0 + s1) + (s2 + s3);
 }
 
 __global__ void solve_finish_kernel(const double* __restrict__ sol, float* __restrict__ alpha, int D) {
@@ -319,7 +359,8 @@ __global__ void solve_finish_kernel(const double* __restrict__ sol, float* __res
 
 // working matrix: D + 1 rows (row D = right-hand side) plus one row of slack for 16-byte accesses at the end
 size_t solve_workspace_bytes(int32_t D) {
-  return align_up((size_t)(D + 2) * solve_ld(D) * 8, 256) + align_up((size_t)D * 8, 256) + 512;
+  return align_up((size_t)(D + 2) * solve_ld(D) * 8, 256) + align_up((size_t)D * 8, 256) +
+         align_up((size_t)((D + kNB - 1) / kNB + 1) * 4, 256) + 512;
 }
 
 // Look-ahead (the classic one): the panel steps are short, serial kernels that leave the GPU mostly idle, so panel
@@ -383,13 +424,15 @@ int solve_normal_equations(const float* ZtZ, const float* Zty, int32_t D, double
   Carver ws(ws_ptr, ws_bytes);
   double* M = ws.take<double>((size_t)(D + 2) * ld);
   double* sol = ws.take<double>((size_t)D);
+  const int n_blk = (D + kNB - 1) / kNB;
+  int* flags = ws.take<int>((size_t)n_blk + 1);            // [n_blk] block-solved flags + the CTA ticket
   if (!ws_ptr || ((uintptr_t)ws_ptr & 255) != 0 || !ws.fits()) return QMLL_ERR_WORKSPACE;
   std::lock_guard<std::mutex> lock(g_solve_mutex);
   SolveSide* side = nullptr;
   if (int rc = solve_side(&side)) return rc;
   cudaStream_t hi = side->hi;
   double* y = M + (size_t)D * ld;                           // row D: b on entry, y = L^-1 b after the factorisation
-  solve_prepare_kernel<<<dim3((unsigned)((D + 1023) / 1024), (unsigned)(D + 1)), 256, 0, st>>>(ZtZ, Zty, D, ld, lambda, M, y, info);
+  solve_prepare_kernel<<<dim3((unsigned)((D + 1023) / 1024), (unsigned)(D + 1)), 256, 0, st>>>(ZtZ, Zty, D, ld, lambda, M, y, info, flags, n_blk + 1);
   QMLL_LAUNCH_CHECK("solve_prepare_kernel");
   QMLL_SOLVE_CUDA(cudaEventRecord(side->ev_main, st));
   QMLL_SOLVE_CUDA(cudaStreamWaitEvent(hi, side->ev_main, 0));
@@ -417,11 +460,8 @@ int solve_normal_equations(const float* ZtZ, const float* Zty, int32_t D, double
   }
   QMLL_SOLVE_CUDA(cudaEventRecord(side->ev_hi, hi));
   QMLL_SOLVE_CUDA(cudaStreamWaitEvent(st, side->ev_hi, 0));
-  for (int k0 = (D - 1) / kNB * kNB; k0 >= 0; k0 -= kNB) {  // L^T alpha = y: running y in row D, alpha into sol
-    const int nb = D - k0 < kNB ? D - k0 : kNB;
-    trsv_back_kernel<<<k0 > 0 ? (k0 + 127) / 128 : 1, 128, 0, st>>>(M, ld, k0, nb, y, sol);
-    QMLL_LAUNCH_CHECK("trsv_back_kernel");
-  }
+  trsv_back_kernel<<<(D + 127) / 128, 128, 0, st>>>(M, D, ld, y, sol, flags, flags + n_blk);   // L^T alpha = y
+  QMLL_LAUNCH_CHECK("trsv_back_kernel");
   solve_finish_kernel<<<(D + 255) / 256, 256, 0, st>>>(sol, alpha, D);
   QMLL_LAUNCH_CHECK("solve_finish_kernel");
   return QMLL_OK;
