@@ -38,7 +38,7 @@ def parse():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-configs", action="store_true", help="skip the per-config block (C2, C3, C5)")
-    ap.add_argument("--only-config", default=None, choices=["c2", "c3", "c5", "fchl19_cell"],
+    ap.add_argument("--only-config", default=None, choices=["c2", "c3", "c5", "fchl19_cell", "solve"],
                     help="run only this entry of the per-config block and print it (used for the ncu captures in profiles/)")
     ap.add_argument("--force-rows", default="auto", choices=["auto", "fwht", "mma", "mma2"],
                     help="how the force rows are computed (qmll_sorf_forward_mode); the bench line uses auto")
@@ -64,6 +64,8 @@ def peaks():
         out.update({"fadd_per_s": p["alu"]["0"]["per_s"], "fadd_source": "measured (profiles/peaks_r2.json, FADD loop on all SMs)",
                     "tf32_burst": p["tensor"]["tf32_tflops_burst"], "tf32_sustained": p["tensor"]["tf32_tflops_sustained"],
                     "mufu_per_s": p["alu"]["9"]["per_s"]})
+        if "14" in p["alu"]:
+            out["dmma_fma_per_s"] = p["alu"]["14"]["per_s"]
     return out
 
 
@@ -430,6 +432,9 @@ def ours_arm(args):
         sms = e0.elapsed_time(e1)
         line["solve"] = {"D": D, "lambda": lam, "ms": sms, "info": int(info.item()),
                          "fp64_tflops": (D ** 3 / 3.0) / (sms * 1e-3) / 1e12}
+        if "dmma_fma_per_s" in pk:      # measured FP64 tensor-core (DMMA) rate: 2 flops per FMA
+            line["solve"]["frac_of_fp64_peak"] = line["solve"]["fp64_tflops"] * 1e12 / (2.0 * pk["dmma_fma_per_s"])
+            line["solve"]["fp64_peak_tflops"] = 2.0 * pk["dmma_fma_per_s"] / 1e12
     del A, ZtZ, dt_, di_
     pkg.release_workspaces()
     torch.cuda.empty_cache()
@@ -538,6 +543,8 @@ def other_configs(pk, reps, rows_mode=0, only=None):
         torch.cuda.empty_cache()
     if only is None or only == "fchl19_cell":
         out["fchl19_cell"] = fchl19_config(pk, tm)
+    if only == "solve":
+        out["solve"] = solve_config(pk, tm)
     return out
 
 
@@ -596,6 +603,29 @@ def fchl19_config(pk, tm):
     o["fchl19_backward_ms"] = tm(lambda: pkg.qmll_fchl19_backward(fp, r, e, idx, wv, nbr_shift=sh, forces=F))
     tot = o["fchl19_rho_ms"] + o["project_x_ms"] + o["backward_g_ms"] + o["project_back_ms"] + o["fchl19_backward_ms"]
     o.update({"coordinates_to_forces_ms": tot, "us_per_atom": tot * 1e3 / na})
+    pkg.release_workspaces()
+    torch.cuda.empty_cache()
+    return o
+
+
+def solve_config(pk, tm, D=16384):
+    """qmll_solve alone on a synthetic SPD system of the bench step's size (Gram matrix of a seeded Gaussian A with
+    D + 512 rows; the bench line's own `solve` entry uses the step's ZtZ instead)."""
+    import torch
+    import paper_2206_01580_b200 as pkg
+    g = torch.Generator(device="cuda").manual_seed(16384)
+    A = torch.randn((D + 512, D), device="cuda", generator=g) / D ** 0.5
+    ZtZ = A.T @ A
+    Zty = torch.randn((D,), device="cuda", generator=g)
+    del A
+    lam = 1e-3
+    ms = tm(lambda: pkg.qmll_solve(ZtZ, Zty, lam))
+    alpha, info = pkg.qmll_solve(ZtZ, Zty, lam)
+    res = ((ZtZ.double() @ alpha.double() + lam * alpha.double() - Zty.double()).norm() / Zty.double().norm()).item()
+    o = {"D": D, "lambda": lam, "ms": ms, "info": int(info.item()), "relative_residual_fp32_alpha": res,
+         "fp64_tflops": (D ** 3 / 3.0) / (ms * 1e-3) / 1e12}
+    if "dmma_fma_per_s" in pk:
+        o["frac_of_fp64_peak"] = o["fp64_tflops"] * 1e12 / (2.0 * pk["dmma_fma_per_s"])
     pkg.release_workspaces()
     torch.cuda.empty_cache()
     return o
