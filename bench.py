@@ -135,45 +135,77 @@ def reference_arm(args):
 
 # ------------------------------------------------------------------------------------------------ clocks
 class ClockSampler:
+    """SM clock, power and throttle reasons DURING the timed region: an in-process NVML thread (20 ms period, first
+    sample immediately), or -- if pynvml is missing -- an `nvidia-smi -lms 20` child (which needs ~0.5 s to start and
+    returned no sample at all on a fresh box for a 1 s timed region)."""
     Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
          "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
 
     def __init__(self, index):
-        self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        import threading
+        self.rows, self.p, self.t, self.halt = [], None, None, threading.Event()
         try:
-            self.p = subprocess.Popen(["nvidia-smi", "-i", str(index), f"--query-gpu={self.Q}",
-                                       "--format=csv,noheader,nounits", "-lms", "20"], stdout=self.f,
-                                      stderr=subprocess.DEVNULL)
+            import pynvml
+            pynvml.nvmlInit()
+            vis = os.environ.get("CUDA_VISIBLE_DEVICES", "")
+            ids = [v for v in vis.split(",") if v.strip()]
+            phys = int(ids[index]) if ids and all(v.strip().isdigit() for v in ids) and index < len(ids) else index
+            h = pynvml.nvmlDeviceGetHandleByIndex(phys)
+            mx = float(pynvml.nvmlDeviceGetMaxClockInfo(h, pynvml.NVML_CLOCK_SM))
+            get_reasons = getattr(pynvml, "nvmlDeviceGetCurrentClocksEventReasons", None) or \
+                pynvml.nvmlDeviceGetCurrentClocksThrottleReasons
+            bits = {"hw_slowdown": 0x8, "sw_thermal_slowdown": 0x20, "hw_thermal_slowdown": 0x40, "sw_power_cap": 0x4}
+
+            def loop():
+                while not self.halt.is_set():
+                    try:
+                        r = int(get_reasons(h))
+                        self.rows.append((float(pynvml.nvmlDeviceGetClockInfo(h, pynvml.NVML_CLOCK_SM)), mx,
+                                          pynvml.nvmlDeviceGetPowerUsage(h) / 1e3, [n for n, b in bits.items() if r & b]))
+                    except Exception:
+                        pass
+                    self.halt.wait(0.02)
+
+            self.t = threading.Thread(target=loop, daemon=True)
+            self.t.start()
+            self.how = "nvml thread"
         except Exception:
-            self.p = None
+            self.how = "nvidia-smi -lms 20"
+            self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+            try:
+                self.p = subprocess.Popen(["nvidia-smi", "-i", str(index), f"--query-gpu={self.Q}",
+                                           "--format=csv,noheader,nounits", "-lms", "20"], stdout=self.f,
+                                          stderr=subprocess.DEVNULL)
+            except Exception:
+                self.p = None
 
     def stop(self):
         out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": []}
-        if self.p is None:
-            return out
-        self.p.terminate()
-        try:
-            self.p.wait(timeout=5)
-        except Exception:
-            self.p.kill()
-        self.f.flush()
-        self.f.seek(0)
-        rows = [r.strip().split(",") for r in self.f.read().strip().splitlines() if r.strip()]
-        self.f.close()
-        os.unlink(self.f.name)
-        sm, reasons, mx, pw = [], set(), None, []
-        for r in rows:
+        if self.t is not None:
+            self.halt.set()
+            self.t.join(timeout=2)
+        elif self.p is not None:
+            self.p.terminate()
             try:
-                sm.append(float(r[0])); mx = float(r[1]); pw.append(float(r[2]))
+                self.p.wait(timeout=5)
             except Exception:
-                continue
-            for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), r[3:7]):
-                if v.strip().lower().startswith("active"):
-                    reasons.add(name)
-        if sm:
-            sm.sort()
-            out.update({"sm_mhz": sm[len(sm) // 2], "sm_max_mhz": mx, "reasons": sorted(reasons),
-                        "power_w_max": max(pw) if pw else None, "samples": len(sm)})
+                self.p.kill()
+            self.f.flush()
+            self.f.seek(0)
+            for r in [r.strip().split(",") for r in self.f.read().strip().splitlines() if r.strip()]:
+                try:
+                    names = ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")
+                    self.rows.append((float(r[0]), float(r[1]), float(r[2]),
+                                      [n for n, v in zip(names, r[3:7]) if v.strip().lower().startswith("active")]))
+                except Exception:
+                    continue
+            self.f.close()
+            os.unlink(self.f.name)
+        if self.rows:
+            sm = sorted(r[0] for r in self.rows)
+            out.update({"sm_mhz": sm[len(sm) // 2], "sm_max_mhz": self.rows[-1][1],
+                        "reasons": sorted({n for r in self.rows for n in r[3]}),
+                        "power_w_max": max(r[2] for r in self.rows), "samples": len(sm), "how": self.how})
         return out
 
 
