@@ -9,8 +9,8 @@
 // substitution in one kernel whose CTAs hand the solved blocks to one another through flags (trsv_back_kernel).
 // syrk_update_kernel is the O(D^3) part: 128 x 64 tiles on the FP64 tensor-core path (mma.sync.m8n8k4.f64, DMMA: the
 // measured peak, profiles/peaks_r2.json kinds 13 / 14, is 18.5 T FMA/s against 17.0 for scalar DFMA, with 1/8 of the
-// instructions and 1/5 of the shared-memory loads), operands through a 3-stage cp.async ring, two CTAs per SM so that
-// the read-modify-write epilogue of one overlaps the main loop of the other.
+// instructions and 1/5 of the shared-memory loads), operands through a 2-stage cp.async ring, three CTAs per SM (the
+// third fills the issue gaps between a warp's dependent DMMAs: pipe 82 % -> 90 % busy).
 // `info` (device int) follows LAPACK: 0 = success, k > 0 = the leading minor of order k is not positive definite (the
 // factorisation then carries NaNs).  The working matrix has leading dimension ld = D rounded up to 8 (16-byte copies).
 #include <mutex>
@@ -180,7 +180,7 @@ __global__ void __launch_bounds__(128) trsm_panel_kernel(double* __restrict__ M,
 // k lane % 4; B the same with the row as n), so the stages are plain copies: [rows][16 k] with a row pitch of 20
 // doubles (conflict-free LDS.64 for the 8 rows x 4 k a fragment touches), filled by 16-byte cp.async (zero-filled
 // beyond kn and beyond the last row).  n_rows = D + 1: the extra row carries the right-hand side.
-constexpr int kUM = 128, kUN = 64, kUK = 16, kUPitch = 20, kUStages = 3;
+constexpr int kUM = 128, kUN = 64, kUK = 16, kUPitch = 20, kUStages = 2;
 constexpr int kUStageDoubles = (kUM + kUN) * kUPitch;
 constexpr int kUSmemBytes = kUStages * kUStageDoubles * 8;
 
@@ -191,7 +191,7 @@ __device__ __forceinline__ void dmma_m8n8k4(double& c0, double& c1, double a, do
   asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0, %1}, {%2}, {%3}, {%0, %1};" : "+d"(c0), "+d"(c1) : "d"(a), "d"(b));
 }
 
-__global__ void __launch_bounds__(128, 2) syrk_update_kernel(double* __restrict__ M, int n_rows, int ld, int r0, int c0,
+__global__ void __launch_bounds__(128, 3) syrk_update_kernel(double* __restrict__ M, int n_rows, int ld, int r0, int c0,
                                                              int c1, int k0, int kn) {
   const int i0 = r0 + blockIdx.x * kUM, j0 = c0 + blockIdx.y * kUN;
   if (j0 >= c1 || j0 > i0 + kUM - 1) return;          // tile entirely above the diagonal or outside the column range
