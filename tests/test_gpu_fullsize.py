@@ -188,3 +188,26 @@ def test_c5_full_cell_against_oracle(q):
     Fo = oracle.forces_w(w)
     assert rel(F.cpu().numpy(), Fo) <= TOL_F
     assert rel(F2.cpu().numpy(), Fo) <= TOL_F
+
+
+def test_solve_at_the_bench_size(q):
+    """qmll_solve at D = 16384 (the step's normal equations; the oracle's unblocked Cholesky would need ~1e12 flops on
+    the host).  Properties that hold at any size: the FP64 residual of the fp32 alpha is at the fp32 rounding level,
+    and alpha agrees with a library FP64 solve (torch.linalg, cuSOLVER) of the same system."""
+    pkg, wio, torch = q
+    D = 16384
+    g = torch.Generator(device="cuda").manual_seed(7)
+    A = torch.randn((D + 512, D), device="cuda", generator=g) / D ** 0.5
+    ZtZ = A.T @ A
+    del A
+    Zty = torch.randn((D,), device="cuda", generator=g)
+    lam = 1e-3
+    alpha, info = pkg.qmll_solve(ZtZ, Zty, lam)
+    assert int(info.item()) == 0
+    M = torch.tril(ZtZ.double())
+    M = M + torch.tril(M, -1).T                         # the symmetric matrix the solve reads (lower triangle)
+    M.diagonal().add_(lam)
+    res = (M @ alpha.double() - Zty.double()).norm() / Zty.double().norm()
+    assert float(res) <= 1e-5
+    ref = torch.linalg.solve(M, Zty.double())
+    assert float((alpha.double() - ref).norm() / ref.norm()) <= 1e-6
