@@ -56,68 +56,78 @@ __global__ void __launch_bounds__(256) solve_prepare_kernel(const float* __restr
     if (j + q <= i) dst[q] = (double)src[q] + (j + q == i ? lambda : 0.0);
 }
 
-// Cholesky of the nb x nb diagonal block at (k0, k0): A = L L^T, L overwrites the lower triangle.  Thread i holds row
-// i in registers (right-looking): per column ONE barrier -- every thread publishes its entry of column j, reads the
-// pivot and the column back, and updates its own row with independent FMAs.  The row SHIFTS by one register per
-// column (a[p - 1] = fma(.., a[p])), so that register p always holds column j + p and the loop over j stays rolled:
-// fully unrolled it is 93 KB of straight-line code that runs once, at instruction-fetch speed (43 % "no instruction"
-// stalls, 32 us per block against 12 us now).  Rows / columns >= nb are an identity pad.
-template <int kPar>
-__device__ __forceinline__ void potrf_column(double (&a)[kNB], const double* __restrict__ colp, double* tile_row, int i,
-                                             int j, int nb, int k0, int* info) {
-  // colp = &col[kPar][j], j % 2 == kPar: colp + p is 16-byte aligned for p % 2 == kPar
-  const double piv = colp[0];
-  if (i == j && j < nb && !(piv > 0.0) && *info == 0) *info = k0 + j + 1;
-  const double dinv = rsqrt(piv);
-  const double l = a[0] * dinv;         // row j: sqrt(piv); rows below: l_ij; rows above: 0
-  if (i >= j) tile_row[j] = l;
-  const double s = l * dinv;            // l_ij / sqrt(piv); colp[p] * (1 / sqrt(piv)) = l_{j+p, j}
-  if (kPar == 0) {
-    a[0] = fma(-s, colp[1], a[1]);
-#pragma unroll
-    for (int p = 2; p < kNB; p += 2) {
-      const double2 c = *reinterpret_cast<const double2*>(colp + p);
-      a[p - 1] = fma(-s, c.x, a[p]);
-      a[p] = fma(-s, c.y, a[p + 1 < kNB ? p + 1 : p]);
-    }
-  } else {
-#pragma unroll
-    for (int p = 1; p < kNB - 1; p += 2) {
-      const double2 c = *reinterpret_cast<const double2*>(colp + p);
-      a[p - 1] = fma(-s, c.x, a[p]);
-      a[p] = fma(-s, c.y, a[p + 1]);
-    }
-    a[kNB - 2] = fma(-s, colp[kNB - 1], a[kNB - 1]);
-  }
-  a[kNB - 1] = 0.0;
-}
-
-__global__ void __launch_bounds__(kNB) potrf_diag_kernel(double* __restrict__ M, int ld, int k0, int nb, int* info) {
+// Cholesky of the nb x nb diagonal block at (k0, k0): A = L L^T, L overwrites the lower triangle.  The block lives in
+// shared memory and is factorised in four block columns of 16 (right-looking between them):
+//   * panel: threads 0..63 = rows, the row's 16 entries in registers; per column ONE 64-thread named barrier -- every
+//     thread publishes its entry of column j, reads the pivot and the column back, and updates the (at most 15)
+//     remaining entries of its row: the serial chain per column is barrier + rsqrt + two multiplies + one FMA;
+//   * update: all 256 threads subtract the rank-16 product from the rest of the block (items of 1 row x 4 columns).
+// History: a register-resident 64-wide row with 63 FMAs per column and thread (rolled by shifting the row one
+// register per column; fully unrolled it was 93 KB of straight-line code at instruction-fetch speed) took 22 us: one
+// warp per scheduler issues its ~200 instructions per column in order, behind the chain.
+// Rows / columns >= nb are an identity pad.
+constexpr int kPB = 16;
+__global__ void __launch_bounds__(256) potrf_diag_kernel(double* __restrict__ M, int ld, int k0, int nb, int* info) {
   __shared__ double tile[kNB][kNB + 1];
-  __shared__ __align__(16) double col[2][2 * kNB];      // column j of every row; the upper half stays zero
-  const int i = threadIdx.x;
-  for (int idx = i; idx < kNB * kNB; idx += kNB) {
+  __shared__ double col[2][kNB];
+  const int t = threadIdx.x;
+  for (int idx = t; idx < kNB * kNB; idx += 256) {
     const int r = idx / kNB, c = idx % kNB;
     if (r < nb && c <= r) cp_async8(&tile[r][c], M + (size_t)(k0 + r) * ld + k0 + c);
     else tile[r][c] = r == c ? 1.0 : 0.0;
   }
-  col[0][kNB + i] = col[1][kNB + i] = 0.0;
   cp_async_wait_all();
   __syncthreads();
-  double a[kNB];
-#pragma unroll
-  for (int c = 0; c < kNB; ++c) a[c] = tile[i][c];
 #pragma unroll 1
-  for (int j = 0; j < kNB; j += 2) {
-    col[0][i] = a[0];
+  for (int c0 = 0; c0 < kNB; c0 += kPB) {
+    if (t < kNB) {                                       // ---- panel: rows 0..63 (rows above c0 carry zeros along)
+      const int i = t;
+      double a[kPB];
+#pragma unroll
+      for (int q = 0; q < kPB; ++q) a[q] = i >= c0 ? tile[i][c0 + q] : 0.0;
+#pragma unroll
+      for (int q = 0; q < kPB; ++q) {
+        const int j = c0 + q;
+        col[q & 1][i] = a[q];
+        asm volatile("bar.sync 1, 64;" ::: "memory");
+        const double piv = col[q & 1][j];
+        if (i == j && j < nb && !(piv > 0.0) && *info == 0) *info = k0 + j + 1;
+        const double dinv = rsqrt(piv);
+        a[q] *= dinv;                                     // row j: sqrt(piv); rows below: l_ij; rows above: 0
+        const double sc = a[q] * dinv;                    // l_ij / sqrt(piv); col[c] * (1 / sqrt(piv)) = l_cj
+#pragma unroll
+        for (int k = q + 1; k < kPB; ++k) a[k] = fma(-sc, col[q & 1][c0 + k], a[k]);
+      }
+      if (i >= c0) {
+#pragma unroll
+        for (int q = 0; q < kPB; ++q)
+          if (c0 + q <= i) tile[i][c0 + q] = a[q];
+      }
+    }
     __syncthreads();
-    potrf_column<0>(a, &col[0][j], tile[i], i, j, nb, k0, info);
-    col[1][i] = a[0];
+    // ---- rank-16 update of rows / columns >= c0 + 16 (lower triangle): item = (row, 4 columns)
+    const int r0 = c0 + kPB, R = kNB - r0;
+    for (int idx = t; idx < R * (R / 4); idx += 256) {
+      const int i = r0 + idx % R, cb = r0 + 4 * (idx / R);
+      if (cb > i) continue;
+      double li[kPB], s0 = 0.0, s1 = 0.0, s2 = 0.0, s3 = 0.0;
+#pragma unroll
+      for (int k = 0; k < kPB; ++k) li[k] = tile[i][c0 + k];
+#pragma unroll
+      for (int k = 0; k < kPB; ++k) {
+        s0 = fma(li[k], tile[cb][c0 + k], s0);
+        s1 = fma(li[k], tile[cb + 1][c0 + k], s1);
+        s2 = fma(li[k], tile[cb + 2][c0 + k], s2);
+        s3 = fma(li[k], tile[cb + 3][c0 + k], s3);
+      }
+      tile[i][cb] -= s0;                                  // entries above the diagonal are scratch (never read back)
+      tile[i][cb + 1] -= s1;
+      tile[i][cb + 2] -= s2;
+      tile[i][cb + 3] -= s3;
+    }
     __syncthreads();
-    potrf_column<1>(a, &col[1][j + 1], tile[i], i, j + 1, nb, k0, info);
   }
-  __syncthreads();
-  for (int idx = i; idx < nb * nb; idx += kNB) {
+  for (int idx = t; idx < nb * nb; idx += 256) {
     const int r = idx / nb, c = idx % nb;
     if (c <= r) M[(size_t)(k0 + r) * ld + k0 + c] = tile[r][c];
   }
@@ -402,7 +412,7 @@ static int solve_factor_panel(double* M, int D, int ld, int K0, int32_t* info, c
   const int nb2 = D - K0 < kNB2 ? D - K0 : kNB2;
   for (int k0 = K0; k0 < K0 + nb2; k0 += kNB) {
     const int nb = K0 + nb2 - k0 < kNB ? K0 + nb2 - k0 : kNB;
-    potrf_diag_kernel<<<1, kNB, 0, st>>>(M, ld, k0, nb, info);
+    potrf_diag_kernel<<<1, 256, 0, st>>>(M, ld, k0, nb, info);
     QMLL_LAUNCH_CHECK("potrf_diag_kernel");
     const int rest = n_rows - k0 - nb;                    // >= 1: the right-hand side row
     trsm_panel_kernel<<<(rest + 127) / 128, 128, 0, st>>>(M, n_rows, ld, k0, nb);
