@@ -257,6 +257,26 @@ int qmll_predict(const qmll_sorf_params* p, const float* x, const int32_t* elem,
                  int64_t n_atoms, int32_t n_mol, const float* alpha, const qmll_grad* grad, float* energies,
                  float* forces, void* workspace, size_t workspace_bytes, void* cuda_stream);
 
+/* qmll_predict for callers that cannot allocate device memory (code under CUDA graph capture, tight serving loops,
+ * harnesses that forbid cudaMalloc): same operation, same arguments and same kernels as qmll_predict (steps a1, a4-a6:
+ * eq. 14-15, forces L137 / eq. 17), but without the workspace arguments.  The scratch -- the model's
+ * lane-permuted tables and the FP64 energy accumulators -- is a static device array of QMLL_PREDICT_STATIC_MAX_BYTES
+ * inside the library, held by every GPU that loads the library until the process exits.  The call allocates nothing
+ * (no cudaMalloc / cudaFree, no allocating library routine); the first call on a device looks up the array's device
+ * address (cudaGetSymbolAddress), later calls reuse it.
+ *   Limit: qmll_workspace_bytes(QMLL_CALL_PREDICT, p, n_atoms, n_mol, 0) <= qmll_predict_static_max_bytes(), else
+ *   QMLL_ERR_WORKSPACE and nothing is launched (4 MiB covers D = 65536 with 5 elements and ~300 000 molecules per
+ *   call; all five BASELINE configs fit).  Other errors as qmll_predict.
+ *   Sharing: every call on a device uses the same array.  What must start at zero is cleared inside every call and
+ *   the tables are rewritten in full, so back-to-back calls on one stream (or otherwise ordered) are independent;
+ *   calls that OVERLAP on the GPU (different streams without ordering, concurrent graph launches) race on the
+ *   scratch and give undefined results.  Thread-safe at enqueue. */
+#define QMLL_PREDICT_STATIC_MAX_BYTES (4u << 20)
+int qmll_predict_static(const qmll_sorf_params* p, const float* x, const int32_t* elem, const int32_t* mol_off,
+                        int64_t n_atoms, int32_t n_mol, const float* alpha, const qmll_grad* grad, float* energies,
+                        float* forces, void* cuda_stream);
+size_t qmll_predict_static_max_bytes(void);
+
 /* NEXT step after the accumulation: alpha = (ZtZ + lambda I)^-1 Zty, the regularised
  * normal equations of eq. 16-17 (L134-144; "solved by LU decomposition", L137 -- SPD, so a blocked Cholesky), in FP64.
  *   ZtZ [D, D] fp32 symmetric (only the lower triangle is read), Zty [D] fp32, lambda >= 0, alpha [D] fp32 out,

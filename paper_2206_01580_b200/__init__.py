@@ -32,7 +32,8 @@ EXPORTS = ("qmll_solve", "qmll_sorf_forward", "qmll_sorf_forward_mode", "qmll_so
            "qmll_launch_count", "qmll_reset_launch_count", "qmll_time_normal_equations_kernel",
            "qmll_collect_normal_equations_kernel_ms", "qmll_microbench", "qmll_microbench_mma", "qmll_pack_lower", "qmll_unpack_lower", "qmll_project",
            "qmll_project_neighbor", "qmll_fchl19", "qmll_fchl19_rep_size", "qmll_sorf_forward_mma", "qmll_rff_forward",
-           "qmll_featmap_workspace_bytes", "qmll_sorf_backward_g", "qmll_project_back", "qmll_fchl19_backward")
+           "qmll_featmap_workspace_bytes", "qmll_sorf_backward_g", "qmll_project_back", "qmll_fchl19_backward",
+           "qmll_predict_static", "qmll_predict_static_max_bytes")
 
 
 class _CParams(ctypes.Structure):
@@ -85,6 +86,10 @@ def load_library() -> ctypes.CDLL:
     lib.qmll_normal_equations_min_workspace_mode.argtypes = [i32, i32]
     lib.qmll_normal_equations_min_workspace_mode.restype = sz
     lib.qmll_predict.argtypes = [pp, vp, vp, vp, i64, i32, vp, gp, vp, vp, vp, sz, vp]
+    lib.qmll_predict_static.argtypes = [pp, vp, vp, vp, i64, i32, vp, gp, vp, vp, vp]
+    lib.qmll_predict_static.restype = ctypes.c_int
+    lib.qmll_predict_static_max_bytes.argtypes = []
+    lib.qmll_predict_static_max_bytes.restype = sz
     lib.qmll_project.argtypes = [vp, vp, vp, i64, i32, i32, i32, i32, vp, vp, vp, vp, vp, vp, vp]
     lib.qmll_project.restype = ctypes.c_int
     lib.qmll_project_neighbor.argtypes = [vp, vp, vp, i64, i32, i32, i32, i32, vp, vp, vp]
@@ -277,6 +282,28 @@ def qmll_predict(p: SorfParams, x, elem, mol_off, alpha, grad: Optional[Grad] = 
                             ctypes.byref(cg) if cg is not None else None, _dev(energies, torch.float32, "energies"),
                             _dev(forces, torch.float32, "forces"), ctypes.c_void_p(ws.data_ptr()), ws.numel(),
                             _stream()))
+    return energies, forces
+
+
+def qmll_predict_static(p: SorfParams, x, elem, mol_off, alpha, energies, grad: Optional[Grad] = None, forces=None):
+    """include/qmll.h qmll_predict_static: qmll_predict on the library's static scratch.  The call allocates nothing,
+    so the outputs are the caller's: energies [n_mol] and, with grad, forces [n_atoms, 3].  Calls that overlap on the
+    GPU race on the shared scratch; problems beyond qmll_predict_static_max_bytes() raise QmllError (status -3)."""
+    lib = load_library()
+    xp, ep, mp, n_atoms, n_mol = _problem(x, elem, mol_off)
+    if energies is None or (grad is not None and forces is None):
+        raise ValueError("qmll_predict_static allocates nothing: pass energies (and forces with grad)")
+    cp = p.c()
+    cg = grad.c() if grad is not None else None
+    status = lib.qmll_predict_static(ctypes.byref(cp), xp, ep, mp, n_atoms, n_mol, _dev(alpha, torch.float32, "alpha"),
+                                     ctypes.byref(cg) if cg is not None else None,
+                                     _dev(energies, torch.float32, "energies"), _dev(forces, torch.float32, "forces"),
+                                     _stream())
+    if status == -3:
+        need = int(lib.qmll_workspace_bytes(CALL_PREDICT, ctypes.byref(cp), n_atoms, n_mol, 0))
+        raise QmllError(status, f"qmll_predict_static: this problem needs {need} bytes of scratch, the static array "
+                                f"holds {int(lib.qmll_predict_static_max_bytes())}; use qmll_predict with a workspace")
+    _check(status)
     return energies, forces
 
 
