@@ -70,6 +70,14 @@ def test_host_side_argument_checks_need_no_gpu(lib):
     assert l.qmll_normal_equations_mode(None, None, 4, 256, 0, None, None, None, 0, 9, None) == -1
     assert l.qmll_predict(None, None, None, None, 0, 0, None, None, None, None, None, 0, None) == -1
     assert l.qmll_sorf_backward_forces(None, None, None, None, 0, 0, None, None, None, None, 0, None) == -1
+    # the static-scratch prediction: null / invalid parameters and problems beyond the array are rejected on the host
+    assert l.qmll_predict_static(None, None, None, None, 0, 0, None, None, None, None, None) == -1
+    assert int(l.qmll_predict_static_max_bytes()) == 4 << 20
+    bad = pkg._CParams(48, 96, 3, 2, 1.0, None, None)                      # d not a power of two
+    assert l.qmll_predict_static(ctypes.byref(bad), None, None, None, 0, 0, None, None, None, None, None) == -1
+    big = pkg._CParams(256, 65536, 3, 16, 1.0, None, None)                 # 4.9 MB of tables
+    assert l.qmll_workspace_bytes(pkg.CALL_PREDICT, ctypes.byref(big), 0, 1000, 0) > 4 << 20
+    assert l.qmll_predict_static(ctypes.byref(big), None, None, None, 0, 1000, None, None, None, None, None) == -3
 
 
 def test_next_row_entry_points_check_arguments_on_the_host(lib):
