@@ -238,6 +238,16 @@ __device__ __forceinline__ void contract_neighbor_atom(const float* __restrict__
   }
 }
 
+// L2 prefetch of [ptr, ptr + floats): 4 KB pieces spread over the lanes (cp.async.bulk.prefetch.L2; pieces stay
+// inside the range, 16-byte aligned).
+__device__ __forceinline__ void l2_prefetch_range(const float* ptr, size_t floats, int lane) {
+  const uintptr_t b = ((uintptr_t)ptr + 15) & ~(uintptr_t)15, e = (uintptr_t)(ptr + floats) & ~(uintptr_t)15;
+  for (uintptr_t q = b + (uintptr_t)lane * 4096; q < e; q += (uintptr_t)kWarp * 4096) {
+    const uint32_t sz = e - q < 4096 ? (uint32_t)(e - q) : 4096u;
+    asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(q), "r"(sz) : "memory");
+  }
+}
+
 template <typename S>
 struct PredSmem {
   static constexpr int kWarps = kPredThreads / kWarp;
@@ -274,9 +284,24 @@ sorf_predict_kernel(const float* __restrict__ x, const int32_t* __restrict__ ele
 #pragma unroll
       for (int q = 0; q < S::E4; ++q) acc[q * kWarp + lane] = make_float4(0.f, 0.f, 0.f, 0.f);
     }
+    int M = 0;                                  // the molecule that owns the atom (found once, before the chain)
+    if (have && (energy_acc != nullptr || (kNeedG && grad.layout == QMLL_GRAD_DENSE)))
+      M = owner_molecule(mol_off, n_mol, a);
 #pragma unroll 1
     for (int sg = 0; sg < n_sg; ++sg) {
       if (!have) continue;
+      if (kNeedG && sg == n_sg - 1) {
+        // The atom's gradient block is streamed exactly once, after the chain, by this warp: ask for it in L2 when
+        // the last stack group starts (early enough to land, late enough that the blocks of all resident warps --
+        // 83 KB each on config 4 -- do not crowd L2).  Measured: config 4 inference 3.70 -> 3.58 ms, config 5 2.06 -> 1.94.
+        if (grad.layout == QMLL_GRAD_DENSE) {
+          const int lo = __ldg(mol_off + M), np_ = __ldg(mol_off + M + 1) - lo;
+          l2_prefetch_range(grad.dense + __ldg(grad.dense_off + M) + (size_t)(a - lo) * S::d * 3 * np_,
+                            (size_t)S::d * 3 * np_, lane);
+        } else if (grad.layout == QMLL_GRAD_NEIGHBOR) {
+          l2_prefetch_range(grad.nbr_val + (size_t)a * grad.K * S::d * 3, (size_t)grad.K * S::d * 3, lane);
+        }
+      }
       f32x2 v[S::E2];
       load_row<S>(v, x + (size_t)a * S::d, p);
       const float4* b4 = bias4 + ((size_t)e * n_sg + sg) * (S::E4 * kWarp) + lane;
@@ -335,9 +360,8 @@ sorf_predict_kernel(const float* __restrict__ x, const int32_t* __restrict__ ele
       }
     }
     if (!have) continue;
-    int M = 0, m_lo = 0, n = 0;
+    int m_lo = 0, n = 0;
     if (energy_acc != nullptr || (kNeedG && grad.layout == QMLL_GRAD_DENSE)) {
-      M = owner_molecule(mol_off, n_mol, a);
       m_lo = __ldg(mol_off + M);
       n = __ldg(mol_off + M + 1) - m_lo;
     }
