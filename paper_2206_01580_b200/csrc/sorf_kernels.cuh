@@ -274,6 +274,7 @@ sorf_predict_kernel(const float* __restrict__ x, const int32_t* __restrict__ ele
   const float4* alpha4 = reinterpret_cast<const float4*>(alpha_s);
   const f32x2 c2 = pk(c, c);
 
+  int M = 0;
 #pragma unroll 1
   for (int a0 = a_block; a0 < a_stop; a0 += kWarps) {
     const int a = a0 + warp;
@@ -284,9 +285,12 @@ sorf_predict_kernel(const float* __restrict__ x, const int32_t* __restrict__ ele
 #pragma unroll
       for (int q = 0; q < S::E4; ++q) acc[q * kWarp + lane] = make_float4(0.f, 0.f, 0.f, 0.f);
     }
-    int M = 0;                                  // the molecule that owns the atom (found once, before the chain)
-    if (have && (energy_acc != nullptr || (kNeedG && grad.layout == QMLL_GRAD_DENSE)))
-      M = owner_molecule(mol_off, n_mol, a);
+    // the molecule that owns the atom, found before the chain: a binary search for the warp's first atom, then a walk
+    // (the warp's atoms increase; empty molecules are stepped over)
+    if (have && (energy_acc != nullptr || (kNeedG && grad.layout == QMLL_GRAD_DENSE))) {
+      if (a0 == a_block) M = owner_molecule(mol_off, n_mol, a);
+      else while (__ldg(mol_off + M + 1) <= a) ++M;
+    }
 #pragma unroll 1
     for (int sg = 0; sg < n_sg; ++sg) {
       if (!have) continue;
