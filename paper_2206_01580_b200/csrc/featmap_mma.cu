@@ -7,11 +7,12 @@
 //
 // Why it pays on B200: per feature the FWHT chain costs T log2(d) adds + T sign flips on the fp32 pipe (~1 ps at the
 // measured 25 T adds/s); the explicit product costs 2 d MACs per pass on tcgen05, 2 passes for SORF (x split hi/lo, W
-// exact) = 0.37 ps at d = 128.  Measured (config 3, profiles/r2_fchl19_featmap.md): 22-23 ms against 30.5 ms; the tensor
-// pipe and MUFU are each ~28 % busy, the instruction issue of the epilogue (14.5 warp instructions per 32 features x 1
-// atom) is what bounds the kernel.
+// exact) = 0.37 ps at d = 128.  Measured (config 3, profiles/r2_fchl19_featmap.md): 20 ms against 30.5 ms.  The epilogue
+// warps are latency-bound (0.52 instructions per cycle and scheduler with the 16 epilogue warps of one CTA), so at
+// d = 128 TWO CTAs share an SM (64 KB of W, 2 stages, 256 TMEM columns each: 22.8 -> 20 ms, issue rate 0.77).
 //
-// Dataflow: W tiles are the stationary operand (128 KB of shared memory: 4 stacks at d = 128, 1 stack at d = 256), so
+// Dataflow: W tiles are the stationary operand (d = 128: 64 KB = 2 stacks per CTA, two CTAs per SM; d = 256: 128 KB =
+// 1 stack, one CTA per SM), so
 // the atoms are first SORTED BY ELEMENT inside groups of 8192 atoms (stable, so the atoms of a molecule that share an
 // element stay adjacent; group-local, so that the reductions into a molecule's row of Z stay in L2) into tiles of kNT
 // columns that never mix elements; x rows are gathered, scaled by one power of two per tile and split into
@@ -286,10 +287,12 @@ struct FmCfg {
   static constexpr int d = D_;
   static constexpr int kKB = D_ / kKBlk;
   static constexpr int kParts = kRff ? 2 : 1;                                  // W parts in shared memory (hi, lo)
-  static constexpr int kG = (D_ <= 128 ? 4 : 2) / kParts;                      // 128-feature tiles per task
+  static constexpr int kCtas = D_ <= 128 ? 2 : 1;                              // CTAs per SM
+  static constexpr int kG = (D_ <= 128 ? 4 : 2) / kParts / kCtas;              // 128-feature tiles per task
   static constexpr int kNT = fm_nt(D_);                                        // atoms per tile
-  static constexpr int kStages = D_ <= 128 ? 4 : 3;
-  static constexpr int kTBufRaw = 512 / (kG * kNT);
+  static constexpr int kStages = kCtas == 2 ? 2 : (D_ <= 128 ? 4 : 3);
+  static constexpr int kTmemCols = 512 / kCtas;
+  static constexpr int kTBufRaw = kTmemCols / (kG * kNT);
   static constexpr int kTBuf = kTBufRaw > 4 ? 4 : kTBufRaw;
   static constexpr uint32_t kABytes = kParts * kG * kKB * kTileBytes;          // 128 KB
   static constexpr uint32_t kStageBytes = 2 * kNT * 128;                       // hi + lo tile of one k-block
@@ -303,7 +306,7 @@ struct FmCfg {
 };
 
 template <int D_, bool kRff>
-__global__ void __launch_bounds__(FmCfg<D_, kRff>::kThreads, 1)
+__global__ void __launch_bounds__(FmCfg<D_, kRff>::kThreads, FmCfg<D_, kRff>::kCtas)
 featmap_mma_kernel(const int* __restrict__ tile_elem, const int* __restrict__ n_tiles_ptr,
                    const uint32_t* __restrict__ end_mask, const int* __restrict__ run_mol, int D, int n_ft, float c, const float* __restrict__ c_elem,
                    float nrm, const __half* __restrict__ Wh, const __half* __restrict__ Wl,
@@ -335,7 +338,7 @@ featmap_mma_kernel(const int* __restrict__ tile_elem, const int* __restrict__ n_
     fence_mbarrier_init();
   }
   if (warp == 2) {
-    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], 512;" ::"r"(smem_u32(tmem_ptr_smem))
+    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(tmem_ptr_smem)), "n"(C::kTmemCols)
                  : "memory");
     asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
   }
@@ -561,7 +564,7 @@ featmap_mma_kernel(const int* __restrict__ tile_elem, const int* __restrict__ n_
   __syncthreads();
   if (warp == 2) {
     tcgen05_fence_after();
-    asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, 512;" ::"r"(tmem_base) : "memory");
+    asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "n"(C::kTmemCols) : "memory");
   }
 }
 
@@ -639,7 +642,7 @@ static int launch_featmap(int n_elem, int D, float c, const float* c_elem, const
   const int n_ft = (D + kTile - 1) / kTile;
   const int n_chunks = (int)((tiles + kFmChunkTiles - 1) / kFmChunkTiles);
   const long long n_tasks = (long long)n_chunks * ((n_ft + C::kG - 1) / C::kG);
-  const int grid = (int)(n_tasks < device_sm_count() ? n_tasks : device_sm_count());
+  const int grid = (int)(n_tasks < device_sm_count() * C::kCtas ? n_tasks : device_sm_count() * C::kCtas);
   const float nrm = (float)sqrt(2.0 / (double)D);
   kern<<<grid, C::kThreads, C::kSmem, st>>>(tile_elem, key_tile0 + n_keys, end_mask, run_mol, D, n_ft, c, c_elem, nrm, Wh, Wl, Xh, Xl,
                                             inv_scale, bias, n_chunks, small ? 1 : D, Z);
