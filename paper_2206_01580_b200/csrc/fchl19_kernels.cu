@@ -19,10 +19,11 @@
 //     global atomics); the block of the central atom is minus the sum of the others (translation invariance) and is
 //     accumulated in shared memory.
 // The Jacobian is the big output: (K + 1) rep 3 floats per atom (15 625-atom cell, K = 64: 8.8 GB).  Measured
-// (profiles/r2_fchl19_featmap.md): 3.9 ms = 2.25 TB/s of writes (0.35 of the HBM copy peak) with 58 % of the issue
-// slots busy at 16 warps / SM -- issue-bound (~170 k warp instructions per atom), not yet write-bound.
+// (profiles/r2_fchl19_featmap.md): 2.9 ms = 3.0 TB/s of writes (0.46 of the HBM copy peak) at 32 warps / SM (four
+// blocks: tables sized by K, 64 registers) -- issue-bound (~170 k warp instructions per atom), not yet write-bound;
+// 3.9 ms with two blocks per SM.
 // Mode 2 (qmll_fchl19_backward) is the Jacobian-free backward pass: the same loops, but every lane multiplies what it
-// would have written by dE/d rho and the warp reduces to one force vector per neighbour (2.0 ms, nothing materialised).
+// would have written by dE/d rho and the warp reduces to one force vector per neighbour (1.65 ms, nothing materialised).
 #include <math_constants.h>
 
 #include "qmll_common.cuh"
@@ -37,36 +38,44 @@ constexpr int kFchlMaxElem = 16;
 
 struct FchlDev {
   int E, n2, n3, rep, K;
+  int cap;                            // rows of the shared-memory neighbour tables: min(K rounded up to 4, kFchlMaxN)
   float eta2, eta3, N2, N3, c3d;      // c3d = c3 * 2 exp(-zeta^2 / 2)   (n = 1 Fourier terms, reading B5)
   float rcut, inv_rcut, rs2_step, rs3_step, norm3;
 };
 
 struct FchlSmem {
-  float *vx, *vy, *vz, *rr, *fc, *dfc;   // [kFchlMaxN] sorted neighbour table: vector i -> j, length, f, f'
-  int *ne, *nslot;                       // [kFchlMaxN] element, neighbour slot q
+  float *vx, *vy, *vz, *rr, *fc, *dfc;   // [cap] sorted neighbour table: vector i -> j, length, f, f'
+  int *ne, *nslot;                       // [cap] element, neighbour slot q
   int* e_start;                          // [kFchlMaxElem + 1] first sorted index of every element
   int* misc;                             // [4]: nn, n_invalid
   int* inv_list;                         // [K] slots that hold no neighbour inside r_cut
   float* rho_acc;                        // [rep]
   float* self_acc;                       // [3 rep]
-  float* pair_tab;                       // [warps][kFchlMaxN][kPairF]
+  float* pair_tab;                       // [warps][cap][kPairF]
   float* stage;                          // [warps][192]
 };
 
+// The tables hold `cap` neighbours: no more than K slots can be inside r_cut, so K (not the library-wide maximum) sizes
+// them -- 36 KB instead of 76 KB per block at K = 64, which is what lets 4-5 blocks share an SM.
+__host__ __device__ inline int fchl_cap(int K) {
+  const int k4 = (K + 3) & ~3;
+  return k4 < 4 ? 4 : (k4 > kFchlMaxN ? kFchlMaxN : k4);
+}
 __host__ __device__ inline size_t fchl_smem_floats(int rep, int K, bool jac) {
-  return (size_t)8 * kFchlMaxN + 32 + 8 + (size_t)K + (size_t)rep + (jac ? (size_t)3 * rep : 0) +
-         (size_t)kFchlWarps * kFchlMaxN * kPairF + (size_t)kFchlWarps * 192 + 16;
+  const size_t cap = (size_t)fchl_cap(K);
+  return 8 * cap + 32 + 8 + (size_t)K + (size_t)rep + (jac ? (size_t)3 * rep : 0) + (size_t)kFchlWarps * cap * kPairF +
+         (size_t)kFchlWarps * 192 + 16;
 }
 
-__device__ __forceinline__ FchlSmem fchl_carve(float* sm, int rep, int K, bool jac) {
+__device__ __forceinline__ FchlSmem fchl_carve(float* sm, int rep, int K, int cap, bool jac) {
   FchlSmem s;
-  s.pair_tab = sm;  sm += kFchlWarps * kFchlMaxN * kPairF;      // first: 16-byte aligned float4 rows
+  s.pair_tab = sm;  sm += kFchlWarps * cap * kPairF;            // first: 16-byte aligned float4 rows
   s.stage = sm;     sm += kFchlWarps * 192;
-  s.vx = sm; s.vy = sm + kFchlMaxN; s.vz = sm + 2 * kFchlMaxN; s.rr = sm + 3 * kFchlMaxN;
-  s.fc = sm + 4 * kFchlMaxN; s.dfc = sm + 5 * kFchlMaxN;
-  s.ne = reinterpret_cast<int*>(sm + 6 * kFchlMaxN);
-  s.nslot = s.ne + kFchlMaxN;
-  s.e_start = s.nslot + kFchlMaxN;
+  s.vx = sm; s.vy = sm + cap; s.vz = sm + 2 * cap; s.rr = sm + 3 * cap;
+  s.fc = sm + 4 * cap; s.dfc = sm + 5 * cap;
+  s.ne = reinterpret_cast<int*>(sm + 6 * cap);
+  s.nslot = s.ne + cap;
+  s.e_start = s.nslot + cap;
   s.misc = s.e_start + 32;
   s.inv_list = s.misc + 8;
   s.rho_acc = reinterpret_cast<float*>(s.inv_list + K);
@@ -86,14 +95,14 @@ __device__ __forceinline__ void f_cut_pair(float r, const FchlDev& P, float* f, 
 // components are stored and summed in on-chip memory"): F[j] -= sum_k w_i[k] d rho_i[k] / d r_j for every neighbour
 // image j, F[i] += the same sum (translation invariance), with w_i = dE / d rho_i given -- no Jacobian is materialised.
 template <int kMode>
-__global__ void __launch_bounds__(kFchlThreads, 2)
+__global__ void __launch_bounds__(kFchlThreads, kMode == 0 ? 5 : 4)
 fchl19_kernel(const FchlDev P, const float* __restrict__ r, const int32_t* __restrict__ elem,
               const int32_t* __restrict__ nbr_idx, const float* __restrict__ nbr_shift, long long n_atoms,
               float* __restrict__ rho, int32_t* __restrict__ jac_idx, float* __restrict__ jac_val,
               int32_t* __restrict__ info, const float* __restrict__ w_in, float* __restrict__ forces) {
   constexpr bool kJac = kMode == 1, kVjp = kMode == 2, kGrad = kMode != 0;
   extern __shared__ __align__(16) float sm_raw[];
-  const FchlSmem S = fchl_carve(sm_raw, P.rep, P.K, kGrad);
+  const FchlSmem S = fchl_carve(sm_raw, P.rep, P.K, P.cap, kGrad);
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const long long i = blockIdx.x;
   const int rep = P.rep, K = P.K, off3 = P.E * P.n2;
@@ -124,17 +133,17 @@ fchl19_kernel(const FchlDev P, const float* __restrict__ r, const int32_t* __res
       const unsigned imask = __ballot_sync(0xffffffffu, q < K && !valid);
       const unsigned lt = (1u << lane) - 1u;
       const int pos = cnt + __popc(mask & lt);
-      if (valid && pos < kFchlMaxN) {
+      if (valid && pos < P.cap) {
         S.vx[pos] = dx; S.vy[pos] = dy; S.vz[pos] = dz; S.rr[pos] = sqrtf(d2);
         S.ne[pos] = __ldg(elem + j); S.nslot[pos] = kVjp ? j : q;     // backward: the atom that receives the force
       }
       if (q < K && !valid) S.inv_list[n_inv + __popc(imask & lt)] = q;
-      if (kJac && q < K) jac_idx[i * (K + 1) + 1 + q] = (valid && pos < kFchlMaxN) ? j : -1;
+      if (kJac && q < K) jac_idx[i * (K + 1) + 1 + q] = (valid && pos < P.cap) ? j : -1;
       cnt += __popc(mask);
       n_inv += __popc(imask);
     }
     if (lane == 0) {
-      if (cnt > kFchlMaxN) { atomicMax(info, (int)(i < 0x7fffffff ? i + 1 : 0x7fffffff)); cnt = kFchlMaxN; }
+      if (cnt > P.cap) { atomicMax(info, (int)(i < 0x7fffffff ? i + 1 : 0x7fffffff)); cnt = P.cap; }
       S.misc[0] = cnt; S.misc[1] = n_inv;
       if (kJac) jac_idx[i * (K + 1)] = (int32_t)i;
     }
@@ -178,7 +187,7 @@ fchl19_kernel(const FchlDev P, const float* __restrict__ r, const int32_t* __res
   }
 
   // ---- phase 1: one warp per neighbour slot ----
-  float* pt = S.pair_tab + warp * (kFchlMaxN * kPairF);
+  float* pt = S.pair_tab + warp * (P.cap * kPairF);
   float* stage = S.stage + warp * 192;
   const float* wv = S.self_acc;                 // kVjp: dE / d rho_i
   float self_x = 0.f, self_y = 0.f, self_z = 0.f;
@@ -364,7 +373,7 @@ int fchl19_launch(const qmll_fchl19_params* fp, const float* r, const int32_t* e
                   const int32_t* nbr_idx, const float* nbr_shift, int32_t K, float* rho, int32_t* jac_idx,
                   float* jac_val, int32_t* info, const float* w_in, float* forces, cudaStream_t st) {
   FchlDev P;
-  P.E = fp->n_elem; P.n2 = fp->n2; P.n3 = fp->n3; P.rep = fchl19_rep_size(fp); P.K = K;
+  P.E = fp->n_elem; P.n2 = fp->n2; P.n3 = fp->n3; P.rep = fchl19_rep_size(fp); P.K = K; P.cap = fchl_cap(K);
   P.eta2 = fp->eta2; P.eta3 = fp->eta3; P.N2 = fp->two_body_decay; P.N3 = fp->three_body_decay;
   P.c3d = (float)((double)fp->three_body_weight * 2.0 * exp(-0.5 * (double)fp->zeta * (double)fp->zeta));
   P.rcut = fp->r_cut; P.inv_rcut = 1.f / fp->r_cut;
