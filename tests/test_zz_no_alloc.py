@@ -85,7 +85,7 @@ def test_static_scratch_call_allocates_no_device_memory(q):
         pkg.qmll_predict_static(dp.params, dp.x, dp.elem, dp.mol_off, dp.alpha, E, dp.grad, F)
     torch.cuda.synchronize()
     free1, _ = torch.cuda.mem_get_info()
-    assert free1 == free0 and torch.cuda.memory_allocated() == allocated0
+    assert free1 >= free0 and torch.cuda.memory_allocated() == allocated0      # free device memory did not shrink
     E_ref, F_ref = pkg.qmll_predict(dp.params, dp.x, dp.elem, dp.mol_off, dp.alpha, dp.grad)
     assert rel(E, E_ref) <= TOL and rel(F, F_ref) <= TOL_F
 
