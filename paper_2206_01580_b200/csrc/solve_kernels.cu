@@ -296,11 +296,13 @@ __device__ __forceinline__ void st_release_gpu(int* p, int v) {
   asm volatile("st.release.gpu.global.s32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
 }
 
+constexpr int kTrsvSmemBytes = (2 * kNB * (kNB + 1) + 2 * kNB) * 8;
 __global__ void __launch_bounds__(128) trsv_back_kernel(const double* __restrict__ M, int D, int ld,
                                                         const double* __restrict__ y, double* __restrict__ sol,
                                                         int* __restrict__ flags, int* __restrict__ ticket) {
-  __shared__ double l[kNB][kNB + 1];
-  __shared__ double dinv[kNB];
+  extern __shared__ __align__(16) double tsm[];           // the two diagonal blocks this CTA owns + their 1 / l_cc
+  double (*tiles)[kNB][kNB + 1] = reinterpret_cast<double (*)[kNB][kNB + 1]>(tsm);
+  double (*dinv2)[kNB] = reinterpret_cast<double (*)[kNB]>(tsm + 2 * kNB * (kNB + 1));
   __shared__ double s_sol[kNB];
   __shared__ double s_run[2 * kNB];
   __shared__ int s_b;
@@ -311,6 +313,20 @@ __global__ void __launch_bounds__(128) trsv_back_kernel(const double* __restrict
   const int j = b * 128 + t;
   double r = j < D ? y[j] : 0.0;
   const int n_blk = (D + kNB - 1) / kNB;
+  // both owned diagonal blocks are fetched now: by the time their turn comes (after every later block) they are here,
+  // and the load is off the chain of dependent block solves
+  for (int o = 0; o < 2; ++o) {
+    const int kb = 2 * b + o, k0 = kb * kNB, nb = kb < n_blk ? (D - k0 < kNB ? D - k0 : kNB) : 0;
+    for (int idx = t; idx < kNB * kNB; idx += 128) {
+      const int rr = idx / kNB, c = idx % kNB;
+      if (rr < nb && c <= rr) cp_async8(&tiles[o][rr][c], M + (size_t)(k0 + rr) * ld + k0 + c);
+      else tiles[o][rr][c] = rr == c ? 1.0 : 0.0;
+    }
+  }
+  cp_async_wait_all();
+  __syncthreads();
+  dinv2[t >> 6][t & 63] = 1.0 / tiles[t >> 6][t & 63][t & 63];
+  __syncthreads();
   for (int kb = n_blk - 1; kb >= 2 * b; --kb) {
     const int k0 = kb * kNB, nb = D - k0 < kNB ? D - k0 : kNB;
     const bool upd = j < k0;                              // this entry receives block kb's term
@@ -318,15 +334,9 @@ __global__ void __launch_bounds__(128) trsv_back_kernel(const double* __restrict
 #pragma unroll
     for (int m = 0; m < kNB; ++m) lc[m] = (upd && m < nb) ? M[(size_t)(k0 + m) * ld + j] : 0.0;
     if ((kb >> 1) == b) {                                 // owner: diagonal solve
-      for (int idx = t; idx < kNB * kNB; idx += 128) {
-        const int rr = idx / kNB, c = idx % kNB;
-        if (rr < nb && c <= rr) cp_async8(&l[rr][c], M + (size_t)(k0 + rr) * ld + k0 + c);
-        else l[rr][c] = rr == c ? 1.0 : 0.0;
-      }
+      const double (*l)[kNB + 1] = tiles[kb & 1];
+      const double* dinv = dinv2[kb & 1];
       s_run[t] = r;
-      cp_async_wait_all();
-      __syncthreads();
-      if (t < kNB) dinv[t] = 1.0 / l[t][t];
       __syncthreads();
       if (t < 32) {
         const int o = (kb & 1) * kNB;                     // the block's entries sit in threads o .. o + 63
@@ -397,6 +407,8 @@ static int solve_side(SolveSide** out) {
     if (cudaEventCreateWithFlags(&s.ev_main, cudaEventDisableTiming) != cudaSuccess) return QMLL_ERR_CUDA;
     if (cudaEventCreateWithFlags(&s.ev_hi, cudaEventDisableTiming) != cudaSuccess) return QMLL_ERR_CUDA;
     if (cudaFuncSetAttribute(syrk_update_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kUSmemBytes) != cudaSuccess)
+      return QMLL_ERR_CUDA;
+    if (cudaFuncSetAttribute(trsv_back_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kTrsvSmemBytes) != cudaSuccess)
       return QMLL_ERR_CUDA;
     s.ready = true;
   }
@@ -470,7 +482,7 @@ int solve_normal_equations(const float* ZtZ, const float* Zty, int32_t D, double
   }
   QMLL_SOLVE_CUDA(cudaEventRecord(side->ev_hi, hi));
   QMLL_SOLVE_CUDA(cudaStreamWaitEvent(st, side->ev_hi, 0));
-  trsv_back_kernel<<<(D + 127) / 128, 128, 0, st>>>(M, D, ld, y, sol, flags, flags + n_blk);   // L^T alpha = y
+  trsv_back_kernel<<<(D + 127) / 128, 128, kTrsvSmemBytes, st>>>(M, D, ld, y, sol, flags, flags + n_blk);   // L^T alpha = y
   QMLL_LAUNCH_CHECK("trsv_back_kernel");
   solve_finish_kernel<<<(D + 255) / 256, 256, 0, st>>>(sol, alpha, D);
   QMLL_LAUNCH_CHECK("solve_finish_kernel");
