@@ -335,6 +335,30 @@ def test_solve_reports_non_positive_definite(q):
     assert int(info.item()) == 334
 
 
+def test_solve_is_bit_reproducible_across_repeats_and_streams(q):
+    """The look-ahead fork / join and the flag hand-over of the backward substitution leave no room for a race: every
+    element of the factor has one writer, so repeated solves (alternating streams) must be bit-identical."""
+    pkg, wio, torch = q
+    g = torch.Generator(device="cuda").manual_seed(11)
+    for D in (577, 1000, 2048):
+        A = torch.randn((D + 300, D), device="cuda", generator=g) / D ** 0.5
+        ZtZ = A.T @ A
+        Zty = torch.randn((D,), device="cuda", generator=g)
+        ref, info = pkg.qmll_solve(ZtZ, Zty, 1e-3)
+        torch.cuda.synchronize()
+        assert int(info.item()) == 0
+        s = torch.cuda.Stream()
+        for k in range(24):
+            if k % 2:
+                with torch.cuda.stream(s):
+                    a, _ = pkg.qmll_solve(ZtZ, Zty, 1e-3)
+                s.synchronize()
+            else:
+                a, _ = pkg.qmll_solve(ZtZ, Zty, 1e-3)
+                torch.cuda.synchronize()
+            assert torch.equal(a, ref)
+
+
 def test_solve_on_a_side_stream_and_under_graph_capture(q):
     """qmll_solve forks panel work onto an internal stream (look-ahead): the result must not depend on the caller's
     stream, and the fork / join must be capturable."""
