@@ -537,6 +537,9 @@ def other_configs(pk, reps, rows_mode=0, only=None):
                 Zm = torch.empty((nm, D), dtype=torch.float32, device="cuda")
                 t = tm(lambda: pkg.qmll_sorf_forward_mma(p, dp.x, dp.elem, dp.mol_off, Z=Zm))
                 cos_s = na * D / (t * 1e-3)
+                Em = torch.empty((nm,), dtype=torch.float32, device="cuda")
+                te = tm(lambda: pkg.qmll_energies(pkg.qmll_sorf_forward_mma(p, dp.x, dp.elem, dp.mol_off, Z=Zm), dp.alpha, energies=Em))
+                o.update({"predict_energies_mma_ms": te, "predict_energies_mma_molecules_per_s": nm / (te * 1e-3)})
                 o.update({"forward_mma_ms": t, "forward_mma_molecules_per_s": nm / (t * 1e-3),
                           "forward_mma_useful_f16_tflops": 2.0 * 2.0 * m.d * D * na / (t * 1e-3) / 1e12,
                           "forward_mma_cos_frac_of_mufu_peak": cos_s / pk.get("mufu_per_s", 4.3e12)})

@@ -33,7 +33,7 @@ EXPORTS = ("qmll_solve", "qmll_sorf_forward", "qmll_sorf_forward_mode", "qmll_so
            "qmll_collect_normal_equations_kernel_ms", "qmll_microbench", "qmll_microbench_mma", "qmll_pack_lower", "qmll_unpack_lower", "qmll_project",
            "qmll_project_neighbor", "qmll_fchl19", "qmll_fchl19_rep_size", "qmll_sorf_forward_mma", "qmll_rff_forward",
            "qmll_featmap_workspace_bytes", "qmll_sorf_backward_g", "qmll_project_back", "qmll_fchl19_backward",
-           "qmll_predict_static", "qmll_predict_static_max_bytes")
+           "qmll_predict_static", "qmll_predict_static_max_bytes", "qmll_energies")
 
 
 class _CParams(ctypes.Structure):
@@ -88,6 +88,8 @@ def load_library() -> ctypes.CDLL:
     lib.qmll_predict.argtypes = [pp, vp, vp, vp, i64, i32, vp, gp, vp, vp, vp, sz, vp]
     lib.qmll_predict_static.argtypes = [pp, vp, vp, vp, i64, i32, vp, gp, vp, vp, vp]
     lib.qmll_predict_static.restype = ctypes.c_int
+    lib.qmll_energies.argtypes = [vp, vp, i64, i32, vp, vp]
+    lib.qmll_energies.restype = ctypes.c_int
     lib.qmll_predict_static_max_bytes.argtypes = []
     lib.qmll_predict_static_max_bytes.restype = sz
     lib.qmll_project.argtypes = [vp, vp, vp, i64, i32, i32, i32, i32, vp, vp, vp, vp, vp, vp, vp]
@@ -283,6 +285,17 @@ def qmll_predict(p: SorfParams, x, elem, mol_off, alpha, grad: Optional[Grad] = 
                             _dev(forces, torch.float32, "forces"), ctypes.c_void_p(ws.data_ptr()), ws.numel(),
                             _stream()))
     return energies, forces
+
+
+def qmll_energies(Z, alpha, energies=None):
+    """energies [n_mol] = Z @ alpha: include/qmll.h qmll_energies (step a4 for a caller that holds Z)."""
+    lib = load_library()
+    n_mol, D = int(Z.shape[0]), int(Z.shape[1])
+    if energies is None:
+        energies = torch.empty((n_mol,), dtype=torch.float32, device=Z.device)
+    _check(lib.qmll_energies(_dev(Z, torch.float32, "Z"), _dev(alpha, torch.float32, "alpha"), n_mol, D,
+                             _dev(energies, torch.float32, "energies"), _stream()))
+    return energies
 
 
 def qmll_predict_static(p: SorfParams, x, elem, mol_off, alpha, energies, grad: Optional[Grad] = None, forces=None):

@@ -392,6 +392,13 @@ int qmll_unpack_lower(const float* packed, int32_t D, float* ZtZ, void* cuda_str
   return syrk_unpack_lower(packed, D, ZtZ, static_cast<cudaStream_t>(cuda_stream));
 }
 
+int qmll_energies(const float* Z, const float* alpha, int64_t n_mol, int32_t D, float* energies, void* cuda_stream) {
+  if (n_mol < 0 || D <= 0 || !alpha || (n_mol > 0 && (!Z || !energies))) return QMLL_ERR_INVALID_ARG;
+  int rc = check_device();
+  if (rc) return rc;
+  return energies_from_z(Z, alpha, n_mol, D, energies, static_cast<cudaStream_t>(cuda_stream));
+}
+
 int qmll_solve(const float* ZtZ, const float* Zty, int32_t D, double lambda, float* alpha, int32_t* info,
                void* workspace, size_t workspace_bytes, void* cuda_stream) {
   if (!ZtZ || !Zty || !alpha || !info || D <= 0 || !(lambda >= 0.0)) return QMLL_ERR_INVALID_ARG;

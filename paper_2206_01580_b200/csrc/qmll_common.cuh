@@ -114,6 +114,7 @@ int syrk_pack_lower(const float* C, int32_t D, float* packed, cudaStream_t st);
 int syrk_unpack_lower(const float* packed, int32_t D, float* C, cudaStream_t st);
 
 // ---- solve (solve_kernels.cu) ------------------------------------------------------------------------------
+int energies_from_z(const float* Z, const float* alpha, int64_t n_mol, int32_t D, float* energies, cudaStream_t st);
 size_t solve_workspace_bytes(int32_t D);
 int solve_normal_equations(const float* ZtZ, const float* Zty, int32_t D, double lambda, float* alpha, int32_t* info,
                            void* ws, size_t ws_bytes, cudaStream_t st);

@@ -70,6 +70,7 @@ def test_host_side_argument_checks_need_no_gpu(lib):
     assert l.qmll_normal_equations_mode(None, None, 4, 256, 0, None, None, None, 0, 9, None) == -1
     assert l.qmll_predict(None, None, None, None, 0, 0, None, None, None, None, None, 0, None) == -1
     assert l.qmll_sorf_backward_forces(None, None, None, None, 0, 0, None, None, None, None, 0, None) == -1
+    assert l.qmll_energies(None, None, 4, 16, None, None) == -1 and l.qmll_energies(None, None, -1, 16, None, None) == -1
     # the static-scratch prediction: null / invalid parameters and problems beyond the array are rejected on the host
     assert l.qmll_predict_static(None, None, None, None, 0, 0, None, None, None, None, None) == -1
     assert int(l.qmll_predict_static_max_bytes()) == 4 << 20

@@ -107,6 +107,32 @@ def test_rff_with_the_dense_sorf_matrix_reproduces_sorf(q):
     assert rel(pkg.qmll_sorf_forward_mma(dp.params, dp.x, dp.elem, dp.mol_off).cpu().numpy(), Zo) <= TOL
 
 
+@pytest.mark.parametrize("n_mol,D", [(1, 4), (7, 130), (33, 1024), (300, 8192), (5, 3)])
+def test_energies_from_z_matches_oracle(q, n_mol, D):
+    """qmll_energies (step a4 on a given Z, eq. 15) against the oracle's FP64 product; odd D takes the scalar path."""
+    pkg, wio, torch = q
+    rng = np.random.default_rng(n_mol + D)
+    Z = rng.standard_normal((n_mol, D)).astype(np.float32)
+    alpha = (rng.standard_normal(D) / np.sqrt(D)).astype(np.float32)
+    E = pkg.qmll_energies(torch.from_numpy(Z).cuda(), torch.from_numpy(alpha).cuda())
+    torch.cuda.synchronize()
+    assert rel(E.cpu().numpy(), oracle.energy(Z, alpha)) <= TOL
+    assert pkg.qmll_energies(torch.empty((0, D), device="cuda"), torch.from_numpy(alpha).cuda()).shape == (0,)
+
+
+def test_feature_map_plus_energies_is_the_energy_only_prediction(q):
+    """Tensor-core feature map + qmll_energies = energies of qmll_predict, against the oracle (config 2 shape, 200
+    molecules) -- the energies-only prediction of the f4 variants."""
+    pkg, wio, torch = q
+    w = make_workload("c2", n_mol=200, with_grad=False)
+    dp = wio.device_problem(w)
+    E = pkg.qmll_energies(pkg.qmll_sorf_forward_mma(dp.params, dp.x, dp.elem, dp.mol_off), dp.alpha)
+    E_fwht, _ = pkg.qmll_predict(dp.params, dp.x, dp.elem, dp.mol_off, dp.alpha)
+    torch.cuda.synchronize()
+    Eo = oracle.energy(oracle.forward_w(w), w.alpha)
+    assert rel(E.cpu().numpy(), Eo) <= TOL and rel(E_fwht.cpu().numpy(), Eo) <= TOL
+
+
 def test_sorf_forward_mma_fullsize_c3(q):
     """Config 3 at full size (100 000 molecules, 1.6 M atoms, D = 16384) in the launch configuration bench.py times
     (configs.c3.forward_mma_ms): 64 sampled molecules against the oracle, all of Z against the register-FWHT path."""
@@ -127,6 +153,13 @@ def test_sorf_forward_mma_fullsize_c3(q):
     num = float((Z - Z2).double().norm())
     den = float(Z2.double().norm())
     assert num / den <= TOL
+    # energies of all 100 000 molecules from this Z: the sampled ones against the oracle, all against qmll_predict
+    E = pkg.qmll_energies(Z, dp.alpha)
+    E_fwht, _ = pkg.qmll_predict(dp.params, dp.x, dp.elem, dp.mol_off, dp.alpha)
+    torch.cuda.synchronize()
+    Eo = oracle.energy(Z[torch.from_numpy(mols).cuda()].cpu().numpy(), w.alpha)
+    assert rel(E.cpu().numpy()[mols], Eo) <= TOL
+    assert float((E - E_fwht).double().norm() / E_fwht.double().norm()) <= TOL
 
 
 def test_sorf_forward_mma_offsets_beyond_31_bits(q):
